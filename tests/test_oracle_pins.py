@@ -1,0 +1,352 @@
+"""Pins for the CPU oracle: each checks the oracle against something other than itself --
+closed forms the paper fixes, brute force on tiny inputs, torch float64 library routines,
+algebraic invariants (BASELINE.json north_star: "hand-rolled conv1d versus a naive triple loop,
+linearity of the histogram under track permutation, bias-only output for empty intervals, the
+400 mm / 4000-bin / 0.1 mm geometry").  CPU only.
+"""
+import os
+
+import numpy as np
+import pytest
+import torch
+import torch.nn.functional as F
+
+from oracle import pvf_oracle as O
+from pvf_inputs import make_events, make_weights, unet_layer_shapes, fc_layer_shapes
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "geometry_and_sizes.txt")
+
+
+def _golden():
+    d = {}
+    with open(GOLDEN) as f:
+        for line in f:
+            line = line.split("#")[0].strip()
+            if line:
+                k, v = line.split()
+                d[k] = float(v)
+    return d
+
+
+# ---------------------------------------------------------------- geometry
+def test_geometry_closed_forms():
+    g = _golden()
+    assert O.N_INTERVALS == g["n_intervals"] and O.N_BINS == g["n_bins"]
+    assert O.N_INTERVALS * O.N_BINS * O.BIN_WIDTH_MM == pytest.approx(g["region_mm"], abs=1e-12)
+    assert O.N_GLOBAL_BINS == 4000
+    assert O.Z_MIN_MM == g["z_min_mm"] and O.BIN_WIDTH_MM == g["bin_width_mm"]
+    assert O.bin_centre_mm(0) == pytest.approx(-199.95, abs=1e-12)
+    assert O.bin_centre_mm(3999) == pytest.approx(199.95, abs=1e-12)
+    assert O.MAX_PEAKS == g["max_peaks"] and float(O.PEAK_THRESHOLD) == pytest.approx(g["peak_threshold"])
+    assert O.FC_CHANNELS * O.N_BINS == g["fc_out"]
+
+
+def test_interval_assignment_cases():
+    z = np.array([-200.0, 199.99, -190.0 + 0.35, 0.0, 200.0, -200.01, np.nan, np.inf, -0.05], np.float32)
+    iv, zrel, nonfinite = O.assign_intervals(z)
+    assert iv[0] == 0 and zrel[0] == 0.0
+    assert iv[1] == 39
+    assert iv[2] == 1 and zrel[2] == pytest.approx(0.035, abs=2e-6)
+    assert iv[3] == 20 and zrel[3] == pytest.approx(0.0, abs=1e-6)
+    assert iv[4] == -1 and iv[5] == -1            # outside [-200, 200): dropped
+    assert iv[6] == -1 and iv[7] == -1 and nonfinite[6] and nonfinite[7]
+    assert iv[8] == 19 and zrel[8] == pytest.approx(0.995, abs=2e-6)
+    assert np.all((zrel >= 0) & (zrel < 1))
+    # every bin centre falls in the interval that holds it, with zrel = (l + 0.5)/100
+    g = np.arange(4000)
+    iv, zrel, _ = O.assign_intervals(O.bin_centre_mm(g).astype(np.float32))
+    assert np.array_equal(iv, g // 100)
+    assert np.allclose(zrel, ((g % 100) + 0.5) / 100.0, atol=3e-6)
+
+
+def test_sizes_from_config():
+    g = _golden()
+    w = make_weights("rand", 1)
+    assert len(w.fc_w) == g["fc_layers"]
+    assert sum(a.size for a in w.fc_w + w.fc_b) == g["fc_params"]
+    assert sum(a.size for a in w.conv_w + w.conv_b) == g["unet_params"]
+    assert w.fc_w[0].shape == (25, g["n_features"]) and w.fc_w[5].shape == (g["fc_out"], 25)
+    L = [100, 50, 25, 50, 100, 100]
+    mac = sum(l * co * ci * k for l, (co, ci, k) in zip(L, unet_layer_shapes(64)))
+    assert mac == g["unet_mac_per_interval"]
+
+
+# ---------------------------------------------------------------- conv1d
+def _naive_conv(x, W, b):
+    N, Cin, L = x.shape
+    Cout, _, K = W.shape
+    p = (K - 1) // 2
+    y = np.zeros((N, Cout, L))
+    for n in range(N):
+        for co in range(Cout):
+            for l in range(L):
+                acc = b[co]
+                for ci in range(Cin):
+                    for j in range(K):
+                        m = l + j - p
+                        if 0 <= m < L:
+                            acc += W[co, ci, j] * x[n, ci, m]
+                y[n, co, l] = acc
+    return y
+
+
+@pytest.mark.parametrize("Cin,Cout,K,L", [(2, 3, 5, 7), (3, 2, 3, 4), (1, 1, 25, 10), (4, 2, 15, 9)])
+def test_conv1d_vs_naive_loop(Cin, Cout, K, L):
+    rng = np.random.default_rng(7)
+    x = rng.normal(size=(2, Cin, L))
+    W = rng.normal(size=(Cout, Cin, K))
+    b = rng.normal(size=Cout)
+    assert np.allclose(O.conv1d_same(x, W, b), _naive_conv(x, W, b), rtol=0, atol=1e-12)
+
+
+@pytest.mark.parametrize("Cin,Cout,K,L", [(8, 64, 25, 100), (64, 64, 15, 50), (64, 64, 5, 25), (128, 64, 25, 100)])
+def test_conv1d_vs_torch_float64(Cin, Cout, K, L):
+    rng = np.random.default_rng(8)
+    x = rng.normal(size=(3, Cin, L))
+    W = rng.normal(size=(Cout, Cin, K))
+    b = rng.normal(size=Cout)
+    ref = F.conv1d(torch.from_numpy(x), torch.from_numpy(W), torch.from_numpy(b), padding=(K - 1) // 2).numpy()
+    assert np.allclose(O.conv1d_same(x, W, b), ref, rtol=0, atol=1e-11)
+
+
+def test_conv1d_delta_kernel_and_shift():
+    rng = np.random.default_rng(9)
+    x = rng.normal(size=(2, 3, 20))
+    W = np.zeros((3, 3, 7))
+    for c in range(3):
+        W[c, c, 3] = 1.0
+    b = np.array([0.5, -1.0, 2.0])
+    assert np.allclose(O.conv1d_same(x, W, b), x + b[None, :, None], atol=1e-15)
+    # off-centre delta: tap j = p + s reads x[l + s]  (cross-correlation, not convolution)
+    W2 = np.zeros((1, 1, 7))
+    W2[0, 0, 5] = 1.0
+    y = O.conv1d_same(x[:, :1], W2, np.zeros(1))
+    assert np.allclose(y[:, 0, :-2], x[:, 0, 2:]) and np.all(y[:, 0, -2:] == 0)
+    # interior shift equivariance
+    Wr = rng.normal(size=(2, 3, 5))
+    xs = np.zeros((1, 3, 40))
+    xs[:, :, 10:20] = rng.normal(size=(1, 3, 10))
+    y0 = O.conv1d_same(xs, Wr, np.zeros(2))
+    y1 = O.conv1d_same(np.roll(xs, 7, axis=2), Wr, np.zeros(2))
+    assert np.allclose(np.roll(y0, 7, axis=2), y1, atol=1e-14)
+
+
+# ---------------------------------------------------------------- pointwise + pool + upsample + FC
+def test_pointwise_closed_forms_and_torch():
+    assert O.softplus(0.0) == pytest.approx(np.log(2.0), abs=1e-15)
+    v = np.linspace(-40, 40, 401)
+    assert np.allclose(O.softplus(v) - O.softplus(-v), v, atol=1e-12)
+    assert O.sigmoid(0.0) == 0.5
+    assert np.allclose(O.sigmoid(v) + O.sigmoid(-v), 1.0, atol=1e-15)
+    tv = torch.from_numpy(v)
+    assert np.allclose(O.softplus(v), F.softplus(tv, beta=1.0, threshold=1e9).numpy(), atol=1e-13)
+    assert np.allclose(O.sigmoid(v), torch.sigmoid(tv).numpy(), atol=1e-15)
+    assert np.allclose(O.leaky_relu(v), F.leaky_relu(tv, 0.01).numpy(), atol=0)
+    assert O.leaky_relu(np.array([-2.0]))[0] == -0.02
+
+
+def test_pool_upsample_vs_torch():
+    rng = np.random.default_rng(3)
+    x = rng.normal(size=(2, 5, 100))
+    tx = torch.from_numpy(x)
+    assert np.array_equal(O.maxpool2(x), F.max_pool1d(tx, 2).numpy())
+    assert np.array_equal(O.upsample2_nearest(x), F.interpolate(tx, scale_factor=2, mode="nearest").numpy())
+    assert O.maxpool2(O.maxpool2(x)).shape[-1] == 25
+    assert np.array_equal(O.maxpool2(O.upsample2_nearest(x)), x)
+
+
+def _torch_fc(x, w):
+    h = torch.from_numpy(x)
+    for k in range(5):
+        h = F.leaky_relu(F.linear(h, torch.from_numpy(w.fc_w[k]).double(), torch.from_numpy(w.fc_b[k]).double()), 0.01)
+    return F.softplus(F.linear(h, torch.from_numpy(w.fc_w[5]).double(), torch.from_numpy(w.fc_b[5]).double()),
+                      beta=1.0, threshold=1e9).numpy()
+
+
+@pytest.mark.parametrize("kind", ["rand", "peaky"])
+def test_fc_vs_torch_float64(kind):
+    w = make_weights(kind, 5)
+    rng = np.random.default_rng(4)
+    x = rng.normal(size=(17, 9))
+    out = O.fc_forward(x, w.fc_w, w.fc_b)
+    assert out.shape == (17, 800)
+    assert np.allclose(out, _torch_fc(x, w), rtol=1e-13, atol=1e-13)
+    assert np.all(out > 0)  # softplus
+
+
+# ---------------------------------------------------------------- histogram invariants
+def test_histogram_permutation_additivity_sum():
+    w = make_weights("rand", 2)
+    ev = make_events("run3", 3, 11)
+    H, flags = O.histogram(ev.feat, ev.event_offsets, w.fc_w, w.fc_b)
+    assert H.shape == (3, 40, 8, 100)
+    # permutation of tracks inside each event
+    rng = np.random.default_rng(0)
+    perm = np.concatenate([ev.event_offsets[e] + rng.permutation(ev.event_offsets[e + 1] - ev.event_offsets[e])
+                           for e in range(3)])
+    Hp, _ = O.histogram(ev.feat[:, perm], ev.event_offsets, w.fc_w, w.fc_b)
+    assert np.allclose(H, Hp, rtol=1e-12, atol=1e-12)
+    # total = sum over in-range tracks of their 800 contributions
+    iv, zrel, _ = O.assign_intervals(ev.feat[0])
+    x = ev.feat.astype(np.float64).T.copy()
+    x[:, 0] = zrel
+    contrib = O.fc_forward(x[iv >= 0], w.fc_w, w.fc_b)
+    assert H.sum() == pytest.approx(contrib.sum(), rel=1e-12)
+    # additivity: event made of two track lists = sum of the two histograms; duplicate doubles
+    a = ev.feat[:, ev.event_offsets[0]:ev.event_offsets[1]]
+    b = ev.feat[:, ev.event_offsets[1]:ev.event_offsets[2]]
+    Ha, _ = O.histogram(a, [0, a.shape[1]], w.fc_w, w.fc_b)
+    Hb, _ = O.histogram(b, [0, b.shape[1]], w.fc_w, w.fc_b)
+    Hab, _ = O.histogram(np.concatenate([a, b], axis=1), [0, a.shape[1] + b.shape[1]], w.fc_w, w.fc_b)
+    assert np.allclose(Hab, Ha + Hb, rtol=1e-12, atol=1e-12)
+    Haa, _ = O.histogram(np.concatenate([a, a], axis=1), [0, 2 * a.shape[1]], w.fc_w, w.fc_b)
+    assert np.allclose(Haa, 2 * Ha, rtol=1e-12, atol=1e-12)
+    # a single track lands in exactly one interval, as its FC output
+    one = np.array([[-190.0 + 0.35, 0.01, -0.02, .1, .2, .1, .15, .12, .2]], np.float32).T
+    H1, _ = O.histogram(one, [0, 1], w.fc_w, w.fc_b)
+    xx = one.astype(np.float64).T.copy()
+    xx[0, 0] = float(O.assign_intervals(one[0])[1][0])
+    assert np.count_nonzero(H1.reshape(40, -1).any(axis=1)) == 1
+    assert np.allclose(H1[0, 1].reshape(-1), O.fc_forward(xx, w.fc_w, w.fc_b)[0], atol=1e-15)
+
+
+def test_dropped_and_nonfinite_tracks_are_flagged():
+    w = make_weights("rand", 2)
+    feat = np.full((9, 3), 0.1, np.float32)
+    feat[0] = [0.0, 250.0, np.nan]
+    H, flags = O.histogram(feat, [0, 3], w.fc_w, w.fc_b)
+    assert flags[0] == (O.FLAG_TRACK_DROPPED | O.FLAG_NONFINITE)
+    H0, f0 = O.histogram(feat[:, :1], [0, 1], w.fc_w, w.fc_b)
+    assert f0[0] == 0 and np.array_equal(H, H0)
+
+
+# ---------------------------------------------------------------- empty intervals / whole model
+def test_empty_intervals_bias_only():
+    w = make_weights("rand", 3)
+    Z = np.zeros((2, 8, 100))
+    e1 = O.leaky_relu(O.conv1d_same(Z, w.conv_w[0], w.conv_b[0]))
+    assert np.allclose(e1, O.leaky_relu(w.conv_b[0].astype(np.float64))[None, :, None], atol=1e-15)
+    ev = make_events("single", 1, 1000)
+    out = O.run(ev.feat, ev.event_offsets, w, want_hist=True)
+    empty = ~out["hist"][0].reshape(40, -1).any(axis=1)
+    assert empty.sum() >= 38
+    P = out["probs"][0].reshape(40, 100)
+    ref = O.unet_probs(np.zeros((1, 40, 8, 100)), w.conv_w, w.conv_b)[0].reshape(40, 100)[0]
+    for i in np.nonzero(empty)[0]:
+        assert np.array_equal(P[i], ref)
+
+
+def _torch_unet(H, w):
+    t = lambda a: torch.from_numpy(np.asarray(a)).double()
+    conv = lambda x, k: F.conv1d(x, t(w.conv_w[k]), t(w.conv_b[k]), padding=(w.conv_w[k].shape[2] - 1) // 2)
+    x = t(H)
+    e1 = F.leaky_relu(conv(x, 0), 0.01)
+    e2 = F.leaky_relu(conv(F.max_pool1d(e1, 2), 1), 0.01)
+    bt = F.leaky_relu(conv(F.max_pool1d(e2, 2), 2), 0.01)
+    d2 = F.leaky_relu(conv(torch.cat([F.interpolate(bt, scale_factor=2, mode="nearest"), e2], 1), 3), 0.01)
+    d1 = F.leaky_relu(conv(torch.cat([F.interpolate(d2, scale_factor=2, mode="nearest"), e1], 1), 4), 0.01)
+    return torch.sigmoid(conv(d1, 5))[:, 0].numpy()
+
+
+@pytest.mark.parametrize("kind,channels", [("rand", 64), ("peaky", 64), ("rand", 32), ("rand", 16)])
+def test_whole_model_vs_torch_composition(kind, channels):
+    w = make_weights(kind, 1, channels)
+    ev = make_events("single", 1, 1000)
+    out = O.run(ev.feat, ev.event_offsets, w, want_hist=True)
+    # FC + histogram through torch: per track, scatter-add
+    iv, zrel, _ = O.assign_intervals(ev.feat[0])
+    x = ev.feat.astype(np.float64).T.copy()
+    x[:, 0] = zrel
+    contrib = _torch_fc(x, w)
+    H = np.zeros((40, 8, 100))
+    for t in range(x.shape[0]):
+        H[iv[t]] += contrib[t].reshape(8, 100)
+    assert np.allclose(out["hist"][0], H, rtol=1e-12, atol=1e-12)
+    p = _torch_unet(H, w).reshape(4000)
+    assert np.max(np.abs(out["probs"][0].astype(np.float64) - p)) <= 1e-7  # float32 cast of a 1e-12-accurate value
+    p64 = O.sigmoid(O.unet_logits(H, w.conv_w, w.conv_b)).reshape(4000)
+    assert np.max(np.abs(p64 - p)) <= 1e-12
+
+
+# ---------------------------------------------------------------- peak finder hand cases
+def _P(**spikes):
+    P = np.zeros(4000, np.float32)
+    for g, v in spikes.items():
+        P[int(g[1:])] = v
+    return P
+
+
+def test_peaks_symmetric_triangle():
+    P = np.zeros(4000, np.float32)
+    P[1498:1503] = [0.1, 0.3, 0.6, 0.3, 0.1]
+    z, pr, bn, c, n = O.find_peaks_event(P)
+    assert c == 1 and n == 1 and bn[0] == 1500 and pr[0] == np.float32(0.6)
+    assert z[0] == pytest.approx(float(O.bin_centre_mm(1500)), abs=2e-5)   # delta = 0 exactly
+    f32 = np.float32
+    assert z[0] == f32(f32(f32(1500.0) + f32(0.5)) * f32(0.1)) + f32(-200.0)
+
+
+def test_peaks_asymmetric_centroid_value():
+    P = np.zeros(4000, np.float32)
+    P[10:13] = [0.2, 0.4, 0.4 - 1e-3]
+    z, pr, bn, c, n = O.find_peaks_event(P)
+    assert c == 1 and bn[0] == 11
+    w = P[8:15].astype(np.float64)
+    delta = (w * np.arange(-3, 4)).sum() / w.sum()
+    assert z[0] == pytest.approx(-200 + (11.5 + delta) * 0.1, abs=3e-5)
+
+
+def test_peaks_plateau_edges_threshold_cap():
+    P = np.zeros(4000, np.float32)
+    P[100:104] = 0.5                       # plateau: left-most bin only
+    P[0] = 0.2                             # g = 0 edge
+    P[3999] = 0.3                          # g = 3999 edge
+    P[2000] = np.float32(0.01)             # == threshold: not a peak
+    P[2100] = np.nextafter(np.float32(0.01), np.float32(1))
+    z, pr, bn, c, n = O.find_peaks_event(P)
+    assert list(bn[:c]) == [0, 100, 2100, 3999]
+    # edge centroids use the truncated window
+    assert z[0] == pytest.approx(-200 + 0.5 * 0.1, abs=2e-5)
+    assert z[3] == pytest.approx(-200 + 3999.5 * 0.1, abs=2e-5)
+    # 33 spikes: 32 kept in ascending order + overflow flag
+    P2 = np.zeros((1, 4000), np.float32)
+    P2[0, 50:50 + 33 * 10:10] = 0.9
+    out = O.find_peaks(P2)
+    assert out["count"][0] == 32 and out["flags"][0] == O.FLAG_PEAK_OVERFLOW
+    assert list(out["bin"][0]) == list(range(50, 50 + 320, 10))
+    # NaN never peaks; neighbours of NaN: comparisons with NaN are false
+    P3 = np.zeros(4000, np.float32)
+    P3[500] = np.nan
+    P3[700] = 0.4
+    z, pr, bn, c, n = O.find_peaks_event(P3)
+    assert list(bn[:c]) == [700]
+    # interval boundary is not special: a maximum at bin 100 with a larger left neighbour at 99
+    P4 = np.zeros(4000, np.float32)
+    P4[99], P4[100] = 0.5, 0.4
+    assert list(O.find_peaks_event(P4)[2][:1]) == [99] and O.find_peaks_event(P4)[3] == 1
+
+
+def test_match_and_tau_stable():
+    assert O.match_peaks([10, 20, 30], [11, 19, 40]) == (2, 3, 1)
+    assert O.match_peaks([10, 11], [10]) == (1, 2, 0)
+    assert O.match_peaks([], [5]) == (0, 0, 1)
+    P = np.zeros(4000)
+    P[100], P[101], P[102] = 0.5, 0.2, 0.4995
+    assert O.tau_stable_peaks(P, [100], 1e-3) == []      # P[102] too close
+    P[102] = 0.3
+    assert O.tau_stable_peaks(P, [100], 1e-3) == [100]
+    # property: any perturbation within tau keeps a tau-stable peak within +-1 bin
+    rng = np.random.default_rng(5)
+    w = make_weights("rand", 1)
+    ev = make_events("run3", 2, 77)
+    out = O.run(ev.feat, ev.event_offsets, w)
+    tau = 1e-3
+    for e in range(2):
+        P = out["probs"][e]
+        all_bins = np.nonzero((P > 0.01) & (P > np.r_[-np.inf, P[:-1]]) & (P >= np.r_[P[1:], -np.inf]))[0]
+        stable = O.tau_stable_peaks(P, all_bins, tau)
+        assert len(stable) > 0
+        Q = (P.astype(np.float64) + rng.uniform(-tau, tau, 4000)).astype(np.float32)
+        qb = np.nonzero((Q > 0.01) & (Q > np.r_[-np.inf, Q[:-1]]) & (Q >= np.r_[Q[1:], -np.inf]))[0]
+        m, nref, _ = O.match_peaks(stable, qb)
+        assert m == nref
