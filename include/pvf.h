@@ -1,0 +1,167 @@
+/* pvf.h -- C ABI of the B200-native PVFinder inference hot path.
+ *
+ * What it computes (section 2, lines 27-31; sizes from BASELINE.json config 0):
+ *   tracks (9 features, SoA) -> per-track 6-layer FC 9->25x5->800 -> deterministic sum into one
+ *   [8,100] histogram for each of the 40 z-intervals of every event -> 1D UNet (64 channels) per
+ *   interval -> sigmoid -> 4000 probabilities per event -> local-maximum peak finding.
+ *
+ * Shape of the boundary: a spec frozen at init (the paper's TensorSpec), one
+ * workspace pool allocated once (the paper's fixed 16 MB arena), per-call non-owning
+ * views of caller-owned SoA buffers (TensorView), a single caller-supplied stream with no
+ * allocation, no host synchronisation and no default-stream work inside the call,
+ * and a status enum for graceful degradation.
+ *
+ * All entry points are thread-compatible (one handle = one user at a time).  Unless noted,
+ * "device" pointers are CUDA device memory owned by the caller, "host" pointers are ordinary
+ * host memory.  No PyTorch types appear here.
+ */
+#ifndef PVF_H
+#define PVF_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define PVF_API __attribute__((visibility("default")))
+#else
+#define PVF_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pvf_ctx* pvf_handle;
+
+typedef enum {
+  PVF_OK = 0,
+  PVF_ERR_ARG = 1,         /* NULL / negative / inconsistent argument; nothing enqueued */
+  PVF_ERR_CONFIG = 2,      /* configuration not supported by this build */
+  PVF_ERR_CAPACITY = 3,    /* n_events > max_events or n_tracks > max_tracks; nothing enqueued */
+  PVF_ERR_CUDA = 4,        /* a CUDA runtime call failed (see pvf_last_cuda_error) */
+  PVF_ERR_UNSUPPORTED = 5  /* valid request this build cannot serve (e.g. stage timing disabled) */
+} pvf_status;
+
+/* Arithmetic of the UNet convolutions (the FC stage and the peak finder are always FP32). */
+typedef enum {
+  PVF_PREC_FP32 = 0, /* FP32 FMA direct convolution (CUDA cores); reference-accuracy path */
+  PVF_PREC_TF32 = 1, /* tcgen05 kind::tf32, operands RN-rounded to TF32, FP32 accumulate in TMEM */
+  PVF_PREC_BF16 = 2  /* tcgen05 kind::f16 with BF16 operands, FP32 accumulate in TMEM */
+} pvf_precision;
+
+/* Bits of pvf_peaks.event_flags (data-dependent anomalies never fail the call: PAPER.md:57). */
+#define PVF_FLAG_PEAK_OVERFLOW 1u /* more than max_peaks maxima; the first max_peaks are kept */
+#define PVF_FLAG_TRACK_DROPPED 2u /* >=1 track outside [z_min, z_min+400mm) or non-finite */
+#define PVF_FLAG_NONFINITE 4u     /* >=1 track with non-finite z_poca */
+
+/* Frozen at pvf_create (the paper's TensorSpec).  Fields marked (fixed) must hold
+ * the stated value in this build, anything else returns PVF_ERR_CONFIG. */
+typedef struct {
+  int32_t n_intervals;     /* (fixed) 40  -- PAPER.md:27 */
+  int32_t n_bins;          /* (fixed) 100 -- PAPER.md:27 */
+  float z_min_mm;          /* (fixed) -200 */
+  float bin_width_mm;      /* (fixed) 0.1 */
+  int32_t fc_in;           /* (fixed) 9   -- PAPER.md:27 */
+  int32_t fc_hidden;       /* (fixed) 25 */
+  int32_t hist_channels;   /* (fixed) 8   -- PAPER.md:29 */
+  int32_t unet_channels;   /* 64 (deployed), 32 or 16 (PAPER.md:84 roadmap) */
+  int32_t k_e1, k_e2, k_b, k_d2, k_d1; /* (fixed) 25, 15, 5, 15, 25 */
+  float leaky_slope;       /* (fixed) 0.01 */
+  float peak_threshold;    /* any finite value; config 0 uses 0.01 */
+  int32_t peak_halfwidth;  /* (fixed) 3 */
+  int32_t max_peaks;       /* (fixed) 32 */
+  int32_t precision;       /* pvf_precision */
+  int32_t split_mask;      /* TF32/BF16 only: bit L (0=e1,1=e2,2=b,3=d2,4=d1) = 3-pass hi/lo split
+                              precision for that conv layer */
+  int32_t max_events;      /* capacity the pool is sized for (>= 1) */
+  int64_t max_tracks;      /* capacity the pool is sized for (>= 1) */
+  int32_t enable_stage_timing; /* pre-creates CUDA events around the four stages; default 0 */
+  int32_t enable_host_io;  /* reserve pool space for pvf_run_host's device staging; default 0 */
+} pvf_config;
+
+/* Fill *cfg with BASELINE.json config 0 (64 channels, FP32) and the given capacities. */
+PVF_API void pvf_default_config(pvf_config* cfg, int32_t max_events, int64_t max_tracks);
+
+/* HOST pointers, PyTorch layouts, float32; copied and re-packed at create, not retained. */
+typedef struct {
+  const float* fc_w[6];   /* Linear weight [out][in] row-major: 25x9, 4 x 25x25, 800x25 */
+  const float* fc_b[6];   /* [out] */
+  const float* conv_w[6]; /* Conv1d weight [C_out][C_in][K]; order e1, e2, b, d2, d1, head */
+  const float* conv_b[6]; /* [C_out] */
+} pvf_weights;
+
+/* DEVICE pointers, caller-owned, read-only: Structure-of-Arrays track buffers. */
+typedef struct {
+  const float* feat[9];         /* each [n_tracks]: z_poca, x_poca, y_poca, e0..e5 (mm) */
+  const int32_t* event_offsets; /* [n_events+1] ascending, offsets[0]=0, offsets[n_events]=n_tracks */
+  int64_t n_tracks;             /* host scalar */
+} pvf_tracks;
+
+/* DEVICE pointers, caller-owned, written by the call. */
+typedef struct {
+  float* z_mm;          /* [n_events*max_peaks] centroid z; unused slots 0 */
+  float* prob;          /* [n_events*max_peaks] P at the peak bin; unused slots 0 */
+  int32_t* bin;         /* [n_events*max_peaks] global bin 0..3999 ascending; unused slots -1 */
+  int32_t* count;       /* [n_events] = min(found, max_peaks) */
+  uint32_t* event_flags;/* [n_events] PVF_FLAG_* bits; may be NULL */
+} pvf_peaks;
+
+/* Bytes of device memory the pool needs for this configuration (0 on invalid config). */
+PVF_API size_t pvf_workspace_bytes(const pvf_config* cfg);
+
+/* Create a context: validates cfg, packs the weights, makes ONE cudaMalloc for the pool
+ * (weights + sort scratch + histogram + staging).  The current CUDA device is used. */
+PVF_API pvf_status pvf_create(const pvf_weights* w, const pvf_config* cfg, pvf_handle* out);
+
+/* Same with a caller-supplied device pool (Allen-style fixed pool): ZERO device
+ * allocation.  dev_pool must be 256-byte aligned and hold >= pvf_workspace_bytes(cfg). */
+PVF_API pvf_status pvf_create_in_pool(const pvf_weights* w, const pvf_config* cfg, void* dev_pool,
+                              size_t pool_bytes, pvf_handle* out);
+
+/* The whole hot path for n_events events, enqueued on cuda_stream (a cudaStream_t; NULL is
+ * rejected so that nothing can leak onto the default stream).  No allocation, no
+ * host sync.  out_probs: device float [n_events, n_intervals*n_bins]; out_peaks: device views.
+ * Errors detectable on the host return non-OK and enqueue nothing; n_events == 0 is a no-op. */
+PVF_API pvf_status pvf_run(pvf_handle h, const pvf_tracks* tracks, int32_t n_events, float* out_probs,
+                   const pvf_peaks* out_peaks, void* cuda_stream);
+
+/* Same computation with HOST buffers: H2D of the nine feature arrays + offsets, pvf_run, D2H of
+ * probabilities (skipped if host_probs == NULL) and peaks, then one stream synchronise.  Needs
+ * enable_host_io.  feat/event_offsets/peaks fields are host pointers here (pinned memory makes the
+ * copies asynchronous but is not required). */
+PVF_API pvf_status pvf_run_host(pvf_handle h, const pvf_tracks* host_tracks, int32_t n_events,
+                        float* host_probs, const pvf_peaks* host_peaks, void* cuda_stream);
+
+/* Peak finder alone on caller-supplied device probabilities [n_events, 4000] (the bit-exactness
+ * test of BASELINE.json north_star runs through this entry point). */
+PVF_API pvf_status pvf_find_peaks(pvf_handle h, const float* probs, int32_t n_events,
+                          const pvf_peaks* out_peaks, void* cuda_stream);
+
+/* UNet + sigmoid alone on a caller-supplied device histogram [n_events,40,8,100] (canonical
+ * [B,C,L] layout of PAPER.md:31) -> out_probs [n_events,4000].  Test/diagnostic entry point. */
+PVF_API pvf_status pvf_run_unet(pvf_handle h, const float* hist, int32_t n_events, float* out_probs,
+                        void* cuda_stream);
+
+/* Copy the histogram of the last pvf_run ([n_events,40,8,100] float, canonical layout) into
+ * dev_out, enqueued on cuda_stream. */
+PVF_API pvf_status pvf_debug_copy_histogram(pvf_handle h, float* dev_out, int32_t n_events, void* cuda_stream);
+
+/* Mean stage times in ms over the pvf_run calls made since the previous call of this function (at
+ * most the 64 most recent): [0] interval sort, [1] FC + segmented sum, [2] UNet, [3] peaks; measured
+ * with CUDA events recorded on the run's stream.  Caller must have synchronised that stream.
+ * Needs enable_stage_timing; PVF_ERR_UNSUPPORTED if no run was recorded. */
+PVF_API pvf_status pvf_stage_times_ms(pvf_handle h, float out_ms[4]);
+
+/* Number of kernels pvf_run enqueues for n_events (host arithmetic; for launch accounting). */
+PVF_API int32_t pvf_launches_per_run(pvf_handle h, int32_t n_events);
+
+PVF_API pvf_status pvf_destroy(pvf_handle h);
+
+PVF_API const char* pvf_status_string(pvf_status s);
+PVF_API const char* pvf_last_cuda_error(pvf_handle h); /* "" if none */
+PVF_API const char* pvf_build_info(void);              /* arch + compiler string of this library */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PVF_H */

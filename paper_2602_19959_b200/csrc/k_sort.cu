@@ -1,0 +1,89 @@
+// a0 -- interval assignment + stable per-event counting sort of tracks by z-interval.
+//
+// PAPER.md:27 (40 intervals x 100 bins over 400 mm), BASELINE.json config 0 ("Each track adds to the
+// interval holding its z_poca"), north_star (b) "tracks are sorted by interval and summed in a fixed
+// order".  The float32 recipe (reading O2): u = (z + 200f) * 0.1f with separately rounded
+// add and multiply, i = floor(u); a track is dropped when z is non-finite or i is outside [0, 40).
+//
+// One warp per event.  Output: perm[event_offsets[e] + k] = original track index of the k-th kept
+// track of event e in (interval, original index) order; seg_off/seg_cnt[e*40 + i] = start (absolute
+// index into perm) and length of interval i's run.  Integer shared-memory atomics only count;
+// placement uses match/ballot ranks, so the order is the stable one and is reproducible.
+#include "pvf_internal.cuh"
+
+namespace pvf {
+
+constexpr int kSortWarps = 4;
+
+__global__ void __launch_bounds__(kSortWarps * 32)
+k_sort(const float* __restrict__ z_poca, const int32_t* __restrict__ event_offsets, int n_events,
+       int32_t* __restrict__ perm, int32_t* __restrict__ seg_off, int32_t* __restrict__ seg_cnt,
+       uint32_t* __restrict__ flags) {
+  __shared__ int s_cnt[kSortWarps][kIntervals];
+  __shared__ int s_base[kSortWarps][kIntervals];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int e = blockIdx.x * kSortWarps + warp;
+  if (e >= n_events) return;   // whole warp exits together; no block-level barrier below
+  int* cnt = s_cnt[warp];
+  int* base = s_base[warp];
+  for (int i = lane; i < kIntervals; i += 32) cnt[i] = 0;
+  __syncwarp();
+  const int lo = event_offsets[e], hi = event_offsets[e + 1];
+  uint32_t fl = 0;
+  for (int t = lo + lane; t < hi; t += 32) {
+    bool nf;
+    float zr;
+    int iv = interval_of(z_poca[t], zr, nf);
+    if (iv >= 0) atomicAdd(&cnt[iv], 1);
+    else fl |= PVF_FLAG_TRACK_DROPPED | (nf ? PVF_FLAG_NONFINITE : 0u);
+  }
+  fl = __reduce_or_sync(0xffffffffu, fl);
+  __syncwarp();
+  // exclusive scan of the 40 counts (lane handles i = lane and i = lane + 32)
+  int c0 = cnt[lane];
+  int c1 = (lane + 32 < kIntervals) ? cnt[lane + 32] : 0;
+  int s0 = c0;
+  for (int d = 1; d < 32; d <<= 1) {
+    int v = __shfl_up_sync(0xffffffffu, s0, d);
+    if (lane >= d) s0 += v;
+  }
+  int tot0 = __shfl_sync(0xffffffffu, s0, 31);
+  int s1 = c1;
+  for (int d = 1; d < 32; d <<= 1) {
+    int v = __shfl_up_sync(0xffffffffu, s1, d);
+    if (lane >= d) s1 += v;
+  }
+  base[lane] = s0 - c0;
+  seg_off[(size_t)e * kIntervals + lane] = lo + s0 - c0;
+  seg_cnt[(size_t)e * kIntervals + lane] = c0;
+  if (lane + 32 < kIntervals) {
+    base[lane + 32] = tot0 + s1 - c1;
+    seg_off[(size_t)e * kIntervals + lane + 32] = lo + tot0 + s1 - c1;
+    seg_cnt[(size_t)e * kIntervals + lane + 32] = c1;
+  }
+  if (lane == 0) flags[e] = fl;
+  __syncwarp();
+  // stable placement, 32 tracks at a time in original order
+  for (int c = lo; c < hi; c += 32) {
+    const int t = c + lane;
+    int key = -1;
+    if (t < hi) { bool nf; float zr; key = interval_of(z_poca[t], zr, nf); }
+    const unsigned grp = __match_any_sync(0xffffffffu, key);
+    const int rank = __popc(grp & ((1u << lane) - 1u));
+    int pos = -1;
+    if (key >= 0) pos = lo + base[key] + rank;
+    __syncwarp();
+    if (key >= 0 && rank == 0) base[key] += __popc(grp);
+    __syncwarp();
+    if (pos >= 0) perm[pos] = t;
+  }
+}
+
+void launch_sort(const float* z_poca, const int32_t* event_offsets, int n_events, int32_t* perm,
+                 int32_t* seg_off, int32_t* seg_cnt, uint32_t* flags, cudaStream_t s) {
+  if (n_events <= 0) return;
+  const int grid = (n_events + kSortWarps - 1) / kSortWarps;
+  k_sort<<<grid, kSortWarps * 32, 0, s>>>(z_poca, event_offsets, n_events, perm, seg_off, seg_cnt, flags);
+}
+
+}  // namespace pvf

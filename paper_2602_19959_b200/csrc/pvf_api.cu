@@ -1,0 +1,397 @@
+// C-ABI glue: configuration checks, the single workspace pool, weight packing, stage sequencing.
+// Declarations and the passages they follow: include/pvf.h.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "pvf_internal.cuh"
+
+using namespace pvf;
+
+#define PVF_STR2(x) #x
+#define PVF_STR(x) PVF_STR2(x)
+
+struct pvf_ctx {
+  pvf_config cfg;
+  bool owns_pool = false;
+  unsigned char* pool = nullptr;
+  size_t pool_bytes = 0;
+  int device = 0;
+  int sm_count = 148;
+  // sub-allocations of the pool
+  float* fc_params = nullptr;
+  float* conv_f32 = nullptr;      // PyTorch-layout conv params (FP32 path + head of every path)
+  UnetParamsF32 conv_ptrs{};
+  void* tc_packed = nullptr;
+  int32_t* perm = nullptr;
+  int32_t* seg_off = nullptr;
+  int32_t* seg_cnt = nullptr;
+  uint32_t* flags = nullptr;
+  float* hist = nullptr;
+  // host-io staging (enable_host_io)
+  float* st_feat = nullptr;
+  int32_t* st_off = nullptr;
+  float* st_probs = nullptr;
+  float* st_z = nullptr;
+  float* st_prob = nullptr;
+  int32_t* st_bin = nullptr;
+  int32_t* st_count = nullptr;
+  uint32_t* st_flags = nullptr;
+  static constexpr int kTimedRuns = 64;   // ring of per-run event sets (stage timing)
+  cudaEvent_t ev[kTimedRuns][5] = {};
+  int64_t timed_runs = 0;                 // runs recorded since the last pvf_stage_times_ms
+  int32_t last_n_events = 0;
+  std::string cuda_err;
+};
+
+namespace {
+
+size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+
+struct Layout {
+  size_t fc_params, conv_f32, tc_packed, perm, seg_off, seg_cnt, flags, hist;
+  size_t st_feat, st_off, st_probs, st_z, st_prob, st_bin, st_count, st_flags, total;
+  size_t conv_w_off[6], conv_b_off[6];  // float offsets inside conv_f32
+};
+
+void conv_shapes(int C, int shp[6][3]) {
+  const int s[6][3] = {{C, kHistCh, 25}, {C, C, 15}, {C, C, 5}, {C, 2 * C, 15}, {C, 2 * C, 25}, {1, C, 1}};
+  memcpy(shp, s, sizeof(s));
+}
+
+bool config_ok(const pvf_config* c) {
+  if (!c) return false;
+  if (c->n_intervals != kIntervals || c->n_bins != kBins) return false;
+  if (c->z_min_mm != -200.0f || c->bin_width_mm != 0.1f) return false;
+  if (c->fc_in != kFcIn || c->fc_hidden != kFcHidden || c->hist_channels != kHistCh) return false;
+  if (c->unet_channels != 64 && c->unet_channels != 32 && c->unet_channels != 16) return false;
+  if (c->k_e1 != 25 || c->k_e2 != 15 || c->k_b != 5 || c->k_d2 != 15 || c->k_d1 != 25) return false;
+  if (c->leaky_slope != kLeaky) return false;
+  if (!(c->peak_threshold == c->peak_threshold)) return false;
+  if (c->peak_halfwidth != kPeakHalf || c->max_peaks != kMaxPeaks) return false;
+  if (c->precision < PVF_PREC_FP32 || c->precision > PVF_PREC_BF16) return false;
+  if (c->split_mask < 0 || c->split_mask > 31) return false;
+  if (c->max_events < 1 || c->max_tracks < 1 || c->max_tracks > 0x7fffffffLL) return false;
+  return true;
+}
+
+Layout make_layout(const pvf_config* c) {
+  Layout L{};
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes); return r; };
+  L.fc_params = take(sizeof(float) * kFcTotal);
+  int shp[6][3];
+  conv_shapes(c->unet_channels, shp);
+  size_t f = 0;
+  for (int k = 0; k < 6; ++k) {
+    L.conv_w_off[k] = f; f += (size_t)shp[k][0] * shp[k][1] * shp[k][2]; f = (f + 63) / 64 * 64;
+    L.conv_b_off[k] = f; f += shp[k][0]; f = (f + 63) / 64 * 64;
+  }
+  L.conv_f32 = take(sizeof(float) * f);
+  L.tc_packed = take(c->precision == PVF_PREC_FP32 ? 0 : unet_tc_packed_bytes(c->unet_channels, c->precision, c->split_mask));
+  const size_t E = (size_t)c->max_events, T = (size_t)c->max_tracks;
+  L.perm = take(sizeof(int32_t) * T);
+  L.seg_off = take(sizeof(int32_t) * E * kIntervals);
+  L.seg_cnt = take(sizeof(int32_t) * E * kIntervals);
+  L.flags = take(sizeof(uint32_t) * E);
+  L.hist = take(sizeof(float) * E * kIntervals * kFcOut);
+  if (c->enable_host_io) {
+    L.st_feat = take(sizeof(float) * 9 * T);
+    L.st_off = take(sizeof(int32_t) * (E + 1));
+    L.st_probs = take(sizeof(float) * E * kGlobalBins);
+    L.st_z = take(sizeof(float) * E * kMaxPeaks);
+    L.st_prob = take(sizeof(float) * E * kMaxPeaks);
+    L.st_bin = take(sizeof(int32_t) * E * kMaxPeaks);
+    L.st_count = take(sizeof(int32_t) * E);
+    L.st_flags = take(sizeof(uint32_t) * E);
+  }
+  L.total = o;
+  return L;
+}
+
+pvf_status fail_cuda(pvf_ctx* h, cudaError_t e, const char* where) {
+  if (h) h->cuda_err = std::string(where) + ": " + cudaGetErrorString(e);
+  return PVF_ERR_CUDA;
+}
+
+#define PVF_CUDA(h, call)                                             \
+  do {                                                                \
+    cudaError_t e__ = (call);                                         \
+    if (e__ != cudaSuccess) return fail_cuda((h), e__, #call);        \
+  } while (0)
+
+bool peaks_ok(const pvf_peaks* p) { return p && p->z_mm && p->prob && p->bin && p->count; }
+
+pvf_status create_impl(const pvf_weights* w, const pvf_config* cfg, void* dev_pool, size_t pool_bytes,
+                       pvf_handle* out) {
+  if (!out) return PVF_ERR_ARG;
+  *out = nullptr;
+  if (!w || !cfg) return PVF_ERR_ARG;
+  if (!config_ok(cfg)) return PVF_ERR_CONFIG;
+  for (int k = 0; k < 6; ++k)
+    if (!w->fc_w[k] || !w->fc_b[k] || !w->conv_w[k] || !w->conv_b[k]) return PVF_ERR_ARG;
+  const Layout L = make_layout(cfg);
+  pvf_ctx* h = new (std::nothrow) pvf_ctx();
+  if (!h) return PVF_ERR_ARG;
+  h->cfg = *cfg;
+  cudaError_t e = cudaGetDevice(&h->device);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, h->device);
+  if (e != cudaSuccess) { delete h; return PVF_ERR_CUDA; }
+  if (dev_pool) {
+    if (pool_bytes < L.total || (reinterpret_cast<uintptr_t>(dev_pool) & 255u)) { delete h; return PVF_ERR_CAPACITY; }
+    h->pool = static_cast<unsigned char*>(dev_pool);
+  } else {
+    void* p = nullptr;
+    e = cudaMalloc(&p, L.total);
+    if (e != cudaSuccess) { delete h; return PVF_ERR_CUDA; }
+    h->pool = static_cast<unsigned char*>(p);
+    h->owns_pool = true;
+  }
+  h->pool_bytes = L.total;
+  unsigned char* B = h->pool;
+  h->fc_params = reinterpret_cast<float*>(B + L.fc_params);
+  h->conv_f32 = reinterpret_cast<float*>(B + L.conv_f32);
+  h->tc_packed = B + L.tc_packed;
+  h->perm = reinterpret_cast<int32_t*>(B + L.perm);
+  h->seg_off = reinterpret_cast<int32_t*>(B + L.seg_off);
+  h->seg_cnt = reinterpret_cast<int32_t*>(B + L.seg_cnt);
+  h->flags = reinterpret_cast<uint32_t*>(B + L.flags);
+  h->hist = reinterpret_cast<float*>(B + L.hist);
+  if (cfg->enable_host_io) {
+    h->st_feat = reinterpret_cast<float*>(B + L.st_feat);
+    h->st_off = reinterpret_cast<int32_t*>(B + L.st_off);
+    h->st_probs = reinterpret_cast<float*>(B + L.st_probs);
+    h->st_z = reinterpret_cast<float*>(B + L.st_z);
+    h->st_prob = reinterpret_cast<float*>(B + L.st_prob);
+    h->st_bin = reinterpret_cast<int32_t*>(B + L.st_bin);
+    h->st_count = reinterpret_cast<int32_t*>(B + L.st_count);
+    h->st_flags = reinterpret_cast<uint32_t*>(B + L.st_flags);
+  }
+  // ---- pack + upload weights (synchronous copies: create is not on the hot path)
+  {
+    std::vector<float> fc(kFcTotal);
+    memcpy(&fc[kFcW0], w->fc_w[0], sizeof(float) * 225);
+    memcpy(&fc[kFcB0], w->fc_b[0], sizeof(float) * 25);
+    for (int k = 0; k < 4; ++k) {
+      memcpy(&fc[kFcHid + kFcHidStride * k], w->fc_w[k + 1], sizeof(float) * 625);
+      memcpy(&fc[kFcHid + kFcHidStride * k + 625], w->fc_b[k + 1], sizeof(float) * 25);
+    }
+    memcpy(&fc[kFcW5], w->fc_w[5], sizeof(float) * 20000);
+    memcpy(&fc[kFcB5], w->fc_b[5], sizeof(float) * 800);
+    e = cudaMemcpy(h->fc_params, fc.data(), sizeof(float) * kFcTotal, cudaMemcpyHostToDevice);
+  }
+  int shp[6][3];
+  conv_shapes(cfg->unet_channels, shp);
+  for (int k = 0; k < 6 && e == cudaSuccess; ++k) {
+    e = cudaMemcpy(h->conv_f32 + L.conv_w_off[k], w->conv_w[k],
+                   sizeof(float) * shp[k][0] * shp[k][1] * shp[k][2], cudaMemcpyHostToDevice);
+    if (e == cudaSuccess)
+      e = cudaMemcpy(h->conv_f32 + L.conv_b_off[k], w->conv_b[k], sizeof(float) * shp[k][0], cudaMemcpyHostToDevice);
+    h->conv_ptrs.w[k] = h->conv_f32 + L.conv_w_off[k];
+    h->conv_ptrs.b[k] = h->conv_f32 + L.conv_b_off[k];
+  }
+  if (e == cudaSuccess) {
+    if (cfg->precision == PVF_PREC_FP32) {
+      e = unet_simt_setup(cfg->unet_channels);
+    } else {
+      const size_t nb = unet_tc_packed_bytes(cfg->unet_channels, cfg->precision, cfg->split_mask);
+      std::vector<unsigned char> img(nb);
+      unet_tc_pack(w, cfg->unet_channels, cfg->precision, cfg->split_mask, img.data());
+      e = cudaMemcpy(h->tc_packed, img.data(), nb, cudaMemcpyHostToDevice);
+      if (e == cudaSuccess) e = unet_tc_setup(cfg->unet_channels, cfg->precision, cfg->split_mask);
+    }
+  }
+  if (e == cudaSuccess && cfg->enable_stage_timing)
+    for (int r = 0; r < pvf_ctx::kTimedRuns; ++r)
+      for (int k = 0; k < 5 && e == cudaSuccess; ++k) e = cudaEventCreate(&h->ev[r][k]);
+  if (e != cudaSuccess) {
+    pvf_destroy(h);
+    return e == cudaErrorInvalidValue && cfg->precision != PVF_PREC_FP32 ? PVF_ERR_CONFIG : PVF_ERR_CUDA;
+  }
+  *out = h;
+  return PVF_OK;
+}
+
+void enqueue_unet(pvf_ctx* h, const float* hist, int n_events, float* out_probs, cudaStream_t s) {
+  const int n_int = n_events * kIntervals;
+  if (h->cfg.precision == PVF_PREC_FP32)
+    launch_unet_simt(hist, n_int, h->conv_ptrs, h->cfg.unet_channels, out_probs, s);
+  else
+    launch_unet_tc(hist, n_int, h->tc_packed, h->cfg.unet_channels, h->cfg.precision, h->cfg.split_mask,
+                   out_probs, h->sm_count, s);
+}
+
+}  // namespace
+
+extern "C" {
+
+void pvf_default_config(pvf_config* c, int32_t max_events, int64_t max_tracks) {
+  if (!c) return;
+  memset(c, 0, sizeof(*c));
+  c->n_intervals = kIntervals; c->n_bins = kBins; c->z_min_mm = -200.0f; c->bin_width_mm = 0.1f;
+  c->fc_in = kFcIn; c->fc_hidden = kFcHidden; c->hist_channels = kHistCh; c->unet_channels = 64;
+  c->k_e1 = 25; c->k_e2 = 15; c->k_b = 5; c->k_d2 = 15; c->k_d1 = 25;
+  c->leaky_slope = kLeaky; c->peak_threshold = 0.01f; c->peak_halfwidth = kPeakHalf; c->max_peaks = kMaxPeaks;
+  c->precision = PVF_PREC_FP32; c->split_mask = 0;
+  c->max_events = max_events; c->max_tracks = max_tracks;
+  c->enable_stage_timing = 0; c->enable_host_io = 0;
+}
+
+size_t pvf_workspace_bytes(const pvf_config* cfg) {
+  if (!config_ok(cfg)) return 0;
+  return make_layout(cfg).total;
+}
+
+pvf_status pvf_create(const pvf_weights* w, const pvf_config* cfg, pvf_handle* out) {
+  return create_impl(w, cfg, nullptr, 0, out);
+}
+
+pvf_status pvf_create_in_pool(const pvf_weights* w, const pvf_config* cfg, void* dev_pool, size_t pool_bytes,
+                              pvf_handle* out) {
+  if (!dev_pool) return PVF_ERR_ARG;
+  return create_impl(w, cfg, dev_pool, pool_bytes, out);
+}
+
+pvf_status pvf_run(pvf_handle h, const pvf_tracks* t, int32_t n_events, float* out_probs,
+                   const pvf_peaks* pk, void* cuda_stream) {
+  if (!h || !t || !cuda_stream || n_events < 0) return PVF_ERR_ARG;
+  if (n_events == 0) return PVF_OK;
+  if (!out_probs || !peaks_ok(pk) || !t->event_offsets || t->n_tracks < 0) return PVF_ERR_ARG;
+  for (int k = 0; k < 9; ++k)
+    if (!t->feat[k] && t->n_tracks > 0) return PVF_ERR_ARG;
+  if (n_events > h->cfg.max_events || t->n_tracks > h->cfg.max_tracks) return PVF_ERR_CAPACITY;
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  const bool timing = h->cfg.enable_stage_timing != 0;
+  cudaEvent_t* ev = h->ev[h->timed_runs % pvf_ctx::kTimedRuns];
+  if (timing) cudaEventRecord(ev[0], s);
+  launch_sort(t->feat[0], t->event_offsets, n_events, h->perm, h->seg_off, h->seg_cnt, h->flags, s);
+  if (timing) cudaEventRecord(ev[1], s);
+  launch_fc_hist(t->feat, t->event_offsets, h->perm, h->seg_off, h->seg_cnt, h->fc_params, n_events, h->hist, s);
+  if (timing) cudaEventRecord(ev[2], s);
+  enqueue_unet(h, h->hist, n_events, out_probs, s);
+  if (timing) cudaEventRecord(ev[3], s);
+  launch_peaks(out_probs, n_events, h->cfg.peak_threshold, h->flags, pk->z_mm, pk->prob, pk->bin, pk->count,
+               pk->event_flags, s);
+  if (timing) { cudaEventRecord(ev[4], s); ++h->timed_runs; }
+  h->last_n_events = n_events;
+  cudaError_t e = cudaPeekAtLastError();
+  if (e != cudaSuccess) return fail_cuda(h, e, "pvf_run launch");
+  return PVF_OK;
+}
+
+pvf_status pvf_run_host(pvf_handle h, const pvf_tracks* t, int32_t n_events, float* host_probs,
+                        const pvf_peaks* pk, void* cuda_stream) {
+  if (!h || !t || !cuda_stream || n_events < 0) return PVF_ERR_ARG;
+  if (!h->cfg.enable_host_io) return PVF_ERR_UNSUPPORTED;
+  if (n_events == 0) return PVF_OK;
+  if (!peaks_ok(pk) || !t->event_offsets || t->n_tracks < 0) return PVF_ERR_ARG;
+  if (n_events > h->cfg.max_events || t->n_tracks > h->cfg.max_tracks) return PVF_ERR_CAPACITY;
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  const size_t T = (size_t)t->n_tracks, cap = (size_t)h->cfg.max_tracks, E = (size_t)n_events;
+  pvf_tracks d{};
+  for (int k = 0; k < 9; ++k) {
+    if (T) PVF_CUDA(h, cudaMemcpyAsync(h->st_feat + cap * k, t->feat[k], sizeof(float) * T, cudaMemcpyHostToDevice, s));
+    d.feat[k] = h->st_feat + cap * k;
+  }
+  PVF_CUDA(h, cudaMemcpyAsync(h->st_off, t->event_offsets, sizeof(int32_t) * (E + 1), cudaMemcpyHostToDevice, s));
+  d.event_offsets = h->st_off;
+  d.n_tracks = t->n_tracks;
+  pvf_peaks dp{h->st_z, h->st_prob, h->st_bin, h->st_count, h->st_flags};
+  pvf_status st = pvf_run(h, &d, n_events, h->st_probs, &dp, cuda_stream);
+  if (st != PVF_OK) return st;
+  if (host_probs) PVF_CUDA(h, cudaMemcpyAsync(host_probs, h->st_probs, sizeof(float) * E * kGlobalBins, cudaMemcpyDeviceToHost, s));
+  PVF_CUDA(h, cudaMemcpyAsync(pk->z_mm, h->st_z, sizeof(float) * E * kMaxPeaks, cudaMemcpyDeviceToHost, s));
+  PVF_CUDA(h, cudaMemcpyAsync(pk->prob, h->st_prob, sizeof(float) * E * kMaxPeaks, cudaMemcpyDeviceToHost, s));
+  PVF_CUDA(h, cudaMemcpyAsync(pk->bin, h->st_bin, sizeof(int32_t) * E * kMaxPeaks, cudaMemcpyDeviceToHost, s));
+  PVF_CUDA(h, cudaMemcpyAsync(pk->count, h->st_count, sizeof(int32_t) * E, cudaMemcpyDeviceToHost, s));
+  if (pk->event_flags)
+    PVF_CUDA(h, cudaMemcpyAsync(pk->event_flags, h->st_flags, sizeof(uint32_t) * E, cudaMemcpyDeviceToHost, s));
+  PVF_CUDA(h, cudaStreamSynchronize(s));
+  return PVF_OK;
+}
+
+pvf_status pvf_find_peaks(pvf_handle h, const float* probs, int32_t n_events, const pvf_peaks* pk, void* cuda_stream) {
+  if (!h || !cuda_stream || n_events < 0) return PVF_ERR_ARG;
+  if (n_events == 0) return PVF_OK;
+  if (!probs || !peaks_ok(pk)) return PVF_ERR_ARG;
+  launch_peaks(probs, n_events, h->cfg.peak_threshold, nullptr, pk->z_mm, pk->prob, pk->bin, pk->count,
+               pk->event_flags, static_cast<cudaStream_t>(cuda_stream));
+  cudaError_t e = cudaPeekAtLastError();
+  if (e != cudaSuccess) return fail_cuda(h, e, "pvf_find_peaks launch");
+  return PVF_OK;
+}
+
+pvf_status pvf_run_unet(pvf_handle h, const float* hist, int32_t n_events, float* out_probs, void* cuda_stream) {
+  if (!h || !cuda_stream || n_events < 0) return PVF_ERR_ARG;
+  if (n_events == 0) return PVF_OK;
+  if (!hist || !out_probs) return PVF_ERR_ARG;
+  if (n_events > h->cfg.max_events) return PVF_ERR_CAPACITY;
+  enqueue_unet(h, hist, n_events, out_probs, static_cast<cudaStream_t>(cuda_stream));
+  cudaError_t e = cudaPeekAtLastError();
+  if (e != cudaSuccess) return fail_cuda(h, e, "pvf_run_unet launch");
+  return PVF_OK;
+}
+
+pvf_status pvf_debug_copy_histogram(pvf_handle h, float* dev_out, int32_t n_events, void* cuda_stream) {
+  if (!h || !dev_out || !cuda_stream || n_events < 0) return PVF_ERR_ARG;
+  if (n_events > h->last_n_events) return PVF_ERR_ARG;
+  if (n_events == 0) return PVF_OK;
+  PVF_CUDA(h, cudaMemcpyAsync(dev_out, h->hist, sizeof(float) * (size_t)n_events * kIntervals * kFcOut,
+                              cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(cuda_stream)));
+  return PVF_OK;
+}
+
+pvf_status pvf_stage_times_ms(pvf_handle h, float out_ms[4]) {
+  if (!h || !out_ms) return PVF_ERR_ARG;
+  if (!h->cfg.enable_stage_timing || h->timed_runs == 0) return PVF_ERR_UNSUPPORTED;
+  const int64_t n = h->timed_runs < pvf_ctx::kTimedRuns ? h->timed_runs : pvf_ctx::kTimedRuns;
+  double acc[4] = {0, 0, 0, 0};
+  for (int64_t r = h->timed_runs - n; r < h->timed_runs; ++r) {
+    cudaEvent_t* ev = h->ev[r % pvf_ctx::kTimedRuns];
+    for (int k = 0; k < 4; ++k) {
+      float ms = 0.f;
+      PVF_CUDA(h, cudaEventElapsedTime(&ms, ev[k], ev[k + 1]));
+      acc[k] += ms;
+    }
+  }
+  for (int k = 0; k < 4; ++k) out_ms[k] = (float)(acc[k] / (double)n);
+  h->timed_runs = 0;
+  return PVF_OK;
+}
+
+int32_t pvf_launches_per_run(pvf_handle h, int32_t n_events) {
+  if (!h || n_events <= 0) return 0;
+  return 1 /*sort*/ + fc_hist_launches(n_events) + 1 /*unet*/ + 1 /*peaks*/;
+}
+
+pvf_status pvf_destroy(pvf_handle h) {
+  if (!h) return PVF_ERR_ARG;
+  for (int r = 0; r < pvf_ctx::kTimedRuns; ++r)
+    for (int k = 0; k < 5; ++k)
+      if (h->ev[r][k]) cudaEventDestroy(h->ev[r][k]);
+  if (h->owns_pool && h->pool) cudaFree(h->pool);
+  delete h;
+  return PVF_OK;
+}
+
+const char* pvf_status_string(pvf_status s) {
+  switch (s) {
+    case PVF_OK: return "PVF_OK";
+    case PVF_ERR_ARG: return "PVF_ERR_ARG";
+    case PVF_ERR_CONFIG: return "PVF_ERR_CONFIG";
+    case PVF_ERR_CAPACITY: return "PVF_ERR_CAPACITY";
+    case PVF_ERR_CUDA: return "PVF_ERR_CUDA";
+    case PVF_ERR_UNSUPPORTED: return "PVF_ERR_UNSUPPORTED";
+  }
+  return "PVF_ERR_?";
+}
+
+const char* pvf_last_cuda_error(pvf_handle h) { return h ? h->cuda_err.c_str() : ""; }
+
+const char* pvf_build_info(void) {
+  return "pvfinder-b200 sm_100a nvcc " __VERSION__ " cuda " PVF_STR(CUDART_VERSION);
+}
+
+}  // extern "C"

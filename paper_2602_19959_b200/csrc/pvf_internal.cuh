@@ -1,0 +1,75 @@
+// Internal declarations shared by the kernels and the C-ABI glue (pvf_api.cu).
+// The geometry is frozen (include/pvf.h marks the fields "fixed"), BASELINE.json config 0.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/pvf.h"
+
+namespace pvf {
+
+constexpr int kIntervals = 40;
+constexpr int kBins = 100;
+constexpr int kGlobalBins = kIntervals * kBins;  // 4000
+constexpr int kFcIn = 9;
+constexpr int kFcHidden = 25;
+constexpr int kHistCh = 8;
+constexpr int kFcOut = kHistCh * kBins;          // 800
+constexpr int kMaxPeaks = 32;
+constexpr int kPeakHalf = 3;
+constexpr float kLeaky = 0.01f;
+
+// Packed FC parameters in device memory (floats), see pack_fc() in pvf_api.cu:
+//   [0,225)      W0 [25][9]        [225,250)    b0
+//   250 + 650*k  W_{k+1} [25][25], then b_{k+1} [25]      (k = 0..3)
+//   2850         W5 [800][25]      22850        b5 [800]
+constexpr int kFcW0 = 0, kFcB0 = 225, kFcHid = 250, kFcHidStride = 650;
+constexpr int kFcW5 = 2850, kFcB5 = 22850, kFcTotal = 23650;
+
+struct ConvShape { int cin, cout, k, len; };
+
+#ifdef __CUDACC__
+// DESIGN.md reading O2 (float32, separately rounded add and multiply, no FMA):
+//   u = (z + 200f) * 0.1f;  i = floor(u);  zrel = u - i  (exact);  dropped if non-finite or i outside [0,40).
+__device__ __forceinline__ int interval_of(float z, float& zrel, bool& nonfinite) {
+  nonfinite = !isfinite(z);
+  zrel = 0.0f;
+  if (nonfinite) return -1;
+  const float u = __fmul_rn(__fadd_rn(z, 200.0f), 0.1f);
+  const float fl = floorf(u);
+  if (!(fl >= 0.0f && fl < (float)kIntervals)) return -1;
+  zrel = __fsub_rn(u, fl);
+  return (int)fl;
+}
+#endif
+
+// a0: interval assignment + stable per-event counting sort (k_sort.cu)
+void launch_sort(const float* z_poca, const int32_t* event_offsets, int n_events, int32_t* perm,
+                 int32_t* seg_off, int32_t* seg_cnt, uint32_t* flags, cudaStream_t s);
+
+// a1+a2: per-track FC and fixed-order segmented sum into H [n_events,40,8,100] (k_fc.cu)
+void launch_fc_hist(const float* const feat[9], const int32_t* event_offsets, const int32_t* perm,
+                    const int32_t* seg_off, const int32_t* seg_cnt, const float* fc_params,
+                    int n_events, float* hist, cudaStream_t s);
+int fc_hist_launches(int n_events);
+
+// a3, FP32 CUDA-core path (k_unet_simt.cu).  conv params: PyTorch layout, floats.
+struct UnetParamsF32 { const float* w[6]; const float* b[6]; };
+cudaError_t unet_simt_setup(int channels);
+void launch_unet_simt(const float* hist, int n_intervals_total, const UnetParamsF32& p, int channels,
+                      float* probs, cudaStream_t s);
+
+// a3, tcgen05/TMEM path (k_unet_tc.cu)
+struct UnetTcPlan;   // opaque; owns nothing on the device (pool pointers only)
+size_t unet_tc_packed_bytes(int channels, int precision, int split_mask);
+// packs PyTorch-layout host weights into the shared-memory image order the kernel streams
+void unet_tc_pack(const pvf_weights* w, int channels, int precision, int split_mask, void* host_dst);
+cudaError_t unet_tc_setup(int channels, int precision, int split_mask);
+void launch_unet_tc(const float* hist, int n_intervals_total, const void* packed_dev, int channels,
+                    int precision, int split_mask, float* probs, int sm_count, cudaStream_t s);
+
+// a4: peak finder (k_peaks.cu)
+void launch_peaks(const float* probs, int n_events, float threshold, const uint32_t* flags_in,
+                  float* z_mm, float* prob, int32_t* bin, int32_t* count, uint32_t* flags_out,
+                  cudaStream_t s);
+
+}  // namespace pvf

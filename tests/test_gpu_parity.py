@@ -1,0 +1,320 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element on the
+same seeded inputs.  Tolerances:
+  peak finder on identical probabilities ........ bit-exact            (north_star)
+  interval sort / counts / flags ................ bit-exact            (integer work)
+  histogram H (FP32 FC vs FP64 oracle) .......... 2e-5 relative to max(|H|, 1)
+  probabilities, FP32 path ...................... 2e-5 absolute
+  probabilities, TF32 path ...................... 1e-3 absolute        (north_star)
+  probabilities, BF16 path ...................... 2e-2 absolute        (north_star / config 4)
+  peaks end to end .............................. within 1 bin on >= 99.9 % of oracle peaks (peaky),
+                                                  100 % of tau-stable peaks (any weights)
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle import pvf_oracle as O
+from pvf_inputs import make_events, make_weights, select_events
+import paper_2602_19959_b200 as pkg
+from paper_2602_19959_b200 import PVFinder
+
+TOL = {"fp32": 2e-5, "tf32": 1e-3, "bf16": 2e-2}
+SPLIT = {"fp32": 0, "tf32": 1, "bf16": 0}
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    import __graft_entry__ as entry
+    entry.build()
+    assert torch.cuda.is_available()
+    torch.cuda.set_device(0)
+
+
+def _dev(ev):
+    return torch.from_numpy(ev.feat).cuda(), torch.from_numpy(ev.event_offsets).cuda()
+
+
+def _run(pvf, ev, n=None):
+    n = ev.n_events if n is None else n
+    feat, off = _dev(ev)
+    probs = torch.full((max(n, 1), 4000), -1.0, device="cuda")
+    pk = pvf.alloc_peaks(max(n, 1))
+    s = torch.cuda.Stream()
+    pvf.run(feat, off, n, probs, pk, stream=s)
+    s.synchronize()
+    return probs, pk
+
+
+def _make(w, ev, prec="fp32", **kw):
+    return PVFinder(w, max_events=max(ev.n_events, 1), max_tracks=max(ev.n_tracks, 1), precision=prec,
+                    split_mask=kw.pop("split_mask", SPLIT[prec]), **kw)
+
+
+def _np(pk):
+    return {k: v.cpu().numpy() for k, v in pk.items()}
+
+
+# ------------------------------------------------------------------ a4: peak finder, bit exact
+def test_peaks_bit_exact_on_identical_probabilities():
+    rng = np.random.default_rng(11)
+    E = 37
+    P = rng.random((E, 4000), dtype=np.float32) ** 8            # many small values, few large
+    P[0] = 0.0                                                   # no peaks
+    P[1] = 0.5                                                   # one plateau over everything: peak at 0
+    P[2] = 0.0; P[2, 100:104] = 0.5; P[2, 0] = 0.2; P[2, 3999] = 0.3; P[2, 2000] = np.float32(0.01)
+    P[3] = 0.0; P[3, 50:50 + 33 * 10:10] = 0.9                   # 33 spikes -> overflow
+    P[4] = 0.0; P[4, 500] = np.nan; P[4, 700] = 0.4
+    P[5] = np.linspace(0, 1, 4000, dtype=np.float32)             # monotone: single peak at the end
+    P[6] = 0.0; P[6, 99], P[6, 100] = 0.4, 0.5                   # across an interval boundary
+    ref = O.find_peaks(P)
+    w = make_weights("rand", 1)
+    pvf = PVFinder(w, max_events=E, max_tracks=1)
+    pk = pvf.alloc_peaks(E)
+    s = torch.cuda.Stream()
+    pvf.find_peaks(torch.from_numpy(P).cuda(), E, pk, stream=s)
+    s.synchronize()
+    got = _np(pk)
+    assert np.array_equal(got["count"], ref["count"])
+    assert np.array_equal(got["bin"], ref["bin"])
+    assert np.array_equal(got["prob"].view(np.uint32), ref["prob"].view(np.uint32))
+    assert np.array_equal(got["z"].view(np.uint32), ref["z"].view(np.uint32))
+    assert np.array_equal(got["flags"].astype(np.uint32) & 1, ref["flags"] & 1)
+    assert got["count"][3] == 32 and got["flags"][3] & 1
+
+
+# ------------------------------------------------------------------ a0 + a1 + a2: histogram
+@pytest.mark.parametrize("kind", ["rand", "peaky"])
+def test_histogram_parity_and_determinism(kind):
+    ev = make_events("run3", 48, 1001)
+    w = make_weights(kind, 1)
+    ref = O.run(ev.feat, ev.event_offsets, w, want_hist=True)
+    pvf = _make(w, ev)
+    probs, pk = _run(pvf, ev)
+    H = torch.empty(ev.n_events, 40, 8, 100, device="cuda")
+    s = torch.cuda.Stream()
+    pvf.debug_copy_histogram(H, ev.n_events, stream=s)
+    s.synchronize()
+    Hn = H.cpu().numpy().astype(np.float64)
+    err = np.abs(Hn - ref["hist"]) / np.maximum(np.abs(ref["hist"]), 1.0)
+    assert err.max() <= 2e-5
+    assert np.array_equal(Hn == 0, ref["hist"] == 0)            # empty intervals are exactly zero
+    # determinism: a second run is bit-identical
+    probs2, pk2 = _run(pvf, ev)
+    H2 = torch.empty_like(H)
+    pvf.debug_copy_histogram(H2, ev.n_events, stream=s)
+    s.synchronize()
+    assert torch.equal(H, H2) and torch.equal(probs, probs2)
+    assert all(torch.equal(pk[k], pk2[k]) for k in pk)
+    # permutation of tracks inside events changes H only by FP32 summation order
+    rng = np.random.default_rng(0)
+    perm = np.concatenate([ev.event_offsets[e] + rng.permutation(ev.event_offsets[e + 1] - ev.event_offsets[e])
+                           for e in range(ev.n_events)])
+    evp = type(ev)(np.ascontiguousarray(ev.feat[:, perm]), ev.event_offsets, ev.pv_z)
+    _run(pvf, evp)
+    pvf.debug_copy_histogram(H2, ev.n_events, stream=s)
+    s.synchronize()
+    assert torch.allclose(H, H2, rtol=1e-5, atol=1e-5)
+
+
+def test_edge_events_empty_dropped_nonfinite_and_long():
+    w = make_weights("rand", 3)
+    base = make_events("pileup", 3, 9)
+    long_n = 700                                                 # > 3 tiles of the FC kernel
+    rng = np.random.default_rng(2)
+    feats, offs = [], [0]
+
+    def add(f):
+        feats.append(f)
+        offs.append(offs[-1] + f.shape[1])
+
+    add(np.zeros((9, 0), np.float32))                            # event 0: empty
+    f = base.feat[:, base.event_offsets[0]:base.event_offsets[1]].copy()
+    f[0, 0], f[0, 1], f[0, 2], f[0, 3] = 250.0, -200.5, np.nan, np.inf
+    add(f)                                                       # event 1: dropped + non-finite
+    fl = np.tile(base.feat[:, :70], (1, 10))[:, :long_n].copy()
+    fl[0] = rng.uniform(-3.0, 3.0, long_n).astype(np.float32)    # 700 tracks in one or two intervals
+    add(fl)
+    add(np.zeros((9, 0), np.float32))                            # event 3: empty again
+    one = base.feat[:, 5:6].copy()
+    one[0, 0] = np.float32(199.99)
+    add(one)                                                     # event 4: single track in the last interval
+    ev = type(base)(np.ascontiguousarray(np.concatenate(feats, axis=1)), np.array(offs, np.int32), [None] * 5)
+    ref = O.run(ev.feat, ev.event_offsets, w, want_hist=True)
+    pvf = _make(w, ev)
+    probs, pk = _run(pvf, ev)
+    H = torch.empty(5, 40, 8, 100, device="cuda")
+    s = torch.cuda.Stream()
+    pvf.debug_copy_histogram(H, 5, stream=s)
+    s.synchronize()
+    Hn = H.cpu().numpy().astype(np.float64)
+    assert (np.abs(Hn - ref["hist"]) / np.maximum(np.abs(ref["hist"]), 1.0)).max() <= 2e-5
+    assert np.all(Hn[0] == 0) and np.all(Hn[3] == 0)
+    got = _np(pk)
+    assert np.array_equal(got["flags"].astype(np.uint32), ref["flags"])
+    assert got["flags"][1] & pkg.FLAG_TRACK_DROPPED and got["flags"][1] & pkg.FLAG_NONFINITE
+    assert np.max(np.abs(probs.cpu().numpy().astype(np.float64) - ref["probs"])) <= TOL["fp32"]
+    # empty events give the bias-only vector UNet(0) in every interval
+    P = probs.cpu().numpy().reshape(5, 40, 100)
+    assert np.all(P[0] == P[0, 0]) and np.array_equal(P[0], P[3])
+
+
+# ------------------------------------------------------------------ a3 + whole path
+def _available(prec, w, ev):
+    try:
+        return _make(w, ev, prec)
+    except pkg.PVFError as exc:
+        if exc.status == pkg.PVF_ERR_CONFIG:
+            pytest.skip(f"precision {prec} not built yet")
+        raise
+
+
+@pytest.mark.parametrize("prec", ["fp32", "tf32", "bf16"])
+@pytest.mark.parametrize("kind", ["rand", "peaky"])
+def test_whole_path_parity(prec, kind):
+    ev = make_events("run3", 48, 1001)
+    w = make_weights(kind, 1)
+    ref = O.run(ev.feat, ev.event_offsets, w)
+    pvf = _available(prec, w, ev)
+    probs, pk = _run(pvf, ev)
+    Pg = probs.cpu().numpy()
+    err = np.abs(Pg.astype(np.float64) - ref["probs"]).max(axis=1)
+    assert err.max() <= TOL[prec], f"max|dP| per event: {err.max():.3e}"
+    got = _np(pk)
+    tau = max(float(err.max()), 1e-7)
+    m_all = n_all = m_st = n_st = 0
+    for e in range(ev.n_events):
+        cand = np.nonzero((ref["probs"][e] > 0.01) & (ref["probs"][e] > np.r_[-np.inf, ref["probs"][e][:-1]])
+                          & (ref["probs"][e] >= np.r_[ref["probs"][e][1:], -np.inf]))[0]
+        gcand = np.nonzero((Pg[e] > 0.01) & (Pg[e] > np.r_[-np.inf, Pg[e][:-1]]) & (Pg[e] >= np.r_[Pg[e][1:], -np.inf]))[0]
+        st = O.tau_stable_peaks(ref["probs"][e], cand, tau)
+        m, n, _ = O.match_peaks(st, gcand)
+        m_st += m; n_st += n
+        if ref["peaks"]["count"][e] < 32 and got["count"][e] < 32:
+            m, n, _ = O.match_peaks(ref["peaks"]["bin"][e], got["bin"][e])
+            m_all += m; n_all += n
+    assert m_st == n_st, f"tau-stable peaks matched {m_st}/{n_st}"
+    if kind == "peaky":
+        assert n_all > 100 and m_all >= 0.999 * n_all, f"peaks matched {m_all}/{n_all}"
+    # the library's own peak finder on its own probabilities is the oracle's definition, bit for bit
+    own = O.find_peaks(Pg)
+    assert np.array_equal(own["bin"], got["bin"]) and np.array_equal(own["z"].view(np.uint32), got["z"].view(np.uint32))
+
+
+@pytest.mark.parametrize("prec", ["fp32", "tf32", "bf16"])
+@pytest.mark.parametrize("ch", [32, 16])
+def test_width_sweep_parity(prec, ch):
+    ev = make_events("run3", 16, 1004)
+    w = make_weights("rand", 1, ch)
+    ref = O.run(ev.feat, ev.event_offsets, w)
+    pvf = _available(prec, w, ev)
+    probs, _ = _run(pvf, ev)
+    assert np.abs(probs.cpu().numpy().astype(np.float64) - ref["probs"]).max() <= TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["fp32", "tf32", "bf16"])
+def test_unet_entry_point_on_synthetic_histograms(prec):
+    """UNet alone: zero input (bias-only), one-hot inputs at the interval edges (padding), large values."""
+    w = make_weights("rand", 5)
+    E = 3
+    H = np.zeros((E, 40, 8, 100), np.float32)
+    H[1, 0, 0, 0] = 3.0; H[1, 0, 7, 99] = 2.0; H[1, 39, 3, 50] = 5.0; H[1, 17, :, 49:51] = 1.5
+    H[2] = np.random.default_rng(3).gamma(2.0, 4.0, size=(40, 8, 100)).astype(np.float32)
+    ref = O.unet_probs(H.astype(np.float64), w.conv_w, w.conv_b)
+    ev = make_events("single", 1, 1)
+    try:
+        pvf = PVFinder(w, max_events=E, max_tracks=1, precision=prec, split_mask=SPLIT[prec])
+    except pkg.PVFError as exc:
+        if exc.status == pkg.PVF_ERR_CONFIG:
+            pytest.skip(f"precision {prec} not built yet")
+        raise
+    out = torch.empty(E, 4000, device="cuda")
+    s = torch.cuda.Stream()
+    pvf.run_unet(torch.from_numpy(H).cuda(), E, out, stream=s)
+    s.synchronize()
+    got = out.cpu().numpy()
+    assert np.abs(got.astype(np.float64) - ref).max() <= TOL[prec]
+    assert np.all(got[0].reshape(40, 100) == got[0, :100])       # identical bias-only vector everywhere
+
+
+# ------------------------------------------------------------------ boundary behaviour
+def test_boundary_contract():
+    ev = make_events("run3", 4, 77)
+    w = make_weights("rand", 1)
+    pvf = _make(w, ev)
+    feat, off = _dev(ev)
+    probs = torch.full((4, 4000), -1.0, device="cuda")
+    pk = pvf.alloc_peaks(4)
+    s = torch.cuda.Stream()
+    pvf.run(feat, off, 0, probs, pk, stream=s)                   # n_events = 0: OK and a no-op
+    s.synchronize()
+    assert float(probs.min()) == -1.0
+    import ctypes as C
+    ts, ps = pvf._tracks_struct(feat, off), pvf._peaks_struct(pk)
+    st = pvf.lib.pvf_run(pvf.handle, C.byref(ts), 4, C.c_void_p(probs.data_ptr()), C.byref(ps), None)
+    assert st == pkg.PVF_ERR_ARG                                 # NULL (default) stream rejected: PAPER.md:53
+    st = pvf.lib.pvf_run(pvf.handle, C.byref(ts), 5, C.c_void_p(probs.data_ptr()), C.byref(ps), C.c_void_p(s.cuda_stream))
+    assert st == pkg.PVF_ERR_CAPACITY
+    st = pvf.lib.pvf_run(pvf.handle, C.byref(ts), -1, C.c_void_p(probs.data_ptr()), C.byref(ps), C.c_void_p(s.cuda_stream))
+    assert st == pkg.PVF_ERR_ARG
+    s.synchronize()
+    assert float(probs.min()) == -1.0                            # nothing was enqueued by the failed calls
+    with pytest.raises(pkg.PVFError):
+        pvf.stage_times_ms()                                     # timing not enabled
+    # caller-supplied pool: zero allocation inside create (Allen-style fixed pool)
+    nbytes = pvf.workspace_bytes()
+    pool = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
+    pvf2 = PVFinder(w, max_events=4, max_tracks=ev.n_tracks, pool=pool)
+    p1, k1 = _run(pvf, ev)
+    p2, k2 = _run(pvf2, ev)
+    assert torch.equal(p1, p2) and torch.equal(k1["bin"], k2["bin"])
+    too_small = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    with pytest.raises(pkg.PVFError):
+        PVFinder(w, max_events=4, max_tracks=ev.n_tracks, pool=too_small)
+
+
+def test_host_io_and_stage_timing():
+    ev = make_events("run3", 6, 78)
+    w = make_weights("peaky", 1)
+    pvf = _make(w, ev, stage_timing=True, host_io=True)
+    probs, pk = _run(pvf, ev)
+    t = pvf.stage_times_ms()
+    assert len(t) == 4 and all(v >= 0 for v in t)
+    assert pvf.launches_per_run(6) == 4
+    hfeat = torch.from_numpy(ev.feat).pin_memory()
+    hoff = torch.from_numpy(ev.event_offsets).pin_memory()
+    hprobs = torch.empty(6, 4000).pin_memory()
+    hpk = pvf.alloc_peaks(6, pinned=True)
+    s = torch.cuda.Stream()
+    pvf.run_host(hfeat, hoff, 6, hprobs, hpk, stream=s)          # synchronises internally
+    assert torch.equal(hprobs, probs.cpu()) and torch.equal(hpk["bin"], pk["bin"].cpu())
+    assert torch.equal(hpk["z"], pk["z"].cpu())
+
+
+# ------------------------------------------------------------------ full size, bench launch configuration
+@pytest.mark.parametrize("prec", ["tf32", "bf16", "fp32"])
+def test_full_batch_sampled_events(prec):
+    """BASELINE.json config 2 (16000 events) in the launch configuration bench.py times; the oracle
+    computes sampled events one by one; properties hold for every event."""
+    E = 16000 if prec != "fp32" else 2000
+    ev = make_events("run3", E, 1002)
+    w = make_weights("peaky", 1)
+    pvf = _available(prec, w, ev)
+    probs, pk = _run(pvf, ev)
+    sample = [0, 1, E // 2, E - 2, E - 1, 4097, 777][: 7 if E > 5000 else 5]
+    sub = select_events(ev, sample)
+    ref = O.run(sub.feat, sub.event_offsets, w)
+    got = probs[sample].cpu().numpy()
+    assert np.abs(got.astype(np.float64) - ref["probs"]).max() <= TOL[prec]
+    gb = pk["bin"][sample].cpu().numpy()
+    for i in range(len(sample)):
+        m, n, _ = O.match_peaks(ref["peaks"]["bin"][i], gb[i])
+        assert m >= n - 1
+    # properties at any size: probabilities in (0,1); peak bins ascending, counts consistent
+    assert float(probs.min()) > 0.0 and float(probs.max()) < 1.0 and bool(torch.isfinite(probs).all())
+    cnt = pk["count"].cpu().numpy()
+    bins = pk["bin"].cpu().numpy()
+    assert np.all((bins >= 0).sum(axis=1) == cnt)
+    d = np.diff(bins, axis=1)
+    assert np.all((d > 0) | (bins[:, 1:] < 0))
