@@ -250,6 +250,93 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
   }
 }
 
+// Compile-time description of conv layer L (0 = e1 ... 4 = d1) as the MMA issuer sees it.
+template <int C, bool BF16, int L>
+struct Lay {
+  using G = Geo<C, BF16>;
+  static constexpr int TAPS = taps_of(L);
+  static constexpr int PAD = (TAPS - 1) / 2;
+  static constexpr int NKB = (L == 0) ? 1 : (L <= 2 ? C / G::KPM : 2 * C / G::KPM);   // K blocks per tap
+  static constexpr int STEPS = TAPS * NKB;                                            // (e1 split: x3, runtime)
+  static constexpr int LEAD = (L == 0 || L == 4) ? G::LEAD1 : ((L == 1 || L == 3) ? G::LEAD2 : G::LEAD3);
+  static constexpr int LBO = (L == 0 || L == 4) ? G::LBO1 : ((L == 1 || L == 3) ? G::LBO2 : G::LBO3);
+  static constexpr int NT = (L == 0 || L == 4) ? G::T : ((L == 1 || L == 3) ? G::T / 2 : (G::T + 3) / 4);
+  static constexpr int HALF = (L >= 3) ? NKB / 2 : NKB;        // K blocks served by the first source buffer
+  static constexpr int SRC0 = (L == 0) ? G::OFF_X0 : (L == 1) ? G::OFF_R : (L == 2) ? G::OFF_R + G::SZ_L2
+                              : (L == 3) ? G::OFF_R + G::SZ_L2 /* U2 */ : G::OFF_R /* U1 */;
+  static constexpr int SRC1 = (L == 3) ? G::OFF_R /* E2 */ : (L == 4) ? G::OFF_E1 : SRC0;
+  // byte offset (from the CTA's shared-memory base) of the first chunk of K block kk
+  __host__ __device__ static constexpr int a_off(int kk) {
+    return kk < HALF ? SRC0 + 2 * kk * LBO : SRC1 + 2 * (kk - HALF) * LBO;
+  }
+};
+
+template <bool BF16>
+__device__ __forceinline__ void mma_lh(uint32_t d, uint32_t a_lo, uint32_t a_hi, uint32_t b_lo, uint32_t b_hi,
+                                       uint32_t idesc, uint32_t acc) {
+  if (BF16) mma_f16_lh(d, a_lo, a_hi, b_lo, b_hi, idesc, acc);
+  else mma_tf32_lh(d, a_lo, a_hi, b_lo, b_hi, idesc, acc);
+}
+
+struct RingState { int ring; uint32_t phase; };
+
+// All MMAs of layer L for the group: tap-major over ring stages, every stage used by all NT tiles.
+// The warp walks the (uniform) schedule; one elected lane issues a whole stage worth of MMAs whose
+// descriptors differ from the stage origin by compile-time constants.
+template <int C, bool BF16, int L>
+__device__ __forceinline__ void mma_layer(uint32_t sb, uint32_t tmem_acc, uint32_t bar0, RingState& rs,
+                                          int steps_rt) {
+  using G = Geo<C, BF16>;
+  using Y = Lay<C, BF16, L>;
+  constexpr int SPS = G::SPS;
+  static_assert(Y::HALF % SPS == 0 || SPS % Y::NKB == 0, "a ring stage is either part of one source's K blocks or whole taps");
+  constexpr uint32_t idesc = instr_desc(BF16 ? kFmtBF16 : kFmtTF32, 128, C);
+  constexpr uint32_t hi = (128u >> 4) | (1u << 14);                    // SBO = 128 B, descriptor version 1
+  constexpr uint32_t a_lbo = (uint32_t)(Y::LBO >> 4) << 16;
+  constexpr uint32_t b_lbo = (uint32_t)((C * 16) >> 4) << 16;
+  const int steps = (L == 0) ? steps_rt : Y::STEPS;
+  for (int f = 0; f < steps; f += SPS) {
+    const int n = min(SPS, steps - f);
+    mbar_wait(bar0 + 8u * rs.ring, rs.phase);
+    tc_fence_after_sync();
+    const uint32_t b0 = b_lbo + ((sb + G::OFF_RING + rs.ring * kStageBytes) >> 4);
+    uint32_t a0 = a_lbo + (sb >> 4);          // stage origin: descriptor low word of tile 0, step f
+    if (L == 0) {
+      // e1: one K block per step; steps run [pass][tap], pass 1 reads the low-part chunks (split)
+    } else if (Y::HALF >= SPS) {
+      const int j0 = f / Y::NKB, kk0 = f % Y::NKB;
+      const int off = kk0 < Y::HALF ? Y::SRC0 + 2 * kk0 * Y::LBO : Y::SRC1 + 2 * (kk0 - Y::HALF) * Y::LBO;
+      a0 += (uint32_t)(off >> 4) + (uint32_t)(Y::LEAD + j0 - Y::PAD);
+    } else {
+      a0 += (uint32_t)(Y::SRC0 >> 4) + (uint32_t)(Y::LEAD + f / Y::NKB - Y::PAD);
+    }
+    if (elect_one()) {
+#pragma unroll
+      for (int i = 0; i < SPS; ++i) {
+        if (i < n) {
+          uint32_t a;
+          if (L == 0) {
+            const int step = f + i, pass = step / 25, j = step - 25 * pass;
+            a = a0 + (uint32_t)((G::OFF_X0 + (pass == 1 ? 2 * G::LBO1 : 0)) >> 4) + (uint32_t)(Y::LEAD + j - Y::PAD);
+          } else if (Y::HALF >= SPS) {
+            a = a0 + (uint32_t)(i * ((2 * Y::LBO) >> 4));
+          } else {
+            a = a0 + (uint32_t)((Y::a_off(i % Y::NKB) - Y::SRC0) >> 4) + (uint32_t)(i / Y::NKB);
+          }
+          const uint32_t b = b0 + (uint32_t)(i * (G::STEP_BYTES >> 4));
+          const uint32_t acc = (i > 0) ? 1u : (f > 0 ? 1u : 0u);
+#pragma unroll
+          for (int t = 0; t < Y::NT; ++t)
+            mma_lh<BF16>(tmem_acc + (uint32_t)(t * C), a + 128u * t, hi, b, hi, idesc, acc);
+        }
+      }
+      mma_commit(bar0 + 8u * (kStages + rs.ring));      // frees the ring slot when these MMAs retire
+    }
+    __syncwarp();
+    if (++rs.ring == kStages) { rs.ring = 0; rs.phase ^= 1u; }
+  }
+}
+
 template <int C, bool BF16>
 __global__ void __launch_bounds__(kTcThreads, 1)
 k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __restrict__ wpack, int split_e1,
@@ -257,7 +344,8 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
   using G = Geo<C, BF16>;
   extern __shared__ __align__(1024) unsigned char smem[];
   const uint32_t sb = smem_u32(smem);
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // provably warp-uniform role index
   float* par = reinterpret_cast<float*>(smem + G::OFF_PAR);
   const uint32_t bar0 = sb + G::OFF_BAR;
   auto full_bar = [&](int s) { return bar0 + 8u * s; };
@@ -305,59 +393,22 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
       }
     }
   } else if (warp == 1) {
-    // ===================== MMA issuer
-    if (lane == 0) {
-      const uint32_t idesc = instr_desc(BF16 ? kFmtBF16 : kFmtTF32, 128, C);
-      const uint64_t desc_hi_b = smem_desc(0, C * 16, 128);
-      int ring = 0;
-      uint32_t phase = 0, epi_phase = 0;
-      for (int g = blockIdx.x; g < n_groups; g += gridDim.x) {
-        for (int l = 0; l < 5; ++l) {
-          // geometry of the layer's input level
-          const int taps = taps_of(l), pad = (taps - 1) / 2;
-          int lead, lbo, ntiles;
-          if (l == 0 || l == 4) { lead = G::LEAD1; lbo = G::LBO1; ntiles = G::T; }
-          else if (l == 1 || l == 3) { lead = G::LEAD2; lbo = G::LBO2; ntiles = G::T / 2; }
-          else { lead = G::LEAD3; lbo = G::LBO3; ntiles = (G::T + 3) / 4; }
-          // source buffers: first half (k blocks < half) and second half of the channel range
-          uint32_t src0, src1;
-          int half;                        // number of k blocks served by src0
-          if (l == 0) { src0 = sb + G::OFF_X0; src1 = src0; half = 4; }
-          else if (l == 1) { src0 = sb + G::OFF_R; src1 = src0; half = P.nkb[1]; }                       // P1
-          else if (l == 2) { src0 = sb + G::OFF_R + G::SZ_L2; src1 = src0; half = P.nkb[2]; }            // P2
-          else if (l == 3) { src0 = sb + G::OFF_R + G::SZ_L2; src1 = sb + G::OFF_R; half = P.nkb[3] / 2; }  // [U2 | E2]
-          else { src0 = sb + G::OFF_R; src1 = sb + G::OFF_E1; half = P.nkb[4] / 2; }                     // [U1 | E1]
-          const uint64_t desc_hi_a = smem_desc(0, (uint32_t)lbo, 128);
-          mbar_wait(epi_bar, epi_phase);
-          epi_phase ^= 1u;
-          tc_fence_after_sync();
-          int j = 0, kk = 0;
-          uint32_t acc = 0;
-          for (int s0 = 0; s0 < P.steps[l]; s0 += G::SPS) {
-            const int n = min(G::SPS, P.steps[l] - s0);
-            mbar_wait(full_bar(ring), phase);
-            tc_fence_after_sync();
-            const uint32_t bstage = sb + G::OFF_RING + ring * kStageBytes;
-            for (int i = 0; i < n; ++i) {
-              uint32_t abase;
-              if (l == 0) abase = src0 + (uint32_t)((kk == 1) ? 2 : 0) * (uint32_t)lbo;   // split: hi, lo, hi
-              else if (kk < half) abase = src0 + (uint32_t)(2 * kk) * (uint32_t)lbo;
-              else abase = src1 + (uint32_t)(2 * (kk - half)) * (uint32_t)lbo;
-              abase += (uint32_t)(lead + j - pad) * 16u;
-              const uint64_t bd = desc_hi_b | (uint64_t)(((bstage + (uint32_t)i * G::STEP_BYTES) >> 4) & 0x3FFFu);
-              for (int t = 0; t < ntiles; ++t) {
-                const uint64_t ad = desc_hi_a | (uint64_t)(((abase + (uint32_t)t * 2048u) >> 4) & 0x3FFFu);
-                if (BF16) mma_f16(tmem_acc + (uint32_t)(t * C), ad, bd, idesc, acc);
-                else mma_tf32(tmem_acc + (uint32_t)(t * C), ad, bd, idesc, acc);
-              }
-              acc = 1;
-              if (++kk == P.nkb[l]) { kk = 0; ++j; }
-            }
-            mma_commit(empty_bar(ring));
-            if (++ring == kStages) { ring = 0; phase ^= 1u; }
-          }
-          mma_commit(accum_bar);
-        }
+    // ===================== MMA issuer (whole warp walks the schedule, one elected lane issues)
+    RingState rs{0, 0u};
+    uint32_t epi_phase = 0;
+    for (int g = blockIdx.x; g < n_groups; g += gridDim.x) {
+#pragma unroll
+      for (int l = 0; l < 5; ++l) {
+        mbar_wait(epi_bar, epi_phase);
+        epi_phase ^= 1u;
+        tc_fence_after_sync();
+        if (l == 0) mma_layer<C, BF16, 0>(sb, tmem_acc, bar0, rs, P.steps[0]);
+        else if (l == 1) mma_layer<C, BF16, 1>(sb, tmem_acc, bar0, rs, 0);
+        else if (l == 2) mma_layer<C, BF16, 2>(sb, tmem_acc, bar0, rs, 0);
+        else if (l == 3) mma_layer<C, BF16, 3>(sb, tmem_acc, bar0, rs, 0);
+        else mma_layer<C, BF16, 4>(sb, tmem_acc, bar0, rs, 0);
+        if (elect_one()) mma_commit(accum_bar);
+        __syncwarp();
       }
     }
   } else {
@@ -440,7 +491,9 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst) {
     const float* W = w->conv_w[l];          // [C][cin][K]
     for (int j = 0; j < K; ++j)
       for (int kk = 0; kk < P.nkb[l]; ++kk) {
-        unsigned char* step = dst + P.w_off[l] + (size_t)(j * P.nkb[l] + kk) * G::STEP_BYTES;
+        // step order inside a layer: [tap][K block]; the e1 split runs [pass][tap] (pass = K block)
+        const size_t step_idx = (l == 0) ? (size_t)kk * K + j : (size_t)j * P.nkb[l] + kk;
+        unsigned char* step = dst + P.w_off[l] + step_idx * G::STEP_BYTES;
         for (int h = 0; h < 2; ++h)
           for (int n = 0; n < C; ++n)
             for (int e = 0; e < G::PER; ++e) {
