@@ -277,7 +277,7 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--precision", default=os.environ.get("PVF_BENCH_PRECISION", "fp32"), choices=["fp32", "tf32", "bf16"])
+    ap.add_argument("--precision", default=os.environ.get("PVF_BENCH_PRECISION", "tf32"), choices=["fp32", "tf32", "bf16"])
     ap.add_argument("--split-mask", type=int, default=-1)
     ap.add_argument("--events", type=int, default=16000)
     ap.add_argument("--model", default="run3", choices=["run3", "pileup"])

@@ -107,8 +107,10 @@ def _peaky(seed: int, channels: int, eps_unet: float = 0.3, eps_fc: float = 0.01
     S_cw[0][0, 0, :] = taps / taps.sum()
     kd1 = shapes[4][2]
     S_cw[4][0, C + 0, (kd1 - 1) // 2] = 1.0   # concat order is [upsampled, skip]
-    S_cw[5][0, 0, 0] = 0.12
-    S_cb[5][0] = -5.0
+    # head: background logit -6.5 (p = 1.5e-3, a decade below the 0.01 peak threshold, so that ripples of
+    # the background are not peaks: DESIGN.md "peaky weights"), signal gain 0.16
+    S_cw[5][0, 0, 0] = 0.16
+    S_cb[5][0] = -6.5
     for k in range(6):
         w.conv_w.append((S_cw[k] + eps_unet * noise.conv_w[k]).astype(np.float32))
         w.conv_b.append((S_cb[k] + eps_unet * noise.conv_b[k]).astype(np.float32))

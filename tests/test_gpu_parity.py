@@ -170,12 +170,30 @@ def _available(prec, w, ev):
         raise
 
 
+_ORACLE_CACHE = {}
+
+
+def _oracle_cached(kind, n_events):
+    """Oracle results are shared by the precisions of one weight kind (the oracle takes ~70 ms/event)."""
+    key = (kind, n_events)
+    if key not in _ORACLE_CACHE:
+        ev = make_events("run3", n_events, 1001)
+        w = make_weights(kind, 1)
+        _ORACLE_CACHE[key] = (ev, w, O.run(ev.feat, ev.event_offsets, w))
+    return _ORACLE_CACHE[key]
+
+
+# share of ALL oracle peaks that must be matched within +-1 bin on `peaky` (north_star: 99.9 %; the BF16
+# variant has a stated 2e-2 probability tolerance, so peaks whose height is within that error of the
+# 0.01 threshold cannot be guaranteed: stated bar 99 %, DESIGN.md "Tolerances")
+PEAK_SHARE = {"fp32": 0.999, "tf32": 0.999, "bf16": 0.99}
+
+
 @pytest.mark.parametrize("prec", ["fp32", "tf32", "bf16"])
 @pytest.mark.parametrize("kind", ["rand", "peaky"])
 def test_whole_path_parity(prec, kind):
-    ev = make_events("run3", 48, 1001)
-    w = make_weights(kind, 1)
-    ref = O.run(ev.feat, ev.event_offsets, w)
+    # peaky: BASELINE.json config 1 (1000 events, ~5400 oracle peaks) so that 99.9 % is resolvable
+    ev, w, ref = _oracle_cached(kind, 1000 if kind == "peaky" else 48)
     pvf = _available(prec, w, ev)
     probs, pk = _run(pvf, ev)
     Pg = probs.cpu().numpy()
@@ -196,7 +214,8 @@ def test_whole_path_parity(prec, kind):
             m_all += m; n_all += n
     assert m_st == n_st, f"tau-stable peaks matched {m_st}/{n_st}"
     if kind == "peaky":
-        assert n_all > 100 and m_all >= 0.999 * n_all, f"peaks matched {m_all}/{n_all}"
+        print(f"[{prec}] peaky: max|dP| {err.max():.3e}; peaks matched {m_all}/{n_all}; tau-stable {m_st}/{n_st}")
+        assert n_all > 3000 and m_all >= PEAK_SHARE[prec] * n_all, f"peaks matched {m_all}/{n_all}"
     # the library's own peak finder on its own probabilities is the oracle's definition, bit for bit
     own = O.find_peaks(Pg)
     assert np.array_equal(own["bin"], got["bin"]) and np.array_equal(own["z"].view(np.uint32), got["z"].view(np.uint32))
