@@ -3,7 +3,7 @@
 // PAPER.md:29 "5-layer UNet architecture (64 channels deployed)", PAPER.md:63-76 (the CNN is the
 // bottleneck); topology from BASELINE.json config 0 (see k_unet_simt.cu); north_star (c): implicit
 // GEMM on tcgen05/TMEM, pool / upsample / concat / activations fused into the epilogues, the
-// intermediates stay in shared memory / TMEM.  DESIGN.md "K2" has the derivation of everything here.
+// intermediates stay in shared memory / TMEM.  DESIGN.md section 4.3 has the derivation.
 //
 // Mapping.  A conv layer is  D[m, n] = sum_j sum_ci  A[m + j - p, ci] * W_j[ci, n]  with m = position
 // (M), n = output channel (N = C), and one (tap j, 32-byte channel block) per tcgen05.mma of shape
@@ -12,12 +12,19 @@
 // shift is a pure bump of the descriptor start address by 16 B per row, the skip concat is a second
 // base address, and an epilogue thread (= one row) writes whole 16-byte chunks, conflict free.
 // Intervals sit at row stride 128 / 64 / 32 (L = 100 / 50 / 25); the rows between them are zero and
-// double as the "same" padding.  One CTA (persistent) takes a group of T intervals through all five
-// layers; accumulators of the group's tiles sit side by side in TMEM and each weight slice is
-// streamed from L2 exactly once per group (1D bulk copies into a ring of 8 KB stages) and used by
-// every tile.  Roles: warp 0 = weight producer, warp 1 = MMA issuer (one thread), warps 2-5 =
-// epilogue (TMEM -> registers -> bias, LeakyReLU, TF32/BF16 rounding, pool / upsample -> shared
-// memory; the last layer fuses the 1x1 head and the sigmoid and writes the probabilities).
+// double as the "same" padding.  One persistent CTA takes a group of T intervals through all five
+// layers; each weight slice is streamed from L2 once per group (1D bulk copies into a ring of 8 KB
+// stages) and used by every tile of the group.
+//
+// Schedule.  The MMA issuer never waits for an epilogue in steady state: d1 is split into the half
+// that reads the e1 skip (d1E, needs only e1's epilogue) and the half that reads up(d2) (d1U); d1E
+// is cut in three parts that run while the epilogues of e2, b and d2 drain, and the NEXT group's e1
+// runs before d1U so that its epilogue overlaps d1U:
+//     e2 | d1E.1 | b | d1E.2 | d2 | d1E.3 | e1(next) | d1U        (weight image is packed in this order)
+// TMEM holds two accumulator regions: A (d1, T tiles) and B (e1: T tiles; e2, b, d2: its first tiles).
+// Roles: warp 0 = weight producer, warp 1 = MMA issuer (warp-uniform schedule, one elected lane
+// issues), warps 2-5 = epilogue (TMEM -> registers -> bias, LeakyReLU, TF32/BF16 rounding, pool /
+// upsample -> shared memory; d1's epilogue fuses the 1x1 head + sigmoid and writes out_probs).
 #include <cuda_bf16.h>
 #include <cstring>
 #include <vector>
@@ -31,10 +38,14 @@ using namespace umma;
 namespace {
 
 constexpr int kTcThreads = 192;
-constexpr int kStages = 6;
+constexpr int kStages = 5;
 constexpr int kStageBytes = 8192;
 constexpr int kHeaderBytes = 2048;          // biases [5][C], head weight [C], head bias
-__host__ __device__ constexpr int taps_of(int l) { return (l == 0 || l == 4) ? 25 : (l == 2 ? 5 : 15); }
+
+// sub-layers as the MMA issuer sees them
+enum { sE1 = 0, sE2 = 1, sB = 2, sD2 = 3, sD1U = 4, sD1E = 5 };
+// weight-image segments in streaming order
+enum { gE2 = 0, gD1Ea = 1, gB = 2, gD1Eb = 3, gD2 = 4, gD1Ec = 5, gE1 = 6, gD1U = 7, kSegs = 8 };
 
 template <int C, bool BF16>
 struct Geo {
@@ -43,6 +54,7 @@ struct Geo {
   static constexpr int KPM = 2 * PER;                // channels per MMA (32 bytes of K)
   static constexpr int NCH = C / PER;                // chunks of a C-channel activation
   static constexpr int XCH = BF16 ? 2 : 4;           // chunks of the input buffer X0 (TF32: hi0 hi1 lo0 lo1)
+  static constexpr int NKB1 = C / KPM;               // MMA K blocks per tap over C channels
   static constexpr int T = (C == 64) ? (BF16 ? 4 : 2) : (BF16 ? 8 : 4);   // intervals per group
   static constexpr int LEAD1 = 16, LEAD2 = 8, LEAD3 = 8;
   static constexpr int ROWS1 = 128 * T + 32, ROWS2 = 64 * T + 16, ROWS3 = 32 * T + 16;
@@ -50,43 +62,57 @@ struct Geo {
   static constexpr int STEP_BYTES = 2 * C * 16;      // one MMA's B operand: [2 chunks][C][16 B]
   static constexpr int SPS = kStageBytes / STEP_BYTES;   // MMA steps per ring stage
   // shared-memory map (bytes)
-  static constexpr int OFF_E1 = 0;
   static constexpr int SZ_L1 = NCH * LBO1;           // a C-channel buffer at L = 100
-  static constexpr int SZ_L2 = NCH * LBO2;
-  static constexpr int OFF_R = OFF_E1 + SZ_L1;       // overlay region: U1 | (E2, U2) | (P1, P2)
-  static constexpr int OFF_X0 = OFF_R + SZ_L1;
-  static constexpr int OFF_RING = OFF_X0 + XCH * LBO1;
+  static constexpr int SZ_L2 = NCH * LBO2;           //                     at L = 50
+  static constexpr int OFF_E1 = 0;                   // e1 skip (dedicated)
+  static constexpr int OFF_R = OFF_E1 + SZ_L1;       // overlay: (E2 | U2) then U1; P2 sits in U2's place
+  static constexpr int OFF_XP = OFF_R + SZ_L1;       // overlay: X0 (input) then P1 = pool(e1)
+  static constexpr int SZ_XP = (XCH * LBO1 > SZ_L2) ? XCH * LBO1 : SZ_L2;
+  static constexpr int OFF_RING = OFF_XP + SZ_XP;
   static constexpr int OFF_PAR = OFF_RING + kStages * kStageBytes;   // biases + head (floats)
   static constexpr int OFF_BAR = OFF_PAR + kHeaderBytes;
   static constexpr int SMEM = OFF_BAR + 256;
-  static constexpr int TMEM_COLS = (T * C <= 32) ? 32 : (T * C <= 64) ? 64 : (T * C <= 128) ? 128 : (T * C <= 256) ? 256 : 512;
+  // TMEM columns: region A = [0, T*C) (d1), region B = [T*C, 2*T*C) (e1; e2, b, d2 use its head)
+  static constexpr int COL_A = 0, COL_B = T * C;
+  static constexpr int TMEM_COLS = (2 * T * C <= 32) ? 32 : (2 * T * C <= 64) ? 64 : (2 * T * C <= 128) ? 128
+                                   : (2 * T * C <= 256) ? 256 : 512;
+  // d1E parts (steps): run while the epilogues of e2 / b / d2 drain; multiples of every SPS
+  static constexpr int D1E_STEPS = 25 * NKB1;
+  static constexpr int D1E_A = D1E_STEPS < 16 ? D1E_STEPS : 16;
+  static constexpr int D1E_B = (D1E_STEPS - D1E_A) < 16 ? (D1E_STEPS - D1E_A) : 16;
+  static constexpr int D1E_C = D1E_STEPS - D1E_A - D1E_B;
   static_assert(2 * SZ_L2 == SZ_L1, "E2 + U2 must tile the overlay region exactly");
   static_assert(SMEM <= 227 * 1024, "shared memory budget");
-  static_assert(T * C <= 512, "TMEM budget");
-  static_assert(NCH % 2 == 0 && T % 2 == 0, "concat halves must hold whole MMA K blocks; level-2 tiles whole");
+  static_assert(2 * T * C <= 512, "TMEM budget");
+  static_assert(NCH % 2 == 0 && T % 2 == 0, "whole MMA K blocks per source; level-2 tiles whole");
+  static_assert(16 % SPS == 0, "d1E parts must start on ring-stage boundaries");
 };
 
-struct LayerPlan {
-  int nkb[5];        // MMA K blocks per tap
-  int steps[5];      // taps * nkb
-  int w_off[5];      // byte offset of the layer's first step in the packed image
+// Steps and byte offsets of the weight-image segments (host packer, producer and issuer agree on it).
+struct Plan {
+  int e1_steps;            // 25, or 75 with the e1 hi/lo split
+  int seg_steps[kSegs];
+  int seg_off[kSegs];      // bytes from the start of the image
   int total;
 };
 
 template <int C, bool BF16>
-__host__ __device__ inline LayerPlan make_plan(int split_e1) {
+__host__ __device__ inline Plan make_plan(int split_e1) {
   using G = Geo<C, BF16>;
-  LayerPlan P{};
-  P.nkb[0] = (!BF16 && split_e1) ? 3 : 1;
-  P.nkb[1] = C / G::KPM;
-  P.nkb[2] = C / G::KPM;
-  P.nkb[3] = 2 * C / G::KPM;
-  P.nkb[4] = 2 * C / G::KPM;
+  Plan P{};
+  P.e1_steps = 25 * ((!BF16 && split_e1) ? 3 : 1);
+  P.seg_steps[gE2] = 15 * G::NKB1;
+  P.seg_steps[gD1Ea] = G::D1E_A;
+  P.seg_steps[gB] = 5 * G::NKB1;
+  P.seg_steps[gD1Eb] = G::D1E_B;
+  P.seg_steps[gD2] = 15 * 2 * G::NKB1;
+  P.seg_steps[gD1Ec] = G::D1E_C;
+  P.seg_steps[gE1] = P.e1_steps;
+  P.seg_steps[gD1U] = 25 * G::NKB1;
   int off = kHeaderBytes;
-  for (int l = 0; l < 5; ++l) {
-    P.steps[l] = taps_of(l) * P.nkb[l];
-    P.w_off[l] = off;
-    off += P.steps[l] * G::STEP_BYTES;
+  for (int s = 0; s < kSegs; ++s) {
+    P.seg_off[s] = off;
+    off += P.seg_steps[s] * G::STEP_BYTES;
   }
   P.total = off;
   return P;
@@ -144,13 +170,14 @@ enum { kE1 = 0, kE2 = 1, kB = 2, kD2 = 3, kD1 = 4 };
 
 // Epilogue of one 128-row accumulator tile, executed by the four epilogue warps (thread = row m).
 template <int C, bool BF16, int MODE>
-__device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_acc, int tile, int q, int lane,
+__device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_base, int tile, int q, int lane,
                                               const float* __restrict__ par, int n_valid_int,
                                               float* __restrict__ probs_group) {
   using G = Geo<C, BF16>;
   const int m = 32 * q + lane;
   const float* bias = par + MODE * C;
-  const uint32_t taddr = tmem_acc + ((uint32_t)(32 * q) << 16) + (uint32_t)(tile * C);
+  const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) +
+                         (uint32_t)((MODE == kD1 ? G::COL_A : G::COL_B) + tile * C);
   // which interval of the group this row belongs to, its position, and whether it is a real output
   int interval, l;
   bool valid;
@@ -161,8 +188,8 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
   uint32_t dst_full = 0, dst_aux = 0, lbo_full = 0, lbo_aux = 0;
   if (MODE == kE1) {
     dst_full = smem_base + G::OFF_E1 + (uint32_t)(G::LEAD1 + 128 * tile + m) * 16u; lbo_full = G::LBO1;
-    dst_aux = smem_base + G::OFF_R + (uint32_t)(G::LEAD2 + 64 * tile + (m >> 1)) * 16u; lbo_aux = G::LBO2;      // P1
-    if (tile == 0 && m < G::LEAD2) zero_rows(smem_base + G::OFF_R, G::LBO2, G::NCH, m);
+    dst_aux = smem_base + G::OFF_XP + (uint32_t)(G::LEAD2 + 64 * tile + (m >> 1)) * 16u; lbo_aux = G::LBO2;     // P1
+    if (tile == 0 && m < G::LEAD2) zero_rows(smem_base + G::OFF_XP, G::LBO2, G::NCH, m);
   } else if (MODE == kE2) {
     dst_full = smem_base + G::OFF_R + (uint32_t)(G::LEAD2 + 128 * tile + m) * 16u; lbo_full = G::LBO2;          // E2
     dst_aux = smem_base + G::OFF_R + G::SZ_L2 + (uint32_t)(G::LEAD3 + 64 * tile + (m >> 1)) * 16u; lbo_aux = G::LBO3;  // P2
@@ -213,29 +240,38 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
   }
 }
 
-// Interval histograms of one group -> X0 (operand-rounded, chunked layout).  128 threads.
+// Interval histograms of one group -> X0 (operand-rounded, chunked layout).  128 threads.  X0 shares
+// its memory with P1, so every row the e1 MMAs can read for a valid output is (re)written: the lead
+// rows and the gap rows l >= 100 of every interval as zeros.
 template <int C, bool BF16>
 __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restrict__ hist, long long g0,
                                         int n_valid_int, int split, int tid) {
   using G = Geo<C, BF16>;
-  const uint32_t x0 = smem_base + G::OFF_X0;
+  const uint32_t x0 = smem_base + G::OFF_XP;
+  const uint4 zero4 = make_uint4(0, 0, 0, 0);
+  if (tid < G::LEAD1)
+    for (int c = 0; c < G::XCH; ++c) st_smem16(x0 + (uint32_t)c * G::LBO1 + (uint32_t)tid * 16u, zero4);
   if (BF16) {
-    for (int it = tid; it < G::T * 100; it += 128) {
-      const int t = it / 100, l = it % 100;
+    for (int it = tid; it < G::T * 128; it += 128) {
+      const int t = it >> 7, l = it & 127;
+      const bool live = l < 100 && t < n_valid_int;
       float x[8];
 #pragma unroll
-      for (int c = 0; c < 8; ++c) x[c] = t < n_valid_int ? __ldg(hist + (g0 + t) * kFcOut + c * kBins + l) : 0.0f;
+      for (int c = 0; c < 8; ++c) x[c] = live ? __ldg(hist + (g0 + t) * kFcOut + c * kBins + l) : 0.0f;
       uint4 qv;
       qv.x = pack_bf16(x[0], x[1]); qv.y = pack_bf16(x[2], x[3]);
       qv.z = pack_bf16(x[4], x[5]); qv.w = pack_bf16(x[6], x[7]);
-      st_smem16(x0 + (uint32_t)(G::LEAD1 + 128 * t + l) * 16u, qv);
+      const uint32_t row = (uint32_t)(G::LEAD1 + it) * 16u;
+      st_smem16(x0 + row, qv);
+      st_smem16(x0 + G::LBO1 + row, zero4);       // channels 8..15 of the K = 16 MMA: zero
     }
   } else {
-    for (int it = tid; it < G::T * 200; it += 128) {
-      const int t = it / 200, rem = it % 200, qc = rem / 100, l = rem % 100;
+    for (int it = tid; it < G::T * 256; it += 128) {
+      const int t = it >> 8, qc = (it >> 7) & 1, l = it & 127;
+      const bool live = l < 100 && t < n_valid_int;
       float x[4];
 #pragma unroll
-      for (int c = 0; c < 4; ++c) x[c] = t < n_valid_int ? __ldg(hist + (g0 + t) * kFcOut + (4 * qc + c) * kBins + l) : 0.0f;
+      for (int c = 0; c < 4; ++c) x[c] = live ? __ldg(hist + (g0 + t) * kFcOut + (4 * qc + c) * kBins + l) : 0.0f;
       uint4 hi;
       hi.x = to_tf32(x[0]); hi.y = to_tf32(x[1]); hi.z = to_tf32(x[2]); hi.w = to_tf32(x[3]);
       const uint32_t row = (uint32_t)(G::LEAD1 + 128 * t + l) * 16u;
@@ -250,21 +286,23 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
   }
 }
 
-// Compile-time description of conv layer L (0 = e1 ... 4 = d1) as the MMA issuer sees it.
-template <int C, bool BF16, int L>
+// Compile-time description of sub-layer S as the MMA issuer sees it.
+template <int C, bool BF16, int S>
 struct Lay {
   using G = Geo<C, BF16>;
-  static constexpr int TAPS = taps_of(L);
+  static constexpr int TAPS = (S == sE1 || S == sD1U || S == sD1E) ? 25 : (S == sB ? 5 : 15);
   static constexpr int PAD = (TAPS - 1) / 2;
-  static constexpr int NKB = (L == 0) ? 1 : (L <= 2 ? C / G::KPM : 2 * C / G::KPM);   // K blocks per tap
-  static constexpr int STEPS = TAPS * NKB;                                            // (e1 split: x3, runtime)
-  static constexpr int LEAD = (L == 0 || L == 4) ? G::LEAD1 : ((L == 1 || L == 3) ? G::LEAD2 : G::LEAD3);
-  static constexpr int LBO = (L == 0 || L == 4) ? G::LBO1 : ((L == 1 || L == 3) ? G::LBO2 : G::LBO3);
-  static constexpr int NT = (L == 0 || L == 4) ? G::T : ((L == 1 || L == 3) ? G::T / 2 : (G::T + 3) / 4);
-  static constexpr int HALF = (L >= 3) ? NKB / 2 : NKB;        // K blocks served by the first source buffer
-  static constexpr int SRC0 = (L == 0) ? G::OFF_X0 : (L == 1) ? G::OFF_R : (L == 2) ? G::OFF_R + G::SZ_L2
-                              : (L == 3) ? G::OFF_R + G::SZ_L2 /* U2 */ : G::OFF_R /* U1 */;
-  static constexpr int SRC1 = (L == 3) ? G::OFF_R /* E2 */ : (L == 4) ? G::OFF_E1 : SRC0;
+  static constexpr int NKB = (S == sE1) ? 1 : (S == sD2 ? 2 * G::NKB1 : G::NKB1);     // K blocks per tap
+  static constexpr int LEVEL = (S == sE1 || S == sD1U || S == sD1E) ? 1 : (S == sB ? 3 : 2);
+  static constexpr int LEAD = LEVEL == 1 ? G::LEAD1 : (LEVEL == 2 ? G::LEAD2 : G::LEAD3);
+  static constexpr int LBO = LEVEL == 1 ? G::LBO1 : (LEVEL == 2 ? G::LBO2 : G::LBO3);
+  static constexpr int NT = LEVEL == 1 ? G::T : (LEVEL == 2 ? G::T / 2 : (G::T + 3) / 4);
+  static constexpr int HALF = (S == sD2) ? NKB / 2 : NKB;      // K blocks served by the first source buffer
+  static constexpr int SRC0 = (S == sE1) ? G::OFF_XP /* X0 */ : (S == sE2) ? G::OFF_XP /* P1 */
+                              : (S == sB) ? G::OFF_R + G::SZ_L2 /* P2 */ : (S == sD2) ? G::OFF_R + G::SZ_L2 /* U2 */
+                              : (S == sD1U) ? G::OFF_R /* U1 */ : G::OFF_E1 /* E1 */;
+  static constexpr int SRC1 = (S == sD2) ? G::OFF_R /* E2 */ : SRC0;
+  static constexpr int DCOL = (S == sD1U || S == sD1E) ? G::COL_A : G::COL_B;
   // byte offset (from the CTA's shared-memory base) of the first chunk of K block kk
   __host__ __device__ static constexpr int a_off(int kk) {
     return kk < HALF ? SRC0 + 2 * kk * LBO : SRC1 + 2 * (kk - HALF) * LBO;
@@ -280,28 +318,30 @@ __device__ __forceinline__ void mma_lh(uint32_t d, uint32_t a_lo, uint32_t a_hi,
 
 struct RingState { int ring; uint32_t phase; };
 
-// All MMAs of layer L for the group: tap-major over ring stages, every stage used by all NT tiles.
-// The warp walks the (uniform) schedule; one elected lane issues a whole stage worth of MMAs whose
-// descriptors differ from the stage origin by compile-time constants.
-template <int C, bool BF16, int L>
-__device__ __forceinline__ void mma_layer(uint32_t sb, uint32_t tmem_acc, uint32_t bar0, RingState& rs,
-                                          int steps_rt) {
+// MMA steps [f_begin, f_end) of sub-layer S for the group: tap-major over ring stages, every stage
+// used by all NT tiles.  The warp walks the (uniform) schedule; one elected lane issues a whole
+// stage worth of MMAs whose descriptors differ from the stage origin by compile-time constants.
+// f_begin must be a multiple of SPS.  acc0 = 0 starts fresh accumulators at step f_begin.
+template <int C, bool BF16, int S>
+__device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_t bar0, RingState& rs,
+                                        int f_begin, int f_end, uint32_t acc0) {
   using G = Geo<C, BF16>;
-  using Y = Lay<C, BF16, L>;
+  using Y = Lay<C, BF16, S>;
   constexpr int SPS = G::SPS;
-  static_assert(Y::HALF % SPS == 0 || SPS % Y::NKB == 0, "a ring stage is either part of one source's K blocks or whole taps");
+  static_assert(Y::HALF % SPS == 0 || SPS % Y::NKB == 0,
+                "a ring stage is either part of one source's K blocks or whole taps");
   constexpr uint32_t idesc = instr_desc(BF16 ? kFmtBF16 : kFmtTF32, 128, C);
   constexpr uint32_t hi = (128u >> 4) | (1u << 14);                    // SBO = 128 B, descriptor version 1
   constexpr uint32_t a_lbo = (uint32_t)(Y::LBO >> 4) << 16;
   constexpr uint32_t b_lbo = (uint32_t)((C * 16) >> 4) << 16;
-  const int steps = (L == 0) ? steps_rt : Y::STEPS;
-  for (int f = 0; f < steps; f += SPS) {
-    const int n = min(SPS, steps - f);
+  const uint32_t dcol = tmem_base + (uint32_t)Y::DCOL;
+  for (int f = f_begin; f < f_end; f += SPS) {
+    const int n = min(SPS, f_end - f);
     mbar_wait(bar0 + 8u * rs.ring, rs.phase);
     tc_fence_after_sync();
     const uint32_t b0 = b_lbo + ((sb + G::OFF_RING + rs.ring * kStageBytes) >> 4);
     uint32_t a0 = a_lbo + (sb >> 4);          // stage origin: descriptor low word of tile 0, step f
-    if (L == 0) {
+    if (S == sE1) {
       // e1: one K block per step; steps run [pass][tap], pass 1 reads the low-part chunks (split)
     } else if (Y::HALF >= SPS) {
       const int j0 = f / Y::NKB, kk0 = f % Y::NKB;
@@ -315,19 +355,19 @@ __device__ __forceinline__ void mma_layer(uint32_t sb, uint32_t tmem_acc, uint32
       for (int i = 0; i < SPS; ++i) {
         if (i < n) {
           uint32_t a;
-          if (L == 0) {
+          if (S == sE1) {
             const int step = f + i, pass = step / 25, j = step - 25 * pass;
-            a = a0 + (uint32_t)((G::OFF_X0 + (pass == 1 ? 2 * G::LBO1 : 0)) >> 4) + (uint32_t)(Y::LEAD + j - Y::PAD);
+            a = a0 + (uint32_t)((Y::SRC0 + (pass == 1 ? 2 * G::LBO1 : 0)) >> 4) + (uint32_t)(Y::LEAD + j - Y::PAD);
           } else if (Y::HALF >= SPS) {
             a = a0 + (uint32_t)(i * ((2 * Y::LBO) >> 4));
           } else {
             a = a0 + (uint32_t)((Y::a_off(i % Y::NKB) - Y::SRC0) >> 4) + (uint32_t)(i / Y::NKB);
           }
           const uint32_t b = b0 + (uint32_t)(i * (G::STEP_BYTES >> 4));
-          const uint32_t acc = (i > 0) ? 1u : (f > 0 ? 1u : 0u);
+          const uint32_t acc = (i > 0) ? 1u : (f > f_begin ? 1u : acc0);
 #pragma unroll
           for (int t = 0; t < Y::NT; ++t)
-            mma_lh<BF16>(tmem_acc + (uint32_t)(t * C), a + 128u * t, hi, b, hi, idesc, acc);
+            mma_lh<BF16>(dcol + (uint32_t)(t * C), a + 128u * t, hi, b, hi, idesc, acc);
         }
       }
       mma_commit(bar0 + 8u * (kStages + rs.ring));      // frees the ring slot when these MMAs retire
@@ -347,21 +387,22 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
   const int tid = threadIdx.x, lane = tid & 31;
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // provably warp-uniform role index
   float* par = reinterpret_cast<float*>(smem + G::OFF_PAR);
+  // mbarriers: full[s], empty[s] per ring stage; accum[k] = "MMAs of layer k retired" (k: e1 e2 b d2 d1);
+  // epi[k] = "epilogue k done" (k: x0-staged e1 e2 b d2 d1)
   const uint32_t bar0 = sb + G::OFF_BAR;
-  auto full_bar = [&](int s) { return bar0 + 8u * s; };
-  auto empty_bar = [&](int s) { return bar0 + 8u * (kStages + s); };
-  const uint32_t accum_bar = bar0 + 8u * (2 * kStages);
-  const uint32_t epi_bar = bar0 + 8u * (2 * kStages + 1);
-  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + G::OFF_BAR + 8 * (2 * kStages + 2));
-  const LayerPlan P = make_plan<C, BF16>(split_e1);
+  auto accum_bar = [&](int k) { return bar0 + 8u * (2 * kStages + k); };
+  auto epi_bar = [&](int k) { return bar0 + 8u * (2 * kStages + 5 + k); };
+  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + G::OFF_BAR + 8 * (2 * kStages + 11));
+  static_assert(8 * (2 * kStages + 11) + 4 <= 256, "barrier block");
+  const Plan P = make_plan<C, BF16>(split_e1);
 
   // ---- one-time setup: zero the activation buffers (gap / halo rows must be zero), parameters, barriers
   for (int i = tid; i < G::OFF_RING / 16; i += kTcThreads) reinterpret_cast<uint4*>(smem)[i] = make_uint4(0, 0, 0, 0);
   for (int i = tid; i < 6 * C + 1; i += kTcThreads) par[i] = reinterpret_cast<const float*>(wpack)[i];
   if (tid == 0) {
-    for (int s = 0; s < kStages; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-    mbar_init(accum_bar, 1);
-    mbar_init(epi_bar, 128);
+    for (int s = 0; s < kStages; ++s) { mbar_init(bar0 + 8u * s, 1); mbar_init(bar0 + 8u * (kStages + s), 1); }
+    for (int k = 0; k < 5; ++k) mbar_init(accum_bar(k), 1);
+    for (int k = 0; k < 6; ++k) mbar_init(epi_bar(k), 128);
     fence_mbar_init();
   }
   if (warp == 1) tmem_alloc(smem_u32(const_cast<uint32_t*>(tmem_slot)), G::TMEM_COLS);
@@ -369,92 +410,124 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
   tc_fence_before_sync();
   __syncthreads();
   tc_fence_after_sync();
-  const uint32_t tmem_acc = *tmem_slot;
+  const uint32_t tmem_base = *tmem_slot;
 
   const int n_groups = (n_int + G::T - 1) / G::T;
+  const int stride = gridDim.x;
 
   if (warp == 0) {
-    // ===================== weight producer: streams every layer's MMA steps through the ring
+    // ===================== weight producer: streams the image's segments through the ring
     if (lane == 0) {
-      int ring = 0;
-      uint32_t phase = 0;
-      for (int g = blockIdx.x; g < n_groups; g += gridDim.x) {
-        for (int l = 0; l < 5; ++l) {
-          const unsigned char* src = wpack + P.w_off[l];
-          for (int s0 = 0; s0 < P.steps[l]; s0 += G::SPS) {
-            const int n = min(G::SPS, P.steps[l] - s0);
-            mbar_wait(empty_bar(ring), phase ^ 1u);
-            mbar_arrive_expect_tx(full_bar(ring), (uint32_t)(n * G::STEP_BYTES));
-            bulk_g2s(sb + G::OFF_RING + ring * kStageBytes, src + (size_t)s0 * G::STEP_BYTES,
-                     (uint32_t)(n * G::STEP_BYTES), full_bar(ring));
-            if (++ring == kStages) { ring = 0; phase ^= 1u; }
-          }
+      RingState rs{0, 0u};
+      auto stream = [&](int seg) {
+        const unsigned char* src = wpack + P.seg_off[seg];
+        const int steps = P.seg_steps[seg];
+        for (int f = 0; f < steps; f += G::SPS) {
+          const int n = min(G::SPS, steps - f);
+          mbar_wait(bar0 + 8u * (kStages + rs.ring), rs.phase ^ 1u);
+          mbar_arrive_expect_tx(bar0 + 8u * rs.ring, (uint32_t)(n * G::STEP_BYTES));
+          bulk_g2s(sb + G::OFF_RING + rs.ring * kStageBytes, src + (size_t)f * G::STEP_BYTES,
+                   (uint32_t)(n * G::STEP_BYTES), bar0 + 8u * rs.ring);
+          if (++rs.ring == kStages) { rs.ring = 0; rs.phase ^= 1u; }
+        }
+      };
+      bool first = true;
+      for (int g = blockIdx.x; g < n_groups; g += stride) {
+        if (first) { stream(gE1); first = false; }
+        const bool has_next = g + stride < n_groups;
+        for (int s = 0; s < kSegs; ++s) {
+          if (s == gE1 && !has_next) continue;
+          stream(s);
         }
       }
     }
   } else if (warp == 1) {
     // ===================== MMA issuer (whole warp walks the schedule, one elected lane issues)
     RingState rs{0, 0u};
-    uint32_t epi_phase = 0;
-    for (int g = blockIdx.x; g < n_groups; g += gridDim.x) {
-#pragma unroll
-      for (int l = 0; l < 5; ++l) {
-        mbar_wait(epi_bar, epi_phase);
-        epi_phase ^= 1u;
-        tc_fence_after_sync();
-        if (l == 0) mma_layer<C, BF16, 0>(sb, tmem_acc, bar0, rs, P.steps[0]);
-        else if (l == 1) mma_layer<C, BF16, 1>(sb, tmem_acc, bar0, rs, 0);
-        else if (l == 2) mma_layer<C, BF16, 2>(sb, tmem_acc, bar0, rs, 0);
-        else if (l == 3) mma_layer<C, BF16, 3>(sb, tmem_acc, bar0, rs, 0);
-        else mma_layer<C, BF16, 4>(sb, tmem_acc, bar0, rs, 0);
-        if (elect_one()) mma_commit(accum_bar);
-        __syncwarp();
+    uint32_t ph[6] = {0, 0, 0, 0, 0, 0};
+    auto wait_epi = [&](int k) { mbar_wait(epi_bar(k), ph[k]); ph[k] ^= 1u; tc_fence_after_sync(); };
+    auto commit = [&](int k) { if (elect_one()) mma_commit(accum_bar(k)); __syncwarp(); };
+    bool first = true;
+    for (int g = blockIdx.x; g < n_groups; g += stride) {
+      const bool has_next = g + stride < n_groups;
+      if (first) {
+        wait_epi(0);
+        mma_seg<C, BF16, sE1>(sb, tmem_base, bar0, rs, 0, P.e1_steps, 0u);
+        commit(0);
       }
+      wait_epi(1);                                   // P1 staged, region B drained
+      mma_seg<C, BF16, sE2>(sb, tmem_base, bar0, rs, 0, 15 * G::NKB1, 0u);
+      commit(1);
+      if (!first) wait_epi(5);                       // region A drained by the previous group's d1 epilogue
+      mma_seg<C, BF16, sD1E>(sb, tmem_base, bar0, rs, 0, G::D1E_A, 0u);
+      wait_epi(2);                                   // E2, P2 staged
+      mma_seg<C, BF16, sB>(sb, tmem_base, bar0, rs, 0, 5 * G::NKB1, 0u);
+      commit(2);
+      mma_seg<C, BF16, sD1E>(sb, tmem_base, bar0, rs, G::D1E_A, G::D1E_A + G::D1E_B, 1u);
+      wait_epi(3);                                   // U2 staged
+      mma_seg<C, BF16, sD2>(sb, tmem_base, bar0, rs, 0, 15 * 2 * G::NKB1, 0u);
+      commit(3);
+      mma_seg<C, BF16, sD1E>(sb, tmem_base, bar0, rs, G::D1E_A + G::D1E_B, G::D1E_STEPS, 1u);
+      wait_epi(4);                                   // U1 staged, region B drained
+      if (has_next) {
+        wait_epi(0);                                 // next group's X0 staged
+        mma_seg<C, BF16, sE1>(sb, tmem_base, bar0, rs, 0, P.e1_steps, 0u);
+        commit(0);
+      }
+      mma_seg<C, BF16, sD1U>(sb, tmem_base, bar0, rs, 0, 25 * G::NKB1, 1u);
+      commit(4);
+      first = false;
     }
   } else {
     // ===================== epilogue warps (128 threads): thread = accumulator row
     const int q = warp & 3, et = tid - 64;
-    uint32_t acc_phase = 0;
+    uint32_t pa[5] = {0, 0, 0, 0, 0};
+    auto wait_acc = [&](int k) { mbar_wait(accum_bar(k), pa[k]); pa[k] ^= 1u; tc_fence_after_sync(); };
+    auto done = [&](int k) { fence_proxy_async_smem(); tc_fence_before_sync(); mbar_arrive(epi_bar(k)); };
     bool first = true;
-    for (int g = blockIdx.x; g < n_groups; g += gridDim.x) {
+    for (int g = blockIdx.x; g < n_groups; g += stride) {
       const long long g0 = (long long)g * G::T;
       const int n_valid = (int)min((long long)G::T, (long long)n_int - g0);
+      const bool has_next = g + stride < n_groups;
+      const long long gn0 = (long long)(g + stride) * G::T;
+      const int n_valid_next = has_next ? (int)min((long long)G::T, (long long)n_int - gn0) : 0;
+      float* pg = probs + g0 * kBins;
       if (first) {
         load_x0<C, BF16>(sb, hist, g0, n_valid, split_e1, et);
-        fence_proxy_async_smem();
-        mbar_arrive(epi_bar);
+        done(0);
+        wait_acc(0);
+        for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kE1>(sb, tmem_base, t, q, lane, par, n_valid, pg);
+        done(1);
         first = false;
       }
-      float* pg = probs + g0 * kBins;
-#pragma unroll 1
-      for (int l = 0; l < 5; ++l) {
-        if (l == 4) {
-          // the next group's input is staged while this group's d1 MMAs run (X0 is dead after e1)
-          const int gn = g + gridDim.x;
-          if (gn < n_groups) {
-            const long long gn0 = (long long)gn * G::T;
-            load_x0<C, BF16>(sb, hist, gn0, (int)min((long long)G::T, (long long)n_int - gn0), split_e1, et);
-          }
-        }
-        mbar_wait(accum_bar, acc_phase);
-        acc_phase ^= 1u;
-        tc_fence_after_sync();
-        if (l == 0) { for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kE1>(sb, tmem_acc, t, q, lane, par, n_valid, pg); }
-        else if (l == 1) { for (int t = 0; t < G::T / 2; ++t) epilogue_tile<C, BF16, kE2>(sb, tmem_acc, t, q, lane, par, n_valid, pg); }
-        else if (l == 2) { for (int t = 0; t < (G::T + 3) / 4; ++t) epilogue_tile<C, BF16, kB>(sb, tmem_acc, t, q, lane, par, n_valid, pg); }
-        else if (l == 3) { for (int t = 0; t < G::T / 2; ++t) epilogue_tile<C, BF16, kD2>(sb, tmem_acc, t, q, lane, par, n_valid, pg); }
-        else { for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kD1>(sb, tmem_acc, t, q, lane, par, n_valid, pg); }
-        fence_proxy_async_smem();
-        tc_fence_before_sync();
-        mbar_arrive(epi_bar);
+      wait_acc(1);
+      for (int t = 0; t < G::T / 2; ++t) epilogue_tile<C, BF16, kE2>(sb, tmem_base, t, q, lane, par, n_valid, pg);
+      done(2);
+      if (has_next) {                                // P1 is dead (e2's MMAs retired): stage the next input
+        load_x0<C, BF16>(sb, hist, gn0, n_valid_next, split_e1, et);
+        done(0);
       }
+      wait_acc(2);
+      for (int t = 0; t < (G::T + 3) / 4; ++t) epilogue_tile<C, BF16, kB>(sb, tmem_base, t, q, lane, par, n_valid, pg);
+      done(3);
+      wait_acc(3);
+      for (int t = 0; t < G::T / 2; ++t) epilogue_tile<C, BF16, kD2>(sb, tmem_base, t, q, lane, par, n_valid, pg);
+      done(4);
+      if (has_next) {
+        wait_acc(0);
+        for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kE1>(sb, tmem_base, t, q, lane, par, n_valid_next, pg);
+        done(1);
+      }
+      wait_acc(4);
+      for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kD1>(sb, tmem_base, t, q, lane, par, n_valid, pg);
+      done(5);
     }
   }
   tc_fence_before_sync();
   __syncthreads();
   if (warp == 1) {
     __syncwarp();
-    tmem_dealloc(tmem_acc, G::TMEM_COLS);
+    tmem_dealloc(tmem_base, G::TMEM_COLS);
   }
 }
 
@@ -476,42 +549,49 @@ uint16_t bf16_rne(float v) {
   return (uint16_t)(u >> 16);
 }
 
+// Packs PyTorch-layout conv weights [C_out][C_in][K] into the image the kernel streams: a 2 KB header
+// (biases [5][C], head weight [C], head bias) and, per segment in streaming order, per MMA step, the
+// B operand [2 chunks][C out][16 B of input channels], operand-rounded (TF32: RN ties away; BF16: RNE).
 template <int C, bool BF16>
 void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst) {
   using G = Geo<C, BF16>;
-  const LayerPlan P = make_plan<C, BF16>(split_e1);
+  const Plan P = make_plan<C, BF16>(split_e1);
   memset(dst, 0, P.total);
   float* hdr = reinterpret_cast<float*>(dst);
   for (int l = 0; l < 5; ++l) memcpy(hdr + l * C, w->conv_b[l], sizeof(float) * C);
   memcpy(hdr + 5 * C, w->conv_w[5], sizeof(float) * C);
   hdr[6 * C] = w->conv_b[5][0];
-  const int cin[5] = {kHistCh, C, C, 2 * C, 2 * C};
-  for (int l = 0; l < 5; ++l) {
-    const int K = taps_of(l);
-    const float* W = w->conv_w[l];          // [C][cin][K]
-    for (int j = 0; j < K; ++j)
-      for (int kk = 0; kk < P.nkb[l]; ++kk) {
-        // step order inside a layer: [tap][K block]; the e1 split runs [pass][tap] (pass = K block)
-        const size_t step_idx = (l == 0) ? (size_t)kk * K + j : (size_t)j * P.nkb[l] + kk;
-        unsigned char* step = dst + P.w_off[l] + step_idx * G::STEP_BYTES;
-        for (int h = 0; h < 2; ++h)
-          for (int n = 0; n < C; ++n)
-            for (int e = 0; e < G::PER; ++e) {
-              int ci = (2 * kk + h) * G::PER + e;
-              int pass = 0;                  // e1 split: k block 0 and 1 carry W_hi, k block 2 carries W_lo
-              if (l == 0 && P.nkb[0] == 3) { ci = h * G::PER + e; pass = kk; }
-              float v = ci < cin[l] ? W[((size_t)n * cin[l] + ci) * K + j] : 0.0f;
-              unsigned char* p = step + ((size_t)h * C + n) * 16 + e * G::ES;
-              if (BF16) {
-                const uint16_t b = bf16_rne(v);
-                memcpy(p, &b, 2);
-              } else {
-                const float hi = tf32_rna(v);
-                const float out = (pass == 2) ? tf32_rna(v - hi) : hi;
-                memcpy(p, &out, 4);
-              }
+  struct SegDef { int seg, layer, cin, taps, nkb, ch_base, f0; };
+  const int A = G::D1E_A, B = G::D1E_B, N1 = G::NKB1;
+  const SegDef defs[kSegs] = {
+      {gE2, 1, C, 15, N1, 0, 0},        {gD1Ea, 4, 2 * C, 25, N1, C, 0},     {gB, 2, C, 5, N1, 0, 0},
+      {gD1Eb, 4, 2 * C, 25, N1, C, A},  {gD2, 3, 2 * C, 15, 2 * N1, 0, 0},   {gD1Ec, 4, 2 * C, 25, N1, C, A + B},
+      {gE1, 0, kHistCh, 25, 1, 0, 0},   {gD1U, 4, 2 * C, 25, N1, 0, 0}};
+  for (const SegDef& d : defs) {
+    const float* W = w->conv_w[d.layer];          // [C][cin][taps]
+    for (int s = 0; s < P.seg_steps[d.seg]; ++s) {
+      const int f = d.f0 + s;                     // step index inside the sub-layer
+      int j, kk, pass = 0;
+      if (d.seg == gE1) { pass = f / 25; j = f % 25; kk = 0; }     // e1 split runs [pass][tap]
+      else { j = f / d.nkb; kk = f % d.nkb; }
+      unsigned char* step = dst + P.seg_off[d.seg] + (size_t)s * G::STEP_BYTES;
+      for (int h = 0; h < 2; ++h)
+        for (int n = 0; n < C; ++n)
+          for (int e = 0; e < G::PER; ++e) {
+            const int cl = (2 * kk + h) * G::PER + e;            // channel inside the sub-layer's range
+            const bool real = (d.seg == gE1) ? cl < kHistCh : true;
+            const float v = real ? W[((size_t)n * d.cin + d.ch_base + cl) * d.taps + j] : 0.0f;
+            unsigned char* p = step + ((size_t)h * C + n) * 16 + e * G::ES;
+            if (BF16) {
+              const uint16_t b = bf16_rne(v);
+              memcpy(p, &b, 2);
+            } else {
+              const float hi = tf32_rna(v);
+              const float out = (pass == 2) ? tf32_rna(v - hi) : hi;   // passes: A_hi W_hi, A_lo W_hi, A_hi W_lo
+              memcpy(p, &out, 4);
             }
-      }
+          }
+    }
   }
 }
 
