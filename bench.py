@@ -234,10 +234,10 @@ def main_ours(args, rank, world, local_rank):
         peak_note = (f"{peaks_src} bf16 sustained {peaks['bf16_tflops_sustained']} TFLOP/s"
                      + ("" if ratio == 1.0 else " x nominal tf32/bf16 ratio 1.1/2.25"))
     achieved = flop / unet_s / 1e12
-    traffic = None
+    traffic = None   # DRAM bytes per launch from the committed ncu --set full capture (per event x E)
     try:
-        with open(os.path.join(ROOT, "profiles", "roofline_traffic.json")) as f:
-            traffic = json.load(f).get(f"{args.precision}_c{args.channels}")
+        with open(os.path.join(ROOT, "profiles", "r01_roofline_traffic.json.txt")) as f:
+            traffic = json.load(f)[f"{args.precision}_c{args.channels}"]["bytes_per_event"] * E
     except Exception:
         pass
     hbm_bytes_fc = (ev.n_tracks * 36 + E * 40 * 800 * 4)
