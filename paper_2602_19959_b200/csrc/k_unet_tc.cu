@@ -38,7 +38,7 @@ using namespace umma;
 namespace {
 
 constexpr int kTcThreads = 192;
-constexpr int kStages = 5;
+constexpr int kMaxStages = 8;
 constexpr int kStageBytes = 8192;
 constexpr int kHeaderBytes = 2048;          // biases [5][C], head weight [C], head bias
 
@@ -57,7 +57,9 @@ struct Geo {
   static constexpr int NKB1 = C / KPM;               // MMA K blocks per tap over C channels
   static constexpr int T = (C == 64) ? (BF16 ? 4 : 2) : (BF16 ? 8 : 4);   // intervals per group
   static constexpr int LEAD1 = 16, LEAD2 = 8, LEAD3 = 8;
-  static constexpr int ROWS1 = 128 * T + 32, ROWS2 = 64 * T + 16, ROWS3 = 32 * T + 16;
+  // rows per chunk = lead halo + T interval slots; reads past the last slot (garbage output rows only)
+  // land in the following chunk / buffer, which is always inside the CTA's allocation
+  static constexpr int ROWS1 = LEAD1 + 128 * T, ROWS2 = LEAD2 + 64 * T, ROWS3 = LEAD3 + 32 * T;
   static constexpr int LBO1 = ROWS1 * 16, LBO2 = ROWS2 * 16, LBO3 = ROWS3 * 16;
   static constexpr int STEP_BYTES = 2 * C * 16;      // one MMA's B operand: [2 chunks][C][16 B]
   static constexpr int SPS = kStageBytes / STEP_BYTES;   // MMA steps per ring stage
@@ -69,7 +71,9 @@ struct Geo {
   static constexpr int OFF_XP = OFF_R + SZ_L1;       // overlay: X0 (input) then P1 = pool(e1)
   static constexpr int SZ_XP = (XCH * LBO1 > SZ_L2) ? XCH * LBO1 : SZ_L2;
   static constexpr int OFF_RING = OFF_XP + SZ_XP;
-  static constexpr int OFF_PAR = OFF_RING + kStages * kStageBytes;   // biases + head (floats)
+  static constexpr int STAGES_FIT = (227 * 1024 - kHeaderBytes - 256 - OFF_RING) / kStageBytes;
+  static constexpr int STAGES = STAGES_FIT < kMaxStages ? STAGES_FIT : kMaxStages;   // weight ring depth
+  static constexpr int OFF_PAR = OFF_RING + STAGES * kStageBytes;   // biases + head (floats)
   static constexpr int OFF_BAR = OFF_PAR + kHeaderBytes;
   static constexpr int SMEM = OFF_BAR + 256;
   // TMEM columns: region A = [0, T*C) (d1), region B = [T*C, 2*T*C) (e1; e2, b, d2 use its head)
@@ -82,7 +86,7 @@ struct Geo {
   static constexpr int D1E_B = (D1E_STEPS - D1E_A) < 16 ? (D1E_STEPS - D1E_A) : 16;
   static constexpr int D1E_C = D1E_STEPS - D1E_A - D1E_B;
   static_assert(2 * SZ_L2 == SZ_L1, "E2 + U2 must tile the overlay region exactly");
-  static_assert(SMEM <= 227 * 1024, "shared memory budget");
+  static_assert(SMEM <= 227 * 1024 && STAGES >= 4, "shared memory budget");
   static_assert(2 * T * C <= 512, "TMEM budget");
   static_assert(NCH % 2 == 0 && T % 2 == 0, "whole MMA K blocks per source; level-2 tiles whole");
   static_assert(16 % SPS == 0, "d1E parts must start on ring-stage boundaries");
@@ -227,9 +231,12 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
 #pragma unroll
       for (int i = 0; i < 16; ++i) pv[i] = fmaxf(v[i], __shfl_xor_sync(0xffffffffu, v[i], 1));
       if ((lane & 1) == 0) store_row16<BF16>(dst_aux, lbo_aux, c0, pv);
-    } else if (exists) {          // kB, kD2: nearest upsample = the same chunk into rows 2m and 2m + 1
-      store_row16<BF16>(dst_full, lbo_full, c0, v);
-      store_row16<BF16>(dst_full + 16u, lbo_full, c0, v);
+    } else if (exists) {          // kB, kD2: nearest upsample = the same chunk into rows 2m and 2m + 1;
+      // groups of four lanes alternate which of the two rows goes first, so that one store instruction
+      // covers all eight 16-byte slots of every 128-byte line evenly (no bank conflicts)
+      const uint32_t swz = (uint32_t)((m >> 2) & 1) * 16u;
+      store_row16<BF16>(dst_full + swz, lbo_full, c0, v);
+      store_row16<BF16>(dst_full + (16u - swz), lbo_full, c0, v);
     }
   }
   if (MODE == kD1) {
@@ -370,10 +377,10 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
             mma_lh<BF16>(dcol + (uint32_t)(t * C), a + 128u * t, hi, b, hi, idesc, acc);
         }
       }
-      mma_commit(bar0 + 8u * (kStages + rs.ring));      // frees the ring slot when these MMAs retire
+      mma_commit(bar0 + 8u * (G::STAGES + rs.ring));      // frees the ring slot when these MMAs retire
     }
     __syncwarp();
-    if (++rs.ring == kStages) { rs.ring = 0; rs.phase ^= 1u; }
+    if (++rs.ring == G::STAGES) { rs.ring = 0; rs.phase ^= 1u; }
   }
 }
 
@@ -390,17 +397,17 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
   // mbarriers: full[s], empty[s] per ring stage; accum[k] = "MMAs of layer k retired" (k: e1 e2 b d2 d1);
   // epi[k] = "epilogue k done" (k: x0-staged e1 e2 b d2 d1)
   const uint32_t bar0 = sb + G::OFF_BAR;
-  auto accum_bar = [&](int k) { return bar0 + 8u * (2 * kStages + k); };
-  auto epi_bar = [&](int k) { return bar0 + 8u * (2 * kStages + 5 + k); };
-  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + G::OFF_BAR + 8 * (2 * kStages + 11));
-  static_assert(8 * (2 * kStages + 11) + 4 <= 256, "barrier block");
+  auto accum_bar = [&](int k) { return bar0 + 8u * (2 * G::STAGES + k); };
+  auto epi_bar = [&](int k) { return bar0 + 8u * (2 * G::STAGES + 5 + k); };
+  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + G::OFF_BAR + 8 * (2 * G::STAGES + 11));
+  static_assert(8 * (2 * G::STAGES + 11) + 4 <= 256, "barrier block");
   const Plan P = make_plan<C, BF16>(split_e1);
 
   // ---- one-time setup: zero the activation buffers (gap / halo rows must be zero), parameters, barriers
   for (int i = tid; i < G::OFF_RING / 16; i += kTcThreads) reinterpret_cast<uint4*>(smem)[i] = make_uint4(0, 0, 0, 0);
   for (int i = tid; i < 6 * C + 1; i += kTcThreads) par[i] = reinterpret_cast<const float*>(wpack)[i];
   if (tid == 0) {
-    for (int s = 0; s < kStages; ++s) { mbar_init(bar0 + 8u * s, 1); mbar_init(bar0 + 8u * (kStages + s), 1); }
+    for (int s = 0; s < G::STAGES; ++s) { mbar_init(bar0 + 8u * s, 1); mbar_init(bar0 + 8u * (G::STAGES + s), 1); }
     for (int k = 0; k < 5; ++k) mbar_init(accum_bar(k), 1);
     for (int k = 0; k < 6; ++k) mbar_init(epi_bar(k), 128);
     fence_mbar_init();
@@ -424,11 +431,11 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
         const int steps = P.seg_steps[seg];
         for (int f = 0; f < steps; f += G::SPS) {
           const int n = min(G::SPS, steps - f);
-          mbar_wait(bar0 + 8u * (kStages + rs.ring), rs.phase ^ 1u);
+          mbar_wait(bar0 + 8u * (G::STAGES + rs.ring), rs.phase ^ 1u);
           mbar_arrive_expect_tx(bar0 + 8u * rs.ring, (uint32_t)(n * G::STEP_BYTES));
           bulk_g2s(sb + G::OFF_RING + rs.ring * kStageBytes, src + (size_t)f * G::STEP_BYTES,
                    (uint32_t)(n * G::STEP_BYTES), bar0 + 8u * rs.ring);
-          if (++rs.ring == kStages) { rs.ring = 0; rs.phase ^= 1u; }
+          if (++rs.ring == G::STAGES) { rs.ring = 0; rs.phase ^= 1u; }
         }
       };
       bool first = true;
