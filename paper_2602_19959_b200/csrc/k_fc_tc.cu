@@ -1,0 +1,388 @@
+// a1 + a2, tensor-core version -- per-track fully connected network with the 25 -> 800 output layer on
+// tcgen05 (FP32-accurate: 3-pass TF32 hi/lo split) and the deterministic segmented sum into the
+// interval histograms H[n_events, 40, 8, 100] done by the epilogue straight out of TMEM.
+//
+// PAPER.md:29 "six FC layers ... combining each track's contribution into a 800-bin histogram (8
+// channels each with 100-bin)"; BASELINE.json config 0 (9->25->25->25->25->25->800, LeakyReLU(0.01),
+// softplus) and north_star (a)/(b): MMA for the FC, tracks sorted by interval and summed in a fixed
+// order, no float atomics.  DESIGN.md section 4.2.
+//
+// Mapping.  The last layer is 88 % of the FC FLOPs.  Per tile of up to 128 sorted tracks of one event
+//     D[o, t] = sum_k W5x[o, k] * hx[t, k],   k < 25: weights x activations, k = 25: bias x 1, K = 32
+// with M = 128 rows = the 100 bins of ONE histogram channel (+28 zero rows), N = 128 tracks.  So an
+// accumulator lane is one output bin and an accumulator column is one track: the epilogue thread that
+// owns lane l walks the columns in sorted-track order, adds softplus(D) into one FP32 register and
+// stores it to H whenever the interval changes -- the same fixed-order sum as k_fc_hist, with no
+// cross-lane reduction and every H element written exactly once (zeros for empty intervals).
+// FP32 accuracy: W5x = W_hi + W_lo and hx = h_hi + h_lo (each part RN-rounded to TF32), three MMAs
+// W_hi h_hi + W_hi h_lo + W_lo h_hi accumulate in FP32 in TMEM (the dropped term is ~2^-22 relative).
+// A CTA serves one half of the outputs (blockIdx.y: channels 0-3 or 4-7; 128 KB of W5x hi+lo resident
+// in shared memory) for a strided subset of the events.  Roles: warps 0-7 epilogue, warp 8 MMA
+// issuer, warps 9-16 = two groups of 128 threads that run the five 25-wide hidden layers (FP32 FMA,
+// thread = track) for alternating tiles and stage h_hi / h_lo as the B operand (double buffered).
+#include <cstring>
+
+#include "pvf_internal.cuh"
+#include "umma.cuh"
+
+namespace pvf {
+using namespace umma;
+
+namespace {
+
+constexpr int kFtThreads = 17 * 32;           // 8 epilogue + 1 MMA + 8 hidden-layer warps
+constexpr int kTile = 128;                   // tracks per tile (MMA N)
+constexpr int kRowsW = 512;                  // 4 channel tiles x 128 rows per CTA half
+constexpr int kLboW = kRowsW * 16;           // 8192: next 16-byte K chunk of the A operand
+constexpr int kLboH = kTile * 16;            // 2048: next 16-byte K chunk of the B operand
+constexpr int kWPart = 8 * kLboW;            // 65536 bytes: one part (hi or lo) of W5x for one half
+constexpr int kHPart = 8 * kLboH;            // 16384 bytes: one part of hx for one tile
+constexpr int kHStride = 28, kWRow = 28;
+
+struct FtSmall {                             // the five hidden layers, zero padded
+  float w0[kFcHidden][12];
+  float b0[28];
+  float wh[4][kFcHidden][kWRow];
+  float bh[4][28];
+};
+
+constexpr int OFF_W = 0;                               // [hi | lo][8 chunks][512 rows][16 B]
+constexpr int OFF_H = OFF_W + 2 * kWPart;              // [buf 0 | 1][hi | lo][8 chunks][128 tracks][16 B]
+constexpr int OFF_SMALL = OFF_H + 4 * kHPart;
+constexpr int OFF_IV = OFF_SMALL + ((int)sizeof(FtSmall) + 127) / 128 * 128;   // int [2][128]
+constexpr int OFF_BARS = OFF_IV + 2 * kTile * 4;
+constexpr int FT_SMEM = OFF_BARS + 128;
+static_assert(FT_SMEM <= 227 * 1024, "shared memory budget");
+// barriers (8 bytes each): h_full[2], h_empty[2], meta_empty[2], acc_full[4], acc_empty[4], then the TMEM slot
+enum { bHFull = 0, bHEmpty = 2, bMeta = 4, bAccFull = 6, bAccEmpty = 10, bSlot = 14 };
+
+__device__ __forceinline__ float leaky_ft(float v) { return v >= 0.0f ? v : kLeaky * v; }
+__device__ __forceinline__ uint32_t tf32_of(float v) {
+  uint32_t r;
+  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(v));
+  return r;
+}
+__device__ __forceinline__ void st16(uint32_t addr, uint4 v) {
+  asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+// softplus(v) = max(v,0) + log(1 + exp(-|v|)) on the SFU (see k_fc.cu)
+// Raw ex2 / lg2 (no range fix-ups needed: the ex2 argument is <= 0, the lg2 argument is in (1, 2]).
+__device__ __forceinline__ float softplus_ft(float v) {
+  const float t = fabsf(v) * -1.4426950408889634f;
+  float e, w;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(t));
+  const float u = 1.0f + e;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(w) : "f"(u));
+  return fmaf(w, 0.6931471805599453f, fmaxf(v, 0.0f));
+}
+
+struct Feat9 { const float* f[9]; };
+
+__global__ void __launch_bounds__(kFtThreads, 1)
+k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* __restrict__ perm,
+             const int32_t* __restrict__ seg_off, const int32_t* __restrict__ seg_cnt,
+             const float* __restrict__ par, const unsigned char* __restrict__ w5img, int n_events,
+             float* __restrict__ hist) {
+  extern __shared__ __align__(1024) unsigned char smem[];
+  const uint32_t sb = smem_u32(smem);
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+  const int half = blockIdx.y;
+  FtSmall& S = *reinterpret_cast<FtSmall*>(smem + OFF_SMALL);
+  int* s_iv = reinterpret_cast<int*>(smem + OFF_IV);
+  auto bar = [&](int k) { return sb + OFF_BARS + 8u * k; };
+  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + OFF_BARS + 8 * bSlot);
+
+  // ---- one-time setup: this half's W5x image, zeroed B buffers, the small layers, barriers, TMEM
+  {
+    const uint4* src = reinterpret_cast<const uint4*>(w5img + (size_t)half * 2 * kWPart);
+    uint4* dst = reinterpret_cast<uint4*>(smem + OFF_W);
+    for (int i = tid; i < 2 * kWPart / 16; i += kFtThreads) dst[i] = __ldg(src + i);
+    uint4* hz = reinterpret_cast<uint4*>(smem + OFF_H);
+    for (int i = tid; i < 4 * kHPart / 16; i += kFtThreads) hz[i] = make_uint4(0, 0, 0, 0);
+  }
+  for (int i = tid; i < kFcHidden * 12; i += kFtThreads) {
+    const int r = i / 12, c = i % 12;
+    S.w0[r][c] = c < kFcIn ? par[kFcW0 + r * kFcIn + c] : 0.0f;
+  }
+  for (int i = tid; i < 28; i += kFtThreads) S.b0[i] = i < kFcHidden ? par[kFcB0 + i] : 0.0f;
+  for (int i = tid; i < 4 * kFcHidden * kWRow; i += kFtThreads) {
+    const int l = i / (kFcHidden * kWRow), r = (i / kWRow) % kFcHidden, c = i % kWRow;
+    S.wh[l][r][c] = c < kFcHidden ? par[kFcHid + l * kFcHidStride + r * kFcHidden + c] : 0.0f;
+  }
+  for (int i = tid; i < 4 * 28; i += kFtThreads) {
+    const int l = i / 28, c = i % 28;
+    S.bh[l][c] = c < kFcHidden ? par[kFcHid + l * kFcHidStride + kFcHidden * kFcHidden + c] : 0.0f;
+  }
+  if (tid == 0) {
+    for (int k = 0; k < 2; ++k) { mbar_init(bar(bHFull + k), 128); mbar_init(bar(bHEmpty + k), 1); mbar_init(bar(bMeta + k), 256); }
+    for (int k = 0; k < 4; ++k) { mbar_init(bar(bAccFull + k), 1); mbar_init(bar(bAccEmpty + k), 128); }
+    fence_mbar_init();
+  }
+  if (warp == 8) tmem_alloc(smem_u32(const_cast<uint32_t*>(tmem_slot)), 512);
+  fence_proxy_async_smem();
+  tc_fence_before_sync();
+  __syncthreads();
+  tc_fence_after_sync();
+  const uint32_t tmem_base = *tmem_slot;
+
+  // kept (in-range) tracks of event e and the start of its run in perm
+  auto kept_of = [&](int e, int& ev_lo) {
+    ev_lo = event_offsets[e];
+    const size_t s = (size_t)e * kIntervals + kIntervals - 1;
+    return seg_off[s] + seg_cnt[s] - ev_lo;
+  };
+
+  if (warp < 8) {
+    // ===================== epilogue: lane = output bin, column = track (sorted order).  Warps 0-3 own
+    // channel tiles 0 and 1, warps 4-7 tiles 2 and 3 (two warps per scheduler hide each other's latency).
+    const int q = warp & 3, mh = warp >> 2;
+    const int r = 32 * q + lane;
+    const bool valid = r < kBins;
+    int it = 0;
+    for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
+      int ev_lo;
+      const int nk = kept_of(e, ev_lo);
+      float* He = hist + (size_t)e * kIntervals * kFcOut + (4 * half + 2 * mh) * kBins + r;   // + iv*800 + mm*100
+      float acc[2] = {0.f, 0.f};
+      int cur[2] = {0, 0};
+      for (int base = 0; base < nk; base += kTile, ++it) {
+        const int buf = it & 1, ntile = min(kTile, nk - base);
+        const bool last = base + kTile >= nk;
+        mbar_wait(bar(bHFull + buf), (uint32_t)((it >> 1) & 1));      // s_iv[buf] is staged
+        const int* ivs = s_iv + buf * kTile;
+#pragma unroll
+        for (int mm = 0; mm < 2; ++mm) {
+          const int mt = 2 * mh + mm;
+          mbar_wait(bar(bAccFull + mt), (uint32_t)(it & 1));
+          tc_fence_after_sync();
+          const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)(mt * kTile);
+          float* Hc = He + mm * kBins;
+          float a = acc[mm];
+          int c = cur[mm];
+          for (int c0 = 0; c0 < ntile; c0 += 16) {
+            uint32_t v[16];
+            tmem_ld_x16(taddr + (uint32_t)c0, v);
+            // intervals of the 16 tracks (broadcast 16-byte loads) while the TMEM load is in flight
+            int ivv[16];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+              const int4 q4 = *reinterpret_cast<const int4*>(ivs + c0 + 4 * k);
+              ivv[4 * k + 0] = q4.x; ivv[4 * k + 1] = q4.y; ivv[4 * k + 2] = q4.z; ivv[4 * k + 3] = q4.w;
+            }
+            tmem_ld_wait();
+            // all 16 softplus first: independent, so the SFU pipeline stays full; columns past the
+            // tile's last track are computed on stale accumulators and then ignored
+            float sp[16];
+#pragma unroll
+            for (int i = 0; i < 16; ++i) sp[i] = softplus_ft(__uint_as_float(v[i]));
+            const int nv = ntile - c0;
+            if (nv >= 16) {
+#pragma unroll
+              for (int i = 0; i < 16; ++i) {
+                if (ivv[i] != c) {           // interval finished: flush (zeros for skipped empty intervals)
+#pragma unroll 1
+                  while (c < ivv[i]) {
+                    if (valid) Hc[c * kFcOut] = a;
+                    a = 0.0f;
+                    ++c;
+                  }
+                }
+                a += sp[i];
+              }
+            } else {
+#pragma unroll 1
+              for (int i = 0; i < nv; ++i) {
+                const int ivt = ivs[c0 + i];
+#pragma unroll 1
+                while (c < ivt) {
+                  if (valid) Hc[c * kFcOut] = a;
+                  a = 0.0f;
+                  ++c;
+                }
+                // sp[] is indexed dynamically here only through this select chain (tail chunk, rare)
+                float x = sp[0];
+#pragma unroll
+                for (int k = 1; k < 16; ++k) x = (i == k) ? sp[k] : x;
+                a += x;
+              }
+            }
+          }
+          if (last) {
+#pragma unroll 1
+            while (c < kIntervals) {
+              if (valid) Hc[c * kFcOut] = a;
+              a = 0.0f;
+              ++c;
+            }
+          }
+          acc[mm] = a;
+          cur[mm] = c;
+          tc_fence_before_sync();
+          mbar_arrive(bar(bAccEmpty + mt));
+        }
+        mbar_arrive(bar(bMeta + buf));
+      }
+      if (nk <= 0 && valid) {                // event without kept tracks: all of its histograms are zero
+        for (int c = 0; c < kIntervals; ++c)
+#pragma unroll
+          for (int mm = 0; mm < 2; ++mm) He[c * kFcOut + mm * kBins] = 0.0f;
+      }
+    }
+  } else if (warp == 8) {
+    // ===================== MMA issuer
+    constexpr uint32_t idesc = instr_desc(kFmtTF32, 128, kTile);
+    constexpr uint32_t hi = (128u >> 4) | (1u << 14);
+    constexpr uint32_t a_lbo = (uint32_t)(kLboW >> 4) << 16, b_lbo = (uint32_t)(kLboH >> 4) << 16;
+    int it = 0;
+    for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
+      int ev_lo;
+      const int nk = kept_of(e, ev_lo);
+      for (int base = 0; base < nk; base += kTile, ++it) {
+        const int buf = it & 1;
+        mbar_wait(bar(bHFull + buf), (uint32_t)((it >> 1) & 1));
+        tc_fence_after_sync();
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt) {
+          mbar_wait(bar(bAccEmpty + mt), (uint32_t)((it & 1) ^ 1));
+          tc_fence_after_sync();
+          if (elect_one()) {
+#pragma unroll
+            for (int pass = 0; pass < 3; ++pass) {       // W_hi h_hi, W_hi h_lo, W_lo h_hi
+#pragma unroll
+              for (int s = 0; s < 4; ++s) {
+                const uint32_t a = a_lbo + ((sb + OFF_W + (pass == 2 ? kWPart : 0) + mt * 2048 + s * 2 * kLboW) >> 4);
+                const uint32_t b = b_lbo + ((sb + OFF_H + buf * 2 * kHPart + (pass == 1 ? kHPart : 0) + s * 2 * kLboH) >> 4);
+                mma_tf32_lh(tmem_base + (uint32_t)(mt * kTile), a, hi, b, hi, idesc, (pass | s) ? 1u : 0u);
+              }
+            }
+            mma_commit(bar(bAccFull + mt));
+            if (mt == 3) mma_commit(bar(bHEmpty + buf));
+          }
+          __syncwarp();
+        }
+      }
+    }
+  } else {
+    // ===================== hidden layers: two groups of 128 threads, thread = track, alternating tiles
+    const int g = (warp - 9) >> 2, i = tid - 288 - 128 * g;
+    const uint32_t hbase = sb + OFF_H + (uint32_t)g * 2 * kHPart + (uint32_t)i * 16u;
+    int it = 0;
+    for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
+      int ev_lo;
+      const int nk = kept_of(e, ev_lo);
+      for (int base = 0; base < nk; base += kTile, ++it) {
+        if ((it & 1) != g) continue;
+        const uint32_t prev = (uint32_t)(((it >> 1) & 1) ^ 1);
+        mbar_wait(bar(bHEmpty + g), prev);         // the MMAs that read this buffer have retired
+        mbar_wait(bar(bMeta + g), prev);           // the epilogue is done with s_iv[g]
+        if (base + i < nk) {
+          const int t = perm[ev_lo + base + i];
+          float zrel;
+          bool nf;
+          const int iv = interval_of(F.f[0][t], zrel, nf);
+          s_iv[g * kTile + i] = iv;
+          const float x[kFcIn] = {zrel, F.f[1][t], F.f[2][t], F.f[3][t], F.f[4][t], F.f[5][t], F.f[6][t], F.f[7][t], F.f[8][t]};
+          float h[32], gg[28];
+#pragma unroll
+          for (int o = 0; o < kFcHidden; ++o) {
+            float a = S.b0[o];
+#pragma unroll
+            for (int k = 0; k < kFcIn; ++k) a = fmaf(S.w0[o][k], x[k], a);
+            h[o] = leaky_ft(a);
+          }
+#pragma unroll
+          for (int l = 0; l < 4; ++l) {
+#pragma unroll
+            for (int o = 0; o < kFcHidden; ++o) {
+              float a = S.bh[l][o];
+              const float4* wr = reinterpret_cast<const float4*>(S.wh[l][o]);
+#pragma unroll
+              for (int q = 0; q < 7; ++q) {
+                const float4 w = wr[q];
+                a = fmaf(w.x, h[4 * q], a);
+                if (4 * q + 1 < kFcHidden) a = fmaf(w.y, h[4 * q + 1], a);
+                if (4 * q + 2 < kFcHidden) a = fmaf(w.z, h[4 * q + 2], a);
+                if (4 * q + 3 < kFcHidden) a = fmaf(w.w, h[4 * q + 3], a);
+              }
+              gg[o] = leaky_ft(a);
+            }
+#pragma unroll
+            for (int o = 0; o < kFcHidden; ++o) h[o] = gg[o];
+          }
+          h[25] = 1.0f;                              // multiplies the bias column of W5x
+#pragma unroll
+          for (int k = 26; k < 32; ++k) h[k] = 0.0f;
+#pragma unroll
+          for (int c = 0; c < 8; ++c) {
+            uint4 vh, vl;
+            vh.x = tf32_of(h[4 * c + 0]); vh.y = tf32_of(h[4 * c + 1]);
+            vh.z = tf32_of(h[4 * c + 2]); vh.w = tf32_of(h[4 * c + 3]);
+            vl.x = tf32_of(h[4 * c + 0] - __uint_as_float(vh.x)); vl.y = tf32_of(h[4 * c + 1] - __uint_as_float(vh.y));
+            vl.z = tf32_of(h[4 * c + 2] - __uint_as_float(vh.z)); vl.w = tf32_of(h[4 * c + 3] - __uint_as_float(vh.w));
+            st16(hbase + (uint32_t)c * kLboH, vh);
+            st16(hbase + kHPart + (uint32_t)c * kLboH, vl);
+          }
+        }
+        fence_proxy_async_smem();
+        mbar_arrive(bar(bHFull + g));
+      }
+    }
+  }
+  tc_fence_before_sync();
+  __syncthreads();
+  if (warp == 8) {
+    __syncwarp();
+    tmem_dealloc(tmem_base, 512);
+  }
+}
+
+float tf32_rna_h(float v) {
+  uint32_t u;
+  memcpy(&u, &v, 4);
+  if ((u & 0x7f800000u) == 0x7f800000u) return v;
+  u = (u + 0x1000u) & 0xffffe000u;
+  float r;
+  memcpy(&r, &u, 4);
+  return r;
+}
+
+}  // namespace
+
+size_t fc_tc_packed_bytes() { return (size_t)2 * 2 * kWPart; }      // 2 halves x (hi | lo)
+
+// W5 [800][25] and b5 [800] (PyTorch layouts) -> per half [hi | lo][8 K chunks][512 rows][4 floats];
+// row 128*mt + r holds output (4*half + mt)*100 + r for r < 100 (zero rows otherwise); K index 25 = bias.
+void fc_tc_pack(const float* w5, const float* b5, void* host_dst) {
+  float* dst = static_cast<float*>(host_dst);
+  memset(dst, 0, fc_tc_packed_bytes());
+  for (int half = 0; half < 2; ++half)
+    for (int mt = 0; mt < 4; ++mt)
+      for (int r = 0; r < kBins; ++r) {
+        const int o = (4 * half + mt) * kBins + r, row = 128 * mt + r;
+        for (int k = 0; k <= kFcHidden; ++k) {
+          const float v = k < kFcHidden ? w5[o * kFcHidden + k] : b5[o];
+          const float hi = tf32_rna_h(v), lo = tf32_rna_h(v - hi);
+          const size_t idx = ((size_t)(k / 4) * kRowsW + row) * 4 + (k % 4);
+          dst[(size_t)half * 2 * (kWPart / 4) + idx] = hi;
+          dst[(size_t)half * 2 * (kWPart / 4) + kWPart / 4 + idx] = lo;
+        }
+      }
+}
+
+cudaError_t fc_tc_setup() {
+  return cudaFuncSetAttribute(k_fc_hist_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM);
+}
+
+void launch_fc_hist_tc(const float* const feat[9], const int32_t* event_offsets, const int32_t* perm,
+                       const int32_t* seg_off, const int32_t* seg_cnt, const float* fc_params, const void* w5img,
+                       int n_events, float* hist, int sm_count, cudaStream_t s) {
+  if (n_events <= 0) return;
+  Feat9 F;
+  for (int k = 0; k < 9; ++k) F.f[k] = feat[k];
+  const int gx = n_events < sm_count / 2 ? n_events : sm_count / 2;
+  k_fc_hist_tc<<<dim3(gx, 2), kFtThreads, FT_SMEM, s>>>(F, event_offsets, perm, seg_off, seg_cnt, fc_params,
+                                                        static_cast<const unsigned char*>(w5img), n_events, hist);
+}
+
+}  // namespace pvf

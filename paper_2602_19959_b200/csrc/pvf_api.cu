@@ -25,6 +25,7 @@ struct pvf_ctx {
   float* conv_f32 = nullptr;      // PyTorch-layout conv params (FP32 path + head of every path)
   UnetParamsF32 conv_ptrs{};
   void* tc_packed = nullptr;
+  void* fc_w5img = nullptr;       // tcgen05 image of the 25 -> 800 layer (TF32 / BF16 modes)
   int32_t* perm = nullptr;
   int32_t* seg_off = nullptr;
   int32_t* seg_cnt = nullptr;
@@ -51,7 +52,7 @@ namespace {
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 struct Layout {
-  size_t fc_params, conv_f32, tc_packed, perm, seg_off, seg_cnt, flags, hist;
+  size_t fc_params, conv_f32, tc_packed, fc_w5img, perm, seg_off, seg_cnt, flags, hist;
   size_t st_feat, st_off, st_probs, st_z, st_prob, st_bin, st_count, st_flags, total;
   size_t conv_w_off[6], conv_b_off[6];  // float offsets inside conv_f32
 };
@@ -92,6 +93,7 @@ Layout make_layout(const pvf_config* c) {
   L.conv_f32 = take(sizeof(float) * f);
   L.tc_packed = take(c->precision == PVF_PREC_FP32 ? 0 : unet_tc_packed_bytes(c->unet_channels, c->precision, c->split_mask));
   const size_t E = (size_t)c->max_events, T = (size_t)c->max_tracks;
+  L.fc_w5img = take(c->precision == PVF_PREC_FP32 ? 0 : fc_tc_packed_bytes());
   L.perm = take(sizeof(int32_t) * T);
   L.seg_off = take(sizeof(int32_t) * E * kIntervals);
   L.seg_cnt = take(sizeof(int32_t) * E * kIntervals);
@@ -154,6 +156,7 @@ pvf_status create_impl(const pvf_weights* w, const pvf_config* cfg, void* dev_po
   h->fc_params = reinterpret_cast<float*>(B + L.fc_params);
   h->conv_f32 = reinterpret_cast<float*>(B + L.conv_f32);
   h->tc_packed = B + L.tc_packed;
+  h->fc_w5img = B + L.fc_w5img;
   h->perm = reinterpret_cast<int32_t*>(B + L.perm);
   h->seg_off = reinterpret_cast<int32_t*>(B + L.seg_off);
   h->seg_cnt = reinterpret_cast<int32_t*>(B + L.seg_cnt);
@@ -201,6 +204,12 @@ pvf_status create_impl(const pvf_weights* w, const pvf_config* cfg, void* dev_po
       unet_tc_pack(w, cfg->unet_channels, cfg->precision, cfg->split_mask, img.data());
       e = cudaMemcpy(h->tc_packed, img.data(), nb, cudaMemcpyHostToDevice);
       if (e == cudaSuccess) e = unet_tc_setup(cfg->unet_channels, cfg->precision, cfg->split_mask);
+      if (e == cudaSuccess) {
+        std::vector<unsigned char> fimg(fc_tc_packed_bytes());
+        fc_tc_pack(w->fc_w[5], w->fc_b[5], fimg.data());
+        e = cudaMemcpy(h->fc_w5img, fimg.data(), fimg.size(), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = fc_tc_setup();
+      }
     }
   }
   if (e == cudaSuccess && cfg->enable_stage_timing)
@@ -268,7 +277,11 @@ pvf_status pvf_run(pvf_handle h, const pvf_tracks* t, int32_t n_events, float* o
   if (timing) cudaEventRecord(ev[0], s);
   launch_sort(t->feat[0], t->event_offsets, n_events, h->perm, h->seg_off, h->seg_cnt, h->flags, s);
   if (timing) cudaEventRecord(ev[1], s);
-  launch_fc_hist(t->feat, t->event_offsets, h->perm, h->seg_off, h->seg_cnt, h->fc_params, n_events, h->hist, s);
+  if (h->cfg.precision == PVF_PREC_FP32)
+    launch_fc_hist(t->feat, t->event_offsets, h->perm, h->seg_off, h->seg_cnt, h->fc_params, n_events, h->hist, s);
+  else
+    launch_fc_hist_tc(t->feat, t->event_offsets, h->perm, h->seg_off, h->seg_cnt, h->fc_params, h->fc_w5img, n_events,
+                      h->hist, h->sm_count, s);
   if (timing) cudaEventRecord(ev[2], s);
   enqueue_unet(h, h->hist, n_events, out_probs, s);
   if (timing) cudaEventRecord(ev[3], s);

@@ -52,6 +52,14 @@ void launch_fc_hist(const float* const feat[9], const int32_t* event_offsets, co
                     int n_events, float* hist, cudaStream_t s);
 int fc_hist_launches(int n_events);
 
+// a1+a2, tensor-core version (k_fc_tc.cu): 25 -> 800 layer as 3-pass TF32 tcgen05 MMAs, sum in the epilogue
+size_t fc_tc_packed_bytes();
+void fc_tc_pack(const float* w5, const float* b5, void* host_dst);
+cudaError_t fc_tc_setup();
+void launch_fc_hist_tc(const float* const feat[9], const int32_t* event_offsets, const int32_t* perm,
+                       const int32_t* seg_off, const int32_t* seg_cnt, const float* fc_params, const void* w5img,
+                       int n_events, float* hist, int sm_count, cudaStream_t s);
+
 // a3, FP32 CUDA-core path (k_unet_simt.cu).  conv params: PyTorch layout, floats.
 struct UnetParamsF32 { const float* w[6]; const float* b[6]; };
 cudaError_t unet_simt_setup(int channels);

@@ -85,12 +85,14 @@ def test_peaks_bit_exact_on_identical_probabilities():
 
 
 # ------------------------------------------------------------------ a0 + a1 + a2: histogram
+# fp32 -> k_fc_hist (FP32 FMA); tf32 -> k_fc_hist_tc (tcgen05, 3-pass TF32 split): same tolerance for both
+@pytest.mark.parametrize("prec", ["fp32", "tf32"])
 @pytest.mark.parametrize("kind", ["rand", "peaky"])
-def test_histogram_parity_and_determinism(kind):
+def test_histogram_parity_and_determinism(kind, prec):
     ev = make_events("run3", 48, 1001)
     w = make_weights(kind, 1)
     ref = O.run(ev.feat, ev.event_offsets, w, want_hist=True)
-    pvf = _make(w, ev)
+    pvf = _make(w, ev, prec)
     probs, pk = _run(pvf, ev)
     H = torch.empty(ev.n_events, 40, 8, 100, device="cuda")
     s = torch.cuda.Stream()
@@ -118,7 +120,8 @@ def test_histogram_parity_and_determinism(kind):
     assert torch.allclose(H, H2, rtol=1e-5, atol=1e-5)
 
 
-def test_edge_events_empty_dropped_nonfinite_and_long():
+@pytest.mark.parametrize("prec", ["fp32", "tf32"])
+def test_edge_events_empty_dropped_nonfinite_and_long(prec):
     w = make_weights("rand", 3)
     base = make_events("pileup", 3, 9)
     long_n = 700                                                 # > 3 tiles of the FC kernel
@@ -142,7 +145,7 @@ def test_edge_events_empty_dropped_nonfinite_and_long():
     add(one)                                                     # event 4: single track in the last interval
     ev = type(base)(np.ascontiguousarray(np.concatenate(feats, axis=1)), np.array(offs, np.int32), [None] * 5)
     ref = O.run(ev.feat, ev.event_offsets, w, want_hist=True)
-    pvf = _make(w, ev)
+    pvf = _make(w, ev, prec)
     probs, pk = _run(pvf, ev)
     H = torch.empty(5, 40, 8, 100, device="cuda")
     s = torch.cuda.Stream()
@@ -154,7 +157,7 @@ def test_edge_events_empty_dropped_nonfinite_and_long():
     got = _np(pk)
     assert np.array_equal(got["flags"].astype(np.uint32), ref["flags"])
     assert got["flags"][1] & pkg.FLAG_TRACK_DROPPED and got["flags"][1] & pkg.FLAG_NONFINITE
-    assert np.max(np.abs(probs.cpu().numpy().astype(np.float64) - ref["probs"])) <= TOL["fp32"]
+    assert np.max(np.abs(probs.cpu().numpy().astype(np.float64) - ref["probs"])) <= TOL[prec]
     # empty events give the bias-only vector UNet(0) in every interval
     P = probs.cpu().numpy().reshape(5, 40, 100)
     assert np.all(P[0] == P[0, 0]) and np.array_equal(P[0], P[3])
