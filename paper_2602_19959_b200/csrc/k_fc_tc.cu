@@ -144,22 +144,22 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
       int ev_lo;
       const int nk = kept_of(e, ev_lo);
       float* He = hist + (size_t)e * kIntervals * kFcOut + (4 * half + 2 * mh) * kBins + r;   // + iv*800 + mm*100
-      float acc[2] = {0.f, 0.f};
-      int cur[2] = {0, 0};
+      float acc0 = 0.f, acc1 = 0.f;              // running sums of the two channel tiles (no dynamic indexing)
+      int cur0 = 0, cur1 = 0;
       for (int base = 0; base < nk; base += kTile, ++it) {
         const int buf = it & 1, ntile = min(kTile, nk - base);
         const bool last = base + kTile >= nk;
         mbar_wait(bar(bHFull + buf), (uint32_t)((it >> 1) & 1));      // s_iv[buf] is staged
         const int* ivs = s_iv + buf * kTile;
-#pragma unroll
+#pragma unroll 1
         for (int mm = 0; mm < 2; ++mm) {
           const int mt = 2 * mh + mm;
           mbar_wait(bar(bAccFull + mt), (uint32_t)(it & 1));
           tc_fence_after_sync();
           const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)(mt * kTile);
           float* Hc = He + mm * kBins;
-          float a = acc[mm];
-          int c = cur[mm];
+          float a = mm ? acc1 : acc0;
+          int c = mm ? cur1 : cur0;
           for (int c0 = 0; c0 < ntile; c0 += 16) {
             uint32_t v[16];
             tmem_ld_x16(taddr + (uint32_t)c0, v);
@@ -216,8 +216,7 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
               ++c;
             }
           }
-          acc[mm] = a;
-          cur[mm] = c;
+          if (mm) { acc1 = a; cur1 = c; } else { acc0 = a; cur0 = c; }
           tc_fence_before_sync();
           mbar_arrive(bar(bAccEmpty + mt));
         }
@@ -291,7 +290,7 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
             for (int k = 0; k < kFcIn; ++k) a = fmaf(S.w0[o][k], x[k], a);
             h[o] = leaky_ft(a);
           }
-#pragma unroll
+#pragma unroll 1                  // four identical layers share one copy of the code (I-cache footprint)
           for (int l = 0; l < 4; ++l) {
 #pragma unroll
             for (int o = 0; o < kFcHidden; ++o) {
