@@ -42,7 +42,9 @@ typedef enum {
   PVF_ERR_UNSUPPORTED = 5  /* valid request this build cannot serve (e.g. stage timing disabled) */
 } pvf_status;
 
-/* Arithmetic of the UNet convolutions (the FC stage and the peak finder are always FP32). */
+/* Arithmetic of the UNet convolutions.  The peak finder is always FP32; the FC stage is always FP32-accurate:
+ * FP32 FMAs in PVF_PREC_FP32, and in the tensor-core modes FP32 FMAs for the 25-wide layers plus a 3-pass
+ * TF32 hi/lo split with FP32 accumulation for the 25 -> 800 layer. */
 typedef enum {
   PVF_PREC_FP32 = 0, /* FP32 FMA direct convolution (CUDA cores); reference-accuracy path */
   PVF_PREC_TF32 = 1, /* tcgen05 kind::tf32, operands RN-rounded to TF32, FP32 accumulate in TMEM */
