@@ -39,7 +39,7 @@ namespace {
 
 constexpr int kTcThreads = 192;
 constexpr int kMaxStages = 8;
-constexpr int kStageBytes = 8192;
+constexpr int kStageBytes = 16384;
 constexpr int kHeaderBytes = 2048;          // biases [5][C], head weight [C], head bias
 
 // sub-layers as the MMA issuer sees them
@@ -55,13 +55,14 @@ struct Geo {
   static constexpr int NCH = C / PER;                // chunks of a C-channel activation
   static constexpr int XCH = BF16 ? 2 : 4;           // chunks of the input buffer X0 (TF32: hi0 hi1 lo0 lo1)
   static constexpr int NKB1 = C / KPM;               // MMA K blocks per tap over C channels
-  static constexpr int T = (C == 64) ? (BF16 ? 4 : 2) : (BF16 ? 8 : 4);   // intervals per group
+  static constexpr int NOUT = 2 * C;                 // MMA N: the outputs of an (even, odd) tap pair side by side
+  static constexpr int T = (C == 64) ? 2 : (C == 32 ? 4 : (BF16 ? 8 : 4));   // intervals per group (TMEM: 4*T*C <= 512)
   static constexpr int LEAD1 = 16, LEAD2 = 8, LEAD3 = 8;
   // rows per chunk = lead halo + T interval slots; reads past the last slot (garbage output rows only)
   // land in the following chunk / buffer, which is always inside the CTA's allocation
   static constexpr int ROWS1 = LEAD1 + 128 * T, ROWS2 = LEAD2 + 64 * T, ROWS3 = LEAD3 + 32 * T;
   static constexpr int LBO1 = ROWS1 * 16, LBO2 = ROWS2 * 16, LBO3 = ROWS3 * 16;
-  static constexpr int STEP_BYTES = 2 * C * 16;      // one MMA's B operand: [2 chunks][C][16 B]
+  static constexpr int STEP_BYTES = 2 * NOUT * 16;   // one MMA's B operand: [2 chunks][2C rows][16 B]
   static constexpr int SPS = kStageBytes / STEP_BYTES;   // MMA steps per ring stage
   // shared-memory map (bytes)
   static constexpr int SZ_L1 = NCH * LBO1;           // a C-channel buffer at L = 100
@@ -71,30 +72,33 @@ struct Geo {
   static constexpr int OFF_XP = OFF_R + SZ_L1;       // overlay: X0 (input) then P1 = pool(e1)
   static constexpr int SZ_XP = (XCH * LBO1 > SZ_L2) ? XCH * LBO1 : SZ_L2;
   static constexpr int OFF_RING = OFF_XP + SZ_XP;
-  static constexpr int STAGES_FIT = (227 * 1024 - kHeaderBytes - 256 - OFF_RING) / kStageBytes;
+  static constexpr int SCR_BYTES = 2 * 4 * C * 4;    // epilogue row-exchange scratch: [2 buffers][4 warps][C floats]
+  static constexpr int STAGES_FIT = (227 * 1024 - kHeaderBytes - 256 - SCR_BYTES - OFF_RING) / kStageBytes;
   static constexpr int STAGES = STAGES_FIT < kMaxStages ? STAGES_FIT : kMaxStages;   // weight ring depth
   static constexpr int OFF_PAR = OFF_RING + STAGES * kStageBytes;   // biases + head (floats)
-  static constexpr int OFF_BAR = OFF_PAR + kHeaderBytes;
+  static constexpr int OFF_SCR = OFF_PAR + kHeaderBytes;
+  static constexpr int OFF_BAR = OFF_SCR + SCR_BYTES;
   static constexpr int SMEM = OFF_BAR + 256;
-  // TMEM columns: region A = [0, T*C) (d1), region B = [T*C, 2*T*C) (e1; e2, b, d2 use its head)
-  static constexpr int COL_A = 0, COL_B = T * C;
-  static constexpr int TMEM_COLS = (2 * T * C <= 32) ? 32 : (2 * T * C <= 64) ? 64 : (2 * T * C <= 128) ? 128
-                                   : (2 * T * C <= 256) ? 256 : 512;
+  // TMEM columns: region A = [0, T*2C) (d1), region B = [T*2C, 2*T*2C) (e1; e2, b, d2 use its head);
+  // an accumulator tile is 2C columns: E0 (even taps) | E1 (odd taps)
+  static constexpr int COL_A = 0, COL_B = T * NOUT;
+  static constexpr int TMEM_COLS = (2 * T * NOUT <= 32) ? 32 : (2 * T * NOUT <= 64) ? 64 : (2 * T * NOUT <= 128) ? 128
+                                   : (2 * T * NOUT <= 256) ? 256 : 512;
   // d1E parts (steps): run while the epilogues of e2 / b / d2 drain; multiples of every SPS
-  static constexpr int D1E_STEPS = 25 * NKB1;
+  static constexpr int D1E_STEPS = 13 * NKB1;        // 13 tap pairs
   static constexpr int D1E_A = D1E_STEPS < 16 ? D1E_STEPS : 16;
   static constexpr int D1E_B = (D1E_STEPS - D1E_A) < 16 ? (D1E_STEPS - D1E_A) : 16;
   static constexpr int D1E_C = D1E_STEPS - D1E_A - D1E_B;
   static_assert(2 * SZ_L2 == SZ_L1, "E2 + U2 must tile the overlay region exactly");
-  static_assert(SMEM <= 227 * 1024 && STAGES >= 4, "shared memory budget");
-  static_assert(2 * T * C <= 512, "TMEM budget");
+  static_assert(SMEM <= 227 * 1024 && STAGES >= 3, "shared memory budget");
+  static_assert(2 * T * NOUT <= 512, "TMEM budget");
   static_assert(NCH % 2 == 0 && T % 2 == 0, "whole MMA K blocks per source; level-2 tiles whole");
   static_assert(16 % SPS == 0, "d1E parts must start on ring-stage boundaries");
 };
 
 // Steps and byte offsets of the weight-image segments (host packer, producer and issuer agree on it).
 struct Plan {
-  int e1_steps;            // 25, or 75 with the e1 hi/lo split
+  int e1_steps;            // 13 tap pairs, x3 with the e1 hi/lo split
   int seg_steps[kSegs];
   int seg_off[kSegs];      // bytes from the start of the image
   int total;
@@ -104,15 +108,15 @@ template <int C, bool BF16>
 __host__ __device__ inline Plan make_plan(int split_e1) {
   using G = Geo<C, BF16>;
   Plan P{};
-  P.e1_steps = 25 * ((!BF16 && split_e1) ? 3 : 1);
-  P.seg_steps[gE2] = 15 * G::NKB1;
+  P.e1_steps = 13 * ((!BF16 && split_e1) ? 3 : 1);
+  P.seg_steps[gE2] = 8 * G::NKB1;
   P.seg_steps[gD1Ea] = G::D1E_A;
-  P.seg_steps[gB] = 5 * G::NKB1;
+  P.seg_steps[gB] = 3 * G::NKB1;
   P.seg_steps[gD1Eb] = G::D1E_B;
-  P.seg_steps[gD2] = 15 * 2 * G::NKB1;
+  P.seg_steps[gD2] = 8 * 2 * G::NKB1;
   P.seg_steps[gD1Ec] = G::D1E_C;
   P.seg_steps[gE1] = P.e1_steps;
-  P.seg_steps[gD1U] = 25 * G::NKB1;
+  P.seg_steps[gD1U] = 13 * G::NKB1;
   int off = kHeaderBytes;
   for (int s = 0; s < kSegs; ++s) {
     P.seg_off[s] = off;
@@ -176,12 +180,28 @@ enum { kE1 = 0, kE2 = 1, kB = 2, kD2 = 3, kD1 = 4 };
 template <int C, bool BF16, int MODE>
 __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_base, int tile, int q, int lane,
                                               const float* __restrict__ par, int n_valid_int,
-                                              float* __restrict__ probs_group) {
+                                              float* __restrict__ probs_group, float* __restrict__ scr) {
   using G = Geo<C, BF16>;
   const int m = 32 * q + lane;
   const float* bias = par + MODE * C;
+  // accumulator tile: columns [0, C) = E0 (even taps), [C, 2C) = E1 (odd taps); output row m = E0[m] + E1[m+1]
   const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) +
-                         (uint32_t)((MODE == kD1 ? G::COL_A : G::COL_B) + tile * C);
+                         (uint32_t)((MODE == kD1 ? G::COL_A : G::COL_B) + tile * G::NOUT);
+  // Row m + 1 of lane 31 lives in the next warp's TMEM quadrant: lane 0 of every warp publishes its E1 row
+  // in shared memory (scr: [4 warps][C], double buffered by the caller), one named barrier per tile.
+#pragma unroll 1
+  for (int c0 = 0; c0 < C; c0 += 16) {
+    uint32_t r[16];
+    tmem_ld_x16(taddr + (uint32_t)(C + c0), r);
+    tmem_ld_wait();
+    if (lane == 0) {
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        *reinterpret_cast<uint4*>(scr + q * C + c0 + 4 * k) = make_uint4(r[4 * k], r[4 * k + 1], r[4 * k + 2], r[4 * k + 3]);
+    }
+  }
+  asm volatile("bar.sync 1, 128;" ::: "memory");
+  const float* nxt = scr + (q + 1) * C;          // E1 row of the next quadrant's first lane (q = 3: unused)
   // which interval of the group this row belongs to, its position, and whether it is a real output
   int interval, l;
   bool valid;
@@ -209,12 +229,17 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
   float logit = 0.0f;
 #pragma unroll 1
   for (int c0 = 0; c0 < C; c0 += 16) {
-    uint32_t r[16];
+    uint32_t r[16], r1[16];
     tmem_ld_x16(taddr + (uint32_t)c0, r);
+    tmem_ld_x16(taddr + (uint32_t)(C + c0), r1);
     tmem_ld_wait();
     float v[16];
 #pragma unroll
-    for (int i = 0; i < 16; ++i) v[i] = lrelu(__uint_as_float(r[i]) + bias[c0 + i]);
+    for (int i = 0; i < 16; ++i) {
+      float up = __shfl_down_sync(0xffffffffu, __uint_as_float(r1[i]), 1);
+      if (lane == 31) up = (q < 3) ? nxt[c0 + i] : 0.0f;
+      v[i] = lrelu(__uint_as_float(r[i]) + up + bias[c0 + i]);
+    }
     if (MODE == kD1) {
       const float* hw = par + 5 * C;
 #pragma unroll
@@ -299,6 +324,7 @@ struct Lay {
   using G = Geo<C, BF16>;
   static constexpr int TAPS = (S == sE1 || S == sD1U || S == sD1E) ? 25 : (S == sB ? 5 : 15);
   static constexpr int PAD = (TAPS - 1) / 2;
+  static constexpr int PAIRS = (TAPS + 1) / 2;                 // (even, odd) tap pairs; the last odd tap is zero
   static constexpr int NKB = (S == sE1) ? 1 : (S == sD2 ? 2 * G::NKB1 : G::NKB1);     // K blocks per tap
   static constexpr int LEVEL = (S == sE1 || S == sD1U || S == sD1E) ? 1 : (S == sB ? 3 : 2);
   static constexpr int LEAD = LEVEL == 1 ? G::LEAD1 : (LEVEL == 2 ? G::LEAD2 : G::LEAD3);
@@ -337,10 +363,10 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
   constexpr int SPS = G::SPS;
   static_assert(Y::HALF % SPS == 0 || SPS % Y::NKB == 0,
                 "a ring stage is either part of one source's K blocks or whole taps");
-  constexpr uint32_t idesc = instr_desc(BF16 ? kFmtBF16 : kFmtTF32, 128, C);
+  constexpr uint32_t idesc = instr_desc(BF16 ? kFmtBF16 : kFmtTF32, 128, G::NOUT);
   constexpr uint32_t hi = (128u >> 4) | (1u << 14);                    // SBO = 128 B, descriptor version 1
   constexpr uint32_t a_lbo = (uint32_t)(Y::LBO >> 4) << 16;
-  constexpr uint32_t b_lbo = (uint32_t)((C * 16) >> 4) << 16;
+  constexpr uint32_t b_lbo = (uint32_t)((G::NOUT * 16) >> 4) << 16;
   const uint32_t dcol = tmem_base + (uint32_t)Y::DCOL;
   for (int f = f_begin; f < f_end; f += SPS) {
     const int n = min(SPS, f_end - f);
@@ -349,13 +375,13 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
     const uint32_t b0 = b_lbo + ((sb + G::OFF_RING + rs.ring * kStageBytes) >> 4);
     uint32_t a0 = a_lbo + (sb >> 4);          // stage origin: descriptor low word of tile 0, step f
     if (S == sE1) {
-      // e1: one K block per step; steps run [pass][tap], pass 1 reads the low-part chunks (split)
+      // e1: one K block per step; steps run [pass][tap pair], pass 1 reads the low-part chunks (split)
     } else if (Y::HALF >= SPS) {
       const int j0 = f / Y::NKB, kk0 = f % Y::NKB;
       const int off = kk0 < Y::HALF ? Y::SRC0 + 2 * kk0 * Y::LBO : Y::SRC1 + 2 * (kk0 - Y::HALF) * Y::LBO;
-      a0 += (uint32_t)(off >> 4) + (uint32_t)(Y::LEAD + j0 - Y::PAD);
+      a0 += (uint32_t)(off >> 4) + (uint32_t)(Y::LEAD + 2 * j0 - Y::PAD);
     } else {
-      a0 += (uint32_t)(Y::SRC0 >> 4) + (uint32_t)(Y::LEAD + f / Y::NKB - Y::PAD);
+      a0 += (uint32_t)(Y::SRC0 >> 4) + (uint32_t)(Y::LEAD + 2 * (f / Y::NKB) - Y::PAD);
     }
     if (elect_one()) {
 #pragma unroll
@@ -363,18 +389,18 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
         if (i < n) {
           uint32_t a;
           if (S == sE1) {
-            const int step = f + i, pass = step / 25, j = step - 25 * pass;
-            a = a0 + (uint32_t)((Y::SRC0 + (pass == 1 ? 2 * G::LBO1 : 0)) >> 4) + (uint32_t)(Y::LEAD + j - Y::PAD);
+            const int step = f + i, pass = step / 13, u = step - 13 * pass;
+            a = a0 + (uint32_t)((Y::SRC0 + (pass == 1 ? 2 * G::LBO1 : 0)) >> 4) + (uint32_t)(Y::LEAD + 2 * u - Y::PAD);
           } else if (Y::HALF >= SPS) {
             a = a0 + (uint32_t)(i * ((2 * Y::LBO) >> 4));
           } else {
-            a = a0 + (uint32_t)((Y::a_off(i % Y::NKB) - Y::SRC0) >> 4) + (uint32_t)(i / Y::NKB);
+            a = a0 + (uint32_t)((Y::a_off(i % Y::NKB) - Y::SRC0) >> 4) + (uint32_t)(2 * (i / Y::NKB));
           }
           const uint32_t b = b0 + (uint32_t)(i * (G::STEP_BYTES >> 4));
           const uint32_t acc = (i > 0) ? 1u : (f > f_begin ? 1u : acc0);
 #pragma unroll
           for (int t = 0; t < Y::NT; ++t)
-            mma_lh<BF16>(dcol + (uint32_t)(t * C), a + 128u * t, hi, b, hi, idesc, acc);
+            mma_lh<BF16>(dcol + (uint32_t)(t * G::NOUT), a + 128u * t, hi, b, hi, idesc, acc);
         }
       }
       mma_commit(bar0 + 8u * (G::STAGES + rs.ring));      // frees the ring slot when these MMAs retire
@@ -463,16 +489,16 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
         commit(0);
       }
       wait_epi(1);                                   // P1 staged, region B drained
-      mma_seg<C, BF16, sE2>(sb, tmem_base, bar0, rs, 0, 15 * G::NKB1, 0u);
+      mma_seg<C, BF16, sE2>(sb, tmem_base, bar0, rs, 0, 8 * G::NKB1, 0u);
       commit(1);
       if (!first) wait_epi(5);                       // region A drained by the previous group's d1 epilogue
       mma_seg<C, BF16, sD1E>(sb, tmem_base, bar0, rs, 0, G::D1E_A, 0u);
       wait_epi(2);                                   // E2, P2 staged
-      mma_seg<C, BF16, sB>(sb, tmem_base, bar0, rs, 0, 5 * G::NKB1, 0u);
+      mma_seg<C, BF16, sB>(sb, tmem_base, bar0, rs, 0, 3 * G::NKB1, 0u);
       commit(2);
       mma_seg<C, BF16, sD1E>(sb, tmem_base, bar0, rs, G::D1E_A, G::D1E_A + G::D1E_B, 1u);
       wait_epi(3);                                   // U2 staged
-      mma_seg<C, BF16, sD2>(sb, tmem_base, bar0, rs, 0, 15 * 2 * G::NKB1, 0u);
+      mma_seg<C, BF16, sD2>(sb, tmem_base, bar0, rs, 0, 8 * 2 * G::NKB1, 0u);
       commit(3);
       mma_seg<C, BF16, sD1E>(sb, tmem_base, bar0, rs, G::D1E_A + G::D1E_B, G::D1E_STEPS, 1u);
       wait_epi(4);                                   // U1 staged, region B drained
@@ -481,13 +507,16 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
         mma_seg<C, BF16, sE1>(sb, tmem_base, bar0, rs, 0, P.e1_steps, 0u);
         commit(0);
       }
-      mma_seg<C, BF16, sD1U>(sb, tmem_base, bar0, rs, 0, 25 * G::NKB1, 1u);
+      mma_seg<C, BF16, sD1U>(sb, tmem_base, bar0, rs, 0, 13 * G::NKB1, 1u);
       commit(4);
       first = false;
     }
   } else {
     // ===================== epilogue warps (128 threads): thread = accumulator row
     const int q = warp & 3, et = tid - 64;
+    float* scr0 = reinterpret_cast<float*>(smem + G::OFF_SCR);
+    int ecount = 0;                          // accumulator tiles drained so far (selects the scratch buffer)
+    auto scr = [&]() { return scr0 + (ecount++ & 1) * 4 * C; };
     uint32_t pa[5] = {0, 0, 0, 0, 0};
     auto wait_acc = [&](int k) { mbar_wait(accum_bar(k), pa[k]); pa[k] ^= 1u; tc_fence_after_sync(); };
     auto done = [&](int k) { fence_proxy_async_smem(); tc_fence_before_sync(); mbar_arrive(epi_bar(k)); };
@@ -503,30 +532,30 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
         load_x0<C, BF16>(sb, hist, g0, n_valid, split_e1, et);
         done(0);
         wait_acc(0);
-        for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kE1>(sb, tmem_base, t, q, lane, par, n_valid, pg);
+        for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kE1>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr());
         done(1);
         first = false;
       }
       wait_acc(1);
-      for (int t = 0; t < G::T / 2; ++t) epilogue_tile<C, BF16, kE2>(sb, tmem_base, t, q, lane, par, n_valid, pg);
+      for (int t = 0; t < G::T / 2; ++t) epilogue_tile<C, BF16, kE2>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr());
       done(2);
       if (has_next) {                                // P1 is dead (e2's MMAs retired): stage the next input
         load_x0<C, BF16>(sb, hist, gn0, n_valid_next, split_e1, et);
         done(0);
       }
       wait_acc(2);
-      for (int t = 0; t < (G::T + 3) / 4; ++t) epilogue_tile<C, BF16, kB>(sb, tmem_base, t, q, lane, par, n_valid, pg);
+      for (int t = 0; t < (G::T + 3) / 4; ++t) epilogue_tile<C, BF16, kB>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr());
       done(3);
       wait_acc(3);
-      for (int t = 0; t < G::T / 2; ++t) epilogue_tile<C, BF16, kD2>(sb, tmem_base, t, q, lane, par, n_valid, pg);
+      for (int t = 0; t < G::T / 2; ++t) epilogue_tile<C, BF16, kD2>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr());
       done(4);
       if (has_next) {
         wait_acc(0);
-        for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kE1>(sb, tmem_base, t, q, lane, par, n_valid_next, pg);
+        for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kE1>(sb, tmem_base, t, q, lane, par, n_valid_next, pg, scr());
         done(1);
       }
       wait_acc(4);
-      for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kD1>(sb, tmem_base, t, q, lane, par, n_valid, pg);
+      for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kD1>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr());
       done(5);
     }
   }
@@ -558,7 +587,8 @@ uint16_t bf16_rne(float v) {
 
 // Packs PyTorch-layout conv weights [C_out][C_in][K] into the image the kernel streams: a 2 KB header
 // (biases [5][C], head weight [C], head bias) and, per segment in streaming order, per MMA step, the
-// B operand [2 chunks][C out][16 B of input channels], operand-rounded (TF32: RN ties away; BF16: RNE).
+// B operand [2 chunks][2C rows: C outputs of tap 2u, then of tap 2u+1][16 B of input channels],
+// operand-rounded (TF32: RN ties away; BF16: RNE).
 template <int C, bool BF16>
 void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst) {
   using G = Geo<C, BF16>;
@@ -578,17 +608,18 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst) {
     const float* W = w->conv_w[d.layer];          // [C][cin][taps]
     for (int s = 0; s < P.seg_steps[d.seg]; ++s) {
       const int f = d.f0 + s;                     // step index inside the sub-layer
-      int j, kk, pass = 0;
-      if (d.seg == gE1) { pass = f / 25; j = f % 25; kk = 0; }     // e1 split runs [pass][tap]
-      else { j = f / d.nkb; kk = f % d.nkb; }
+      int u, kk, pass = 0;                        // tap pair, K block
+      if (d.seg == gE1) { pass = f / 13; u = f % 13; kk = 0; }     // e1 split runs [pass][tap pair]
+      else { u = f / d.nkb; kk = f % d.nkb; }
       unsigned char* step = dst + P.seg_off[d.seg] + (size_t)s * G::STEP_BYTES;
       for (int h = 0; h < 2; ++h)
-        for (int n = 0; n < C; ++n)
+        for (int n = 0; n < G::NOUT; ++n)         // rows [0, C): even tap 2u, rows [C, 2C): odd tap 2u + 1
           for (int e = 0; e < G::PER; ++e) {
+            const int co = n % C, j = 2 * u + n / C;
             const int cl = (2 * kk + h) * G::PER + e;            // channel inside the sub-layer's range
-            const bool real = (d.seg == gE1) ? cl < kHistCh : true;
-            const float v = real ? W[((size_t)n * d.cin + d.ch_base + cl) * d.taps + j] : 0.0f;
-            unsigned char* p = step + ((size_t)h * C + n) * 16 + e * G::ES;
+            const bool real = j < d.taps && ((d.seg == gE1) ? cl < kHistCh : true);
+            const float v = real ? W[((size_t)co * d.cin + d.ch_base + cl) * d.taps + j] : 0.0f;
+            unsigned char* p = step + ((size_t)h * G::NOUT + n) * 16 + e * G::ES;
             if (BF16) {
               const uint16_t b = bf16_rne(v);
               memcpy(p, &b, 2);
