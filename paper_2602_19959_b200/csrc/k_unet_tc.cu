@@ -6,8 +6,10 @@
 // intermediates stay in shared memory / TMEM.  DESIGN.md section 4.3 has the derivation.
 //
 // Mapping.  A conv layer is  D[m, n] = sum_j sum_ci  A[m + j - p, ci] * W_j[ci, n]  with m = position
-// (M), n = output channel (N = C), and one (tap j, 32-byte channel block) per tcgen05.mma of shape
-// 128 x C x (8 TF32 | 16 BF16).  Activations live in shared memory in the K-major no-swizzle UMMA
+// (M), n = output channel.  Taps are taken in (even, odd) pairs that share one read of A:
+//     D[m] = E0[m] + E1[m + 1],   E0[m] = sum_u A[m + 2u - p] W_2u,   E1[m'] = sum_u A[m' + 2u - p] W_2u+1
+// so one (tap pair u, 32-byte channel block) is one tcgen05.mma of shape 128 x 2C x (8 TF32 | 16 BF16)
+// with B = [W_2u | W_2u+1]; the epilogue adds the E1 half of the next row.  Activations live in shared memory in the K-major no-swizzle UMMA
 // layout  [channel chunk of 16 B][row][16 B]  (core matrix = 8 rows x 16 B contiguous), so a tap
 // shift is a pure bump of the descriptor start address by 16 B per row, the skip concat is a second
 // base address, and an epilogue thread (= one row) writes whole 16-byte chunks, conflict free.
