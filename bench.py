@@ -1,7 +1,7 @@
 """bench.py -- throughput of the PVFinder hot path on B200 (contract: see DESIGN.md "Measurement").
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
-                    [--precision tf32|bf16|fp32] [--events E] [--model run3|pileup] [--channels C]
+                    [--precision tf32|bf16|fp16|fp32] [--events E] [--model run3|pileup] [--channels C]
 
 One "step" = one pass of the whole hot path (interval sort, FC + segmented sum, UNet, peak finder:
 SURVEY.md section 8a rows a0-a4) over one batch of synthetic events (BASELINE.json config 2: 16000
@@ -229,7 +229,7 @@ def main_ours(args, rank, world, local_rank):
         bound, peak = "alu", 148 * 128 * 2 * 1.965e9 / 1e12
         peak_note = "FP32 FMA: 148 SM x 128 lanes x 2 FLOP x 1.965 GHz (B200_PROFILING.md unit counts)"
     else:
-        ratio = 1.0 if args.precision == "bf16" else 1.1 / 2.25
+        ratio = 1.0 if args.precision in ("bf16", "fp16") else 1.1 / 2.25
         bound, peak = "tensor", peaks["bf16_tflops_sustained"] * ratio
         peak_note = (f"{peaks_src} bf16 sustained {peaks['bf16_tflops_sustained']} TFLOP/s"
                      + ("" if ratio == 1.0 else " x nominal tf32/bf16 ratio 1.1/2.25"))
@@ -244,7 +244,7 @@ def main_ours(args, rank, world, local_rank):
     out = {
         "metric": METRIC, "value": value, "unit": "events/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": {"fp32": "f32", "tf32": "tf32", "bf16": "bf16"}[args.precision],
+        "vs_baseline": None, "dtype": {"fp32": "f32", "tf32": "tf32", "bf16": "bf16", "fp16": "f16"}[args.precision],
         "data": "synthetic",
         "config": {"workload": f"BASELINE.json config {'3' if args.model == 'pileup' else '2'}: {E} events/GPU, "
                                f"model {args.model}, {ev.n_tracks} tracks, UNet {args.channels} ch, weights {args.weights}",
@@ -277,7 +277,7 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--precision", default=os.environ.get("PVF_BENCH_PRECISION", "tf32"), choices=["fp32", "tf32", "bf16"])
+    ap.add_argument("--precision", default=os.environ.get("PVF_BENCH_PRECISION", "tf32"), choices=["fp32", "tf32", "bf16", "fp16"])
     ap.add_argument("--split-mask", type=int, default=-1)
     ap.add_argument("--events", type=int, default=16000)
     ap.add_argument("--model", default="run3", choices=["run3", "pileup"])

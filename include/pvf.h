@@ -48,7 +48,8 @@ typedef enum {
 typedef enum {
   PVF_PREC_FP32 = 0, /* FP32 FMA direct convolution (CUDA cores); reference-accuracy path */
   PVF_PREC_TF32 = 1, /* tcgen05 kind::tf32, operands RN-rounded to TF32, FP32 accumulate in TMEM */
-  PVF_PREC_BF16 = 2  /* tcgen05 kind::f16 with BF16 operands, FP32 accumulate in TMEM */
+  PVF_PREC_BF16 = 2, /* tcgen05 kind::f16 with BF16 operands, FP32 accumulate in TMEM */
+  PVF_PREC_FP16 = 3  /* tcgen05 kind::f16 with FP16 operands (the paper's roadmap precision) */
 } pvf_precision;
 
 /* Bits of pvf_peaks.event_flags (data-dependent anomalies never fail the call: PAPER.md:57). */
@@ -73,7 +74,7 @@ typedef struct {
   int32_t peak_halfwidth;  /* (fixed) 3 */
   int32_t max_peaks;       /* (fixed) 32 */
   int32_t precision;       /* pvf_precision */
-  int32_t split_mask;      /* TF32/BF16 only: bit L (0=e1,1=e2,2=b,3=d2,4=d1) = 3-pass hi/lo split
+  int32_t split_mask;      /* TF32 only: bit L (0=e1,1=e2,2=b,3=d2,4=d1) = 3-pass hi/lo split
                               precision for that conv layer */
   int32_t max_events;      /* capacity the pool is sized for (>= 1) */
   int64_t max_tracks;      /* capacity the pool is sized for (>= 1) */

@@ -37,7 +37,7 @@ constexpr int kLboW = kRowsW * 16;           // 8192: next 16-byte K chunk of th
 constexpr int kLboH = kTile * 16;            // 2048: next 16-byte K chunk of the B operand
 constexpr int kWPart = 8 * kLboW;            // 65536 bytes: one part (hi or lo) of W5x for one half
 constexpr int kHPart = 8 * kLboH;            // 16384 bytes: one part of hx for one tile
-constexpr int kHStride = 28, kWRow = 28;
+constexpr int kWRow = 28;
 
 struct FtSmall {                             // the five hidden layers, zero padded
   float w0[kFcHidden][12];

@@ -28,6 +28,7 @@
 // issues), warps 2-5 = epilogue (TMEM -> registers -> bias, LeakyReLU, TF32/BF16 rounding, pool /
 // upsample -> shared memory; d1's epilogue fuses the 1x1 head + sigmoid and writes out_probs).
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <cstring>
 #include <vector>
 
@@ -49,7 +50,9 @@ enum { sE1 = 0, sE2 = 1, sB = 2, sD2 = 3, sD1U = 4, sD1E = 5 };
 // weight-image segments in streaming order
 enum { gE2 = 0, gD1Ea = 1, gB = 2, gD1Eb = 3, gD2 = 4, gD1Ec = 5, gE1 = 6, gD1U = 7, kSegs = 8 };
 
-template <int C, bool BF16>
+// BF16: operand format -- 0 = TF32 (4-byte), 1 = BF16, 2 = FP16 (2-byte; everything that only depends on
+// the operand size treats 1 and 2 alike)
+template <int C, int BF16>
 struct Geo {
   static constexpr int ES = BF16 ? 2 : 4;            // operand element size
   static constexpr int PER = 16 / ES;                // channels per 16-byte chunk
@@ -106,7 +109,7 @@ struct Plan {
   int total;
 };
 
-template <int C, bool BF16>
+template <int C, int BF16>
 __host__ __device__ inline Plan make_plan(int split_e1) {
   using G = Geo<C, BF16>;
   Plan P{};
@@ -135,10 +138,17 @@ __device__ __forceinline__ uint32_t to_tf32(float v) {
   asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(v));
   return r;
 }
-__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
-  const __nv_bfloat162 h = __floats2bfloat162_rn(lo, hi);
+// two floats -> one 32-bit word of 16-bit operands (FMT 1 = BF16, 2 = FP16), round to nearest even
+template <int FMT>
+__device__ __forceinline__ uint32_t pack16(float lo, float hi) {
   uint32_t r;
-  memcpy(&r, &h, 4);
+  if (FMT == 2) {
+    const __half2 h = __floats2half2_rn(lo, hi);
+    memcpy(&r, &h, 4);
+  } else {
+    const __nv_bfloat162 h = __floats2bfloat162_rn(lo, hi);
+    memcpy(&r, &h, 4);
+  }
   return r;
 }
 __device__ __forceinline__ void st_smem16(uint32_t addr, uint4 v) {
@@ -147,16 +157,16 @@ __device__ __forceinline__ void st_smem16(uint32_t addr, uint4 v) {
 
 // 16 consecutive channels of one row -> 16-byte chunks (4 for TF32, 2 for BF16) at
 // dst + chunk * lbo, chunk counted from c0 / PER.
-template <bool BF16>
+template <int BF16>
 __device__ __forceinline__ void store_row16(uint32_t dst_row, uint32_t lbo, int c0, const float (&v)[16]) {
   if (BF16) {
 #pragma unroll
     for (int k = 0; k < 2; ++k) {
       uint4 q;
-      q.x = pack_bf16(v[8 * k + 0], v[8 * k + 1]);
-      q.y = pack_bf16(v[8 * k + 2], v[8 * k + 3]);
-      q.z = pack_bf16(v[8 * k + 4], v[8 * k + 5]);
-      q.w = pack_bf16(v[8 * k + 6], v[8 * k + 7]);
+      q.x = pack16<BF16>(v[8 * k + 0], v[8 * k + 1]);
+      q.y = pack16<BF16>(v[8 * k + 2], v[8 * k + 3]);
+      q.z = pack16<BF16>(v[8 * k + 4], v[8 * k + 5]);
+      q.w = pack16<BF16>(v[8 * k + 6], v[8 * k + 7]);
       st_smem16(dst_row + (uint32_t)(c0 / 8 + k) * lbo, q);
     }
   } else {
@@ -179,7 +189,7 @@ __device__ __forceinline__ void zero_rows(uint32_t buf, uint32_t lbo, int nch, i
 enum { kE1 = 0, kE2 = 1, kB = 2, kD2 = 3, kD1 = 4 };
 
 // Epilogue of one 128-row accumulator tile, executed by the four epilogue warps (thread = row m).
-template <int C, bool BF16, int MODE>
+template <int C, int BF16, int MODE>
 __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_base, int tile, int q, int lane,
                                               const float* __restrict__ par, int n_valid_int,
                                               float* __restrict__ probs_group, float* __restrict__ scr) {
@@ -277,7 +287,7 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
 // Interval histograms of one group -> X0 (operand-rounded, chunked layout).  128 threads.  X0 shares
 // its memory with P1, so every row the e1 MMAs can read for a valid output is (re)written: the lead
 // rows and the gap rows l >= 100 of every interval as zeros.
-template <int C, bool BF16>
+template <int C, int BF16>
 __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restrict__ hist, long long g0,
                                         int n_valid_int, int split, int tid) {
   using G = Geo<C, BF16>;
@@ -293,8 +303,8 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
 #pragma unroll
       for (int c = 0; c < 8; ++c) x[c] = live ? __ldg(hist + (g0 + t) * kFcOut + c * kBins + l) : 0.0f;
       uint4 qv;
-      qv.x = pack_bf16(x[0], x[1]); qv.y = pack_bf16(x[2], x[3]);
-      qv.z = pack_bf16(x[4], x[5]); qv.w = pack_bf16(x[6], x[7]);
+      qv.x = pack16<BF16>(x[0], x[1]); qv.y = pack16<BF16>(x[2], x[3]);
+      qv.z = pack16<BF16>(x[4], x[5]); qv.w = pack16<BF16>(x[6], x[7]);
       const uint32_t row = (uint32_t)(G::LEAD1 + it) * 16u;
       st_smem16(x0 + row, qv);
       st_smem16(x0 + G::LBO1 + row, zero4);       // channels 8..15 of the K = 16 MMA: zero
@@ -321,7 +331,7 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
 }
 
 // Compile-time description of sub-layer S as the MMA issuer sees it.
-template <int C, bool BF16, int S>
+template <int C, int BF16, int S>
 struct Lay {
   using G = Geo<C, BF16>;
   static constexpr int TAPS = (S == sE1 || S == sD1U || S == sD1E) ? 25 : (S == sB ? 5 : 15);
@@ -344,7 +354,7 @@ struct Lay {
   }
 };
 
-template <bool BF16>
+template <int BF16>
 __device__ __forceinline__ void mma_lh(uint32_t d, uint32_t a_lo, uint32_t a_hi, uint32_t b_lo, uint32_t b_hi,
                                        uint32_t idesc, uint32_t acc) {
   if (BF16) mma_f16_lh(d, a_lo, a_hi, b_lo, b_hi, idesc, acc);
@@ -357,7 +367,7 @@ struct RingState { int ring; uint32_t phase; };
 // used by all NT tiles.  The warp walks the (uniform) schedule; one elected lane issues a whole
 // stage worth of MMAs whose descriptors differ from the stage origin by compile-time constants.
 // f_begin must be a multiple of SPS.  acc0 = 0 starts fresh accumulators at step f_begin.
-template <int C, bool BF16, int S>
+template <int C, int BF16, int S>
 __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_t bar0, RingState& rs,
                                         int f_begin, int f_end, uint32_t acc0) {
   using G = Geo<C, BF16>;
@@ -365,7 +375,7 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
   constexpr int SPS = G::SPS;
   static_assert(Y::HALF % SPS == 0 || SPS % Y::NKB == 0,
                 "a ring stage is either part of one source's K blocks or whole taps");
-  constexpr uint32_t idesc = instr_desc(BF16 ? kFmtBF16 : kFmtTF32, 128, G::NOUT);
+  constexpr uint32_t idesc = instr_desc(BF16 == 2 ? kFmtF16 : (BF16 ? kFmtBF16 : kFmtTF32), 128, G::NOUT);
   constexpr uint32_t hi = (128u >> 4) | (1u << 14);                    // SBO = 128 B, descriptor version 1
   constexpr uint32_t a_lbo = (uint32_t)(Y::LBO >> 4) << 16;
   constexpr uint32_t b_lbo = (uint32_t)((G::NOUT * 16) >> 4) << 16;
@@ -412,7 +422,7 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
   }
 }
 
-template <int C, bool BF16>
+template <int C, int BF16>
 __global__ void __launch_bounds__(kTcThreads, 1)
 k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __restrict__ wpack, int split_e1,
           float* __restrict__ probs) {
@@ -587,11 +597,29 @@ uint16_t bf16_rne(float v) {
   return (uint16_t)(u >> 16);
 }
 
+uint16_t fp16_rne(float v) {                 // float -> IEEE binary16, round to nearest even, overflow -> inf
+  uint32_t u;
+  memcpy(&u, &v, 4);
+  const uint32_t sign = (u >> 16) & 0x8000u;
+  u &= 0x7fffffffu;
+  if (u >= 0x7f800000u) return (uint16_t)(sign | (u > 0x7f800000u ? 0x7e00u : 0x7c00u));
+  if (u >= 0x477ff000u) return (uint16_t)(sign | 0x7c00u);                 // >= 65520 rounds to inf
+  if (u < 0x38800000u) {                                                   // subnormal half (or zero)
+    if (u < 0x33000000u) return (uint16_t)sign;
+    const int shift = 126 - (int)(u >> 23);                                // 14 .. 24
+    const uint32_t mant = (u & 0x7fffffu) | 0x800000u;
+    const uint32_t q = mant >> shift, rem = mant & ((1u << shift) - 1u), halfway = 1u << (shift - 1);
+    return (uint16_t)(sign | (q + ((rem > halfway || (rem == halfway && (q & 1u))) ? 1u : 0u)));
+  }
+  const uint32_t r = u + 0xfffu + ((u >> 13) & 1u);                        // round the 13 dropped bits
+  return (uint16_t)(sign | ((r - 0x38000000u) >> 13));
+}
+
 // Packs PyTorch-layout conv weights [C_out][C_in][K] into the image the kernel streams: a 2 KB header
 // (biases [5][C], head weight [C], head bias) and, per segment in streaming order, per MMA step, the
 // B operand [2 chunks][2C rows: C outputs of tap 2u, then of tap 2u+1][16 B of input channels],
 // operand-rounded (TF32: RN ties away; BF16: RNE).
-template <int C, bool BF16>
+template <int C, int BF16>
 void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst) {
   using G = Geo<C, BF16>;
   const Plan P = make_plan<C, BF16>(split_e1);
@@ -623,7 +651,7 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst) {
             const float v = real ? W[((size_t)co * d.cin + d.ch_base + cl) * d.taps + j] : 0.0f;
             unsigned char* p = step + ((size_t)h * G::NOUT + n) * 16 + e * G::ES;
             if (BF16) {
-              const uint16_t b = bf16_rne(v);
+              const uint16_t b = (BF16 == 2) ? fp16_rne(v) : bf16_rne(v);
               memcpy(p, &b, 2);
             } else {
               const float hi = tf32_rna(v);
@@ -635,7 +663,7 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst) {
   }
 }
 
-template <int C, bool BF16>
+template <int C, int BF16>
 void launch_impl(const float* hist, int n_int, const void* packed, int split_e1, float* probs, int sm_count,
                  cudaStream_t s) {
   using G = Geo<C, BF16>;
@@ -645,17 +673,17 @@ void launch_impl(const float* hist, int n_int, const void* packed, int split_e1,
                                                       split_e1, probs);
 }
 
-template <int C, bool BF16>
+template <int C, int BF16>
 cudaError_t setup_impl() {
   return cudaFuncSetAttribute(k_unet_tc<C, BF16>, cudaFuncAttributeMaxDynamicSharedMemorySize, Geo<C, BF16>::SMEM);
 }
 
 #define PVF_TC_DISPATCH(CALL)                                     \
   do {                                                            \
-    const bool bf = precision == PVF_PREC_BF16;                   \
-    if (channels == 64) { if (bf) CALL(64, true); else CALL(64, false); }      \
-    else if (channels == 32) { if (bf) CALL(32, true); else CALL(32, false); } \
-    else { if (bf) CALL(16, true); else CALL(16, false); }        \
+    const int fm = precision == PVF_PREC_BF16 ? 1 : (precision == PVF_PREC_FP16 ? 2 : 0);   \
+    if (channels == 64) { if (fm == 1) CALL(64, 1); else if (fm == 2) CALL(64, 2); else CALL(64, 0); }      \
+    else if (channels == 32) { if (fm == 1) CALL(32, 1); else if (fm == 2) CALL(32, 2); else CALL(32, 0); } \
+    else { if (fm == 1) CALL(16, 1); else if (fm == 2) CALL(16, 2); else CALL(16, 0); }        \
   } while (0)
 
 }  // namespace
@@ -677,7 +705,7 @@ void unet_tc_pack(const pvf_weights* w, int channels, int precision, int split_m
 cudaError_t unet_tc_setup(int channels, int precision, int split_mask) {
   if (channels != 64 && channels != 32 && channels != 16) return cudaErrorInvalidValue;
   if (split_mask & ~1) return cudaErrorInvalidValue;          // only the e1 split is built
-  if (precision == PVF_PREC_BF16 && split_mask) return cudaErrorInvalidValue;
+  if (precision != PVF_PREC_TF32 && split_mask) return cudaErrorInvalidValue;   // the split is a TF32 remedy
   cudaError_t e = cudaSuccess;
 #define PVF_CALL(C_, B_) e = setup_impl<C_, B_>()
   PVF_TC_DISPATCH(PVF_CALL);

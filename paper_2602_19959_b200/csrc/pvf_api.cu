@@ -72,7 +72,7 @@ bool config_ok(const pvf_config* c) {
   if (c->leaky_slope != kLeaky) return false;
   if (!(c->peak_threshold == c->peak_threshold)) return false;
   if (c->peak_halfwidth != kPeakHalf || c->max_peaks != kMaxPeaks) return false;
-  if (c->precision < PVF_PREC_FP32 || c->precision > PVF_PREC_BF16) return false;
+  if (c->precision < PVF_PREC_FP32 || c->precision > PVF_PREC_FP16) return false;
   if (c->split_mask < 0 || c->split_mask > 31) return false;
   if (c->max_events < 1 || c->max_tracks < 1 || c->max_tracks > 0x7fffffffLL) return false;
   return true;

@@ -67,7 +67,6 @@ void launch_unet_simt(const float* hist, int n_intervals_total, const UnetParams
                       float* probs, cudaStream_t s);
 
 // a3, tcgen05/TMEM path (k_unet_tc.cu)
-struct UnetTcPlan;   // opaque; owns nothing on the device (pool pointers only)
 size_t unet_tc_packed_bytes(int channels, int precision, int split_mask);
 // packs PyTorch-layout host weights into the shared-memory image order the kernel streams
 void unet_tc_pack(const pvf_weights* w, int channels, int precision, int split_mask, void* host_dst);

@@ -20,8 +20,9 @@ from pvf_inputs import make_events, make_weights, select_events
 import paper_2602_19959_b200 as pkg
 from paper_2602_19959_b200 import PVFinder
 
-TOL = {"fp32": 2e-5, "tf32": 1e-3, "bf16": 2e-2}
-SPLIT = {"fp32": 0, "tf32": 1, "bf16": 0}
+# fp16 (NEXT-3, the paper's roadmap precision): 10-bit mantissa like TF32 but without the e1 split -> stated 2e-3
+TOL = {"fp32": 2e-5, "tf32": 1e-3, "bf16": 2e-2, "fp16": 2e-3}
+SPLIT = {"fp32": 0, "tf32": 1, "bf16": 0, "fp16": 0}
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -189,10 +190,10 @@ def _oracle_cached(kind, n_events):
 # share of ALL oracle peaks that must be matched within +-1 bin on `peaky` (north_star: 99.9 %; the BF16
 # variant has a stated 2e-2 probability tolerance, so peaks whose height is within that error of the
 # 0.01 threshold cannot be guaranteed: stated bar 99 %)
-PEAK_SHARE = {"fp32": 0.999, "tf32": 0.999, "bf16": 0.99}
+PEAK_SHARE = {"fp32": 0.999, "tf32": 0.999, "bf16": 0.99, "fp16": 0.995}
 
 
-@pytest.mark.parametrize("prec", ["fp32", "tf32", "bf16"])
+@pytest.mark.parametrize("prec", ["fp32", "tf32", "bf16", "fp16"])
 @pytest.mark.parametrize("kind", ["rand", "peaky"])
 def test_whole_path_parity(prec, kind):
     # peaky: BASELINE.json config 1 (1000 events, ~5400 oracle peaks) so that 99.9 % is resolvable
@@ -224,7 +225,7 @@ def test_whole_path_parity(prec, kind):
     assert np.array_equal(own["bin"], got["bin"]) and np.array_equal(own["z"].view(np.uint32), got["z"].view(np.uint32))
 
 
-@pytest.mark.parametrize("prec", ["fp32", "tf32", "bf16"])
+@pytest.mark.parametrize("prec", ["fp32", "tf32", "bf16", "fp16"])
 @pytest.mark.parametrize("ch", [32, 16])
 def test_width_sweep_parity(prec, ch):
     ev = make_events("run3", 16, 1004)
@@ -235,7 +236,7 @@ def test_width_sweep_parity(prec, ch):
     assert np.abs(probs.cpu().numpy().astype(np.float64) - ref["probs"]).max() <= TOL[prec]
 
 
-@pytest.mark.parametrize("prec", ["fp32", "tf32", "bf16"])
+@pytest.mark.parametrize("prec", ["fp32", "tf32", "bf16", "fp16"])
 def test_unet_entry_point_on_synthetic_histograms(prec):
     """UNet alone: zero input (bias-only), one-hot inputs at the interval edges (padding), large values."""
     w = make_weights("rand", 5)
