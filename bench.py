@@ -36,8 +36,19 @@ if ROOT not in sys.path:
 from pvf_inputs import make_events, make_weights, select_events  # noqa: E402
 
 UNET_FLOP_PER_EVENT = {64: 2.5196e9, 32: 0.65562e9, 16: 0.17677e9}
-SEEDS = {"run3": 1002, "pileup": 1003}
+SEEDS = {"run3": 1002, "pileup": 1003, "single": 1000}
 METRIC = "PVFinder events/s (whole hot path) on B200"
+
+
+def _config_id(args):
+    """Which BASELINE.json config the flags correspond to (label only)."""
+    if args.model == "single":
+        return "0"
+    if args.model == "pileup":
+        return "3"
+    if args.channels != 64 or args.precision in ("bf16", "fp16"):
+        return "4"
+    return "1" if args.events == 1000 else "2"
 
 
 def _peaks_file():
@@ -246,10 +257,11 @@ def main_ours(args, rank, world, local_rank):
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": {"fp32": "f32", "tf32": "tf32", "bf16": "bf16", "fp16": "f16"}[args.precision],
         "data": "synthetic",
-        "config": {"workload": f"BASELINE.json config {'3' if args.model == 'pileup' else '2'}: {E} events/GPU, "
+        "config": {"workload": f"BASELINE.json config {_config_id(args)}: {E} events/GPU, "
                                f"model {args.model}, {ev.n_tracks} tracks, UNet {args.channels} ch, weights {args.weights}",
                    "precision": args.precision, "split_mask": split,
-                   "cache": "inputs larger than L2 (107 MB features, 2 GB histogram per step)"},
+                   "cache": ("inputs larger than L2 (107 MB features, 2 GB histogram per step)" if E >= 2000 else
+                             "small batch: inputs fit in L2 (latency-style measurement)")},
         "us_per_event": ms * 1e3 / (args.steps * E),
         "stage_ms": {"sort": stage[0], "fc_hist": stage[1], "unet": stage[2], "peaks": stage[3]},
         "stage_us_per_event": {k: v * 1e3 / E for k, v in zip(("sort", "fc_hist", "unet", "peaks"), stage)},
@@ -280,7 +292,7 @@ def main():
     ap.add_argument("--precision", default=os.environ.get("PVF_BENCH_PRECISION", "tf32"), choices=["fp32", "tf32", "bf16", "fp16"])
     ap.add_argument("--split-mask", type=int, default=-1)
     ap.add_argument("--events", type=int, default=16000)
-    ap.add_argument("--model", default="run3", choices=["run3", "pileup"])
+    ap.add_argument("--model", default="run3", choices=["run3", "pileup", "single"])
     ap.add_argument("--weights", default="peaky", choices=["peaky", "rand"])
     ap.add_argument("--channels", type=int, default=64, choices=[64, 32, 16])
     ap.add_argument("--cpu-sample", type=int, default=64)

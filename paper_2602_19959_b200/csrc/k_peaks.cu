@@ -9,7 +9,7 @@
 //   first 32 in ascending g are kept, count = min(found, 32), overflow flag if found > 32
 //   lo = max(g-3,0), hi = min(g+3,3999); s0 = s1 = 0; for j = lo..hi: s0 += P[j]; s1 += P[j]*(j-g)
 //   z = ((g + 0.5) + s1/s0) * 0.1 + (-200)
-// One warp per event; 32 consecutive bins per step; ordered compaction by ballot.
+// One warp per event; 32 consecutive bins per step, five steps' loads in flight; ordered compaction by ballot.
 #include "pvf_internal.cuh"
 
 namespace pvf {
@@ -26,33 +26,46 @@ k_peaks(const float* __restrict__ probs, int n_events, float thr, const uint32_t
   const float* P = probs + (size_t)e * kGlobalBins;
   const float ninf = __int_as_float(0xff800000);
   int found = 0;
-  for (int g0 = 0; g0 < kGlobalBins; g0 += 32) {
-    const int g = g0 + lane;
-    const float c = P[g];                       // 4000 = 125 * 32: always in range
-    float l = __shfl_up_sync(0xffffffffu, c, 1);
-    float r = __shfl_down_sync(0xffffffffu, c, 1);
-    if (lane == 0) l = g > 0 ? P[g - 1] : ninf;
-    if (lane == 31) r = g < kGlobalBins - 1 ? P[g + 1] : ninf;
-    const bool is_peak = (c > thr) && (c > l) && (c >= r);
-    const unsigned m = __ballot_sync(0xffffffffu, is_peak);
-    const int slot = found + __popc(m & ((1u << lane) - 1u));
-    if (is_peak && slot < kMaxPeaks) {
-      const int lo = max(g - kPeakHalf, 0), hi = min(g + kPeakHalf, kGlobalBins - 1);
-      float s0 = 0.0f, s1 = 0.0f;
-      for (int j = lo; j <= hi; ++j) {
-        const float pj = P[j];
-        s0 = __fadd_rn(s0, pj);
-        s1 = __fadd_rn(s1, __fmul_rn(pj, (float)(j - g)));
+  constexpr int kBatch = 5;                     // 4000 = 25 * 5 * 32: five independent 128-byte loads in flight
+  for (int gb = 0; gb < kGlobalBins; gb += 32 * kBatch) {
+    float cv[kBatch];
+#pragma unroll
+    for (int b = 0; b < kBatch; ++b) cv[b] = P[gb + 32 * b + lane];
+    // neighbours across the 32-bin steps: lane 0 needs the last value of the previous step, lane 31 the
+    // first of the next one; inside the batch they come from the registers of other lanes
+    const float prev_edge = gb > 0 ? P[gb - 1] : ninf;
+    const float next_edge = gb + 32 * kBatch < kGlobalBins ? P[gb + 32 * kBatch] : ninf;
+#pragma unroll
+    for (int b = 0; b < kBatch; ++b) {
+      const int g = gb + 32 * b + lane;
+      const float c = cv[b];
+      float l = __shfl_up_sync(0xffffffffu, c, 1);
+      float r = __shfl_down_sync(0xffffffffu, c, 1);
+      const float l_in = b > 0 ? __shfl_sync(0xffffffffu, cv[b > 0 ? b - 1 : 0], 31) : prev_edge;
+      const float r_in = b + 1 < kBatch ? __shfl_sync(0xffffffffu, cv[b + 1 < kBatch ? b + 1 : b], 0) : next_edge;
+      if (lane == 0) l = l_in;
+      if (lane == 31) r = r_in;
+      const bool is_peak = (c > thr) && (c > l) && (c >= r);
+      const unsigned m = __ballot_sync(0xffffffffu, is_peak);
+      const int slot = found + __popc(m & ((1u << lane) - 1u));
+      if (is_peak && slot < kMaxPeaks) {
+        const int lo = max(g - kPeakHalf, 0), hi = min(g + kPeakHalf, kGlobalBins - 1);
+        float s0 = 0.0f, s1 = 0.0f;
+        for (int j = lo; j <= hi; ++j) {
+          const float pj = P[j];
+          s0 = __fadd_rn(s0, pj);
+          s1 = __fadd_rn(s1, __fmul_rn(pj, (float)(j - g)));
+        }
+        const float delta = __fdiv_rn(s1, s0);
+        const float t = __fadd_rn(__fadd_rn((float)g, 0.5f), delta);
+        const float z = __fadd_rn(__fmul_rn(t, 0.1f), -200.0f);
+        const size_t o = (size_t)e * kMaxPeaks + slot;
+        z_mm[o] = z;
+        prob[o] = c;
+        bin[o] = g;
       }
-      const float delta = __fdiv_rn(s1, s0);
-      const float t = __fadd_rn(__fadd_rn((float)g, 0.5f), delta);
-      const float z = __fadd_rn(__fmul_rn(t, 0.1f), -200.0f);
-      const size_t o = (size_t)e * kMaxPeaks + slot;
-      z_mm[o] = z;
-      prob[o] = c;
-      bin[o] = g;
+      found += __popc(m);
     }
-    found += __popc(m);
   }
   const int kept = min(found, kMaxPeaks);
   if (lane >= kept) {   // kMaxPeaks == 32 == warp size: lane s clears slot s
