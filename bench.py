@@ -163,7 +163,7 @@ def main_ours(args, rank, world, local_rank):
     w = make_weights(args.weights, 1, args.channels)
     split = args.split_mask if args.split_mask >= 0 else (1 if args.precision == "tf32" else 0)
     pvf = PVFinder(w, max_events=E, max_tracks=ev.n_tracks, precision=args.precision, split_mask=split,
-                   stage_timing=True, host_io=True)
+                   stage_timing=True, host_io=True, elide_empty=args.elide_empty)
     feat = torch.from_numpy(ev.feat).cuda()
     off = torch.from_numpy(ev.event_offsets).cuda()
     probs = torch.empty(E, 4000, device="cuda")
@@ -235,6 +235,15 @@ def main_ours(args, rank, world, local_rank):
 
     peaks, peaks_src = _peaks_file()
     flop = UNET_FLOP_PER_EVENT[args.channels] * E
+    nonempty = None
+    if args.elide_empty:
+        # executed-FLOP accounting: only the intervals that hold a track go through the UNet
+        z = ev.feat[0]
+        iv = np.floor((z.astype(np.float32) + np.float32(200.0)) * np.float32(0.1)).astype(np.int64)   # bookkeeping only
+        evi = np.repeat(np.arange(E), np.diff(ev.event_offsets))
+        ok = np.isfinite(z) & (iv >= 0) & (iv < 40)
+        nonempty = float(np.unique(evi[ok] * 40 + iv[ok]).size) / (E * 40)
+        flop *= nonempty
     unet_s = stage[2] * 1e-3
     if args.precision == "fp32":
         bound, peak = "alu", 148 * 128 * 2 * 1.965e9 / 1e12
@@ -260,6 +269,7 @@ def main_ours(args, rank, world, local_rank):
         "config": {"workload": f"BASELINE.json config {_config_id(args)}: {E} events/GPU, "
                                f"model {args.model}, {ev.n_tracks} tracks, UNet {args.channels} ch, weights {args.weights}",
                    "precision": args.precision, "split_mask": split,
+                   "elide_empty_intervals": bool(args.elide_empty), "nonempty_interval_fraction": nonempty,
                    "cache": ("inputs larger than L2 (107 MB features, 2 GB histogram per step)" if E >= 2000 else
                              "small batch: inputs fit in L2 (latency-style measurement)")},
         "us_per_event": ms * 1e3 / (args.steps * E),
@@ -299,6 +309,8 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=16)
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--elide-empty", action="store_true",
+                    help="NEXT-2 mode: UNet only over non-empty intervals (reported with executed-FLOP accounting)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     rank = int(os.environ.get("RANK", "0"))

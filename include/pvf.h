@@ -80,6 +80,10 @@ typedef struct {
   int64_t max_tracks;      /* capacity the pool is sized for (>= 1) */
   int32_t enable_stage_timing; /* pre-creates CUDA events around the four stages; default 0 */
   int32_t enable_host_io;  /* reserve pool space for pvf_run_host's device staging; default 0 */
+  int32_t elide_empty_intervals; /* tensor-core modes only; default 0.  1: the UNet runs only over intervals that
+                              hold at least one track, every empty interval gets the precomputed vector
+                              UNet(0) -- bit-identical output, fewer executed FLOPs (our optimisation, not the
+                              method's: SURVEY.md section 8f NEXT-2; reported separately by bench.py) */
 } pvf_config;
 
 /* Fill *cfg with BASELINE.json config 0 (64 channels, FP32) and the given capacities. */

@@ -37,7 +37,7 @@ class pvf_config(C.Structure):
         ("leaky_slope", C.c_float), ("peak_threshold", C.c_float), ("peak_halfwidth", C.c_int32),
         ("max_peaks", C.c_int32), ("precision", C.c_int32), ("split_mask", C.c_int32),
         ("max_events", C.c_int32), ("max_tracks", C.c_int64), ("enable_stage_timing", C.c_int32),
-        ("enable_host_io", C.c_int32),
+        ("enable_host_io", C.c_int32), ("elide_empty_intervals", C.c_int32),
     ]
 
 
@@ -120,7 +120,8 @@ class PVFinder:
     """One pvf_handle.  Methods mirror the C entry points; tensors are torch CUDA tensors."""
 
     def __init__(self, weights, max_events: int, max_tracks: int, precision="fp32", channels: int | None = None,
-                 split_mask: int = 0, stage_timing: bool = False, host_io: bool = False, pool=None, lib=None,
+                 split_mask: int = 0, stage_timing: bool = False, host_io: bool = False, elide_empty: bool = False,
+                 pool=None, lib=None,
                  **cfg_over):
         import torch  # device memory + streams only
         self.torch = torch
@@ -129,7 +130,7 @@ class PVFinder:
         prec = PRECISIONS[precision] if isinstance(precision, str) else int(precision)
         self.cfg = default_config(self.lib, max_events, max_tracks, unet_channels=ch, precision=prec,
                                   split_mask=split_mask, enable_stage_timing=int(stage_timing),
-                                  enable_host_io=int(host_io), **cfg_over)
+                                  enable_host_io=int(host_io), elide_empty_intervals=int(elide_empty), **cfg_over)
         ws, keep = _weights_struct(weights)
         self.handle = C.c_void_p()
         if pool is None:

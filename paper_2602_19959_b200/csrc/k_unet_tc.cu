@@ -192,7 +192,8 @@ enum { kE1 = 0, kE2 = 1, kB = 2, kD2 = 3, kD1 = 4 };
 template <int C, int BF16, int MODE>
 __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_base, int tile, int q, int lane,
                                               const float* __restrict__ par, int n_valid_int,
-                                              float* __restrict__ probs_group, float* __restrict__ scr) {
+                                              float* __restrict__ probs_group, float* __restrict__ scr,
+                                              const int* __restrict__ list_g) {
   using G = Geo<C, BF16>;
   const int m = 32 * q + lane;
   const float* bias = par + MODE * C;
@@ -279,7 +280,9 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
   if (MODE == kD1) {
     if (valid && interval < n_valid_int) {
       const float a = logit + par[6 * C];
-      probs_group[interval * kBins + l] = 1.0f / (1.0f + expf(-a));
+      // list_g != nullptr: the group's intervals are rows list_g[0..T) of the full output (empty-interval elision)
+      const size_t row = list_g ? (size_t)list_g[interval] : (size_t)interval;
+      probs_group[row * kBins + l] = 1.0f / (1.0f + expf(-a));
     }
   }
 }
@@ -289,7 +292,7 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
 // rows and the gap rows l >= 100 of every interval as zeros.
 template <int C, int BF16>
 __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restrict__ hist, long long g0,
-                                        int n_valid_int, int split, int tid) {
+                                        int n_valid_int, int split, int tid, const int* __restrict__ list) {
   using G = Geo<C, BF16>;
   const uint32_t x0 = smem_base + G::OFF_XP;
   const uint4 zero4 = make_uint4(0, 0, 0, 0);
@@ -299,9 +302,10 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
     for (int it = tid; it < G::T * 128; it += 128) {
       const int t = it >> 7, l = it & 127;
       const bool live = l < 100 && t < n_valid_int;
+      const long long src = !live ? 0 : (list ? (long long)list[g0 + t] : g0 + t);
       float x[8];
 #pragma unroll
-      for (int c = 0; c < 8; ++c) x[c] = live ? __ldg(hist + (g0 + t) * kFcOut + c * kBins + l) : 0.0f;
+      for (int c = 0; c < 8; ++c) x[c] = live ? __ldg(hist + src * kFcOut + c * kBins + l) : 0.0f;
       uint4 qv;
       qv.x = pack16<BF16>(x[0], x[1]); qv.y = pack16<BF16>(x[2], x[3]);
       qv.z = pack16<BF16>(x[4], x[5]); qv.w = pack16<BF16>(x[6], x[7]);
@@ -313,9 +317,10 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
     for (int it = tid; it < G::T * 256; it += 128) {
       const int t = it >> 8, qc = (it >> 7) & 1, l = it & 127;
       const bool live = l < 100 && t < n_valid_int;
+      const long long src = !live ? 0 : (list ? (long long)list[g0 + t] : g0 + t);
       float x[4];
 #pragma unroll
-      for (int c = 0; c < 4; ++c) x[c] = live ? __ldg(hist + (g0 + t) * kFcOut + (4 * qc + c) * kBins + l) : 0.0f;
+      for (int c = 0; c < 4; ++c) x[c] = live ? __ldg(hist + src * kFcOut + (4 * qc + c) * kBins + l) : 0.0f;
       uint4 hi;
       hi.x = to_tf32(x[0]); hi.y = to_tf32(x[1]); hi.z = to_tf32(x[2]); hi.w = to_tf32(x[3]);
       const uint32_t row = (uint32_t)(G::LEAD1 + 128 * t + l) * 16u;
@@ -425,7 +430,10 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
 template <int C, int BF16>
 __global__ void __launch_bounds__(kTcThreads, 1)
 k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __restrict__ wpack, int split_e1,
-          float* __restrict__ probs) {
+          float* __restrict__ probs, const int* __restrict__ list, const int* __restrict__ n_list) {
+  // list / n_list (device, optional): process only intervals list[0 .. *n_list) of hist / probs (elision of
+  // empty intervals); n_int is then only the capacity the grid was sized for
+  if (n_list != nullptr) n_int = *n_list;
   using G = Geo<C, BF16>;
   extern __shared__ __align__(1024) unsigned char smem[];
   const uint32_t sb = smem_u32(smem);
@@ -539,35 +547,37 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
       const bool has_next = g + stride < n_groups;
       const long long gn0 = (long long)(g + stride) * G::T;
       const int n_valid_next = has_next ? (int)min((long long)G::T, (long long)n_int - gn0) : 0;
-      float* pg = probs + g0 * kBins;
+      float* pg = list ? probs : probs + g0 * kBins;
+      const int* lg = list ? list + g0 : nullptr;
+      const int* lgn = list ? list + gn0 : nullptr;
       if (first) {
-        load_x0<C, BF16>(sb, hist, g0, n_valid, split_e1, et);
+        load_x0<C, BF16>(sb, hist, g0, n_valid, split_e1, et, list);
         done(0);
         wait_acc(0);
-        for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kE1>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr());
+        for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kE1>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr(), lg);
         done(1);
         first = false;
       }
       wait_acc(1);
-      for (int t = 0; t < G::T / 2; ++t) epilogue_tile<C, BF16, kE2>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr());
+      for (int t = 0; t < G::T / 2; ++t) epilogue_tile<C, BF16, kE2>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr(), lg);
       done(2);
       if (has_next) {                                // P1 is dead (e2's MMAs retired): stage the next input
-        load_x0<C, BF16>(sb, hist, gn0, n_valid_next, split_e1, et);
+        load_x0<C, BF16>(sb, hist, gn0, n_valid_next, split_e1, et, list);
         done(0);
       }
       wait_acc(2);
-      for (int t = 0; t < (G::T + 3) / 4; ++t) epilogue_tile<C, BF16, kB>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr());
+      for (int t = 0; t < (G::T + 3) / 4; ++t) epilogue_tile<C, BF16, kB>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr(), lg);
       done(3);
       wait_acc(3);
-      for (int t = 0; t < G::T / 2; ++t) epilogue_tile<C, BF16, kD2>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr());
+      for (int t = 0; t < G::T / 2; ++t) epilogue_tile<C, BF16, kD2>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr(), lg);
       done(4);
       if (has_next) {
         wait_acc(0);
-        for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kE1>(sb, tmem_base, t, q, lane, par, n_valid_next, pg, scr());
+        for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kE1>(sb, tmem_base, t, q, lane, par, n_valid_next, pg, scr(), lgn);
         done(1);
       }
       wait_acc(4);
-      for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kD1>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr());
+      for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kD1>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr(), lg);
       done(5);
     }
   }
@@ -665,12 +675,12 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst) {
 
 template <int C, int BF16>
 void launch_impl(const float* hist, int n_int, const void* packed, int split_e1, float* probs, int sm_count,
-                 cudaStream_t s) {
+                 const int* list, const int* n_list, cudaStream_t s) {
   using G = Geo<C, BF16>;
   const int n_groups = (n_int + G::T - 1) / G::T;
   const int grid = n_groups < sm_count ? n_groups : sm_count;
   k_unet_tc<C, BF16><<<grid, kTcThreads, G::SMEM, s>>>(hist, n_int, static_cast<const unsigned char*>(packed),
-                                                      split_e1, probs);
+                                                      split_e1, probs, list, n_list);
 }
 
 template <int C, int BF16>
@@ -714,9 +724,10 @@ cudaError_t unet_tc_setup(int channels, int precision, int split_mask) {
 }
 
 void launch_unet_tc(const float* hist, int n_intervals_total, const void* packed_dev, int channels, int precision,
-                    int split_mask, float* probs, int sm_count, cudaStream_t s) {
+                    int split_mask, float* probs, int sm_count, const int* list, const int* n_list, cudaStream_t s) {
   if (n_intervals_total <= 0) return;
-#define PVF_CALL(C_, B_) launch_impl<C_, B_>(hist, n_intervals_total, packed_dev, split_mask & 1, probs, sm_count, s)
+#define PVF_CALL(C_, B_) \
+  launch_impl<C_, B_>(hist, n_intervals_total, packed_dev, split_mask & 1, probs, sm_count, list, n_list, s)
   PVF_TC_DISPATCH(PVF_CALL);
 #undef PVF_CALL
 }

@@ -25,7 +25,10 @@ struct pvf_ctx {
   float* conv_f32 = nullptr;      // PyTorch-layout conv params (FP32 path + head of every path)
   UnetParamsF32 conv_ptrs{};
   void* tc_packed = nullptr;
-  void* fc_w5img = nullptr;       // tcgen05 image of the 25 -> 800 layer (TF32 / BF16 modes)
+  void* fc_w5img = nullptr;
+  int32_t* el_list = nullptr;     // empty-interval elision: work list, its length, UNet(0)
+  int32_t* el_count = nullptr;
+  float* el_p0 = nullptr;       // tcgen05 image of the 25 -> 800 layer (TF32 / BF16 modes)
   int32_t* perm = nullptr;
   int32_t* seg_off = nullptr;
   int32_t* seg_cnt = nullptr;
@@ -52,7 +55,7 @@ namespace {
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 struct Layout {
-  size_t fc_params, conv_f32, tc_packed, fc_w5img, perm, seg_off, seg_cnt, flags, hist;
+  size_t fc_params, conv_f32, tc_packed, fc_w5img, el_list, el_count, el_p0, perm, seg_off, seg_cnt, flags, hist;
   size_t st_feat, st_off, st_probs, st_z, st_prob, st_bin, st_count, st_flags, total;
   size_t conv_w_off[6], conv_b_off[6];  // float offsets inside conv_f32
 };
@@ -75,6 +78,7 @@ bool config_ok(const pvf_config* c) {
   if (c->precision < PVF_PREC_FP32 || c->precision > PVF_PREC_FP16) return false;
   if (c->split_mask < 0 || c->split_mask > 31) return false;
   if (c->max_events < 1 || c->max_tracks < 1 || c->max_tracks > 0x7fffffffLL) return false;
+  if (c->elide_empty_intervals && c->precision == PVF_PREC_FP32) return false;   // tensor-core modes only
   return true;
 }
 
@@ -94,6 +98,9 @@ Layout make_layout(const pvf_config* c) {
   L.tc_packed = take(c->precision == PVF_PREC_FP32 ? 0 : unet_tc_packed_bytes(c->unet_channels, c->precision, c->split_mask));
   const size_t E = (size_t)c->max_events, T = (size_t)c->max_tracks;
   L.fc_w5img = take(c->precision == PVF_PREC_FP32 ? 0 : fc_tc_packed_bytes());
+  L.el_list = take(c->elide_empty_intervals ? sizeof(int32_t) * E * kIntervals : 0);
+  L.el_count = take(c->elide_empty_intervals ? 256 : 0);
+  L.el_p0 = take(c->elide_empty_intervals ? sizeof(float) * kGlobalBins : 0);
   L.perm = take(sizeof(int32_t) * T);
   L.seg_off = take(sizeof(int32_t) * E * kIntervals);
   L.seg_cnt = take(sizeof(int32_t) * E * kIntervals);
@@ -123,6 +130,9 @@ pvf_status fail_cuda(pvf_ctx* h, cudaError_t e, const char* where) {
     cudaError_t e__ = (call);                                         \
     if (e__ != cudaSuccess) return fail_cuda((h), e__, #call);        \
   } while (0)
+
+void enqueue_unet(pvf_ctx* h, const float* hist, int n_events, float* out_probs, cudaStream_t s,
+                  const int* list = nullptr, const int* n_list = nullptr);
 
 bool peaks_ok(const pvf_peaks* p) { return p && p->z_mm && p->prob && p->bin && p->count; }
 
@@ -157,6 +167,9 @@ pvf_status create_impl(const pvf_weights* w, const pvf_config* cfg, void* dev_po
   h->conv_f32 = reinterpret_cast<float*>(B + L.conv_f32);
   h->tc_packed = B + L.tc_packed;
   h->fc_w5img = B + L.fc_w5img;
+  h->el_list = reinterpret_cast<int32_t*>(B + L.el_list);
+  h->el_count = reinterpret_cast<int32_t*>(B + L.el_count);
+  h->el_p0 = reinterpret_cast<float*>(B + L.el_p0);
   h->perm = reinterpret_cast<int32_t*>(B + L.perm);
   h->seg_off = reinterpret_cast<int32_t*>(B + L.seg_off);
   h->seg_cnt = reinterpret_cast<int32_t*>(B + L.seg_cnt);
@@ -212,6 +225,18 @@ pvf_status create_impl(const pvf_weights* w, const pvf_config* cfg, void* dev_po
       }
     }
   }
+  if (e == cudaSuccess && cfg->elide_empty_intervals) {
+    // UNet(0): one event's worth of zero histograms through the very kernel pvf_run uses, on a private
+    // stream (create is not on the hot path); every interval of it is the constant vector
+    cudaStream_t cs = nullptr;
+    e = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaMemsetAsync(h->hist, 0, sizeof(float) * kIntervals * kFcOut, cs);
+    if (e == cudaSuccess) {
+      enqueue_unet(h, h->hist, 1, h->el_p0, cs);
+      e = cudaStreamSynchronize(cs);
+    }
+    if (cs) cudaStreamDestroy(cs);
+  }
   if (e == cudaSuccess && cfg->enable_stage_timing)
     for (int r = 0; r < pvf_ctx::kTimedRuns; ++r)
       for (int k = 0; k < 5 && e == cudaSuccess; ++k) e = cudaEventCreate(&h->ev[r][k]);
@@ -223,13 +248,14 @@ pvf_status create_impl(const pvf_weights* w, const pvf_config* cfg, void* dev_po
   return PVF_OK;
 }
 
-void enqueue_unet(pvf_ctx* h, const float* hist, int n_events, float* out_probs, cudaStream_t s) {
+void enqueue_unet(pvf_ctx* h, const float* hist, int n_events, float* out_probs, cudaStream_t s, const int* list,
+                  const int* n_list) {
   const int n_int = n_events * kIntervals;
   if (h->cfg.precision == PVF_PREC_FP32)
     launch_unet_simt(hist, n_int, h->conv_ptrs, h->cfg.unet_channels, out_probs, s);
   else
     launch_unet_tc(hist, n_int, h->tc_packed, h->cfg.unet_channels, h->cfg.precision, h->cfg.split_mask,
-                   out_probs, h->sm_count, s);
+                   out_probs, h->sm_count, list, n_list, s);
 }
 
 }  // namespace
@@ -245,7 +271,7 @@ void pvf_default_config(pvf_config* c, int32_t max_events, int64_t max_tracks) {
   c->leaky_slope = kLeaky; c->peak_threshold = 0.01f; c->peak_halfwidth = kPeakHalf; c->max_peaks = kMaxPeaks;
   c->precision = PVF_PREC_FP32; c->split_mask = 0;
   c->max_events = max_events; c->max_tracks = max_tracks;
-  c->enable_stage_timing = 0; c->enable_host_io = 0;
+  c->enable_stage_timing = 0; c->enable_host_io = 0; c->elide_empty_intervals = 0;
 }
 
 size_t pvf_workspace_bytes(const pvf_config* cfg) {
@@ -283,7 +309,12 @@ pvf_status pvf_run(pvf_handle h, const pvf_tracks* t, int32_t n_events, float* o
     launch_fc_hist_tc(t->feat, t->event_offsets, h->perm, h->seg_off, h->seg_cnt, h->fc_params, h->fc_w5img, n_events,
                       h->hist, h->sm_count, s);
   if (timing) cudaEventRecord(ev[2], s);
-  enqueue_unet(h, h->hist, n_events, out_probs, s);
+  if (h->cfg.elide_empty_intervals) {
+    launch_compact_fill(h->seg_cnt, n_events * kIntervals, h->el_list, h->el_count, h->el_p0, out_probs, s);
+    enqueue_unet(h, h->hist, n_events, out_probs, s, h->el_list, h->el_count);
+  } else {
+    enqueue_unet(h, h->hist, n_events, out_probs, s);
+  }
   if (timing) cudaEventRecord(ev[3], s);
   launch_peaks(out_probs, n_events, h->cfg.peak_threshold, h->flags, pk->z_mm, pk->prob, pk->bin, pk->count,
                pk->event_flags, s);
@@ -376,7 +407,8 @@ pvf_status pvf_stage_times_ms(pvf_handle h, float out_ms[4]) {
 
 int32_t pvf_launches_per_run(pvf_handle h, int32_t n_events) {
   if (!h || n_events <= 0) return 0;
-  return 1 /*sort*/ + fc_hist_launches(n_events) + 1 /*unet*/ + 1 /*peaks*/;
+  return 1 /*sort*/ + fc_hist_launches(n_events) + 1 /*unet*/ + 1 /*peaks*/ +
+         (h->cfg.elide_empty_intervals ? 2 /*work list, constant fill*/ : 0);
 }
 
 pvf_status pvf_destroy(pvf_handle h) {

@@ -71,8 +71,14 @@ size_t unet_tc_packed_bytes(int channels, int precision, int split_mask);
 // packs PyTorch-layout host weights into the shared-memory image order the kernel streams
 void unet_tc_pack(const pvf_weights* w, int channels, int precision, int split_mask, void* host_dst);
 cudaError_t unet_tc_setup(int channels, int precision, int split_mask);
+// list / n_list (device, optional): run only over intervals list[0 .. *n_list) (empty-interval elision)
 void launch_unet_tc(const float* hist, int n_intervals_total, const void* packed_dev, int channels,
-                    int precision, int split_mask, float* probs, int sm_count, cudaStream_t s);
+                    int precision, int split_mask, float* probs, int sm_count, const int* list, const int* n_list,
+                    cudaStream_t s);
+
+// NEXT-2, empty-interval elision (k_compact.cu): work list of non-empty intervals + constant fill of the rest
+void launch_compact_fill(const int32_t* seg_cnt, int n_total, int32_t* list, int32_t* n_list, const float* p0,
+                         float* probs, cudaStream_t s);
 
 // a4: peak finder (k_peaks.cu)
 void launch_peaks(const float* probs, int n_events, float threshold, const uint32_t* flags_in,

@@ -261,6 +261,32 @@ def test_unet_entry_point_on_synthetic_histograms(prec):
     assert np.all(got[0].reshape(40, 100) == got[0, :100])       # identical bias-only vector everywhere
 
 
+# ------------------------------------------------------------------ NEXT-2: empty-interval elision
+@pytest.mark.parametrize("prec", ["tf32", "bf16", "fp16"])
+def test_empty_interval_elision_is_bit_identical(prec):
+    """The UNet run only over non-empty intervals + the constant UNet(0) vector elsewhere must reproduce the
+    plain path bit for bit (an interval's result does not depend on its group mates); includes an event
+    without tracks and a batch whose non-empty count is not a multiple of the group size."""
+    base = make_events("run3", 37, 555)
+    feats = [base.feat[:, : base.event_offsets[20]], np.zeros((9, 0), np.float32), base.feat[:, base.event_offsets[20]:]]
+    offs = np.concatenate([base.event_offsets[:21], base.event_offsets[20:] ]).astype(np.int32)
+    ev = type(base)(np.ascontiguousarray(np.concatenate(feats, axis=1)), offs, [None] * 38)
+    w = make_weights("peaky", 2)
+    plain = _make(w, ev, prec)
+    elided = _make(w, ev, prec, elide_empty=True)
+    p1, k1 = _run(plain, ev)
+    p2, k2 = _run(elided, ev)
+    assert torch.equal(p1, p2)
+    assert all(torch.equal(k1[k], k2[k]) for k in k1)
+    assert elided.launches_per_run(ev.n_events) == plain.launches_per_run(ev.n_events) + 2
+    P = p2.cpu().numpy().reshape(38, 40, 100)
+    assert np.all(P[20] == P[20, 0])                              # the empty event: UNet(0) everywhere
+    p3, _ = _run(elided, ev)                                      # and again (work-list order may differ)
+    assert torch.equal(p2, p3)
+    with pytest.raises(pkg.PVFError):
+        _make(w, ev, "fp32", elide_empty=True)                    # tensor-core modes only
+
+
 # ------------------------------------------------------------------ boundary behaviour
 def test_boundary_contract():
     ev = make_events("run3", 4, 77)
