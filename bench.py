@@ -103,6 +103,26 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def rank_seed(model, rank):
+    """Every rank is a replica with its OWN batch (events are independent): no collective
+    on the data path, weak scaling."""
+    return SEEDS[model] + rank
+
+
+def max_over_ranks(values, dist, device):
+    """Device-timed durations -> the slowest rank's (the job is as fast as its slowest replica)."""
+    import torch
+    t = torch.tensor(list(values), device=device, dtype=torch.float64)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def whole_job_rate(world, events_per_rank, steps, ms):
+    """Whole-job events/s: all ranks' events over the max-over-ranks time."""
+    return world * events_per_rank * steps / (ms * 1e-3)
+
+
 def run_oracle_sample(ev, w, n_sample):
     """Oracle timed as it stands on the first n_sample events.  Returns (events/s, seconds, threads)."""
     from oracle import pvf_oracle as O   # bench.py's cpu_baseline / reference legs may execute oracle/
@@ -159,7 +179,7 @@ def main_ours(args, rank, world, local_rank):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     E = args.events
-    ev = make_events(args.model, E, SEEDS[args.model] + rank)
+    ev = make_events(args.model, E, rank_seed(args.model, rank))
     w = make_weights(args.weights, 1, args.channels)
     split = args.split_mask if args.split_mask >= 0 else (1 if args.precision == "tf32" else 0)
     pvf = PVFinder(w, max_events=E, max_tracks=ev.n_tracks, precision=args.precision, split_mask=split,
@@ -222,16 +242,13 @@ def main_ours(args, rank, world, local_rank):
     h2d = int(hfeat.numel() * 4 + hoff.numel() * 4)
     d2h = int(hprobs.numel() * 4 + sum(v.numel() * v.element_size() for v in hpk.values()))
 
-    t = torch.tensor([ms, ms_e2e], device="cuda", dtype=torch.float64)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms, ms_e2e = float(t[0]), float(t[1])
+    ms, ms_e2e = max_over_ranks([ms, ms_e2e], dist, "cuda")
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return
-    value = world * E * args.steps / (ms * 1e-3)
-    e2e_value = world * E * n_e2e / (ms_e2e * 1e-3)
+    value = whole_job_rate(world, E, args.steps, ms)
+    e2e_value = whole_job_rate(world, E, n_e2e, ms_e2e)
 
     peaks, peaks_src = _peaks_file()
     flop = UNET_FLOP_PER_EVENT[args.channels] * E
