@@ -104,16 +104,44 @@ def fc_forward(x, fc_w, fc_b):
 # O4 histogram -- PAPER.md:29 "combining each track's contribution into a 800-bin histogram";
 # PAPER.md:49 (garbled "B=40, C=64, L=800") read as B = 40 intervals, C = 8, L = 100  [READING].
 # ----------------------------------------------------------------------------------------------
-def histogram(feat, event_offsets, fc_w, fc_b):
+def boundary_neighbours(interval, zrel, margin_mm):
+    """NEXT-1 -- PAPER.md:49 "tracks on boundaries of intervals are part of two intervals".
+    [READING] (the paper gives no margin): a kept track whose z lies within ``margin_mm`` of its
+    interval's lower (upper) edge ALSO contributes to the previous (next) interval, there with
+    z_rel' = z_rel + 1 (z_rel - 1), i.e. still measured from that interval's lower edge; intervals -1 and
+    40 do not exist.  Decisions and z_rel' in float32:  m = margin_mm * 0.1f;  lower side iff
+    z_rel < m;  upper side iff z_rel >= 1f - m  (margin < 5 mm, so never both).
+    Returns (neighbour int32 [T]: -1 none else the extra interval, zrel2 float32 [T])."""
+    f32 = np.float32
+    m = f32(f32(margin_mm) * f32(0.1))
+    interval = np.asarray(interval, np.int32)
+    zrel = np.asarray(zrel, np.float32)
+    nb = np.full(interval.shape, -1, np.int32)
+    z2 = np.zeros(interval.shape, np.float32)
+    if not (m > 0):
+        return nb, z2
+    assert m < f32(0.5)
+    lower = (interval > 0) & (zrel < m)
+    upper = (interval >= 0) & (interval < N_INTERVALS - 1) & (zrel >= f32(f32(1.0) - m)) & ~lower
+    nb[lower] = interval[lower] - 1
+    z2[lower] = (zrel[lower] + f32(1.0)).astype(np.float32)
+    nb[upper] = interval[upper] + 1
+    z2[upper] = (zrel[upper] - f32(1.0)).astype(np.float32)
+    return nb, z2
+
+
+def histogram(feat, event_offsets, fc_w, fc_b, boundary_margin_mm=0.0):
     """feat float32 [9, T] SoA, event_offsets int [E+1] -> (H float64 [E,40,8,100], flags uint32 [E]).
 
     H[e,i,c,l] = sum over in-range tracks t of event e with interval(t) = i, in ascending track
-    index, of fc(x_t)[c*100 + l]; empty intervals are exactly 0.
+    index, of fc(x_t)[c*100 + l]; empty intervals are exactly 0.  With boundary_margin_mm > 0 (NEXT-1)
+    boundary tracks add a second contribution to the neighbouring interval (boundary_neighbours).
     """
     feat = np.asarray(feat, np.float32)
     off = np.asarray(event_offsets, np.int64)
     E = off.shape[0] - 1
     interval, zrel, nonfinite = assign_intervals(feat[0])
+    nb, zrel2 = boundary_neighbours(interval, zrel, boundary_margin_mm)
     x = feat.astype(np.float64).T.copy()           # [T, 9]
     x[:, 0] = zrel.astype(np.float64)
     H = np.zeros((E, N_INTERVALS, FC_CHANNELS, N_BINS), np.float64)
@@ -133,6 +161,13 @@ def histogram(feat, event_offsets, fc_w, fc_b):
         contrib = fc_forward(x[lo:hi][keep], fc_w, fc_b)       # [n, 800]
         for n, t in enumerate(keep):                            # ascending original index
             H[e, iv[t]] += contrib[n].reshape(FC_CHANNELS, N_BINS)
+        extra = np.nonzero(nb[lo:hi] >= 0)[0]                   # NEXT-1: second contribution of boundary tracks
+        if extra.size:
+            x2 = x[lo:hi][extra].copy()
+            x2[:, 0] = zrel2[lo:hi][extra].astype(np.float64)
+            contrib2 = fc_forward(x2, fc_w, fc_b)
+            for n, t in enumerate(extra):
+                H[e, nb[lo + t]] += contrib2[n].reshape(FC_CHANNELS, N_BINS)
     return H, flags
 
 
@@ -260,7 +295,8 @@ def find_peaks(P):
 # ----------------------------------------------------------------------------------------------
 # whole path (call stack of PAPER.md:27-31): tracks -> FC -> histogram -> UNet -> sigmoid -> peaks
 # ----------------------------------------------------------------------------------------------
-def run(feat, event_offsets, weights, chunk_events=16, want_hist=False, operand_round=None):
+def run(feat, event_offsets, weights, chunk_events=16, want_hist=False, operand_round=None,
+        boundary_margin_mm=0.0):
     """Returns dict(probs float32 [E,4000], peaks dict, flags uint32 [E][, hist float64 [E,40,8,100]]).
     Events are processed in chunks only to bound memory; each event's result depends on its own
     tracks alone."""
@@ -273,7 +309,7 @@ def run(feat, event_offsets, weights, chunk_events=16, want_hist=False, operand_
     for lo in range(0, E, chunk_events):
         hi = min(lo + chunk_events, E)
         sub_off = off[lo:hi + 1] - off[lo]
-        H, fl = histogram(feat[:, off[lo]:off[hi]], sub_off, weights.fc_w, weights.fc_b)
+        H, fl = histogram(feat[:, off[lo]:off[hi]], sub_off, weights.fc_w, weights.fc_b, boundary_margin_mm)
         probs[lo:hi] = unet_probs(H, weights.conv_w, weights.conv_b, operand_round)
         flags[lo:hi] = fl
         if want_hist:

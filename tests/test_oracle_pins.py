@@ -350,3 +350,36 @@ def test_match_and_tau_stable():
         qb = np.nonzero((Q > 0.01) & (Q > np.r_[-np.inf, Q[:-1]]) & (Q >= np.r_[Q[1:], -np.inf]))[0]
         m, nref, _ = O.match_peaks(stable, qb)
         assert m == nref
+
+
+# ---------------------------------------------------------------- NEXT-1: boundary tracks in two intervals
+def test_boundary_tracks_contribute_to_the_neighbouring_interval():
+    """PAPER.md:49 "tracks on boundaries of intervals are part of two intervals": margin 0 is the plain
+    histogram; with a margin a track near an edge adds fc([z_rel +- 1, ...]) to the neighbour -- checked
+    against fc_forward called by hand on a three-track event; region edges have no outside neighbour."""
+    from pvf_inputs import make_weights
+    w = make_weights("rand", 4)
+    feat = np.zeros((9, 4), np.float32)
+    feat[1:] = 0.05
+    feat[0] = [-190.0 + 0.2, -200.0 + 0.1, 199.95, -185.0]       # lower edge of interval 1; region edges; mid-interval
+    off = np.array([0, 4], np.int32)
+    H0, _ = O.histogram(feat, off, w.fc_w, w.fc_b)
+    H0b, _ = O.histogram(feat, off, w.fc_w, w.fc_b, boundary_margin_mm=0.0)
+    assert np.array_equal(H0, H0b)
+    H1, _ = O.histogram(feat, off, w.fc_w, w.fc_b, boundary_margin_mm=0.5)
+    iv, zrel, _ = O.assign_intervals(feat[0])
+    assert list(iv) == [1, 0, 39, 1]
+    nb, z2 = O.boundary_neighbours(iv, zrel, 0.5)
+    assert list(nb) == [0, -1, -1, -1]                           # only the first track has a second interval
+    assert abs(float(z2[0]) - 1.02) < 1e-5
+    x = feat[:, 0].astype(np.float64).copy()
+    x[0] = float(z2[0])
+    extra = O.fc_forward(x[None, :], w.fc_w, w.fc_b)[0].reshape(8, 100)
+    assert np.allclose(H1[0, 0] - H0[0, 0], extra, rtol=0, atol=1e-12)
+    assert np.array_equal(H1[0, 1:], H0[0, 1:])                  # nothing else changes
+    # upper side: a track 0.3 mm below the upper edge of interval 7 also lands in interval 8 with z_rel - 1
+    feat2 = feat[:, :1].copy()
+    feat2[0, 0] = -200.0 + 80.0 - 0.3
+    iv2, zr2, _ = O.assign_intervals(feat2[0])
+    nb2, z22 = O.boundary_neighbours(iv2, zr2, 0.5)
+    assert iv2[0] == 7 and nb2[0] == 8 and abs(float(z22[0]) + 0.03) < 1e-5
