@@ -84,6 +84,9 @@ typedef struct {
                               hold at least one track, every empty interval gets the precomputed vector
                               UNet(0) -- bit-identical output, fewer executed FLOPs (our optimisation, not the
                               method's: SURVEY.md section 8f NEXT-2; reported separately by bench.py) */
+  float boundary_margin_mm; /* default 0 = "each track adds to the interval holding its z_poca" (BASELINE.json
+                              config 0).  > 0 (< 4.9): a track within this distance of an interval edge also
+                              contributes to the neighbouring interval, PAPER.md:49 (NEXT-1; R12) */
 } pvf_config;
 
 /* Fill *cfg with BASELINE.json config 0 (64 channels, FP32) and the given capacities. */

@@ -82,8 +82,8 @@ k_fc_hist(const float* __restrict__ f0, const float* __restrict__ f1, const floa
   __syncthreads();
 
   for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
-    const int ev_lo = event_offsets[e];
     const size_t seg0 = (size_t)e * kIntervals;
+    const int ev_lo = seg_off[seg0];          // start of the event's run of entries in perm
     const int n_kept = seg_off[seg0 + kIntervals - 1] + seg_cnt[seg0 + kIntervals - 1] - ev_lo;
     float* He = hist + (size_t)e * kIntervals * kFcOut;
     float acc[4] = {0.f, 0.f, 0.f, 0.f};
@@ -92,9 +92,9 @@ k_fc_hist(const float* __restrict__ f0, const float* __restrict__ f1, const floa
       const int ntile = min(kFcThreads, n_kept - base);
       // ---- phase A: hidden layers, one sorted track per thread
       if (tid < ntile) {
-        const int t = perm[ev_lo + base + tid];
-        float zrel; bool nf;
-        const int iv = interval_of(f0[t], zrel, nf);
+        int t;
+        float zrel;
+        const int iv = entry_interval(perm[ev_lo + base + tid], f0, t, zrel);   // own or neighbouring interval (NEXT-1)
         S.iv[tid] = iv;
         float x[kFcIn] = {zrel, f1[t], f2[t], f3[t], f4[t], f5[t], f6[t], f7[t], f8[t]};
         float h[28], g[28];

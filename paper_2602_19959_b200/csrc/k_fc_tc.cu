@@ -128,7 +128,7 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
 
   // kept (in-range) tracks of event e and the start of its run in perm
   auto kept_of = [&](int e, int& ev_lo) {
-    ev_lo = event_offsets[e];
+    ev_lo = seg_off[(size_t)e * kIntervals];            // start of the event's run of entries in perm
     const size_t s = (size_t)e * kIntervals + kIntervals - 1;
     return seg_off[s] + seg_cnt[s] - ev_lo;
   };
@@ -276,10 +276,9 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
         mbar_wait(bar(bHEmpty + g), prev);         // the MMAs that read this buffer have retired
         mbar_wait(bar(bMeta + g), prev);           // the epilogue is done with s_iv[g]
         if (base + i < nk) {
-          const int t = perm[ev_lo + base + i];
+          int t;
           float zrel;
-          bool nf;
-          const int iv = interval_of(F.f[0][t], zrel, nf);
+          const int iv = entry_interval(perm[ev_lo + base + i], F.f[0], t, zrel);   // own or neighbouring interval
           s_iv[g * kTile + i] = iv;
           const float x[kFcIn] = {zrel, F.f[1][t], F.f[2][t], F.f[3][t], F.f[4][t], F.f[5][t], F.f[6][t], F.f[7][t], F.f[8][t]};
           float h[32], gg[28];

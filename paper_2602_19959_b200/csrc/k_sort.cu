@@ -18,7 +18,7 @@ constexpr int kSortWarps = 4;
 __global__ void __launch_bounds__(kSortWarps * 32)
 k_sort(const float* __restrict__ z_poca, const int32_t* __restrict__ event_offsets, int n_events,
        int32_t* __restrict__ perm, int32_t* __restrict__ seg_off, int32_t* __restrict__ seg_cnt,
-       uint32_t* __restrict__ flags) {
+       uint32_t* __restrict__ flags, float mfrac, int two) {
   __shared__ int s_cnt[kSortWarps][kIntervals];
   __shared__ int s_base[kSortWarps][kIntervals];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -29,13 +29,17 @@ k_sort(const float* __restrict__ z_poca, const int32_t* __restrict__ event_offse
   for (int i = lane; i < kIntervals; i += 32) cnt[i] = 0;
   __syncwarp();
   const int lo = event_offsets[e], hi = event_offsets[e + 1];
+  const int plo = two ? 2 * lo : lo;        // start of the event's run in perm (two slots per track with NEXT-1)
   uint32_t fl = 0;
   for (int t = lo + lane; t < hi; t += 32) {
     bool nf;
     float zr;
     int iv = interval_of(z_poca[t], zr, nf);
-    if (iv >= 0) atomicAdd(&cnt[iv], 1);
-    else fl |= PVF_FLAG_TRACK_DROPPED | (nf ? PVF_FLAG_NONFINITE : 0u);
+    if (iv >= 0) {
+      atomicAdd(&cnt[iv], 1);
+      const int nb = neighbour_code(iv, zr, mfrac);      // NEXT-1: boundary tracks count twice
+      if (nb) atomicAdd(&cnt[nb == 1 ? iv - 1 : iv + 1], 1);
+    } else fl |= PVF_FLAG_TRACK_DROPPED | (nf ? PVF_FLAG_NONFINITE : 0u);
   }
   fl = __reduce_or_sync(0xffffffffu, fl);
   __syncwarp();
@@ -54,36 +58,64 @@ k_sort(const float* __restrict__ z_poca, const int32_t* __restrict__ event_offse
     if (lane >= d) s1 += v;
   }
   base[lane] = s0 - c0;
-  seg_off[(size_t)e * kIntervals + lane] = lo + s0 - c0;
+  seg_off[(size_t)e * kIntervals + lane] = plo + s0 - c0;
   seg_cnt[(size_t)e * kIntervals + lane] = c0;
   if (lane + 32 < kIntervals) {
     base[lane + 32] = tot0 + s1 - c1;
-    seg_off[(size_t)e * kIntervals + lane + 32] = lo + tot0 + s1 - c1;
+    seg_off[(size_t)e * kIntervals + lane + 32] = plo + tot0 + s1 - c1;
     seg_cnt[(size_t)e * kIntervals + lane + 32] = c1;
   }
   if (lane == 0) flags[e] = fl;
   __syncwarp();
   // stable placement, 32 tracks at a time in original order
-  for (int c = lo; c < hi; c += 32) {
-    const int t = c + lane;
-    int key = -1;
-    if (t < hi) { bool nf; float zr; key = interval_of(z_poca[t], zr, nf); }
-    const unsigned grp = __match_any_sync(0xffffffffu, key);
-    const int rank = __popc(grp & ((1u << lane) - 1u));
-    int pos = -1;
-    if (key >= 0) pos = lo + base[key] + rank;
-    __syncwarp();
-    if (key >= 0 && rank == 0) base[key] += __popc(grp);
-    __syncwarp();
-    if (pos >= 0) perm[pos] = t;
+  if (!two) {
+    for (int c = lo; c < hi; c += 32) {
+      const int t = c + lane;
+      int key = -1;
+      if (t < hi) { bool nf; float zr; key = interval_of(z_poca[t], zr, nf); }
+      const unsigned grp = __match_any_sync(0xffffffffu, key);
+      const int rank = __popc(grp & ((1u << lane) - 1u));
+      int pos = -1;
+      if (key >= 0) pos = lo + base[key] + rank;
+      __syncwarp();
+      if (key >= 0 && rank == 0) base[key] += __popc(grp);
+      __syncwarp();
+      if (pos >= 0) perm[pos] = t;
+    }
+  } else {
+    // NEXT-1: a lane holds up to two keys (its interval and a neighbour); per interval the entries of the
+    // chunk are placed in lane (= track) order, so the order inside a segment stays "ascending track index"
+    for (int c = lo; c < hi; c += 32) {
+      const int t = c + lane;
+      int key = -1, key2 = -1, code = 0;
+      if (t < hi) {
+        bool nf;
+        float zr;
+        key = interval_of(z_poca[t], zr, nf);
+        code = neighbour_code(key, zr, mfrac);
+        if (code) key2 = code == 1 ? key - 1 : key + 1;
+      }
+      const unsigned present = __ballot_sync(0xffffffffu, key >= 0);
+      if (present == 0u) continue;
+      for (int k = 0; k < kIntervals; ++k) {
+        const bool mine = key == k, mine2 = key2 == k;
+        const unsigned m = __ballot_sync(0xffffffffu, mine || mine2);
+        if (m == 0u) continue;
+        if (mine || mine2) perm[plo + base[k] + __popc(m & ((1u << lane) - 1u))] = t | ((mine ? 0 : code) << kEntryShift);
+        __syncwarp();
+        if (lane == 0) base[k] += __popc(m);
+        __syncwarp();
+      }
+    }
   }
 }
 
 void launch_sort(const float* z_poca, const int32_t* event_offsets, int n_events, int32_t* perm,
-                 int32_t* seg_off, int32_t* seg_cnt, uint32_t* flags, cudaStream_t s) {
+                 int32_t* seg_off, int32_t* seg_cnt, uint32_t* flags, float mfrac, cudaStream_t s) {
   if (n_events <= 0) return;
   const int grid = (n_events + kSortWarps - 1) / kSortWarps;
-  k_sort<<<grid, kSortWarps * 32, 0, s>>>(z_poca, event_offsets, n_events, perm, seg_off, seg_cnt, flags);
+  k_sort<<<grid, kSortWarps * 32, 0, s>>>(z_poca, event_offsets, n_events, perm, seg_off, seg_cnt, flags, mfrac,
+                                          mfrac > 0.0f ? 1 : 0);
 }
 
 }  // namespace pvf

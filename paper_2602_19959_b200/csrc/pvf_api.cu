@@ -79,6 +79,8 @@ bool config_ok(const pvf_config* c) {
   if (c->split_mask < 0 || c->split_mask > 31) return false;
   if (c->max_events < 1 || c->max_tracks < 1 || c->max_tracks > 0x7fffffffLL) return false;
   if (c->elide_empty_intervals && c->precision == PVF_PREC_FP32) return false;   // tensor-core modes only
+  if (!(c->boundary_margin_mm >= 0.0f && c->boundary_margin_mm < 4.9f)) return false;
+  if (c->boundary_margin_mm > 0.0f && c->max_tracks > (int64_t)kEntryMask) return false;
   return true;
 }
 
@@ -101,7 +103,7 @@ Layout make_layout(const pvf_config* c) {
   L.el_list = take(c->elide_empty_intervals ? sizeof(int32_t) * E * kIntervals : 0);
   L.el_count = take(c->elide_empty_intervals ? 256 : 0);
   L.el_p0 = take(c->elide_empty_intervals ? sizeof(float) * kGlobalBins : 0);
-  L.perm = take(sizeof(int32_t) * T);
+  L.perm = take(sizeof(int32_t) * T * (c->boundary_margin_mm > 0.0f ? 2 : 1));   // NEXT-1: two entries per track
   L.seg_off = take(sizeof(int32_t) * E * kIntervals);
   L.seg_cnt = take(sizeof(int32_t) * E * kIntervals);
   L.flags = take(sizeof(uint32_t) * E);
@@ -271,7 +273,7 @@ void pvf_default_config(pvf_config* c, int32_t max_events, int64_t max_tracks) {
   c->leaky_slope = kLeaky; c->peak_threshold = 0.01f; c->peak_halfwidth = kPeakHalf; c->max_peaks = kMaxPeaks;
   c->precision = PVF_PREC_FP32; c->split_mask = 0;
   c->max_events = max_events; c->max_tracks = max_tracks;
-  c->enable_stage_timing = 0; c->enable_host_io = 0; c->elide_empty_intervals = 0;
+  c->enable_stage_timing = 0; c->enable_host_io = 0; c->elide_empty_intervals = 0; c->boundary_margin_mm = 0.0f;
 }
 
 size_t pvf_workspace_bytes(const pvf_config* cfg) {
@@ -301,7 +303,8 @@ pvf_status pvf_run(pvf_handle h, const pvf_tracks* t, int32_t n_events, float* o
   const bool timing = h->cfg.enable_stage_timing != 0;
   cudaEvent_t* ev = h->ev[h->timed_runs % pvf_ctx::kTimedRuns];
   if (timing) cudaEventRecord(ev[0], s);
-  launch_sort(t->feat[0], t->event_offsets, n_events, h->perm, h->seg_off, h->seg_cnt, h->flags, s);
+  launch_sort(t->feat[0], t->event_offsets, n_events, h->perm, h->seg_off, h->seg_cnt, h->flags,
+              h->cfg.boundary_margin_mm * 0.1f, s);
   if (timing) cudaEventRecord(ev[1], s);
   if (h->cfg.precision == PVF_PREC_FP32)
     launch_fc_hist(t->feat, t->event_offsets, h->perm, h->seg_off, h->seg_cnt, h->fc_params, n_events, h->hist, s);

@@ -40,11 +40,34 @@ __device__ __forceinline__ int interval_of(float z, float& zrel, bool& nonfinite
   zrel = __fsub_rn(u, fl);
   return (int)fl;
 }
+// NEXT-1 ("tracks on boundaries of intervals are part of two intervals"; reading R12):
+// with margin fraction mfrac = margin_mm * 0.1f > 0 a kept track with zrel < mfrac also contributes to the
+// previous interval (zrel + 1), one with zrel >= 1 - mfrac to the next (zrel - 1).  A perm entry carries the
+// track index in bits [0,29) and in bits [29,31) which contribution it is: 0 own interval, 1 previous, 2 next.
+constexpr int kEntryShift = 29;
+constexpr int kEntryMask = (1 << kEntryShift) - 1;
+__device__ __forceinline__ int neighbour_code(int iv, float zrel, float mfrac) {
+  if (iv < 0 || !(mfrac > 0.0f)) return 0;
+  if (iv > 0 && zrel < mfrac) return 1;
+  if (iv < kIntervals - 1 && zrel >= __fsub_rn(1.0f, mfrac)) return 2;
+  return 0;
+}
+// interval and relative z of a perm entry; t = the track it refers to
+__device__ __forceinline__ int entry_interval(int ent, const float* __restrict__ z_poca, int& t, float& zrel) {
+  t = ent & kEntryMask;
+  const int which = ent >> kEntryShift;
+  bool nf;
+  int iv = interval_of(z_poca[t], zrel, nf);
+  if (which == 1) { iv -= 1; zrel = __fadd_rn(zrel, 1.0f); }
+  else if (which == 2) { iv += 1; zrel = __fsub_rn(zrel, 1.0f); }
+  return iv;
+}
 #endif
 
-// a0: interval assignment + stable per-event counting sort (k_sort.cu)
+// a0: interval assignment + stable per-event counting sort (k_sort.cu).  mfrac > 0: boundary tracks get a
+// second entry (perm then holds up to 2 entries per track).
 void launch_sort(const float* z_poca, const int32_t* event_offsets, int n_events, int32_t* perm,
-                 int32_t* seg_off, int32_t* seg_cnt, uint32_t* flags, cudaStream_t s);
+                 int32_t* seg_off, int32_t* seg_cnt, uint32_t* flags, float mfrac, cudaStream_t s);
 
 // a1+a2: per-track FC and fixed-order segmented sum into H [n_events,40,8,100] (k_fc.cu)
 void launch_fc_hist(const float* const feat[9], const int32_t* event_offsets, const int32_t* perm,

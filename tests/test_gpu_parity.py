@@ -261,6 +261,43 @@ def test_unet_entry_point_on_synthetic_histograms(prec):
     assert np.all(got[0].reshape(40, 100) == got[0, :100])       # identical bias-only vector everywhere
 
 
+# ------------------------------------------------------------------ NEXT-1: boundary tracks in two intervals
+@pytest.mark.parametrize("prec", ["fp32", "tf32"])
+def test_boundary_tracks_two_intervals(prec):
+    """with a margin, tracks near an interval edge also contribute to the neighbour.  Histogram
+    and probabilities against the oracle run with the same margin; an event packed with edge tracks
+    (including the region's own edges, which have no outside neighbour) and two runs bit-identical."""
+    margin = 0.5
+    base = make_events("run3", 24, 321)
+    rng = np.random.default_rng(5)
+    f = base.feat[:, :200].copy()
+    edges = -200.0 + 10.0 * rng.integers(0, 41, 200)
+    f[0] = np.clip(edges + rng.uniform(-0.6, 0.6, 200), -199.999, 199.999).astype(np.float32)
+    feat = np.ascontiguousarray(np.concatenate([base.feat, f], axis=1))
+    offs = np.concatenate([base.event_offsets, [base.event_offsets[-1] + 200]]).astype(np.int32)
+    ev = type(base)(feat, offs, [None] * 25)
+    w = make_weights("peaky", 3)
+    ref = O.run(ev.feat, ev.event_offsets, w, want_hist=True, boundary_margin_mm=margin)
+    ref0 = O.run(ev.feat, ev.event_offsets, w, want_hist=True)
+    assert np.abs(ref["hist"] - ref0["hist"]).max() > 0.1          # the margin does change the histograms
+    pvf = _make(w, ev, prec, boundary_margin_mm=margin)
+    probs, pk = _run(pvf, ev)
+    H = torch.empty(ev.n_events, 40, 8, 100, device="cuda")
+    s = torch.cuda.Stream()
+    pvf.debug_copy_histogram(H, ev.n_events, stream=s)
+    s.synchronize()
+    Hn = H.cpu().numpy().astype(np.float64)
+    assert (np.abs(Hn - ref["hist"]) / np.maximum(np.abs(ref["hist"]), 1.0)).max() <= 2e-5
+    assert np.array_equal(Hn == 0, ref["hist"] == 0)
+    assert np.abs(probs.cpu().numpy().astype(np.float64) - ref["probs"]).max() <= TOL[prec]
+    probs2, pk2 = _run(pvf, ev)
+    assert torch.equal(probs, probs2) and all(torch.equal(pk[k], pk2[k]) for k in pk)
+    # margin 0 stays the config-0 definition
+    plain = _make(w, ev, prec)
+    p0, _ = _run(plain, ev)
+    assert np.abs(p0.cpu().numpy().astype(np.float64) - ref0["probs"]).max() <= TOL[prec]
+
+
 # ------------------------------------------------------------------ NEXT-2: empty-interval elision
 @pytest.mark.parametrize("prec", ["tf32", "bf16", "fp16"])
 def test_empty_interval_elision_is_bit_identical(prec):
