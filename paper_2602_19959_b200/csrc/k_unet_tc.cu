@@ -182,6 +182,29 @@ __device__ __forceinline__ void store_row16(uint32_t dst_row, uint32_t lbo, int 
   }
 }
 
+// Pooled row (identical in both lanes of a pair): the even lane stores the first half of the 16 channels,
+// the odd lane the second half, so every lane of the store instruction is active.
+template <int BF16>
+__device__ __forceinline__ void store_pooled16(uint32_t dst_row, uint32_t lbo, int c0, const float (&v)[16], int odd) {
+  float h[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) h[i] = odd ? v[8 + i] : v[i];
+  if (BF16) {
+    uint4 q;
+    q.x = pack16<BF16>(h[0], h[1]); q.y = pack16<BF16>(h[2], h[3]);
+    q.z = pack16<BF16>(h[4], h[5]); q.w = pack16<BF16>(h[6], h[7]);
+    st_smem16(dst_row + (uint32_t)(c0 / 8 + odd) * lbo, q);
+  } else {
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      uint4 q;
+      q.x = to_tf32(h[4 * k + 0]); q.y = to_tf32(h[4 * k + 1]);
+      q.z = to_tf32(h[4 * k + 2]); q.w = to_tf32(h[4 * k + 3]);
+      st_smem16(dst_row + (uint32_t)(c0 / 4 + 2 * odd + k) * lbo, q);
+    }
+  }
+}
+
 __device__ __forceinline__ void zero_rows(uint32_t buf, uint32_t lbo, int nch, int row) {
   for (int c = 0; c < nch; ++c) st_smem16(buf + (uint32_t)c * lbo + (uint32_t)row * 16u, make_uint4(0, 0, 0, 0));
 }
@@ -214,7 +237,7 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
     }
   }
   asm volatile("bar.sync 1, 128;" ::: "memory");
-  const float* nxt = scr + (q + 1) * C;          // E1 row of the next quadrant's first lane (q = 3: unused)
+  const float* nxt = scr + (q < 3 ? q + 1 : 3) * C;   // E1 row of the next quadrant's first lane (q = 3: unused)
   // which interval of the group this row belongs to, its position, and whether it is a real output
   int interval, l;
   bool valid;
@@ -246,11 +269,16 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
     tmem_ld_x16(taddr + (uint32_t)c0, r);
     tmem_ld_x16(taddr + (uint32_t)(C + c0), r1);
     tmem_ld_wait();
-    float v[16];
+    float v[16], nx[16];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {             // whole-warp broadcast loads (cheaper than 16 predicated scalar loads)
+      const float4 n4 = *reinterpret_cast<const float4*>(nxt + c0 + 4 * k);
+      nx[4 * k] = n4.x; nx[4 * k + 1] = n4.y; nx[4 * k + 2] = n4.z; nx[4 * k + 3] = n4.w;
+    }
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
       float up = __shfl_down_sync(0xffffffffu, __uint_as_float(r1[i]), 1);
-      if (lane == 31) up = (q < 3) ? nxt[c0 + i] : 0.0f;
+      if (lane == 31) up = (q < 3) ? nx[i] : 0.0f;
       v[i] = lrelu(__uint_as_float(r[i]) + up + bias[c0 + i]);
     }
     if (MODE == kD1) {
@@ -268,7 +296,7 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
       float pv[16];
 #pragma unroll
       for (int i = 0; i < 16; ++i) pv[i] = fmaxf(v[i], __shfl_xor_sync(0xffffffffu, v[i], 1));
-      if ((lane & 1) == 0) store_row16<BF16>(dst_aux, lbo_aux, c0, pv);
+      store_pooled16<BF16>(dst_aux, lbo_aux, c0, pv, lane & 1);   // both lanes of a pair hold the same maxima
     } else if (exists) {          // kB, kD2: nearest upsample = the same chunk into rows 2m and 2m + 1;
       // groups of four lanes alternate which of the two rows goes first, so that one store instruction
       // covers all eight 16-byte slots of every 128-byte line evenly (no bank conflicts)

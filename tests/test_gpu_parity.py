@@ -346,6 +346,17 @@ def test_boundary_contract():
     assert st == pkg.PVF_ERR_ARG
     s.synchronize()
     assert float(probs.min()) == -1.0                            # nothing was enqueued by the failed calls
+    # no device allocation inside pvf_run: free memory is unchanged across calls (the
+    # first call has already loaded the kernels)
+    pvf.run(feat, off, 4, probs, pk, stream=s)
+    s.synchronize()
+    free0, _ = torch.cuda.mem_get_info()
+    for _ in range(3):
+        pvf.run(feat, off, 4, probs, pk, stream=s)
+    s.synchronize()
+    free1, _ = torch.cuda.mem_get_info()
+    assert free1 == free0
+    assert bool((probs > 0).all())
     with pytest.raises(pkg.PVFError):
         pvf.stage_times_ms()                                     # timing not enabled
     # caller-supplied pool: zero allocation inside create (Allen-style fixed pool)
