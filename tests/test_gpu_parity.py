@@ -390,12 +390,13 @@ def test_host_io_and_stage_timing():
 
 
 # ------------------------------------------------------------------ full size, bench launch configuration
-@pytest.mark.parametrize("prec", ["tf32", "bf16", "fp32"])
-def test_full_batch_sampled_events(prec):
-    """BASELINE.json config 2 (16000 events) in the launch configuration bench.py times; the oracle
-    computes sampled events one by one; properties hold for every event."""
+@pytest.mark.parametrize("prec,model", [("tf32", "run3"), ("bf16", "run3"), ("fp32", "run3"), ("tf32", "pileup"),
+                                        ("fp16", "pileup")])
+def test_full_batch_sampled_events(prec, model):
+    """BASELINE.json config 2 / config 3 (16000 events) in the launch configuration bench.py times; the
+    oracle computes sampled events one by one; properties hold for every event."""
     E = 16000 if prec != "fp32" else 2000
-    ev = make_events("run3", E, 1002)
+    ev = make_events(model, E, 1002 if model == "run3" else 1003)
     w = make_weights("peaky", 1)
     pvf = _available(prec, w, ev)
     probs, pk = _run(pvf, ev)
@@ -409,7 +410,8 @@ def test_full_batch_sampled_events(prec):
         m, n, _ = O.match_peaks(ref["peaks"]["bin"][i], gb[i])
         assert m >= n - 1
     # properties at any size: probabilities in (0,1); peak bins ascending, counts consistent
-    assert float(probs.min()) > 0.0 and float(probs.max()) < 1.0 and bool(torch.isfinite(probs).all())
+    # (a float32 sigmoid saturates to exactly 1.0 for logits > ~17: dense pile-up peaks of the toy weights do)
+    assert float(probs.min()) > 0.0 and float(probs.max()) <= 1.0 and bool(torch.isfinite(probs).all())
     cnt = pk["count"].cpu().numpy()
     bins = pk["bin"].cpu().numpy()
     assert np.all((bins >= 0).sum(axis=1) == cnt)
