@@ -87,6 +87,10 @@ typedef struct {
   float boundary_margin_mm; /* default 0 = "each track adds to the interval holding its z_poca" (BASELINE.json
                               config 0).  > 0 (< 4.9): a track within this distance of an interval edge also
                               contributes to the neighbouring interval, PAPER.md:49 (NEXT-1; R12) */
+  int32_t unet_cta_pair;   /* tensor-core modes only; default 0.  1: the UNet kernel runs as clusters of two CTAs that
+                              share every tcgen05.mma (cta_group::2, M = 256): each CTA keeps its own intervals'
+                              activations and half of the weight rows, so the weight stream and the B-operand
+                              reads per SM are halved.  Same arithmetic, bit-identical output */
 } pvf_config;
 
 /* Fill *cfg with BASELINE.json config 0 (64 channels, FP32) and the given capacities. */

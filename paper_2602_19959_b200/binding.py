@@ -38,7 +38,7 @@ class pvf_config(C.Structure):
         ("max_peaks", C.c_int32), ("precision", C.c_int32), ("split_mask", C.c_int32),
         ("max_events", C.c_int32), ("max_tracks", C.c_int64), ("enable_stage_timing", C.c_int32),
         ("enable_host_io", C.c_int32), ("elide_empty_intervals", C.c_int32),
-        ("boundary_margin_mm", C.c_float),
+        ("boundary_margin_mm", C.c_float), ("unet_cta_pair", C.c_int32),
     ]
 
 
@@ -122,7 +122,7 @@ class PVFinder:
 
     def __init__(self, weights, max_events: int, max_tracks: int, precision="fp32", channels: int | None = None,
                  split_mask: int = 0, stage_timing: bool = False, host_io: bool = False, elide_empty: bool = False,
-                 boundary_margin_mm: float = 0.0, pool=None, lib=None,
+                 boundary_margin_mm: float = 0.0, cta_pair: bool = False, pool=None, lib=None,
                  **cfg_over):
         import torch  # device memory + streams only
         self.torch = torch
@@ -132,7 +132,8 @@ class PVFinder:
         self.cfg = default_config(self.lib, max_events, max_tracks, unet_channels=ch, precision=prec,
                                   split_mask=split_mask, enable_stage_timing=int(stage_timing),
                                   enable_host_io=int(host_io), elide_empty_intervals=int(elide_empty),
-                                  boundary_margin_mm=float(boundary_margin_mm), **cfg_over)
+                                  boundary_margin_mm=float(boundary_margin_mm), unet_cta_pair=int(cta_pair),
+                                  **cfg_over)
         ws, keep = _weights_struct(weights)
         self.handle = C.c_void_p()
         if pool is None:

@@ -44,6 +44,7 @@ constexpr int kTcThreads = 192;
 constexpr int kMaxStages = 8;
 constexpr int kStageBytes = 16384;
 constexpr int kHeaderBytes = 2048;          // biases [5][C], head weight [C], head bias
+constexpr int kBarBytes = 512;
 
 // sub-layers as the MMA issuer sees them
 enum { sE1 = 0, sE2 = 1, sB = 2, sD2 = 3, sD1U = 4, sD1E = 5 };
@@ -52,7 +53,10 @@ enum { gE2 = 0, gD1Ea = 1, gB = 2, gD1Eb = 3, gD2 = 4, gD1Ec = 5, gE1 = 6, gD1U 
 
 // BF16: operand format -- 0 = TF32 (4-byte), 1 = BF16, 2 = FP16 (2-byte; everything that only depends on
 // the operand size treats 1 and 2 alike)
-template <int C, int BF16>
+// CG: CTAs per MMA -- 1, or 2 = a cluster of two CTAs (cta_group::2) that run one M = 256 MMA per step: each CTA
+// supplies its own 128 activation rows (its own group of intervals) and HALF of the weight rows (rank 0 the even
+// tap of a pair, rank 1 the odd tap), so per CTA the weight stream and the B-operand reads are halved.
+template <int C, int BF16, int CG = 1>
 struct Geo {
   static constexpr int ES = BF16 ? 2 : 4;            // operand element size
   static constexpr int PER = 16 / ES;                // channels per 16-byte chunk
@@ -67,8 +71,10 @@ struct Geo {
   // land in the following chunk / buffer, which is always inside the CTA's allocation
   static constexpr int ROWS1 = LEAD1 + 128 * T, ROWS2 = LEAD2 + 64 * T, ROWS3 = LEAD3 + 32 * T;
   static constexpr int LBO1 = ROWS1 * 16, LBO2 = ROWS2 * 16, LBO3 = ROWS3 * 16;
-  static constexpr int STEP_BYTES = 2 * NOUT * 16;   // one MMA's B operand: [2 chunks][2C rows][16 B]
-  static constexpr int SPS = kStageBytes / STEP_BYTES;   // MMA steps per ring stage
+  static constexpr int NB = NOUT / CG;               // B-operand rows this CTA holds
+  static constexpr int STEP_BYTES = 2 * NB * 16;     // one MMA's B operand in this CTA: [2 chunks][NB rows][16 B]
+  static constexpr int STAGE_BYTES = kStageBytes / CG;
+  static constexpr int SPS = STAGE_BYTES / STEP_BYTES;   // MMA steps per ring stage (independent of CG)
   // shared-memory map (bytes)
   static constexpr int SZ_L1 = NCH * LBO1;           // a C-channel buffer at L = 100
   static constexpr int SZ_L2 = NCH * LBO2;           //                     at L = 50
@@ -78,12 +84,16 @@ struct Geo {
   static constexpr int SZ_XP = (XCH * LBO1 > SZ_L2) ? XCH * LBO1 : SZ_L2;
   static constexpr int OFF_RING = OFF_XP + SZ_XP;
   static constexpr int SCR_BYTES = 2 * 4 * C * 4;    // epilogue row-exchange scratch: [2 buffers][4 warps][C floats]
-  static constexpr int STAGES_FIT = (227 * 1024 - kHeaderBytes - 256 - SCR_BYTES - OFF_RING) / kStageBytes;
-  static constexpr int STAGES = STAGES_FIT < kMaxStages ? STAGES_FIT : kMaxStages;   // weight ring depth
-  static constexpr int OFF_PAR = OFF_RING + STAGES * kStageBytes;   // biases + head (floats)
+  static constexpr int STAGES_FIT = (227 * 1024 - kHeaderBytes - kBarBytes - SCR_BYTES - OFF_RING) / STAGE_BYTES;
+  static constexpr int MAX_STAGES = CG == 2 ? 12 : kMaxStages;
+  static constexpr int STAGES = STAGES_FIT < MAX_STAGES ? STAGES_FIT : MAX_STAGES;   // weight ring depth
+  static constexpr int OFF_PAR = OFF_RING + STAGES * STAGE_BYTES;   // biases + head (floats)
   static constexpr int OFF_SCR = OFF_PAR + kHeaderBytes;
   static constexpr int OFF_BAR = OFF_SCR + SCR_BYTES;
-  static constexpr int SMEM = OFF_BAR + 256;
+  static constexpr int SMEM = OFF_BAR + kBarBytes;
+  // mbarriers (8 bytes each): full[S] empty[S] peer_full[S] accum[5] epi[6] peer_epi[6], then the TMEM slot
+  static constexpr int BAR_ACCUM = 3 * STAGES, BAR_EPI = BAR_ACCUM + 5, BAR_PEPI = BAR_EPI + 6, BAR_SLOT = BAR_PEPI + 6;
+  static_assert(8 * BAR_SLOT + 4 <= kBarBytes, "barrier block");
   // TMEM columns: region A = [0, T*2C) (d1), region B = [T*2C, 2*T*2C) (e1; e2, b, d2 use its head);
   // an accumulator tile is 2C columns: E0 (even taps) | E1 (odd taps)
   static constexpr int COL_A = 0, COL_B = T * NOUT;
@@ -109,9 +119,10 @@ struct Plan {
   int total;
 };
 
-template <int C, int BF16>
+// With CG = 2 the image is two such images back to back (rank 0 | rank 1), each `total` bytes with its own header.
+template <int C, int BF16, int CG>
 __host__ __device__ inline Plan make_plan(int split_e1) {
-  using G = Geo<C, BF16>;
+  using G = Geo<C, BF16, CG>;
   Plan P{};
   P.e1_steps = 13 * ((!BF16 && split_e1) ? 3 : 1);
   P.seg_steps[gE2] = 8 * G::NKB1;
@@ -387,11 +398,16 @@ struct Lay {
   }
 };
 
-template <int BF16>
+template <int BF16, int CG>
 __device__ __forceinline__ void mma_lh(uint32_t d, uint32_t a_lo, uint32_t a_hi, uint32_t b_lo, uint32_t b_hi,
                                        uint32_t idesc, uint32_t acc) {
-  if (BF16) mma_f16_lh(d, a_lo, a_hi, b_lo, b_hi, idesc, acc);
-  else mma_tf32_lh(d, a_lo, a_hi, b_lo, b_hi, idesc, acc);
+  if (CG == 2) {
+    if (BF16) mma2_f16_lh(d, a_lo, a_hi, b_lo, b_hi, idesc, acc);
+    else mma2_tf32_lh(d, a_lo, a_hi, b_lo, b_hi, idesc, acc);
+  } else {
+    if (BF16) mma_f16_lh(d, a_lo, a_hi, b_lo, b_hi, idesc, acc);
+    else mma_tf32_lh(d, a_lo, a_hi, b_lo, b_hi, idesc, acc);
+  }
 }
 
 struct RingState { int ring; uint32_t phase; };
@@ -400,24 +416,25 @@ struct RingState { int ring; uint32_t phase; };
 // used by all NT tiles.  The warp walks the (uniform) schedule; one elected lane issues a whole
 // stage worth of MMAs whose descriptors differ from the stage origin by compile-time constants.
 // f_begin must be a multiple of SPS.  acc0 = 0 starts fresh accumulators at step f_begin.
-template <int C, int BF16, int S>
+template <int C, int BF16, int CG, int S>
 __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_t bar0, RingState& rs,
                                         int f_begin, int f_end, uint32_t acc0) {
-  using G = Geo<C, BF16>;
+  using G = Geo<C, BF16, CG>;
   using Y = Lay<C, BF16, S>;
   constexpr int SPS = G::SPS;
   static_assert(Y::HALF % SPS == 0 || SPS % Y::NKB == 0,
                 "a ring stage is either part of one source's K blocks or whole taps");
-  constexpr uint32_t idesc = instr_desc(BF16 == 2 ? kFmtF16 : (BF16 ? kFmtBF16 : kFmtTF32), 128, G::NOUT);
+  constexpr uint32_t idesc = instr_desc(BF16 == 2 ? kFmtF16 : (BF16 ? kFmtBF16 : kFmtTF32), 128 * CG, G::NOUT);
   constexpr uint32_t hi = (128u >> 4) | (1u << 14);                    // SBO = 128 B, descriptor version 1
   constexpr uint32_t a_lbo = (uint32_t)(Y::LBO >> 4) << 16;
-  constexpr uint32_t b_lbo = (uint32_t)((G::NOUT * 16) >> 4) << 16;
+  constexpr uint32_t b_lbo = (uint32_t)((G::NB * 16) >> 4) << 16;
   const uint32_t dcol = tmem_base + (uint32_t)Y::DCOL;
   for (int f = f_begin; f < f_end; f += SPS) {
     const int n = min(SPS, f_end - f);
     mbar_wait(bar0 + 8u * rs.ring, rs.phase);
+    if (CG == 2) mbar_wait_cluster(bar0 + 8u * (2 * G::STAGES + rs.ring), rs.phase);   // the peer's half has landed
     tc_fence_after_sync();
-    const uint32_t b0 = b_lbo + ((sb + G::OFF_RING + rs.ring * kStageBytes) >> 4);
+    const uint32_t b0 = b_lbo + ((sb + G::OFF_RING + rs.ring * G::STAGE_BYTES) >> 4);
     uint32_t a0 = a_lbo + (sb >> 4);          // stage origin: descriptor low word of tile 0, step f
     if (S == sE1) {
       // e1: one K block per step; steps run [pass][tap pair], pass 1 reads the low-part chunks (split)
@@ -445,119 +462,168 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
           const uint32_t acc = (i > 0) ? 1u : (f > f_begin ? 1u : acc0);
 #pragma unroll
           for (int t = 0; t < Y::NT; ++t)
-            mma_lh<BF16>(dcol + (uint32_t)(t * G::NOUT), a + 128u * t, hi, b, hi, idesc, acc);
+            mma_lh<BF16, CG>(dcol + (uint32_t)(t * G::NOUT), a + 128u * t, hi, b, hi, idesc, acc);
         }
       }
-      mma_commit(bar0 + 8u * (G::STAGES + rs.ring));      // frees the ring slot when these MMAs retire
+      // frees the ring slot (in both CTAs of a pair) when these MMAs retire
+      if (CG == 2) mma_commit2(bar0 + 8u * (G::STAGES + rs.ring), 3);
+      else mma_commit(bar0 + 8u * (G::STAGES + rs.ring));
     }
     __syncwarp();
     if (++rs.ring == G::STAGES) { rs.ring = 0; rs.phase ^= 1u; }
   }
 }
 
-template <int C, int BF16>
+template <int C, int BF16, int CG>
 __global__ void __launch_bounds__(kTcThreads, 1)
 k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __restrict__ wpack, int split_e1,
           float* __restrict__ probs, const int* __restrict__ list, const int* __restrict__ n_list) {
   // list / n_list (device, optional): process only intervals list[0 .. *n_list) of hist / probs (elision of
   // empty intervals); n_int is then only the capacity the grid was sized for
   if (n_list != nullptr) n_int = *n_list;
-  using G = Geo<C, BF16>;
+  using G = Geo<C, BF16, CG>;
   extern __shared__ __align__(1024) unsigned char smem[];
   const uint32_t sb = smem_u32(smem);
   const int tid = threadIdx.x, lane = tid & 31;
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // provably warp-uniform role index
+  // CG = 2: the two CTAs of a cluster walk the same schedule in lockstep, each on its own group of intervals;
+  // rank 0 (the leader) issues every MMA for both
+  const int rank = CG == 2 ? (int)cluster_ctarank() : 0;
   float* par = reinterpret_cast<float*>(smem + G::OFF_PAR);
-  // mbarriers: full[s], empty[s] per ring stage; accum[k] = "MMAs of layer k retired" (k: e1 e2 b d2 d1);
-  // epi[k] = "epilogue k done" (k: x0-staged e1 e2 b d2 d1)
+  // mbarriers: full[s], empty[s] per ring stage (this CTA's half of the weights); peer_full[s] (leader only: the
+  // peer's half has landed); accum[k] = "MMAs of layer k retired" (k: e1 e2 b d2 d1; multicast to both CTAs);
+  // epi[k] = "this CTA's epilogue k done" (k: x0-staged e1 e2 b d2 d1); peer_epi[k] (leader only: the peer's)
   const uint32_t bar0 = sb + G::OFF_BAR;
-  auto accum_bar = [&](int k) { return bar0 + 8u * (2 * G::STAGES + k); };
-  auto epi_bar = [&](int k) { return bar0 + 8u * (2 * G::STAGES + 5 + k); };
-  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + G::OFF_BAR + 8 * (2 * G::STAGES + 11));
-  static_assert(8 * (2 * G::STAGES + 11) + 4 <= 256, "barrier block");
-  const Plan P = make_plan<C, BF16>(split_e1);
+  auto accum_bar = [&](int k) { return bar0 + 8u * (G::BAR_ACCUM + k); };
+  auto epi_bar = [&](int k) { return bar0 + 8u * (G::BAR_EPI + k); };
+  auto pepi_bar = [&](int k) { return bar0 + 8u * (G::BAR_PEPI + k); };
+  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + G::OFF_BAR + 8 * G::BAR_SLOT);
+  const Plan P = make_plan<C, BF16, CG>(split_e1);
+  const unsigned char* wimg = wpack + (size_t)rank * P.total;       // this CTA's weight image
 
   // ---- one-time setup: zero the activation buffers (gap / halo rows must be zero), parameters, barriers
   for (int i = tid; i < G::OFF_RING / 16; i += kTcThreads) reinterpret_cast<uint4*>(smem)[i] = make_uint4(0, 0, 0, 0);
-  for (int i = tid; i < 6 * C + 1; i += kTcThreads) par[i] = reinterpret_cast<const float*>(wpack)[i];
+  for (int i = tid; i < 6 * C + 1; i += kTcThreads) par[i] = reinterpret_cast<const float*>(wimg)[i];
   if (tid == 0) {
-    for (int s = 0; s < G::STAGES; ++s) { mbar_init(bar0 + 8u * s, 1); mbar_init(bar0 + 8u * (G::STAGES + s), 1); }
+    for (int s = 0; s < G::STAGES; ++s) {
+      mbar_init(bar0 + 8u * s, 1);
+      mbar_init(bar0 + 8u * (G::STAGES + s), 1);
+      mbar_init(bar0 + 8u * (2 * G::STAGES + s), 1);
+    }
     for (int k = 0; k < 5; ++k) mbar_init(accum_bar(k), 1);
-    for (int k = 0; k < 6; ++k) mbar_init(epi_bar(k), 128);
+    for (int k = 0; k < 6; ++k) { mbar_init(epi_bar(k), 128); mbar_init(pepi_bar(k), 128); }
     fence_mbar_init();
   }
-  if (warp == 1) tmem_alloc(smem_u32(const_cast<uint32_t*>(tmem_slot)), G::TMEM_COLS);
+  if (warp == 1) {
+    if (CG == 2) tmem_alloc2(smem_u32(const_cast<uint32_t*>(tmem_slot)), G::TMEM_COLS);
+    else tmem_alloc(smem_u32(const_cast<uint32_t*>(tmem_slot)), G::TMEM_COLS);
+  }
   fence_proxy_async_smem();
   tc_fence_before_sync();
-  __syncthreads();
+  if (CG == 2) cluster_sync_all(); else __syncthreads();
   tc_fence_after_sync();
   const uint32_t tmem_base = *tmem_slot;
 
+  // pair-groups: pair p of the grid takes groups CG*pg + rank for pg = p, p + pairs, ...; a CTA whose group lies
+  // past the end (odd group count) runs the schedule on zeros and stores nothing
   const int n_groups = (n_int + G::T - 1) / G::T;
-  const int stride = gridDim.x;
+  const int n_pg = (n_groups + CG - 1) / CG;
+  const int pg0 = (int)blockIdx.x / CG, stride = (int)gridDim.x / CG;
 
   if (warp == 0) {
-    // ===================== weight producer: streams the image's segments through the ring
+    // ===================== weight producer: streams this CTA's image through the ring
     if (lane == 0) {
       RingState rs{0, 0u};
       auto stream = [&](int seg) {
-        const unsigned char* src = wpack + P.seg_off[seg];
+        const unsigned char* src = wimg + P.seg_off[seg];
         const int steps = P.seg_steps[seg];
         for (int f = 0; f < steps; f += G::SPS) {
           const int n = min(G::SPS, steps - f);
           mbar_wait(bar0 + 8u * (G::STAGES + rs.ring), rs.phase ^ 1u);
           mbar_arrive_expect_tx(bar0 + 8u * rs.ring, (uint32_t)(n * G::STEP_BYTES));
-          bulk_g2s(sb + G::OFF_RING + rs.ring * kStageBytes, src + (size_t)f * G::STEP_BYTES,
+          bulk_g2s(sb + G::OFF_RING + rs.ring * G::STAGE_BYTES, src + (size_t)f * G::STEP_BYTES,
                    (uint32_t)(n * G::STEP_BYTES), bar0 + 8u * rs.ring);
           if (++rs.ring == G::STAGES) { rs.ring = 0; rs.phase ^= 1u; }
         }
       };
       bool first = true;
-      for (int g = blockIdx.x; g < n_groups; g += stride) {
+      for (int pg = pg0; pg < n_pg; pg += stride) {
         if (first) { stream(gE1); first = false; }
-        const bool has_next = g + stride < n_groups;
+        const bool has_next = pg + stride < n_pg;
         for (int s = 0; s < kSegs; ++s) {
           if (s == gE1 && !has_next) continue;
           stream(s);
         }
       }
     }
-  } else if (warp == 1) {
+  } else if (warp == 1 && rank == 0) {
     // ===================== MMA issuer (whole warp walks the schedule, one elected lane issues)
     RingState rs{0, 0u};
     uint32_t ph[6] = {0, 0, 0, 0, 0, 0};
-    auto wait_epi = [&](int k) { mbar_wait(epi_bar(k), ph[k]); ph[k] ^= 1u; tc_fence_after_sync(); };
-    auto commit = [&](int k) { if (elect_one()) mma_commit(accum_bar(k)); __syncwarp(); };
+    auto wait_epi = [&](int k) {
+      mbar_wait(epi_bar(k), ph[k]);
+      if (CG == 2) mbar_wait_cluster(pepi_bar(k), ph[k]);
+      ph[k] ^= 1u;
+      tc_fence_after_sync();
+    };
+    auto commit = [&](int k) {
+      if (elect_one()) {
+        if (CG == 2) mma_commit2(accum_bar(k), 3); else mma_commit(accum_bar(k));
+      }
+      __syncwarp();
+    };
     bool first = true;
-    for (int g = blockIdx.x; g < n_groups; g += stride) {
-      const bool has_next = g + stride < n_groups;
+    for (int pg = pg0; pg < n_pg; pg += stride) {
+      const bool has_next = pg + stride < n_pg;
       if (first) {
         wait_epi(0);
-        mma_seg<C, BF16, sE1>(sb, tmem_base, bar0, rs, 0, P.e1_steps, 0u);
+        mma_seg<C, BF16, CG, sE1>(sb, tmem_base, bar0, rs, 0, P.e1_steps, 0u);
         commit(0);
       }
       wait_epi(1);                                   // P1 staged, region B drained
-      mma_seg<C, BF16, sE2>(sb, tmem_base, bar0, rs, 0, 8 * G::NKB1, 0u);
+      mma_seg<C, BF16, CG, sE2>(sb, tmem_base, bar0, rs, 0, 8 * G::NKB1, 0u);
       commit(1);
       if (!first) wait_epi(5);                       // region A drained by the previous group's d1 epilogue
-      mma_seg<C, BF16, sD1E>(sb, tmem_base, bar0, rs, 0, G::D1E_A, 0u);
+      mma_seg<C, BF16, CG, sD1E>(sb, tmem_base, bar0, rs, 0, G::D1E_A, 0u);
       wait_epi(2);                                   // E2, P2 staged
-      mma_seg<C, BF16, sB>(sb, tmem_base, bar0, rs, 0, 3 * G::NKB1, 0u);
+      mma_seg<C, BF16, CG, sB>(sb, tmem_base, bar0, rs, 0, 3 * G::NKB1, 0u);
       commit(2);
-      mma_seg<C, BF16, sD1E>(sb, tmem_base, bar0, rs, G::D1E_A, G::D1E_A + G::D1E_B, 1u);
+      mma_seg<C, BF16, CG, sD1E>(sb, tmem_base, bar0, rs, G::D1E_A, G::D1E_A + G::D1E_B, 1u);
       wait_epi(3);                                   // U2 staged
-      mma_seg<C, BF16, sD2>(sb, tmem_base, bar0, rs, 0, 8 * 2 * G::NKB1, 0u);
+      mma_seg<C, BF16, CG, sD2>(sb, tmem_base, bar0, rs, 0, 8 * 2 * G::NKB1, 0u);
       commit(3);
-      mma_seg<C, BF16, sD1E>(sb, tmem_base, bar0, rs, G::D1E_A + G::D1E_B, G::D1E_STEPS, 1u);
+      mma_seg<C, BF16, CG, sD1E>(sb, tmem_base, bar0, rs, G::D1E_A + G::D1E_B, G::D1E_STEPS, 1u);
       wait_epi(4);                                   // U1 staged, region B drained
       if (has_next) {
         wait_epi(0);                                 // next group's X0 staged
-        mma_seg<C, BF16, sE1>(sb, tmem_base, bar0, rs, 0, P.e1_steps, 0u);
+        mma_seg<C, BF16, CG, sE1>(sb, tmem_base, bar0, rs, 0, P.e1_steps, 0u);
         commit(0);
       }
-      mma_seg<C, BF16, sD1U>(sb, tmem_base, bar0, rs, 0, 13 * G::NKB1, 1u);
+      mma_seg<C, BF16, CG, sD1U>(sb, tmem_base, bar0, rs, 0, 13 * G::NKB1, 1u);
       commit(4);
       first = false;
+    }
+  } else if (warp == 1) {
+    // ===================== peer CTA of a pair: relay "my half of ring stage s has landed" to the leader
+    if (lane == 0) {
+      RingState rs{0, 0u};
+      const uint32_t lead_bar0 = mapa_rank(bar0, 0);
+      auto relay = [&](int steps) {
+        for (int f = 0; f < steps; f += G::SPS) {
+          mbar_wait(bar0 + 8u * rs.ring, rs.phase);
+          mbar_arrive_cluster(lead_bar0 + 8u * (2 * G::STAGES + rs.ring));
+          if (++rs.ring == G::STAGES) { rs.ring = 0; rs.phase ^= 1u; }
+        }
+      };
+      bool first = true;
+      for (int pg = pg0; pg < n_pg; pg += stride) {
+        if (first) { relay(P.seg_steps[gE1]); first = false; }
+        const bool has_next = pg + stride < n_pg;
+        for (int s = 0; s < kSegs; ++s) {
+          if (s == gE1 && !has_next) continue;
+          relay(P.seg_steps[s]);
+        }
+      }
     }
   } else {
     // ===================== epilogue warps (128 threads): thread = accumulator row
@@ -567,53 +633,60 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
     auto scr = [&]() { return scr0 + (ecount++ & 1) * 4 * C; };
     uint32_t pa[5] = {0, 0, 0, 0, 0};
     auto wait_acc = [&](int k) { mbar_wait(accum_bar(k), pa[k]); pa[k] ^= 1u; tc_fence_after_sync(); };
-    auto done = [&](int k) { fence_proxy_async_smem(); tc_fence_before_sync(); mbar_arrive(epi_bar(k)); };
+    const uint32_t lead_pepi = CG == 2 ? mapa_rank(pepi_bar(0), 0) : 0u;
+    auto done = [&](int k) {
+      fence_proxy_async_smem();
+      tc_fence_before_sync();
+      if (CG == 2 && rank == 1) mbar_arrive_cluster(lead_pepi + 8u * k);
+      else mbar_arrive(epi_bar(k));
+    };
     bool first = true;
-    for (int g = blockIdx.x; g < n_groups; g += stride) {
-      const long long g0 = (long long)g * G::T;
-      const int n_valid = (int)min((long long)G::T, (long long)n_int - g0);
-      const bool has_next = g + stride < n_groups;
-      const long long gn0 = (long long)(g + stride) * G::T;
-      const int n_valid_next = has_next ? (int)min((long long)G::T, (long long)n_int - gn0) : 0;
-      float* pg = list ? probs : probs + g0 * kBins;
+    for (int pg = pg0; pg < n_pg; pg += stride) {
+      const long long g0 = ((long long)pg * CG + rank) * G::T;
+      const int n_valid = (int)max(0LL, min((long long)G::T, (long long)n_int - g0));
+      const bool has_next = pg + stride < n_pg;
+      const long long gn0 = ((long long)(pg + stride) * CG + rank) * G::T;
+      const int n_valid_next = has_next ? (int)max(0LL, min((long long)G::T, (long long)n_int - gn0)) : 0;
+      float* pg_out = list ? probs : probs + g0 * kBins;
       const int* lg = list ? list + g0 : nullptr;
       const int* lgn = list ? list + gn0 : nullptr;
       if (first) {
         load_x0<C, BF16>(sb, hist, g0, n_valid, split_e1, et, list);
         done(0);
         wait_acc(0);
-        for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kE1>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr(), lg);
+        for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kE1>(sb, tmem_base, t, q, lane, par, n_valid, pg_out, scr(), lg);
         done(1);
         first = false;
       }
       wait_acc(1);
-      for (int t = 0; t < G::T / 2; ++t) epilogue_tile<C, BF16, kE2>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr(), lg);
+      for (int t = 0; t < G::T / 2; ++t) epilogue_tile<C, BF16, kE2>(sb, tmem_base, t, q, lane, par, n_valid, pg_out, scr(), lg);
       done(2);
       if (has_next) {                                // P1 is dead (e2's MMAs retired): stage the next input
         load_x0<C, BF16>(sb, hist, gn0, n_valid_next, split_e1, et, list);
         done(0);
       }
       wait_acc(2);
-      for (int t = 0; t < (G::T + 3) / 4; ++t) epilogue_tile<C, BF16, kB>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr(), lg);
+      for (int t = 0; t < (G::T + 3) / 4; ++t) epilogue_tile<C, BF16, kB>(sb, tmem_base, t, q, lane, par, n_valid, pg_out, scr(), lg);
       done(3);
       wait_acc(3);
-      for (int t = 0; t < G::T / 2; ++t) epilogue_tile<C, BF16, kD2>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr(), lg);
+      for (int t = 0; t < G::T / 2; ++t) epilogue_tile<C, BF16, kD2>(sb, tmem_base, t, q, lane, par, n_valid, pg_out, scr(), lg);
       done(4);
       if (has_next) {
         wait_acc(0);
-        for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kE1>(sb, tmem_base, t, q, lane, par, n_valid_next, pg, scr(), lgn);
+        for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kE1>(sb, tmem_base, t, q, lane, par, n_valid_next, pg_out, scr(), lgn);
         done(1);
       }
       wait_acc(4);
-      for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kD1>(sb, tmem_base, t, q, lane, par, n_valid, pg, scr(), lg);
+      for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kD1>(sb, tmem_base, t, q, lane, par, n_valid, pg_out, scr(), lg);
       done(5);
     }
   }
+  __syncwarp();
   tc_fence_before_sync();
-  __syncthreads();
+  if (CG == 2) cluster_sync_all(); else __syncthreads();   // pair: the peer's shared memory and barriers stay alive until both are done
   if (warp == 1) {
     __syncwarp();
-    tmem_dealloc(tmem_base, G::TMEM_COLS);
+    if (CG == 2) tmem_dealloc2(tmem_base, G::TMEM_COLS); else tmem_dealloc(tmem_base, G::TMEM_COLS);
   }
 }
 
@@ -657,11 +730,15 @@ uint16_t fp16_rne(float v) {                 // float -> IEEE binary16, round to
 // (biases [5][C], head weight [C], head bias) and, per segment in streaming order, per MMA step, the
 // B operand [2 chunks][2C rows: C outputs of tap 2u, then of tap 2u+1][16 B of input channels],
 // operand-rounded (TF32: RN ties away; BF16: RNE).
-template <int C, int BF16>
-void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst) {
-  using G = Geo<C, BF16>;
-  const Plan P = make_plan<C, BF16>(split_e1);
-  memset(dst, 0, P.total);
+// CG = 2: two images back to back; rank r's steps hold B rows [r*C, (r+1)*C) only (rank 0 = the even tap of
+// every pair, rank 1 = the odd tap).
+template <int C, int BF16, int CG>
+void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst_all) {
+  using G = Geo<C, BF16, CG>;
+  const Plan P = make_plan<C, BF16, CG>(split_e1);
+  memset(dst_all, 0, (size_t)CG * P.total);
+  for (int rank = 0; rank < CG; ++rank) {
+  unsigned char* dst = dst_all + (size_t)rank * P.total;
   float* hdr = reinterpret_cast<float*>(dst);
   for (int l = 0; l < 5; ++l) memcpy(hdr + l * C, w->conv_b[l], sizeof(float) * C);
   memcpy(hdr + 5 * C, w->conv_w[5], sizeof(float) * C);
@@ -681,13 +758,14 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst) {
       else { u = f / d.nkb; kk = f % d.nkb; }
       unsigned char* step = dst + P.seg_off[d.seg] + (size_t)s * G::STEP_BYTES;
       for (int h = 0; h < 2; ++h)
-        for (int n = 0; n < G::NOUT; ++n)         // rows [0, C): even tap 2u, rows [C, 2C): odd tap 2u + 1
+        for (int nl = 0; nl < G::NB; ++nl)        // rows [0, C): even tap 2u, rows [C, 2C): odd tap 2u + 1
           for (int e = 0; e < G::PER; ++e) {
+            const int n = rank * G::NB + nl;
             const int co = n % C, j = 2 * u + n / C;
             const int cl = (2 * kk + h) * G::PER + e;            // channel inside the sub-layer's range
             const bool real = j < d.taps && ((d.seg == gE1) ? cl < kHistCh : true);
             const float v = real ? W[((size_t)co * d.cin + d.ch_base + cl) * d.taps + j] : 0.0f;
-            unsigned char* p = step + ((size_t)h * G::NOUT + n) * 16 + e * G::ES;
+            unsigned char* p = step + ((size_t)h * G::NB + nl) * 16 + e * G::ES;
             if (BF16) {
               const uint16_t b = (BF16 == 2) ? fp16_rne(v) : bf16_rne(v);
               memcpy(p, &b, 2);
@@ -699,63 +777,88 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst) {
           }
     }
   }
+  }
 }
 
-template <int C, int BF16>
+template <int C, int BF16, int CG>
 void launch_impl(const float* hist, int n_int, const void* packed, int split_e1, float* probs, int sm_count,
                  const int* list, const int* n_list, cudaStream_t s) {
-  using G = Geo<C, BF16>;
+  using G = Geo<C, BF16, CG>;
   const int n_groups = (n_int + G::T - 1) / G::T;
-  const int grid = n_groups < sm_count ? n_groups : sm_count;
-  k_unet_tc<C, BF16><<<grid, kTcThreads, G::SMEM, s>>>(hist, n_int, static_cast<const unsigned char*>(packed),
-                                                      split_e1, probs, list, n_list);
+  const int n_pg = (n_groups + CG - 1) / CG, max_pairs = sm_count / CG;
+  const int grid = CG * (n_pg < max_pairs ? n_pg : max_pairs);
+  if (CG == 1) {
+    k_unet_tc<C, BF16, CG><<<grid, kTcThreads, G::SMEM, s>>>(hist, n_int, static_cast<const unsigned char*>(packed),
+                                                            split_e1, probs, list, n_list);
+  } else {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(kTcThreads);
+    cfg.dynamicSmemBytes = G::SMEM;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = CG;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, k_unet_tc<C, BF16, CG>, hist, n_int, static_cast<const unsigned char*>(packed), split_e1,
+                       probs, list, n_list);
+  }
 }
 
-template <int C, int BF16>
+template <int C, int BF16, int CG>
 cudaError_t setup_impl() {
-  return cudaFuncSetAttribute(k_unet_tc<C, BF16>, cudaFuncAttributeMaxDynamicSharedMemorySize, Geo<C, BF16>::SMEM);
+  return cudaFuncSetAttribute(k_unet_tc<C, BF16, CG>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              Geo<C, BF16, CG>::SMEM);
 }
 
-#define PVF_TC_DISPATCH(CALL)                                     \
+#define PVF_TC_DISPATCH_CG(CALL, CG_)                             \
   do {                                                            \
     const int fm = precision == PVF_PREC_BF16 ? 1 : (precision == PVF_PREC_FP16 ? 2 : 0);   \
-    if (channels == 64) { if (fm == 1) CALL(64, 1); else if (fm == 2) CALL(64, 2); else CALL(64, 0); }      \
-    else if (channels == 32) { if (fm == 1) CALL(32, 1); else if (fm == 2) CALL(32, 2); else CALL(32, 0); } \
-    else { if (fm == 1) CALL(16, 1); else if (fm == 2) CALL(16, 2); else CALL(16, 0); }        \
+    if (channels == 64) { if (fm == 1) CALL(64, 1, CG_); else if (fm == 2) CALL(64, 2, CG_); else CALL(64, 0, CG_); }      \
+    else if (channels == 32) { if (fm == 1) CALL(32, 1, CG_); else if (fm == 2) CALL(32, 2, CG_); else CALL(32, 0, CG_); } \
+    else { if (fm == 1) CALL(16, 1, CG_); else if (fm == 2) CALL(16, 2, CG_); else CALL(16, 0, CG_); }        \
+  } while (0)
+#define PVF_TC_DISPATCH(CALL)                                     \
+  do {                                                            \
+    if (cta_pair) PVF_TC_DISPATCH_CG(CALL, 2); else PVF_TC_DISPATCH_CG(CALL, 1);   \
   } while (0)
 
 }  // namespace
 
-size_t unet_tc_packed_bytes(int channels, int precision, int split_mask) {
+size_t unet_tc_packed_bytes(int channels, int precision, int split_mask, int cta_pair) {
   size_t r = 0;
-#define PVF_CALL(C_, B_) r = (size_t)make_plan<C_, B_>(split_mask & 1).total
+#define PVF_CALL(C_, B_, G_) r = (size_t)G_ * make_plan<C_, B_, G_>(split_mask & 1).total
   PVF_TC_DISPATCH(PVF_CALL);
 #undef PVF_CALL
   return r;
 }
 
-void unet_tc_pack(const pvf_weights* w, int channels, int precision, int split_mask, void* host_dst) {
-#define PVF_CALL(C_, B_) pack_impl<C_, B_>(w, split_mask & 1, static_cast<unsigned char*>(host_dst))
+void unet_tc_pack(const pvf_weights* w, int channels, int precision, int split_mask, int cta_pair, void* host_dst) {
+#define PVF_CALL(C_, B_, G_) pack_impl<C_, B_, G_>(w, split_mask & 1, static_cast<unsigned char*>(host_dst))
   PVF_TC_DISPATCH(PVF_CALL);
 #undef PVF_CALL
 }
 
-cudaError_t unet_tc_setup(int channels, int precision, int split_mask) {
+cudaError_t unet_tc_setup(int channels, int precision, int split_mask, int cta_pair) {
   if (channels != 64 && channels != 32 && channels != 16) return cudaErrorInvalidValue;
   if (split_mask & ~1) return cudaErrorInvalidValue;          // only the e1 split is built
   if (precision != PVF_PREC_TF32 && split_mask) return cudaErrorInvalidValue;   // the split is a TF32 remedy
   cudaError_t e = cudaSuccess;
-#define PVF_CALL(C_, B_) e = setup_impl<C_, B_>()
+#define PVF_CALL(C_, B_, G_) e = setup_impl<C_, B_, G_>()
   PVF_TC_DISPATCH(PVF_CALL);
 #undef PVF_CALL
   return e;
 }
 
 void launch_unet_tc(const float* hist, int n_intervals_total, const void* packed_dev, int channels, int precision,
-                    int split_mask, float* probs, int sm_count, const int* list, const int* n_list, cudaStream_t s) {
+                    int split_mask, int cta_pair, float* probs, int sm_count, const int* list, const int* n_list,
+                    cudaStream_t s) {
   if (n_intervals_total <= 0) return;
-#define PVF_CALL(C_, B_) \
-  launch_impl<C_, B_>(hist, n_intervals_total, packed_dev, split_mask & 1, probs, sm_count, list, n_list, s)
+#define PVF_CALL(C_, B_, G_) \
+  launch_impl<C_, B_, G_>(hist, n_intervals_total, packed_dev, split_mask & 1, probs, sm_count, list, n_list, s)
   PVF_TC_DISPATCH(PVF_CALL);
 #undef PVF_CALL
 }

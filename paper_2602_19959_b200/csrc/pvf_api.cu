@@ -79,6 +79,8 @@ bool config_ok(const pvf_config* c) {
   if (c->split_mask < 0 || c->split_mask > 31) return false;
   if (c->max_events < 1 || c->max_tracks < 1 || c->max_tracks > 0x7fffffffLL) return false;
   if (c->elide_empty_intervals && c->precision == PVF_PREC_FP32) return false;   // tensor-core modes only
+  if (c->unet_cta_pair != 0 && c->unet_cta_pair != 1) return false;
+  if (c->unet_cta_pair && c->precision == PVF_PREC_FP32) return false;           // tensor-core modes only
   if (!(c->boundary_margin_mm >= 0.0f && c->boundary_margin_mm < 4.9f)) return false;
   if (c->boundary_margin_mm > 0.0f && c->max_tracks > (int64_t)kEntryMask) return false;
   return true;
@@ -97,7 +99,7 @@ Layout make_layout(const pvf_config* c) {
     L.conv_b_off[k] = f; f += shp[k][0]; f = (f + 63) / 64 * 64;
   }
   L.conv_f32 = take(sizeof(float) * f);
-  L.tc_packed = take(c->precision == PVF_PREC_FP32 ? 0 : unet_tc_packed_bytes(c->unet_channels, c->precision, c->split_mask));
+  L.tc_packed = take(c->precision == PVF_PREC_FP32 ? 0 : unet_tc_packed_bytes(c->unet_channels, c->precision, c->split_mask, c->unet_cta_pair));
   const size_t E = (size_t)c->max_events, T = (size_t)c->max_tracks;
   L.fc_w5img = take(c->precision == PVF_PREC_FP32 ? 0 : fc_tc_packed_bytes());
   L.el_list = take(c->elide_empty_intervals ? sizeof(int32_t) * E * kIntervals : 0);
@@ -214,11 +216,11 @@ pvf_status create_impl(const pvf_weights* w, const pvf_config* cfg, void* dev_po
     if (cfg->precision == PVF_PREC_FP32) {
       e = unet_simt_setup(cfg->unet_channels);
     } else {
-      const size_t nb = unet_tc_packed_bytes(cfg->unet_channels, cfg->precision, cfg->split_mask);
+      const size_t nb = unet_tc_packed_bytes(cfg->unet_channels, cfg->precision, cfg->split_mask, cfg->unet_cta_pair);
       std::vector<unsigned char> img(nb);
-      unet_tc_pack(w, cfg->unet_channels, cfg->precision, cfg->split_mask, img.data());
+      unet_tc_pack(w, cfg->unet_channels, cfg->precision, cfg->split_mask, cfg->unet_cta_pair, img.data());
       e = cudaMemcpy(h->tc_packed, img.data(), nb, cudaMemcpyHostToDevice);
-      if (e == cudaSuccess) e = unet_tc_setup(cfg->unet_channels, cfg->precision, cfg->split_mask);
+      if (e == cudaSuccess) e = unet_tc_setup(cfg->unet_channels, cfg->precision, cfg->split_mask, cfg->unet_cta_pair);
       if (e == cudaSuccess) {
         std::vector<unsigned char> fimg(fc_tc_packed_bytes());
         fc_tc_pack(w->fc_w[5], w->fc_b[5], fimg.data());
@@ -257,7 +259,7 @@ void enqueue_unet(pvf_ctx* h, const float* hist, int n_events, float* out_probs,
     launch_unet_simt(hist, n_int, h->conv_ptrs, h->cfg.unet_channels, out_probs, s);
   else
     launch_unet_tc(hist, n_int, h->tc_packed, h->cfg.unet_channels, h->cfg.precision, h->cfg.split_mask,
-                   out_probs, h->sm_count, list, n_list, s);
+                   h->cfg.unet_cta_pair, out_probs, h->sm_count, list, n_list, s);
 }
 
 }  // namespace
@@ -274,6 +276,7 @@ void pvf_default_config(pvf_config* c, int32_t max_events, int64_t max_tracks) {
   c->precision = PVF_PREC_FP32; c->split_mask = 0;
   c->max_events = max_events; c->max_tracks = max_tracks;
   c->enable_stage_timing = 0; c->enable_host_io = 0; c->elide_empty_intervals = 0; c->boundary_margin_mm = 0.0f;
+  c->unet_cta_pair = 0;
 }
 
 size_t pvf_workspace_bytes(const pvf_config* cfg) {

@@ -90,14 +90,15 @@ void launch_unet_simt(const float* hist, int n_intervals_total, const UnetParams
                       float* probs, cudaStream_t s);
 
 // a3, tcgen05/TMEM path (k_unet_tc.cu)
-size_t unet_tc_packed_bytes(int channels, int precision, int split_mask);
+// cta_pair: 0 = one CTA per MMA (cta_group::1); 1 = clusters of two CTAs sharing every MMA (cta_group::2)
+size_t unet_tc_packed_bytes(int channels, int precision, int split_mask, int cta_pair);
 // packs PyTorch-layout host weights into the shared-memory image order the kernel streams
-void unet_tc_pack(const pvf_weights* w, int channels, int precision, int split_mask, void* host_dst);
-cudaError_t unet_tc_setup(int channels, int precision, int split_mask);
+void unet_tc_pack(const pvf_weights* w, int channels, int precision, int split_mask, int cta_pair, void* host_dst);
+cudaError_t unet_tc_setup(int channels, int precision, int split_mask, int cta_pair);
 // list / n_list (device, optional): run only over intervals list[0 .. *n_list) (empty-interval elision)
 void launch_unet_tc(const float* hist, int n_intervals_total, const void* packed_dev, int channels,
-                    int precision, int split_mask, float* probs, int sm_count, const int* list, const int* n_list,
-                    cudaStream_t s);
+                    int precision, int split_mask, int cta_pair, float* probs, int sm_count, const int* list,
+                    const int* n_list, cudaStream_t s);
 
 // NEXT-2, empty-interval elision (k_compact.cu): work list of non-empty intervals + constant fill of the rest
 void launch_compact_fill(const int32_t* seg_cnt, int n_total, int32_t* list, int32_t* n_list, const float* p0,

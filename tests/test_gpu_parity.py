@@ -324,6 +324,33 @@ def test_empty_interval_elision_is_bit_identical(prec):
         _make(w, ev, "fp32", elide_empty=True)                    # tensor-core modes only
 
 
+# ------------------------------------------------------------------ CTA pairs (cta_group::2)
+@pytest.mark.parametrize("prec,channels", [("tf32", 64), ("bf16", 64), ("fp16", 64), ("tf32", 32), ("bf16", 32),
+                                           ("tf32", 16), ("bf16", 16)])
+def test_cta_pair_is_bit_identical(prec, channels):
+    """unet_cta_pair = 1 runs the same MMAs as M = 256 instructions shared by two CTAs: identical arithmetic, so the
+    output must equal the one-CTA path bit for bit.  37 events = 1480 intervals: an odd number of groups at T = 8
+    (one CTA of the last pair idles), several pair-groups per cluster, with and without elision."""
+    ev = make_events("run3", 37, 556)
+    w = make_weights("peaky", 3, channels=channels)
+    one = _make(w, ev, prec)
+    two = _make(w, ev, prec, cta_pair=True)
+    p1, k1 = _run(one, ev)
+    p2, k2 = _run(two, ev)
+    assert torch.equal(p1, p2)
+    assert all(torch.equal(k1[k], k2[k]) for k in k1)
+    for n in (1, 3):                                              # 40 / 120 intervals: fewer pairs than SMs
+        q1, _ = _run(one, ev, n)
+        q2, _ = _run(two, ev, n)
+        assert torch.equal(q1[:n], q2[:n])
+    if channels == 64:
+        two_el = _make(w, ev, prec, cta_pair=True, elide_empty=True)
+        p3, _ = _run(two_el, ev)
+        assert torch.equal(p1, p3)
+    with pytest.raises(pkg.PVFError):
+        _make(w, ev, "fp32", cta_pair=True)                       # tensor-core modes only
+
+
 # ------------------------------------------------------------------ boundary behaviour
 def test_boundary_contract():
     ev = make_events("run3", 4, 77)
