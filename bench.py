@@ -184,6 +184,7 @@ def main_ours(args, rank, world, local_rank):
     split = args.split_mask if args.split_mask >= 0 else (1 if args.precision == "tf32" else 0)
     pvf = PVFinder(w, max_events=E, max_tracks=ev.n_tracks, precision=args.precision, split_mask=split,
                    stage_timing=True, host_io=True, elide_empty=args.elide_empty,
+                   cta_pair=bool(args.cta_pair) and args.precision != "fp32",
                    boundary_margin_mm=args.boundary_margin)
     feat = torch.from_numpy(ev.feat).cuda()
     off = torch.from_numpy(ev.event_offsets).cuda()
@@ -287,7 +288,7 @@ def main_ours(args, rank, world, local_rank):
         "config": {"workload": f"BASELINE.json config {_config_id(args)}: {E} events/GPU, "
                                f"model {args.model}, {ev.n_tracks} tracks, UNet {args.channels} ch, weights {args.weights}",
                    "precision": args.precision, "split_mask": split,
-                   "elide_empty_intervals": bool(args.elide_empty), "boundary_margin_mm": args.boundary_margin, "nonempty_interval_fraction": nonempty,
+                   "elide_empty_intervals": bool(args.elide_empty), "unet_cta_pair": bool(args.cta_pair) and args.precision != "fp32", "boundary_margin_mm": args.boundary_margin, "nonempty_interval_fraction": nonempty,
                    "cache": ("inputs larger than L2 (107 MB features, 2 GB histogram per step)" if E >= 2000 else
                              "small batch: inputs fit in L2 (latency-style measurement)")},
         "us_per_event": ms * 1e3 / (args.steps * E),
@@ -329,6 +330,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--boundary-margin", type=float, default=0.0,
                     help="NEXT-1 mode (mm): boundary tracks contribute to two intervals, PAPER.md:49")
+    ap.add_argument("--cta-pair", type=int, default=0, choices=[0, 1],
+                    help="UNet as clusters of two CTAs sharing every MMA (cta_group::2)")
     ap.add_argument("--elide-empty", action="store_true",
                     help="NEXT-2 mode: UNet only over non-empty intervals (reported with executed-FLOP accounting)")
     args = ap.parse_args()
