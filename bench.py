@@ -330,7 +330,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--boundary-margin", type=float, default=0.0,
                     help="NEXT-1 mode (mm): boundary tracks contribute to two intervals, PAPER.md:49")
-    ap.add_argument("--cta-pair", type=int, default=0, choices=[0, 1],
+    ap.add_argument("--cta-pair", type=int, default=1, choices=[0, 1],
                     help="UNet as clusters of two CTAs sharing every MMA (cta_group::2)")
     ap.add_argument("--elide-empty", action="store_true",
                     help="NEXT-2 mode: UNet only over non-empty intervals (reported with executed-FLOP accounting)")

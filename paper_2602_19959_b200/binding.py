@@ -122,13 +122,15 @@ class PVFinder:
 
     def __init__(self, weights, max_events: int, max_tracks: int, precision="fp32", channels: int | None = None,
                  split_mask: int = 0, stage_timing: bool = False, host_io: bool = False, elide_empty: bool = False,
-                 boundary_margin_mm: float = 0.0, cta_pair: bool = False, pool=None, lib=None,
+                 boundary_margin_mm: float = 0.0, cta_pair: bool | None = None, pool=None, lib=None,
                  **cfg_over):
         import torch  # device memory + streams only
         self.torch = torch
         self.lib = lib or load_library()
         ch = channels if channels is not None else getattr(weights, "channels", 64)
         prec = PRECISIONS[precision] if isinstance(precision, str) else int(precision)
+        if cta_pair is None:                 # tensor-core modes default to CTA pairs (cta_group::2): faster, same bits
+            cta_pair = prec != PRECISIONS["fp32"]
         self.cfg = default_config(self.lib, max_events, max_tracks, unet_channels=ch, precision=prec,
                                   split_mask=split_mask, enable_stage_timing=int(stage_timing),
                                   enable_host_io=int(host_io), elide_empty_intervals=int(elide_empty),

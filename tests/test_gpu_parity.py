@@ -333,7 +333,7 @@ def test_cta_pair_is_bit_identical(prec, channels):
     (one CTA of the last pair idles), several pair-groups per cluster, with and without elision."""
     ev = make_events("run3", 37, 556)
     w = make_weights("peaky", 3, channels=channels)
-    one = _make(w, ev, prec)
+    one = _make(w, ev, prec, cta_pair=False)
     two = _make(w, ev, prec, cta_pair=True)
     p1, k1 = _run(one, ev)
     p2, k2 = _run(two, ev)
