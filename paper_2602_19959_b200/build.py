@@ -16,6 +16,7 @@ LIB = os.path.join(HERE, "libpvf.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"]
+FLAGS += os.environ.get("PVF_NVCC_EXTRA", "").split()      # e.g. -DPVF_UNET_PROF (issuer wait-time counters)
 
 
 def _sources():

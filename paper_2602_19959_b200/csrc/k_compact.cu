@@ -45,6 +45,21 @@ k_fill_empty(const int32_t* __restrict__ seg_cnt, int n_total, const float* __re
   for (int l = lane; l < kBins; l += 32) dst[l] = p0[l];
 }
 
+// out[n, 0..800) = seg_cnt[n] > 0 ? hist[n, 0..800) : 0 (one block per interval).
+__global__ void __launch_bounds__(200)
+k_copy_hist_masked(const float* __restrict__ hist, const int32_t* __restrict__ seg_cnt, float* __restrict__ out) {
+  const size_t n = blockIdx.x;
+  const bool live = seg_cnt[n] > 0;
+  const float4* src = reinterpret_cast<const float4*>(hist + n * kFcOut);
+  float4* dst = reinterpret_cast<float4*>(out + n * kFcOut);
+  dst[threadIdx.x] = live ? src[threadIdx.x] : make_float4(0.f, 0.f, 0.f, 0.f);
+}
+
+void launch_copy_hist_masked(const float* hist, const int32_t* seg_cnt, int n_total, float* out, cudaStream_t s) {
+  if (n_total <= 0) return;
+  k_copy_hist_masked<<<n_total, 200, 0, s>>>(hist, seg_cnt, out);
+}
+
 void launch_compact_fill(const int32_t* seg_cnt, int n_total, int32_t* list, int32_t* n_list, const float* p0,
                          float* probs, cudaStream_t s) {
   if (n_total <= 0) return;

@@ -78,11 +78,47 @@ __device__ __forceinline__ float softplus_ft(float v) {
 
 struct Feat9 { const float* f[9]; };
 
+// One step of the ordered segmented sum: track with interval iv and value x joins the running sum a of
+// interval c.  If the interval changes, the finished sum goes to base[c * 800] by a predicated store
+// and the sum restarts from x (0 + x == x exactly).  Written in PTX so that it stays one compare, one
+// 64-bit multiply-add, one predicated store and one select -- no branch (a taken branch per track cost more
+// than the softplus) and no predicate spilling.
+__device__ __forceinline__ void seg_step(float& a, int& c, int iv, float x, float* base) {
+  const float t = a + x;
+  float r;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t.reg .b64 ad;\n\t"
+      "setp.ne.s32 p, %1, %2;\n\t"
+      "mad.wide.s32 ad, %2, 3200, %3;\n\t"
+      "@p st.global.f32 [ad], %4;\n\t"
+      "selp.f32 %0, %5, %6, p;\n\t}"
+      : "=f"(r)
+      : "r"(iv), "r"(c), "l"(base), "f"(a), "f"(x), "f"(t)
+      : "memory");
+  a = r;
+  c = iv;
+}
+static_assert(kFcOut * 4 == 3200, "seg_step's interval stride");
+
+#ifdef PVF_FC_PROF
+// Diagnostic build only (-DPVF_FC_PROF): cycles per role and CTA (lane 0 of one warp per role):
+// [0] epilogue wait h_full, [1] epilogue wait acc_full, [2] epilogue total; [3] MMA wait h_full, [4] MMA wait acc_empty,
+// [5] MMA total; [6] hidden wait h_empty, [7] hidden wait meta, [8] hidden total (group 0), [9] tiles
+__device__ unsigned long long g_fc_prof[160][16];
+#define FC_PROF_T0() const long long prof_t0 = clock64()
+#define FC_PROF_ADD(slot, cond) do { if (cond) g_fc_prof[blockIdx.x + gridDim.x * blockIdx.y][slot] += (unsigned long long)(clock64() - prof_t0); } while (0)
+#define FC_PROF_CNT(slot, cond) do { if (cond) g_fc_prof[blockIdx.x + gridDim.x * blockIdx.y][slot] += 1ull; } while (0)
+#else
+#define FC_PROF_T0() do {} while (0)
+#define FC_PROF_ADD(slot, cond) do {} while (0)
+#define FC_PROF_CNT(slot, cond) do {} while (0)
+#endif
+
 __global__ void __launch_bounds__(kFtThreads, 1)
 k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* __restrict__ perm,
              const int32_t* __restrict__ seg_off, const int32_t* __restrict__ seg_cnt,
              const float* __restrict__ par, const unsigned char* __restrict__ w5img, int n_events,
-             float* __restrict__ hist) {
+             float* __restrict__ hist, float* __restrict__ dump) {
   extern __shared__ __align__(1024) unsigned char smem[];
   const uint32_t sb = smem_u32(smem);
   const int tid = threadIdx.x, lane = tid & 31;
@@ -140,24 +176,30 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
     const int r = 32 * q + lane;
     const bool valid = r < kBins;
     int it = 0;
+    const bool pw = tid == 0;
+    FC_PROF_T0();
     for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
       int ev_lo;
       const int nk = kept_of(e, ev_lo);
       float* He = hist + (size_t)e * kIntervals * kFcOut + (4 * half + 2 * mh) * kBins + r;   // + iv*800 + mm*100
       float acc0 = 0.f, acc1 = 0.f;              // running sums of the two channel tiles (no dynamic indexing)
-      int cur0 = 0, cur1 = 0;
+      int cur0 = 0, cur1 = 0;                    // interval the running sums belong to
       for (int base = 0; base < nk; base += kTile, ++it) {
         const int buf = it & 1, ntile = min(kTile, nk - base);
         const bool last = base + kTile >= nk;
-        mbar_wait(bar(bHFull + buf), (uint32_t)((it >> 1) & 1));      // s_iv[buf] is staged
+        { FC_PROF_T0(); mbar_wait(bar(bHFull + buf), (uint32_t)((it >> 1) & 1)); FC_PROF_ADD(0, pw); }   // s_iv[buf] is staged
+        FC_PROF_CNT(9, pw);
         const int* ivs = s_iv + buf * kTile;
+        if (base == 0) cur0 = cur1 = ivs[0];     // the event's first (lowest) non-empty interval
 #pragma unroll 1
         for (int mm = 0; mm < 2; ++mm) {
           const int mt = 2 * mh + mm;
-          mbar_wait(bar(bAccFull + mt), (uint32_t)(it & 1));
+          { FC_PROF_T0(); mbar_wait(bar(bAccFull + mt), (uint32_t)(it & 1)); FC_PROF_ADD(1, pw); }
           tc_fence_after_sync();
           const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)(mt * kTile);
-          float* Hc = He + mm * kBins;
+          // lanes 100..127 of a tile are not bins: their (meaningless) sums go to the dump slot, so that the
+          // store predicate of seg_step stays warp-uniform
+          float* Hc = valid ? He + mm * kBins : dump + r;
           float a = mm ? acc1 : acc0;
           int c = mm ? cur1 : cur0;
           for (int c0 = 0; c0 < ntile; c0 += 16) {
@@ -172,78 +214,53 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
             }
             tmem_ld_wait();
             // all 16 softplus first: independent, so the SFU pipeline stays full; columns past the
-            // tile's last track are computed on stale accumulators and then ignored
+            // tile's last track are computed on stale accumulators and then masked
             float sp[16];
 #pragma unroll
             for (int i = 0; i < 16; ++i) sp[i] = softplus_ft(__uint_as_float(v[i]));
             const int nv = ntile - c0;
+            // Ordered accumulation without branches (a taken branch per track cost more than the softplus):
+            // when the interval changes the finished sum goes out by a predicated store and the sum restarts
+            // from this track's value (0 + x == x exactly).  Only intervals that hold a track are written --
+            // the UNet kernel never reads the histogram of an empty interval (it takes seg_cnt == 0 as zeros).
             if (nv >= 16) {
 #pragma unroll
-              for (int i = 0; i < 16; ++i) {
-                if (ivv[i] != c) {           // interval finished: flush (zeros for skipped empty intervals)
-#pragma unroll 1
-                  while (c < ivv[i]) {
-                    if (valid) Hc[c * kFcOut] = a;
-                    a = 0.0f;
-                    ++c;
-                  }
-                }
-                a += sp[i];
-              }
-            } else {
-#pragma unroll 1
-              for (int i = 0; i < nv; ++i) {
-                const int ivt = ivs[c0 + i];
-#pragma unroll 1
-                while (c < ivt) {
-                  if (valid) Hc[c * kFcOut] = a;
-                  a = 0.0f;
-                  ++c;
-                }
-                // sp[] is indexed dynamically here only through this select chain (tail chunk, rare)
-                float x = sp[0];
+              for (int i = 0; i < 16; ++i) seg_step(a, c, ivv[i], sp[i], Hc);
+            } else {                              // ragged last chunk: inactive columns add +0 to the same interval
 #pragma unroll
-                for (int k = 1; k < 16; ++k) x = (i == k) ? sp[k] : x;
-                a += x;
+              for (int i = 0; i < 16; ++i) {
+                const bool act = i < nv;
+                seg_step(a, c, act ? ivv[i] : c, act ? sp[i] : 0.0f, Hc);
               }
             }
           }
-          if (last) {
-#pragma unroll 1
-            while (c < kIntervals) {
-              if (valid) Hc[c * kFcOut] = a;
-              a = 0.0f;
-              ++c;
-            }
-          }
+          if (last) Hc[c * kFcOut] = a;            // the event's last non-empty interval
           if (mm) { acc1 = a; cur1 = c; } else { acc0 = a; cur0 = c; }
           tc_fence_before_sync();
           mbar_arrive(bar(bAccEmpty + mt));
         }
         mbar_arrive(bar(bMeta + buf));
       }
-      if (nk <= 0 && valid) {                // event without kept tracks: all of its histograms are zero
-        for (int c = 0; c < kIntervals; ++c)
-#pragma unroll
-          for (int mm = 0; mm < 2; ++mm) He[c * kFcOut + mm * kBins] = 0.0f;
-      }
     }
+    FC_PROF_ADD(2, pw);
   } else if (warp == 8) {
     // ===================== MMA issuer
     constexpr uint32_t idesc = instr_desc(kFmtTF32, 128, kTile);
     constexpr uint32_t hi = (128u >> 4) | (1u << 14);
     constexpr uint32_t a_lbo = (uint32_t)(kLboW >> 4) << 16, b_lbo = (uint32_t)(kLboH >> 4) << 16;
     int it = 0;
+    const bool pw = lane == 0;
+    FC_PROF_T0();
     for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
       int ev_lo;
       const int nk = kept_of(e, ev_lo);
       for (int base = 0; base < nk; base += kTile, ++it) {
         const int buf = it & 1;
-        mbar_wait(bar(bHFull + buf), (uint32_t)((it >> 1) & 1));
+        { FC_PROF_T0(); mbar_wait(bar(bHFull + buf), (uint32_t)((it >> 1) & 1)); FC_PROF_ADD(3, pw); }
         tc_fence_after_sync();
 #pragma unroll
         for (int mt = 0; mt < 4; ++mt) {
-          mbar_wait(bar(bAccEmpty + mt), (uint32_t)((it & 1) ^ 1));
+          { FC_PROF_T0(); mbar_wait(bar(bAccEmpty + mt), (uint32_t)((it & 1) ^ 1)); FC_PROF_ADD(4, pw); }
           tc_fence_after_sync();
           if (elect_one()) {
 #pragma unroll
@@ -262,19 +279,22 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
         }
       }
     }
+    FC_PROF_ADD(5, pw);
   } else {
     // ===================== hidden layers: two groups of 128 threads, thread = track, alternating tiles
     const int g = (warp - 9) >> 2, i = tid - 288 - 128 * g;
     const uint32_t hbase = sb + OFF_H + (uint32_t)g * 2 * kHPart + (uint32_t)i * 16u;
     int it = 0;
+    const bool pw = g == 0 && i == 0;
+    FC_PROF_T0();
     for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
       int ev_lo;
       const int nk = kept_of(e, ev_lo);
       for (int base = 0; base < nk; base += kTile, ++it) {
         if ((it & 1) != g) continue;
         const uint32_t prev = (uint32_t)(((it >> 1) & 1) ^ 1);
-        mbar_wait(bar(bHEmpty + g), prev);         // the MMAs that read this buffer have retired
-        mbar_wait(bar(bMeta + g), prev);           // the epilogue is done with s_iv[g]
+        { FC_PROF_T0(); mbar_wait(bar(bHEmpty + g), prev); FC_PROF_ADD(6, pw); }   // the MMAs that read this buffer have retired
+        { FC_PROF_T0(); mbar_wait(bar(bMeta + g), prev); FC_PROF_ADD(7, pw); }     // the epilogue is done with s_iv[g]
         if (base + i < nk) {
           int t;
           float zrel;
@@ -326,6 +346,7 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
         mbar_arrive(bar(bHFull + g));
       }
     }
+    FC_PROF_ADD(8, pw);
   }
   tc_fence_before_sync();
   __syncthreads();
@@ -374,13 +395,22 @@ cudaError_t fc_tc_setup() {
 
 void launch_fc_hist_tc(const float* const feat[9], const int32_t* event_offsets, const int32_t* perm,
                        const int32_t* seg_off, const int32_t* seg_cnt, const float* fc_params, const void* w5img,
-                       int n_events, float* hist, int sm_count, cudaStream_t s) {
+                       int n_events, float* hist, float* dump, int sm_count, cudaStream_t s) {
   if (n_events <= 0) return;
   Feat9 F;
   for (int k = 0; k < 9; ++k) F.f[k] = feat[k];
   const int gx = n_events < sm_count / 2 ? n_events : sm_count / 2;
   k_fc_hist_tc<<<dim3(gx, 2), kFtThreads, FT_SMEM, s>>>(F, event_offsets, perm, seg_off, seg_cnt, fc_params,
-                                                        static_cast<const unsigned char*>(w5img), n_events, hist);
+                                                        static_cast<const unsigned char*>(w5img), n_events, hist, dump);
 }
+
+#ifdef PVF_FC_PROF
+extern "C" __attribute__((visibility("default"))) int pvf_debug_fc_prof(unsigned long long* host_out, int reset) {
+  cudaDeviceSynchronize();
+  if (host_out) cudaMemcpyFromSymbol(host_out, g_fc_prof, sizeof(g_fc_prof));
+  if (reset) { static unsigned long long z[160][16]; cudaMemcpyToSymbol(g_fc_prof, z, sizeof(z)); }
+  return 0;
+}
+#endif
 
 }  // namespace pvf

@@ -44,7 +44,7 @@ constexpr int kTcThreads = 192;
 constexpr int kMaxStages = 8;
 constexpr int kStageBytes = 16384;
 constexpr int kHeaderBytes = 2048;          // biases [5][C], head weight [C], head bias
-constexpr int kBarBytes = 512;
+constexpr int kBarBytes = 768;
 
 // sub-layers as the MMA issuer sees them
 enum { sE1 = 0, sE2 = 1, sB = 2, sD2 = 3, sD1U = 4, sD1E = 5 };
@@ -85,7 +85,7 @@ struct Geo {
   static constexpr int OFF_RING = OFF_XP + SZ_XP;
   static constexpr int SCR_BYTES = 2 * 4 * C * 4;    // epilogue row-exchange scratch: [2 buffers][4 warps][C floats]
   static constexpr int STAGES_FIT = (227 * 1024 - kHeaderBytes - kBarBytes - SCR_BYTES - OFF_RING) / STAGE_BYTES;
-  static constexpr int MAX_STAGES = CG == 2 ? 12 : kMaxStages;
+  static constexpr int MAX_STAGES = CG == 2 ? 12 : kMaxStages;   // measured: depth >= 6 changes nothing (bf16 and tf32)
   static constexpr int STAGES = STAGES_FIT < MAX_STAGES ? STAGES_FIT : MAX_STAGES;   // weight ring depth
   static constexpr int OFF_PAR = OFF_RING + STAGES * STAGE_BYTES;   // biases + head (floats)
   static constexpr int OFF_SCR = OFF_PAR + kHeaderBytes;
@@ -330,8 +330,11 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
 // its memory with P1, so every row the e1 MMAs can read for a valid output is (re)written: the lead
 // rows and the gap rows l >= 100 of every interval as zeros.
 template <int C, int BF16>
+// seg_cnt (optional): tracks per interval; an interval without tracks is taken as zeros WITHOUT reading hist
+// (the tensor-core FC kernel does not write the histograms of empty intervals).
 __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restrict__ hist, long long g0,
-                                        int n_valid_int, int split, int tid, const int* __restrict__ list) {
+                                        int n_valid_int, int split, int tid, const int* __restrict__ list,
+                                        const int* __restrict__ seg_cnt) {
   using G = Geo<C, BF16>;
   const uint32_t x0 = smem_base + G::OFF_XP;
   const uint4 zero4 = make_uint4(0, 0, 0, 0);
@@ -340,8 +343,9 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
   if (BF16) {
     for (int it = tid; it < G::T * 128; it += 128) {
       const int t = it >> 7, l = it & 127;
-      const bool live = l < 100 && t < n_valid_int;
+      bool live = l < 100 && t < n_valid_int;
       const long long src = !live ? 0 : (list ? (long long)list[g0 + t] : g0 + t);
+      if (live && seg_cnt != nullptr) live = __ldg(seg_cnt + src) > 0;
       float x[8];
 #pragma unroll
       for (int c = 0; c < 8; ++c) x[c] = live ? __ldg(hist + src * kFcOut + c * kBins + l) : 0.0f;
@@ -355,8 +359,9 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
   } else {
     for (int it = tid; it < G::T * 256; it += 128) {
       const int t = it >> 8, qc = (it >> 7) & 1, l = it & 127;
-      const bool live = l < 100 && t < n_valid_int;
+      bool live = l < 100 && t < n_valid_int;
       const long long src = !live ? 0 : (list ? (long long)list[g0 + t] : g0 + t);
+      if (live && seg_cnt != nullptr) live = __ldg(seg_cnt + src) > 0;
       float x[4];
 #pragma unroll
       for (int c = 0; c < 4; ++c) x[c] = live ? __ldg(hist + src * kFcOut + (4 * qc + c) * kBins + l) : 0.0f;
@@ -412,6 +417,17 @@ __device__ __forceinline__ void mma_lh(uint32_t d, uint32_t a_lo, uint32_t a_hi,
 
 struct RingState { int ring; uint32_t phase; };
 
+#ifdef PVF_UNET_PROF
+// Diagnostic build only (-DPVF_UNET_PROF): cycles the MMA issuer spent waiting, per CTA:
+// [0..5] wait_epi(k), [6] ring stage full (own half), [7] ring stage full (peer's half), [8] whole role loop
+__device__ unsigned long long g_unet_prof[160][16];
+#define PVF_PROF_T0() const long long prof_t0 = clock64()
+#define PVF_PROF_ADD(slot) do { if ((threadIdx.x & 31) == 0) g_unet_prof[blockIdx.x][slot] += (unsigned long long)(clock64() - prof_t0); } while (0)
+#else
+#define PVF_PROF_T0() do {} while (0)
+#define PVF_PROF_ADD(slot) do {} while (0)
+#endif
+
 // MMA steps [f_begin, f_end) of sub-layer S for the group: tap-major over ring stages, every stage
 // used by all NT tiles.  The warp walks the (uniform) schedule; one elected lane issues a whole
 // stage worth of MMAs whose descriptors differ from the stage origin by compile-time constants.
@@ -431,8 +447,16 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
   const uint32_t dcol = tmem_base + (uint32_t)Y::DCOL;
   for (int f = f_begin; f < f_end; f += SPS) {
     const int n = min(SPS, f_end - f);
-    mbar_wait(bar0 + 8u * rs.ring, rs.phase);
-    if (CG == 2) mbar_wait_cluster(bar0 + 8u * (2 * G::STAGES + rs.ring), rs.phase);   // the peer's half has landed
+    {
+      PVF_PROF_T0();
+      mbar_wait(bar0 + 8u * rs.ring, rs.phase);
+      PVF_PROF_ADD(6);
+    }
+    if (CG == 2) {
+      PVF_PROF_T0();
+      mbar_wait_cluster(bar0 + 8u * (2 * G::STAGES + rs.ring), rs.phase);   // the peer's half has landed
+      PVF_PROF_ADD(7);
+    }
     tc_fence_after_sync();
     const uint32_t b0 = b_lbo + ((sb + G::OFF_RING + rs.ring * G::STAGE_BYTES) >> 4);
     uint32_t a0 = a_lbo + (sb >> 4);          // stage origin: descriptor low word of tile 0, step f
@@ -477,7 +501,8 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
 template <int C, int BF16, int CG>
 __global__ void __launch_bounds__(kTcThreads, 1)
 k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __restrict__ wpack, int split_e1,
-          float* __restrict__ probs, const int* __restrict__ list, const int* __restrict__ n_list) {
+          float* __restrict__ probs, const int* __restrict__ list, const int* __restrict__ n_list,
+          const int* __restrict__ seg_cnt) {
   // list / n_list (device, optional): process only intervals list[0 .. *n_list) of hist / probs (elision of
   // empty intervals); n_int is then only the capacity the grid was sized for
   if (n_list != nullptr) n_int = *n_list;
@@ -561,8 +586,10 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
     RingState rs{0, 0u};
     uint32_t ph[6] = {0, 0, 0, 0, 0, 0};
     auto wait_epi = [&](int k) {
+      PVF_PROF_T0();
       mbar_wait(epi_bar(k), ph[k]);
       if (CG == 2) mbar_wait_cluster(pepi_bar(k), ph[k]);
+      PVF_PROF_ADD(k);
       ph[k] ^= 1u;
       tc_fence_after_sync();
     };
@@ -573,6 +600,7 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
       __syncwarp();
     };
     bool first = true;
+    PVF_PROF_T0();
     for (int pg = pg0; pg < n_pg; pg += stride) {
       const bool has_next = pg + stride < n_pg;
       if (first) {
@@ -603,6 +631,7 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
       commit(4);
       first = false;
     }
+    PVF_PROF_ADD(8);
   } else if (warp == 1) {
     // ===================== peer CTA of a pair: relay "my half of ring stage s has landed" to the leader
     if (lane == 0) {
@@ -651,7 +680,7 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
       const int* lg = list ? list + g0 : nullptr;
       const int* lgn = list ? list + gn0 : nullptr;
       if (first) {
-        load_x0<C, BF16>(sb, hist, g0, n_valid, split_e1, et, list);
+        load_x0<C, BF16>(sb, hist, g0, n_valid, split_e1, et, list, seg_cnt);
         done(0);
         wait_acc(0);
         for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kE1>(sb, tmem_base, t, q, lane, par, n_valid, pg_out, scr(), lg);
@@ -662,7 +691,7 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
       for (int t = 0; t < G::T / 2; ++t) epilogue_tile<C, BF16, kE2>(sb, tmem_base, t, q, lane, par, n_valid, pg_out, scr(), lg);
       done(2);
       if (has_next) {                                // P1 is dead (e2's MMAs retired): stage the next input
-        load_x0<C, BF16>(sb, hist, gn0, n_valid_next, split_e1, et, list);
+        load_x0<C, BF16>(sb, hist, gn0, n_valid_next, split_e1, et, list, seg_cnt);
         done(0);
       }
       wait_acc(2);
@@ -782,14 +811,14 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst_all) {
 
 template <int C, int BF16, int CG>
 void launch_impl(const float* hist, int n_int, const void* packed, int split_e1, float* probs, int sm_count,
-                 const int* list, const int* n_list, cudaStream_t s) {
+                 const int* list, const int* n_list, const int* seg_cnt, cudaStream_t s) {
   using G = Geo<C, BF16, CG>;
   const int n_groups = (n_int + G::T - 1) / G::T;
   const int n_pg = (n_groups + CG - 1) / CG, max_pairs = sm_count / CG;
   const int grid = CG * (n_pg < max_pairs ? n_pg : max_pairs);
   if (CG == 1) {
     k_unet_tc<C, BF16, CG><<<grid, kTcThreads, G::SMEM, s>>>(hist, n_int, static_cast<const unsigned char*>(packed),
-                                                            split_e1, probs, list, n_list);
+                                                            split_e1, probs, list, n_list, seg_cnt);
   } else {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
@@ -804,7 +833,7 @@ void launch_impl(const float* hist, int n_int, const void* packed, int split_e1,
     cfg.attrs = at;
     cfg.numAttrs = 1;
     cudaLaunchKernelEx(&cfg, k_unet_tc<C, BF16, CG>, hist, n_int, static_cast<const unsigned char*>(packed), split_e1,
-                       probs, list, n_list);
+                       probs, list, n_list, seg_cnt);
   }
 }
 
@@ -855,12 +884,21 @@ cudaError_t unet_tc_setup(int channels, int precision, int split_mask, int cta_p
 
 void launch_unet_tc(const float* hist, int n_intervals_total, const void* packed_dev, int channels, int precision,
                     int split_mask, int cta_pair, float* probs, int sm_count, const int* list, const int* n_list,
-                    cudaStream_t s) {
+                    const int* seg_cnt, cudaStream_t s) {
   if (n_intervals_total <= 0) return;
 #define PVF_CALL(C_, B_, G_) \
-  launch_impl<C_, B_, G_>(hist, n_intervals_total, packed_dev, split_mask & 1, probs, sm_count, list, n_list, s)
+  launch_impl<C_, B_, G_>(hist, n_intervals_total, packed_dev, split_mask & 1, probs, sm_count, list, n_list, seg_cnt, s)
   PVF_TC_DISPATCH(PVF_CALL);
 #undef PVF_CALL
 }
+
+#ifdef PVF_UNET_PROF
+extern "C" __attribute__((visibility("default"))) int pvf_debug_unet_prof(unsigned long long* host_out, int reset) {
+  cudaDeviceSynchronize();
+  if (host_out) cudaMemcpyFromSymbol(host_out, g_unet_prof, sizeof(g_unet_prof));
+  if (reset) { static unsigned long long z[160][16]; cudaMemcpyToSymbol(g_unet_prof, z, sizeof(z)); }
+  return 0;
+}
+#endif
 
 }  // namespace pvf

@@ -109,7 +109,7 @@ Layout make_layout(const pvf_config* c) {
   L.seg_off = take(sizeof(int32_t) * E * kIntervals);
   L.seg_cnt = take(sizeof(int32_t) * E * kIntervals);
   L.flags = take(sizeof(uint32_t) * E);
-  L.hist = take(sizeof(float) * E * kIntervals * kFcOut);
+  L.hist = take(sizeof(float) * (E * kIntervals * kFcOut + (c->precision == PVF_PREC_FP32 ? 0 : kFcDumpFloats)));
   if (c->enable_host_io) {
     L.st_feat = take(sizeof(float) * 9 * T);
     L.st_off = take(sizeof(int32_t) * (E + 1));
@@ -135,8 +135,9 @@ pvf_status fail_cuda(pvf_ctx* h, cudaError_t e, const char* where) {
     if (e__ != cudaSuccess) return fail_cuda((h), e__, #call);        \
   } while (0)
 
+// seg_cnt != nullptr: hist is the pool's histogram as the tensor-core FC kernel leaves it (empty intervals unwritten)
 void enqueue_unet(pvf_ctx* h, const float* hist, int n_events, float* out_probs, cudaStream_t s,
-                  const int* list = nullptr, const int* n_list = nullptr);
+                  const int* list = nullptr, const int* n_list = nullptr, const int* seg_cnt = nullptr);
 
 bool peaks_ok(const pvf_peaks* p) { return p && p->z_mm && p->prob && p->bin && p->count; }
 
@@ -253,13 +254,13 @@ pvf_status create_impl(const pvf_weights* w, const pvf_config* cfg, void* dev_po
 }
 
 void enqueue_unet(pvf_ctx* h, const float* hist, int n_events, float* out_probs, cudaStream_t s, const int* list,
-                  const int* n_list) {
+                  const int* n_list, const int* seg_cnt) {
   const int n_int = n_events * kIntervals;
   if (h->cfg.precision == PVF_PREC_FP32)
     launch_unet_simt(hist, n_int, h->conv_ptrs, h->cfg.unet_channels, out_probs, s);
   else
     launch_unet_tc(hist, n_int, h->tc_packed, h->cfg.unet_channels, h->cfg.precision, h->cfg.split_mask,
-                   h->cfg.unet_cta_pair, out_probs, h->sm_count, list, n_list, s);
+                   h->cfg.unet_cta_pair, out_probs, h->sm_count, list, n_list, seg_cnt, s);
 }
 
 }  // namespace
@@ -313,13 +314,15 @@ pvf_status pvf_run(pvf_handle h, const pvf_tracks* t, int32_t n_events, float* o
     launch_fc_hist(t->feat, t->event_offsets, h->perm, h->seg_off, h->seg_cnt, h->fc_params, n_events, h->hist, s);
   else
     launch_fc_hist_tc(t->feat, t->event_offsets, h->perm, h->seg_off, h->seg_cnt, h->fc_params, h->fc_w5img, n_events,
-                      h->hist, h->sm_count, s);
+                      h->hist, h->hist + (size_t)h->cfg.max_events * kIntervals * kFcOut, h->sm_count, s);
   if (timing) cudaEventRecord(ev[2], s);
   if (h->cfg.elide_empty_intervals) {
     launch_compact_fill(h->seg_cnt, n_events * kIntervals, h->el_list, h->el_count, h->el_p0, out_probs, s);
-    enqueue_unet(h, h->hist, n_events, out_probs, s, h->el_list, h->el_count);
+    enqueue_unet(h, h->hist, n_events, out_probs, s, h->el_list, h->el_count);   // the list holds non-empty intervals only
   } else {
-    enqueue_unet(h, h->hist, n_events, out_probs, s);
+    // tensor-core modes: k_fc_hist_tc leaves the histograms of empty intervals unwritten, the UNet takes them as zeros
+    enqueue_unet(h, h->hist, n_events, out_probs, s, nullptr, nullptr,
+                 h->cfg.precision == PVF_PREC_FP32 ? nullptr : h->seg_cnt);
   }
   if (timing) cudaEventRecord(ev[3], s);
   launch_peaks(out_probs, n_events, h->cfg.peak_threshold, h->flags, pk->z_mm, pk->prob, pk->bin, pk->count,
@@ -388,8 +391,13 @@ pvf_status pvf_debug_copy_histogram(pvf_handle h, float* dev_out, int32_t n_even
   if (!h || !dev_out || !cuda_stream || n_events < 0) return PVF_ERR_ARG;
   if (n_events > h->last_n_events) return PVF_ERR_ARG;
   if (n_events == 0) return PVF_OK;
-  PVF_CUDA(h, cudaMemcpyAsync(dev_out, h->hist, sizeof(float) * (size_t)n_events * kIntervals * kFcOut,
-                              cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(cuda_stream)));
+  if (h->cfg.precision == PVF_PREC_FP32) {
+    PVF_CUDA(h, cudaMemcpyAsync(dev_out, h->hist, sizeof(float) * (size_t)n_events * kIntervals * kFcOut,
+                                cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(cuda_stream)));
+  } else {   // the tensor-core FC kernel writes non-empty intervals only: empty ones are zeros by definition
+    launch_copy_hist_masked(h->hist, h->seg_cnt, n_events * kIntervals, dev_out, static_cast<cudaStream_t>(cuda_stream));
+    PVF_CUDA(h, cudaPeekAtLastError());
+  }
   return PVF_OK;
 }
 

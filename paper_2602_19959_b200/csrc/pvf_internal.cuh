@@ -81,7 +81,9 @@ void fc_tc_pack(const float* w5, const float* b5, void* host_dst);
 cudaError_t fc_tc_setup();
 void launch_fc_hist_tc(const float* const feat[9], const int32_t* event_offsets, const int32_t* perm,
                        const int32_t* seg_off, const int32_t* seg_cnt, const float* fc_params, const void* w5img,
-                       int n_events, float* hist, int sm_count, cudaStream_t s);
+                       int n_events, float* hist, float* dump, int sm_count, cudaStream_t s);
+// dump: kFcDumpFloats floats of scratch that the padding lanes of the accumulator tiles write their sums to
+constexpr size_t kFcDumpFloats = (size_t)kIntervals * kFcOut + 1024;
 
 // a3, FP32 CUDA-core path (k_unet_simt.cu).  conv params: PyTorch layout, floats.
 struct UnetParamsF32 { const float* w[6]; const float* b[6]; };
@@ -96,11 +98,14 @@ size_t unet_tc_packed_bytes(int channels, int precision, int split_mask, int cta
 void unet_tc_pack(const pvf_weights* w, int channels, int precision, int split_mask, int cta_pair, void* host_dst);
 cudaError_t unet_tc_setup(int channels, int precision, int split_mask, int cta_pair);
 // list / n_list (device, optional): run only over intervals list[0 .. *n_list) (empty-interval elision)
+// seg_cnt (device, optional): tracks per interval; intervals with none are taken as zeros without reading hist
 void launch_unet_tc(const float* hist, int n_intervals_total, const void* packed_dev, int channels,
                     int precision, int split_mask, int cta_pair, float* probs, int sm_count, const int* list,
-                    const int* n_list, cudaStream_t s);
+                    const int* n_list, const int* seg_cnt, cudaStream_t s);
 
 // NEXT-2, empty-interval elision (k_compact.cu): work list of non-empty intervals + constant fill of the rest
+// canonical histogram out of the pool's: out[n] = seg_cnt[n] > 0 ? hist[n] : 0 (debug accessor, tensor-core modes)
+void launch_copy_hist_masked(const float* hist, const int32_t* seg_cnt, int n_total, float* out, cudaStream_t s);
 void launch_compact_fill(const int32_t* seg_cnt, int n_total, int32_t* list, int32_t* n_list, const float* p0,
                          float* probs, cudaStream_t s);
 

@@ -36,12 +36,29 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
       : "memory");
   return ok != 0;
 }
+// Same with a suspend-time hint (ns): the thread may sleep in hardware until the phase completes or the
+// time is up, instead of coming back at once and re-issuing (a spinning waiter takes issue slots from
+// the warps it is waiting for).
+#ifndef PVF_MBAR_HINT_NS
+#define PVF_MBAR_HINT_NS 2000
+#endif
+__device__ __forceinline__ bool mbar_try_wait_hint(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+      "selp.b32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok)
+      : "r"(bar), "r"(parity), "r"((uint32_t)PVF_MBAR_HINT_NS)
+      : "memory");
+  return ok != 0;
+}
 // Waits for the phase with the given parity to complete.  A wait that lasts longer than ~2 s of
 // SM clock is a protocol bug: trap instead of hanging the device.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   if (mbar_try_wait(bar, parity)) return;
   const long long t0 = clock64();
-  while (!mbar_try_wait(bar, parity)) {
+  while (!mbar_try_wait_hint(bar, parity)) {
     if (clock64() - t0 > 4000000000LL) __trap();
   }
 }
