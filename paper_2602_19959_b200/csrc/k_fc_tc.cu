@@ -30,7 +30,11 @@ using namespace umma;
 
 namespace {
 
-constexpr int kFtThreads = 17 * 32;           // 8 epilogue + 1 MMA + 8 hidden-layer warps
+constexpr int kEpiWarps = 13;                // one per (accumulator tile, 32-lane quadrant) that holds outputs
+constexpr int kMmaWarp = kEpiWarps;
+constexpr int kHidWarp0 = kMmaWarp + 1;
+constexpr int kFtThreads = (kEpiWarps + 1 + 8) * 32;   // 13 epilogue + 1 MMA + 8 hidden-layer warps
+constexpr int kHalfOut = kFcOut / 2;         // outputs per CTA half, packed densely: row 128 t + r = output 400 half + 128 t + r
 constexpr int kTile = 128;                   // tracks per tile (MMA N)
 constexpr int kRowsW = 512;                  // 4 channel tiles x 128 rows per CTA half
 constexpr int kLboW = kRowsW * 16;           // 8192: next 16-byte K chunk of the A operand
@@ -49,12 +53,14 @@ struct FtSmall {                             // the five hidden layers, zero pad
 constexpr int OFF_W = 0;                               // [hi | lo][8 chunks][512 rows][16 B]
 constexpr int OFF_H = OFF_W + 2 * kWPart;              // [buf 0 | 1][hi | lo][8 chunks][128 tracks][16 B]
 constexpr int OFF_SMALL = OFF_H + 4 * kHPart;
-constexpr int OFF_IV = OFF_SMALL + ((int)sizeof(FtSmall) + 127) / 128 * 128;   // int [2][128]
-constexpr int OFF_BARS = OFF_IV + 2 * kTile * 4;
-constexpr int FT_SMEM = OFF_BARS + 128;
+constexpr int OFF_IV = OFF_SMALL + ((int)sizeof(FtSmall) + 127) / 128 * 128;   // int [4][128]
+constexpr int kIvBufs = 4;                   // interval lists of four tiles in flight: the hidden-layer warps of tile
+                                             // i + 2 must not wait for the epilogue of tile i (measured: they did)
+constexpr int OFF_BARS = OFF_IV + kIvBufs * kTile * 4;
+constexpr int FT_SMEM = OFF_BARS + 256;
 static_assert(FT_SMEM <= 227 * 1024, "shared memory budget");
 // barriers (8 bytes each): h_full[2], h_empty[2], meta_empty[2], acc_full[4], acc_empty[4], then the TMEM slot
-enum { bHFull = 0, bHEmpty = 2, bMeta = 4, bAccFull = 6, bAccEmpty = 10, bSlot = 14 };
+enum { bHFull = 0, bHEmpty = 2, bMeta = 4, bAccFull = 8, bAccEmpty = 12, bSlot = 16 };
 
 __device__ __forceinline__ float leaky_ft(float v) { return v >= 0.0f ? v : kLeaky * v; }
 __device__ __forceinline__ uint32_t tf32_of(float v) {
@@ -151,11 +157,12 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
     S.bh[l][c] = c < kFcHidden ? par[kFcHid + l * kFcHidStride + kFcHidden * kFcHidden + c] : 0.0f;
   }
   if (tid == 0) {
-    for (int k = 0; k < 2; ++k) { mbar_init(bar(bHFull + k), 128); mbar_init(bar(bHEmpty + k), 1); mbar_init(bar(bMeta + k), 256); }
-    for (int k = 0; k < 4; ++k) { mbar_init(bar(bAccFull + k), 1); mbar_init(bar(bAccEmpty + k), 128); }
+    for (int k = 0; k < 2; ++k) { mbar_init(bar(bHFull + k), 128); mbar_init(bar(bHEmpty + k), 1); }
+    for (int k = 0; k < kIvBufs; ++k) mbar_init(bar(bMeta + k), 32 * kEpiWarps);
+    for (int k = 0; k < 4; ++k) { mbar_init(bar(bAccFull + k), 1); mbar_init(bar(bAccEmpty + k), k < 3 ? 128 : 32); }
     fence_mbar_init();
   }
-  if (warp == 8) tmem_alloc(smem_u32(const_cast<uint32_t*>(tmem_slot)), 512);
+  if (warp == kMmaWarp) tmem_alloc(smem_u32(const_cast<uint32_t*>(tmem_slot)), 512);
   fence_proxy_async_smem();
   tc_fence_before_sync();
   __syncthreads();
@@ -169,81 +176,73 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
     return seg_off[s] + seg_cnt[s] - ev_lo;
   };
 
-  if (warp < 8) {
-    // ===================== epilogue: lane = output bin, column = track (sorted order).  Warps 0-3 own
-    // channel tiles 0 and 1, warps 4-7 tiles 2 and 3 (two warps per scheduler hide each other's latency).
-    const int q = warp & 3, mh = warp >> 2;
-    const int r = 32 * q + lane;
-    const bool valid = r < kBins;
+  if (warp < kEpiWarps) {
+    // ===================== epilogue: lane = output, column = track (sorted order).  The 400 outputs of this half
+    // fill accumulator tiles 0-2 and 16 rows of tile 3; warp w owns the 32 rows of quadrant w & 3 of tile w >> 2
+    // (warp 12: the 16 rows of tile 3), so every warp has one tile per 128 tracks.
+    const int q = warp & 3, mt = warp >> 2;
+    const int r = 32 * q + lane, ol = 128 * mt + r;
+    const bool valid = ol < kHalfOut;
     int it = 0;
     const bool pw = tid == 0;
     FC_PROF_T0();
     for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
       int ev_lo;
       const int nk = kept_of(e, ev_lo);
-      float* He = hist + (size_t)e * kIntervals * kFcOut + (4 * half + 2 * mh) * kBins + r;   // + iv*800 + mm*100
-      float acc0 = 0.f, acc1 = 0.f;              // running sums of the two channel tiles (no dynamic indexing)
-      int cur0 = 0, cur1 = 0;                    // interval the running sums belong to
+      // output o = c * 100 + l lives at H[e][interval][o]: the dense row index is the offset itself.  Rows that
+      // hold no output send their (meaningless) sums to the dump slot, so seg_step's store predicate stays
+      // warp-uniform.
+      float* Hc = valid ? hist + (size_t)e * kIntervals * kFcOut + kHalfOut * half + ol : dump + r;   // + iv * 800
+      float a = 0.f;                             // running sum of the current interval
+      int c = 0;                                 // the interval it belongs to
       for (int base = 0; base < nk; base += kTile, ++it) {
         const int buf = it & 1, ntile = min(kTile, nk - base);
         const bool last = base + kTile >= nk;
-        { FC_PROF_T0(); mbar_wait(bar(bHFull + buf), (uint32_t)((it >> 1) & 1)); FC_PROF_ADD(0, pw); }   // s_iv[buf] is staged
+        { FC_PROF_T0(); mbar_wait(bar(bHFull + buf), (uint32_t)((it >> 1) & 1)); FC_PROF_ADD(0, pw); }   // s_iv is staged
         FC_PROF_CNT(9, pw);
-        const int* ivs = s_iv + buf * kTile;
-        if (base == 0) cur0 = cur1 = ivs[0];     // the event's first (lowest) non-empty interval
-#pragma unroll 1
-        for (int mm = 0; mm < 2; ++mm) {
-          const int mt = 2 * mh + mm;
-          { FC_PROF_T0(); mbar_wait(bar(bAccFull + mt), (uint32_t)(it & 1)); FC_PROF_ADD(1, pw); }
-          tc_fence_after_sync();
-          const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)(mt * kTile);
-          // lanes 100..127 of a tile are not bins: their (meaningless) sums go to the dump slot, so that the
-          // store predicate of seg_step stays warp-uniform
-          float* Hc = valid ? He + mm * kBins : dump + r;
-          float a = mm ? acc1 : acc0;
-          int c = mm ? cur1 : cur0;
-          for (int c0 = 0; c0 < ntile; c0 += 16) {
-            uint32_t v[16];
-            tmem_ld_x16(taddr + (uint32_t)c0, v);
-            // intervals of the 16 tracks (broadcast 16-byte loads) while the TMEM load is in flight
-            int ivv[16];
+        const int* ivs = s_iv + (it & (kIvBufs - 1)) * kTile;
+        if (base == 0) c = ivs[0];               // the event's first (lowest) non-empty interval
+        { FC_PROF_T0(); mbar_wait(bar(bAccFull + mt), (uint32_t)(it & 1)); FC_PROF_ADD(1, pw); }
+        tc_fence_after_sync();
+        const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)(mt * kTile);
+        for (int c0 = 0; c0 < ntile; c0 += 16) {
+          uint32_t v[16];
+          tmem_ld_x16(taddr + (uint32_t)c0, v);
+          // intervals of the 16 tracks (broadcast 16-byte loads) while the TMEM load is in flight
+          int ivv[16];
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-              const int4 q4 = *reinterpret_cast<const int4*>(ivs + c0 + 4 * k);
-              ivv[4 * k + 0] = q4.x; ivv[4 * k + 1] = q4.y; ivv[4 * k + 2] = q4.z; ivv[4 * k + 3] = q4.w;
-            }
-            tmem_ld_wait();
-            // all 16 softplus first: independent, so the SFU pipeline stays full; columns past the
-            // tile's last track are computed on stale accumulators and then masked
-            float sp[16];
+          for (int k = 0; k < 4; ++k) {
+            const int4 q4 = *reinterpret_cast<const int4*>(ivs + c0 + 4 * k);
+            ivv[4 * k + 0] = q4.x; ivv[4 * k + 1] = q4.y; ivv[4 * k + 2] = q4.z; ivv[4 * k + 3] = q4.w;
+          }
+          tmem_ld_wait();
+          // all 16 softplus first: independent, so the SFU pipeline stays full; columns past the
+          // tile's last track are computed on stale accumulators and then masked
+          float sp[16];
 #pragma unroll
-            for (int i = 0; i < 16; ++i) sp[i] = softplus_ft(__uint_as_float(v[i]));
-            const int nv = ntile - c0;
-            // Ordered accumulation without branches (a taken branch per track cost more than the softplus):
-            // when the interval changes the finished sum goes out by a predicated store and the sum restarts
-            // from this track's value (0 + x == x exactly).  Only intervals that hold a track are written --
-            // the UNet kernel never reads the histogram of an empty interval (it takes seg_cnt == 0 as zeros).
-            if (nv >= 16) {
+          for (int i = 0; i < 16; ++i) sp[i] = softplus_ft(__uint_as_float(v[i]));
+          const int nv = ntile - c0;
+          // Ordered accumulation without branches (seg_step).  Only intervals that hold a track are written --
+          // the UNet kernel never reads the histogram of an empty interval (it takes seg_cnt == 0 as zeros).
+          if (nv >= 16) {
 #pragma unroll
-              for (int i = 0; i < 16; ++i) seg_step(a, c, ivv[i], sp[i], Hc);
-            } else {                              // ragged last chunk: inactive columns add +0 to the same interval
+            for (int i = 0; i < 16; ++i) seg_step(a, c, ivv[i], sp[i], Hc);
+          } else {                                // ragged last chunk: inactive columns add +0 to the same interval
 #pragma unroll
-              for (int i = 0; i < 16; ++i) {
-                const bool act = i < nv;
-                seg_step(a, c, act ? ivv[i] : c, act ? sp[i] : 0.0f, Hc);
-              }
+            for (int i = 0; i < 16; ++i) {
+              const bool act = i < nv;
+              seg_step(a, c, act ? ivv[i] : c, act ? sp[i] : 0.0f, Hc);
             }
           }
-          if (last) Hc[c * kFcOut] = a;            // the event's last non-empty interval
-          if (mm) { acc1 = a; cur1 = c; } else { acc0 = a; cur0 = c; }
-          tc_fence_before_sync();
-          mbar_arrive(bar(bAccEmpty + mt));
         }
-        mbar_arrive(bar(bMeta + buf));
+        if (last) Hc[c * kFcOut] = a;             // the event's last non-empty interval
+        tc_fence_before_sync();
+        mbar_arrive(bar(bAccEmpty + mt));
+        mbar_arrive(bar(bMeta + (it & (kIvBufs - 1))));
       }
     }
     FC_PROF_ADD(2, pw);
-  } else if (warp == 8) {
+  } else if (warp == kMmaWarp) {
     // ===================== MMA issuer
     constexpr uint32_t idesc = instr_desc(kFmtTF32, 128, kTile);
     constexpr uint32_t hi = (128u >> 4) | (1u << 14);
@@ -282,7 +281,7 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
     FC_PROF_ADD(5, pw);
   } else {
     // ===================== hidden layers: two groups of 128 threads, thread = track, alternating tiles
-    const int g = (warp - 9) >> 2, i = tid - 288 - 128 * g;
+    const int g = (warp - kHidWarp0) >> 2, i = tid - 32 * kHidWarp0 - 128 * g;
     const uint32_t hbase = sb + OFF_H + (uint32_t)g * 2 * kHPart + (uint32_t)i * 16u;
     int it = 0;
     const bool pw = g == 0 && i == 0;
@@ -294,12 +293,13 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
         if ((it & 1) != g) continue;
         const uint32_t prev = (uint32_t)(((it >> 1) & 1) ^ 1);
         { FC_PROF_T0(); mbar_wait(bar(bHEmpty + g), prev); FC_PROF_ADD(6, pw); }   // the MMAs that read this buffer have retired
-        { FC_PROF_T0(); mbar_wait(bar(bMeta + g), prev); FC_PROF_ADD(7, pw); }     // the epilogue is done with s_iv[g]
+        const int ib = it & (kIvBufs - 1);
+        { FC_PROF_T0(); mbar_wait(bar(bMeta + ib), (uint32_t)(((it >> 2) & 1) ^ 1)); FC_PROF_ADD(7, pw); }   // the epilogue is done with s_iv[ib]
         if (base + i < nk) {
           int t;
           float zrel;
           const int iv = entry_interval(perm[ev_lo + base + i], F.f[0], t, zrel);   // own or neighbouring interval
-          s_iv[g * kTile + i] = iv;
+          s_iv[ib * kTile + i] = iv;
           const float x[kFcIn] = {zrel, F.f[1][t], F.f[2][t], F.f[3][t], F.f[4][t], F.f[5][t], F.f[6][t], F.f[7][t], F.f[8][t]};
           float h[32], gg[28];
 #pragma unroll
@@ -350,7 +350,7 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
   }
   tc_fence_before_sync();
   __syncthreads();
-  if (warp == 8) {
+  if (warp == kMmaWarp) {
     __syncwarp();
     tmem_dealloc(tmem_base, 512);
   }
@@ -371,22 +371,21 @@ float tf32_rna_h(float v) {
 size_t fc_tc_packed_bytes() { return (size_t)2 * 2 * kWPart; }      // 2 halves x (hi | lo)
 
 // W5 [800][25] and b5 [800] (PyTorch layouts) -> per half [hi | lo][8 K chunks][512 rows][4 floats];
-// row 128*mt + r holds output (4*half + mt)*100 + r for r < 100 (zero rows otherwise); K index 25 = bias.
+// row 128*mt + r holds output 400*half + 128*mt + r while 128*mt + r < 400 (zero rows otherwise); K index 25 = bias.
 void fc_tc_pack(const float* w5, const float* b5, void* host_dst) {
   float* dst = static_cast<float*>(host_dst);
   memset(dst, 0, fc_tc_packed_bytes());
   for (int half = 0; half < 2; ++half)
-    for (int mt = 0; mt < 4; ++mt)
-      for (int r = 0; r < kBins; ++r) {
-        const int o = (4 * half + mt) * kBins + r, row = 128 * mt + r;
-        for (int k = 0; k <= kFcHidden; ++k) {
-          const float v = k < kFcHidden ? w5[o * kFcHidden + k] : b5[o];
-          const float hi = tf32_rna_h(v), lo = tf32_rna_h(v - hi);
-          const size_t idx = ((size_t)(k / 4) * kRowsW + row) * 4 + (k % 4);
-          dst[(size_t)half * 2 * (kWPart / 4) + idx] = hi;
-          dst[(size_t)half * 2 * (kWPart / 4) + kWPart / 4 + idx] = lo;
-        }
+    for (int row = 0; row < kHalfOut; ++row) {
+      const int o = kHalfOut * half + row;
+      for (int k = 0; k <= kFcHidden; ++k) {
+        const float v = k < kFcHidden ? w5[o * kFcHidden + k] : b5[o];
+        const float hi = tf32_rna_h(v), lo = tf32_rna_h(v - hi);
+        const size_t idx = ((size_t)(k / 4) * kRowsW + row) * 4 + (k % 4);
+        dst[(size_t)half * 2 * (kWPart / 4) + idx] = hi;
+        dst[(size_t)half * 2 * (kWPart / 4) + kWPart / 4 + idx] = lo;
       }
+    }
 }
 
 cudaError_t fc_tc_setup() {
