@@ -142,7 +142,11 @@ PVF_API pvf_status pvf_run(pvf_handle h, const pvf_tracks* tracks, int32_t n_eve
 /* Same computation with HOST buffers: H2D of the nine feature arrays + offsets, pvf_run, D2H of
  * probabilities (skipped if host_probs == NULL) and peaks, then one stream synchronise.  Needs
  * enable_host_io.  feat/event_offsets/peaks fields are host pointers here (pinned memory makes the
- * copies asynchronous but is not required). */
+ * copies asynchronous but is not required; event_offsets[0] must be 0 and event_offsets[n_events] ==
+ * n_tracks).  Batches of >= 4096 events run as a pipeline of 8 chunks: the copies use two streams the
+ * library created at pvf_create (ordered after / before cuda_stream by events), so that H2D of chunk
+ * k+1 and D2H of chunk k-1 overlap the kernels of chunk k; results are identical to pvf_run.  After such
+ * a call pvf_debug_copy_histogram sees the last chunk only; stage timing is not recorded. */
 PVF_API pvf_status pvf_run_host(pvf_handle h, const pvf_tracks* host_tracks, int32_t n_events,
                         float* host_probs, const pvf_peaks* host_peaks, void* cuda_stream);
 

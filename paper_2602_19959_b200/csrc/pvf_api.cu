@@ -43,6 +43,11 @@ struct pvf_ctx {
   int32_t* st_bin = nullptr;
   int32_t* st_count = nullptr;
   uint32_t* st_flags = nullptr;
+  // pvf_run_host only: copy streams and events of the chunk pipeline (H2D of chunk k+1 | compute k | D2H k-1)
+  static constexpr int kHostChunks = 8;
+  cudaStream_t s_in = nullptr, s_out = nullptr;
+  cudaEvent_t ev_in[kHostChunks] = {}, ev_comp[kHostChunks] = {}, ev_fork = nullptr, ev_join = nullptr;
+  bool suppress_timing = false;
   static constexpr int kTimedRuns = 64;   // ring of per-run event sets (stage timing)
   cudaEvent_t ev[kTimedRuns][5] = {};
   int64_t timed_runs = 0;                 // runs recorded since the last pvf_stage_times_ms
@@ -242,6 +247,16 @@ pvf_status create_impl(const pvf_weights* w, const pvf_config* cfg, void* dev_po
     }
     if (cs) cudaStreamDestroy(cs);
   }
+  if (e == cudaSuccess && cfg->enable_host_io) {
+    e = cudaStreamCreateWithFlags(&h->s_in, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&h->s_out, cudaStreamNonBlocking);
+    for (int k = 0; k < pvf_ctx::kHostChunks && e == cudaSuccess; ++k) {
+      e = cudaEventCreateWithFlags(&h->ev_in[k], cudaEventDisableTiming);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_comp[k], cudaEventDisableTiming);
+    }
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming);
+  }
   if (e == cudaSuccess && cfg->enable_stage_timing)
     for (int r = 0; r < pvf_ctx::kTimedRuns; ++r)
       for (int k = 0; k < 5 && e == cudaSuccess; ++k) e = cudaEventCreate(&h->ev[r][k]);
@@ -304,7 +319,7 @@ pvf_status pvf_run(pvf_handle h, const pvf_tracks* t, int32_t n_events, float* o
     if (!t->feat[k] && t->n_tracks > 0) return PVF_ERR_ARG;
   if (n_events > h->cfg.max_events || t->n_tracks > h->cfg.max_tracks) return PVF_ERR_CAPACITY;
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-  const bool timing = h->cfg.enable_stage_timing != 0;
+  const bool timing = h->cfg.enable_stage_timing != 0 && !h->suppress_timing;
   cudaEvent_t* ev = h->ev[h->timed_runs % pvf_ctx::kTimedRuns];
   if (timing) cudaEventRecord(ev[0], s);
   launch_sort(t->feat[0], t->event_offsets, n_events, h->perm, h->seg_off, h->seg_cnt, h->flags,
@@ -343,26 +358,68 @@ pvf_status pvf_run_host(pvf_handle h, const pvf_tracks* t, int32_t n_events, flo
   if (n_events > h->cfg.max_events || t->n_tracks > h->cfg.max_tracks) return PVF_ERR_CAPACITY;
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   const size_t T = (size_t)t->n_tracks, cap = (size_t)h->cfg.max_tracks, E = (size_t)n_events;
+  for (int k = 0; k < 9; ++k)
+    if (!t->feat[k] && T > 0) return PVF_ERR_ARG;
+  // Large batches run as a pipeline of chunks: the H2D copy of chunk k+1 (stream s_in) and the D2H copy of chunk k-1
+  // (stream s_out) overlap the kernels of chunk k on the caller's stream.  Track indices stay absolute (the kernels
+  // index everything through event_offsets), so a chunk is just a window [e0, e1) of the same arrays.
+  const int n_chunks = n_events >= 4096 ? pvf_ctx::kHostChunks : 1;
+  const int32_t* off = t->event_offsets;                     // host pointer here
+  if (n_chunks > 1 && (off[0] != 0 || (size_t)off[E] != T)) return PVF_ERR_ARG;
   pvf_tracks d{};
-  for (int k = 0; k < 9; ++k) {
-    if (T) PVF_CUDA(h, cudaMemcpyAsync(h->st_feat + cap * k, t->feat[k], sizeof(float) * T, cudaMemcpyHostToDevice, s));
-    d.feat[k] = h->st_feat + cap * k;
-  }
-  PVF_CUDA(h, cudaMemcpyAsync(h->st_off, t->event_offsets, sizeof(int32_t) * (E + 1), cudaMemcpyHostToDevice, s));
-  d.event_offsets = h->st_off;
+  for (int k = 0; k < 9; ++k) d.feat[k] = h->st_feat + cap * k;
   d.n_tracks = t->n_tracks;
-  pvf_peaks dp{h->st_z, h->st_prob, h->st_bin, h->st_count, h->st_flags};
-  pvf_status st = pvf_run(h, &d, n_events, h->st_probs, &dp, cuda_stream);
-  if (st != PVF_OK) return st;
-  if (host_probs) PVF_CUDA(h, cudaMemcpyAsync(host_probs, h->st_probs, sizeof(float) * E * kGlobalBins, cudaMemcpyDeviceToHost, s));
-  PVF_CUDA(h, cudaMemcpyAsync(pk->z_mm, h->st_z, sizeof(float) * E * kMaxPeaks, cudaMemcpyDeviceToHost, s));
-  PVF_CUDA(h, cudaMemcpyAsync(pk->prob, h->st_prob, sizeof(float) * E * kMaxPeaks, cudaMemcpyDeviceToHost, s));
-  PVF_CUDA(h, cudaMemcpyAsync(pk->bin, h->st_bin, sizeof(int32_t) * E * kMaxPeaks, cudaMemcpyDeviceToHost, s));
-  PVF_CUDA(h, cudaMemcpyAsync(pk->count, h->st_count, sizeof(int32_t) * E, cudaMemcpyDeviceToHost, s));
-  if (pk->event_flags)
-    PVF_CUDA(h, cudaMemcpyAsync(pk->event_flags, h->st_flags, sizeof(uint32_t) * E, cudaMemcpyDeviceToHost, s));
+  if (n_chunks > 1) {
+    PVF_CUDA(h, cudaEventRecord(h->ev_fork, s));             // the copy streams start after what is already queued on s
+    PVF_CUDA(h, cudaStreamWaitEvent(h->s_in, h->ev_fork, 0));
+    PVF_CUDA(h, cudaStreamWaitEvent(h->s_out, h->ev_fork, 0));
+  }
+  h->suppress_timing = n_chunks > 1;                         // stage timing describes whole-batch pvf_run calls only
+  pvf_status st = PVF_OK;
+  for (int c = 0; c < n_chunks && st == PVF_OK; ++c) {
+    const size_t e0 = E * c / n_chunks, e1 = E * (c + 1) / n_chunks, ne = e1 - e0;
+    const size_t t0 = n_chunks > 1 ? (size_t)off[e0] : 0, t1 = n_chunks > 1 ? (size_t)off[e1] : T;
+    cudaStream_t si = n_chunks > 1 ? h->s_in : s, so = n_chunks > 1 ? h->s_out : s;
+    for (int k = 0; k < 9; ++k)
+      if (t1 > t0)
+        PVF_CUDA(h, cudaMemcpyAsync(h->st_feat + cap * k + t0, t->feat[k] + t0, sizeof(float) * (t1 - t0), cudaMemcpyHostToDevice, si));
+    {   // offsets (e0, e1] -- plus offsets[e0] for the first chunk -- so that no element is copied twice
+      const size_t lo = c == 0 ? e0 : e0 + 1;
+      PVF_CUDA(h, cudaMemcpyAsync(h->st_off + lo, off + lo, sizeof(int32_t) * (e1 + 1 - lo), cudaMemcpyHostToDevice, si));
+    }
+    if (n_chunks > 1) {
+      PVF_CUDA(h, cudaEventRecord(h->ev_in[c], si));
+      PVF_CUDA(h, cudaStreamWaitEvent(s, h->ev_in[c], 0));
+    }
+    d.event_offsets = h->st_off + e0;
+    pvf_peaks dp{h->st_z + e0 * kMaxPeaks, h->st_prob + e0 * kMaxPeaks, h->st_bin + e0 * kMaxPeaks, h->st_count + e0,
+                 h->st_flags + e0};
+    st = pvf_run(h, &d, (int32_t)ne, h->st_probs + e0 * kGlobalBins, &dp, cuda_stream);
+    if (st != PVF_OK) break;
+    if (n_chunks > 1) {
+      PVF_CUDA(h, cudaEventRecord(h->ev_comp[c], s));
+      PVF_CUDA(h, cudaStreamWaitEvent(so, h->ev_comp[c], 0));
+    }
+    if (host_probs)
+      PVF_CUDA(h, cudaMemcpyAsync(host_probs + e0 * kGlobalBins, h->st_probs + e0 * kGlobalBins, sizeof(float) * ne * kGlobalBins,
+                                  cudaMemcpyDeviceToHost, so));
+    PVF_CUDA(h, cudaMemcpyAsync(pk->z_mm + e0 * kMaxPeaks, dp.z_mm, sizeof(float) * ne * kMaxPeaks, cudaMemcpyDeviceToHost, so));
+    PVF_CUDA(h, cudaMemcpyAsync(pk->prob + e0 * kMaxPeaks, dp.prob, sizeof(float) * ne * kMaxPeaks, cudaMemcpyDeviceToHost, so));
+    PVF_CUDA(h, cudaMemcpyAsync(pk->bin + e0 * kMaxPeaks, dp.bin, sizeof(int32_t) * ne * kMaxPeaks, cudaMemcpyDeviceToHost, so));
+    PVF_CUDA(h, cudaMemcpyAsync(pk->count + e0, dp.count, sizeof(int32_t) * ne, cudaMemcpyDeviceToHost, so));
+    if (pk->event_flags)
+      PVF_CUDA(h, cudaMemcpyAsync(pk->event_flags + e0, dp.event_flags, sizeof(uint32_t) * ne, cudaMemcpyDeviceToHost, so));
+  }
+  h->suppress_timing = false;
+  if (n_chunks > 1) {                                        // join: the caller's stream is ordered after both copy streams
+    PVF_CUDA(h, cudaEventRecord(h->ev_join, h->s_out));
+    PVF_CUDA(h, cudaStreamWaitEvent(s, h->ev_join, 0));
+    PVF_CUDA(h, cudaEventRecord(h->ev_join, h->s_in));
+    PVF_CUDA(h, cudaStreamWaitEvent(s, h->ev_join, 0));
+  }
   PVF_CUDA(h, cudaStreamSynchronize(s));
-  return PVF_OK;
+  if (st == PVF_OK) h->last_n_events = n_chunks > 1 ? (int32_t)(E - E * (n_chunks - 1) / n_chunks) : n_events;
+  return st;
 }
 
 pvf_status pvf_find_peaks(pvf_handle h, const float* probs, int32_t n_events, const pvf_peaks* pk, void* cuda_stream) {
@@ -430,6 +487,14 @@ pvf_status pvf_destroy(pvf_handle h) {
   for (int r = 0; r < pvf_ctx::kTimedRuns; ++r)
     for (int k = 0; k < 5; ++k)
       if (h->ev[r][k]) cudaEventDestroy(h->ev[r][k]);
+  for (int k = 0; k < pvf_ctx::kHostChunks; ++k) {
+    if (h->ev_in[k]) cudaEventDestroy(h->ev_in[k]);
+    if (h->ev_comp[k]) cudaEventDestroy(h->ev_comp[k]);
+  }
+  if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+  if (h->ev_join) cudaEventDestroy(h->ev_join);
+  if (h->s_in) cudaStreamDestroy(h->s_in);
+  if (h->s_out) cudaStreamDestroy(h->s_out);
   if (h->owns_pool && h->pool) cudaFree(h->pool);
   delete h;
   return PVF_OK;

@@ -416,6 +416,34 @@ def test_host_io_and_stage_timing():
     assert torch.equal(hpk["z"], pk["z"].cpu())
 
 
+@pytest.mark.parametrize("prec,margin", [("tf32", 0.0), ("fp16", 0.5), ("fp32", 0.0)])
+def test_host_io_chunk_pipeline_matches_device_run(prec, margin):
+    """pvf_run_host on >= 4096 events runs as 8 chunks with the copies on the library's own streams: the host
+    results must equal the device-resident pvf_run of the same batch bit for bit (4101 events: ragged chunks;
+    one event without tracks; with the two-entry sort of NEXT-1 as well)."""
+    base = make_events("run3", 4100, 79)
+    cut = int(base.event_offsets[2050])
+    offs = np.concatenate([base.event_offsets[:2051], base.event_offsets[2050:]]).astype(np.int32)
+    ev = type(base)(base.feat, offs, [None] * 4101)
+    w = make_weights("peaky", 1)
+    E = ev.n_events
+    pvf = _make(w, ev, prec, host_io=True, stage_timing=True, boundary_margin_mm=margin)
+    probs, pk = _run(pvf, ev)
+    pvf.stage_times_ms()
+    hfeat = torch.from_numpy(ev.feat).pin_memory()
+    hoff = torch.from_numpy(ev.event_offsets).pin_memory()
+    hprobs = torch.full((E, 4000), -1.0).pin_memory()
+    hpk = pvf.alloc_peaks(E, pinned=True)
+    s = torch.cuda.Stream()
+    for _ in range(2):                                            # twice: the staging buffers are reused
+        pvf.run_host(hfeat, hoff, E, hprobs, hpk, stream=s)
+        assert torch.equal(hprobs, probs.cpu())
+        for k in pk:
+            assert torch.equal(hpk[k], pk[k].cpu()), k
+    with pytest.raises(pkg.PVFError):
+        pvf.stage_times_ms()                                      # chunked host runs record no stage times
+
+
 # ------------------------------------------------------------------ full size, bench launch configuration
 @pytest.mark.parametrize("prec,model", [("tf32", "run3"), ("bf16", "run3"), ("fp32", "run3"), ("tf32", "pileup"),
                                         ("fp16", "pileup")])
