@@ -113,7 +113,7 @@ struct Geo {
 
 // Steps and byte offsets of the weight-image segments (host packer, producer and issuer agree on it).
 struct Plan {
-  int e1_steps;            // 13 tap pairs, x3 with the e1 hi/lo split
+  int e1_steps;            // 13 tap pairs, x2 with the e1 hi/lo split (TF32 mode)
   int seg_steps[kSegs];
   int seg_off[kSegs];      // bytes from the start of the image
   int total;
@@ -124,7 +124,7 @@ template <int C, int BF16, int CG>
 __host__ __device__ inline Plan make_plan(int split_e1) {
   using G = Geo<C, BF16, CG>;
   Plan P{};
-  P.e1_steps = 13 * ((!BF16 && split_e1) ? 3 : 1);
+  P.e1_steps = 13 * ((!BF16 && split_e1) ? 2 : 1);
   P.seg_steps[gE2] = 8 * G::NKB1;
   P.seg_steps[gD1Ea] = G::D1E_A;
   P.seg_steps[gB] = 3 * G::NKB1;
@@ -356,6 +356,29 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
       st_smem16(x0 + row, qv);
       st_smem16(x0 + G::LBO1 + row, zero4);       // channels 8..15 of the K = 16 MMA: zero
     }
+  } else if (split) {
+    // TF32 mode with the e1 split: the histogram enters as TWO BF16 pieces per value, x = a1 + a2 (+ 2^-17 |x|),
+    // side by side in the K = 16 of one kind::f16 MMA: chunk 0 = a1 of the 8 channels, chunk 1 = a2.  With the
+    // weights as [w1 | w1] (pass 0) and [w2 | 0] (pass 1) two MMAs per tap pair give a1 w1 + a2 w1 + a1 w2, i.e.
+    // ~2^-16 relative per product (plain TF32: 2^-12) for 2/3 of the MMAs a three-pass TF32 split needs.
+    for (int it = tid; it < G::T * 128; it += 128) {
+      const int t = it >> 7, l = it & 127;
+      bool live = l < 100 && t < n_valid_int;
+      const long long src = !live ? 0 : (list ? (long long)list[g0 + t] : g0 + t);
+      if (live && seg_cnt != nullptr) live = __ldg(seg_cnt + src) > 0;
+      float x[8], r[8];
+#pragma unroll
+      for (int c = 0; c < 8; ++c) {
+        x[c] = live ? __ldg(hist + src * kFcOut + c * kBins + l) : 0.0f;
+        r[c] = x[c] - __bfloat162float(__float2bfloat16_rn(x[c]));
+      }
+      uint4 q1, q2;
+      q1.x = pack16<1>(x[0], x[1]); q1.y = pack16<1>(x[2], x[3]); q1.z = pack16<1>(x[4], x[5]); q1.w = pack16<1>(x[6], x[7]);
+      q2.x = pack16<1>(r[0], r[1]); q2.y = pack16<1>(r[2], r[3]); q2.z = pack16<1>(r[4], r[5]); q2.w = pack16<1>(r[6], r[7]);
+      const uint32_t row = (uint32_t)(G::LEAD1 + it) * 16u;
+      st_smem16(x0 + row, q1);
+      st_smem16(x0 + G::LBO1 + row, q2);
+    }
   } else {
     for (int it = tid; it < G::T * 256; it += 128) {
       const int t = it >> 8, qc = (it >> 7) & 1, l = it & 127;
@@ -369,12 +392,6 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
       hi.x = to_tf32(x[0]); hi.y = to_tf32(x[1]); hi.z = to_tf32(x[2]); hi.w = to_tf32(x[3]);
       const uint32_t row = (uint32_t)(G::LEAD1 + 128 * t + l) * 16u;
       st_smem16(x0 + (uint32_t)qc * G::LBO1 + row, hi);
-      if (split) {
-        uint4 lo;
-        lo.x = to_tf32(x[0] - __uint_as_float(hi.x)); lo.y = to_tf32(x[1] - __uint_as_float(hi.y));
-        lo.z = to_tf32(x[2] - __uint_as_float(hi.z)); lo.w = to_tf32(x[3] - __uint_as_float(hi.w));
-        st_smem16(x0 + (uint32_t)(2 + qc) * G::LBO1 + row, lo);
-      }
     }
   }
 }
@@ -434,13 +451,15 @@ __device__ unsigned long long g_unet_prof[160][16];
 // f_begin must be a multiple of SPS.  acc0 = 0 starts fresh accumulators at step f_begin.
 template <int C, int BF16, int CG, int S>
 __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_t bar0, RingState& rs,
-                                        int f_begin, int f_end, uint32_t acc0) {
+                                        int f_begin, int f_end, uint32_t acc0, bool e1x = false) {
+  // e1x (sub-layer e1 of the TF32 kernel only): the split e1 runs as kind::f16 MMAs on BF16 pieces (see load_x0)
   using G = Geo<C, BF16, CG>;
   using Y = Lay<C, BF16, S>;
   constexpr int SPS = G::SPS;
   static_assert(Y::HALF % SPS == 0 || SPS % Y::NKB == 0,
                 "a ring stage is either part of one source's K blocks or whole taps");
   constexpr uint32_t idesc = instr_desc(BF16 == 2 ? kFmtF16 : (BF16 ? kFmtBF16 : kFmtTF32), 128 * CG, G::NOUT);
+  constexpr uint32_t idesc_x = instr_desc(kFmtBF16, 128 * CG, G::NOUT);
   constexpr uint32_t hi = (128u >> 4) | (1u << 14);                    // SBO = 128 B, descriptor version 1
   constexpr uint32_t a_lbo = (uint32_t)(Y::LBO >> 4) << 16;
   constexpr uint32_t b_lbo = (uint32_t)((G::NB * 16) >> 4) << 16;
@@ -461,7 +480,7 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
     const uint32_t b0 = b_lbo + ((sb + G::OFF_RING + rs.ring * G::STAGE_BYTES) >> 4);
     uint32_t a0 = a_lbo + (sb >> 4);          // stage origin: descriptor low word of tile 0, step f
     if (S == sE1) {
-      // e1: one K block per step; steps run [pass][tap pair], pass 1 reads the low-part chunks (split)
+      // e1: one K block per step; steps run [pass][tap pair]; both passes of the split read the same operand
     } else if (Y::HALF >= SPS) {
       const int j0 = f / Y::NKB, kk0 = f % Y::NKB;
       const int off = kk0 < Y::HALF ? Y::SRC0 + 2 * kk0 * Y::LBO : Y::SRC1 + 2 * (kk0 - Y::HALF) * Y::LBO;
@@ -476,7 +495,7 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
           uint32_t a;
           if (S == sE1) {
             const int step = f + i, pass = step / 13, u = step - 13 * pass;
-            a = a0 + (uint32_t)((Y::SRC0 + (pass == 1 ? 2 * G::LBO1 : 0)) >> 4) + (uint32_t)(Y::LEAD + 2 * u - Y::PAD);
+            a = a0 + (uint32_t)(Y::SRC0 >> 4) + (uint32_t)(Y::LEAD + 2 * u - Y::PAD);
           } else if (Y::HALF >= SPS) {
             a = a0 + (uint32_t)(i * ((2 * Y::LBO) >> 4));
           } else {
@@ -485,8 +504,10 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
           const uint32_t b = b0 + (uint32_t)(i * (G::STEP_BYTES >> 4));
           const uint32_t acc = (i > 0) ? 1u : (f > f_begin ? 1u : acc0);
 #pragma unroll
-          for (int t = 0; t < Y::NT; ++t)
-            mma_lh<BF16, CG>(dcol + (uint32_t)(t * G::NOUT), a + 128u * t, hi, b, hi, idesc, acc);
+          for (int t = 0; t < Y::NT; ++t) {
+            if (S == sE1 && BF16 == 0 && e1x) mma_lh<1, CG>(dcol + (uint32_t)(t * G::NOUT), a + 128u * t, hi, b, hi, idesc_x, acc);
+            else mma_lh<BF16, CG>(dcol + (uint32_t)(t * G::NOUT), a + 128u * t, hi, b, hi, idesc, acc);
+          }
         }
       }
       // frees the ring slot (in both CTAs of a pair) when these MMAs retire
@@ -605,7 +626,7 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
       const bool has_next = pg + stride < n_pg;
       if (first) {
         wait_epi(0);
-        mma_seg<C, BF16, CG, sE1>(sb, tmem_base, bar0, rs, 0, P.e1_steps, 0u);
+        mma_seg<C, BF16, CG, sE1>(sb, tmem_base, bar0, rs, 0, P.e1_steps, 0u, split_e1 != 0);
         commit(0);
       }
       wait_epi(1);                                   // P1 staged, region B drained
@@ -624,7 +645,7 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
       wait_epi(4);                                   // U1 staged, region B drained
       if (has_next) {
         wait_epi(0);                                 // next group's X0 staged
-        mma_seg<C, BF16, CG, sE1>(sb, tmem_base, bar0, rs, 0, P.e1_steps, 0u);
+        mma_seg<C, BF16, CG, sE1>(sb, tmem_base, bar0, rs, 0, P.e1_steps, 0u, split_e1 != 0);
         commit(0);
       }
       mma_seg<C, BF16, CG, sD1U>(sb, tmem_base, bar0, rs, 0, 13 * G::NKB1, 1u);
@@ -786,6 +807,24 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst_all) {
       if (d.seg == gE1) { pass = f / 13; u = f % 13; kk = 0; }     // e1 split runs [pass][tap pair]
       else { u = f / d.nkb; kk = f % d.nkb; }
       unsigned char* step = dst + P.seg_off[d.seg] + (size_t)s * G::STEP_BYTES;
+      if (d.seg == gE1 && !BF16 && split_e1) {
+        // split e1 of the TF32 kernel: BF16 pieces w = w1 + w2; pass 0 holds [w1 | w1] (meets [a1 | a2]), pass 1 [w2 | 0]
+        for (int h = 0; h < 2; ++h)
+          for (int nl = 0; nl < G::NB; ++nl)
+            for (int e = 0; e < 8; ++e) {
+              const int n = rank * G::NB + nl;
+              const int co = n % C, j = 2 * u + n / C;
+              const float v = j < d.taps ? W[((size_t)co * d.cin + e) * d.taps + j] : 0.0f;
+              const uint16_t w1 = bf16_rne(v);
+              uint32_t w1bits = (uint32_t)w1 << 16;
+              float w1f;
+              memcpy(&w1f, &w1bits, 4);
+              const uint16_t w2 = bf16_rne(v - w1f);
+              const uint16_t out = pass == 0 ? w1 : (h == 0 ? w2 : (uint16_t)0);
+              memcpy(step + ((size_t)h * G::NB + nl) * 16 + e * 2, &out, 2);
+            }
+        continue;
+      }
       for (int h = 0; h < 2; ++h)
         for (int nl = 0; nl < G::NB; ++nl)        // rows [0, C): even tap 2u, rows [C, 2C): odd tap 2u + 1
           for (int e = 0; e < G::PER; ++e) {
@@ -800,7 +839,7 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst_all) {
               memcpy(p, &b, 2);
             } else {
               const float hi = tf32_rna(v);
-              const float out = (pass == 2) ? tf32_rna(v - hi) : hi;   // passes: A_hi W_hi, A_lo W_hi, A_hi W_lo
+              const float out = hi;
               memcpy(p, &out, 4);
             }
           }
