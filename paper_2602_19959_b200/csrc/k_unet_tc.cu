@@ -30,6 +30,7 @@
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 #include <cstring>
+#include <type_traits>
 #include <vector>
 
 #include "pvf_internal.cuh"
@@ -40,7 +41,9 @@ using namespace umma;
 
 namespace {
 
-constexpr int kTcThreads = 192;
+constexpr int kEpiSets = 2;                 // two sets of four epilogue warps (a warp reaches TMEM lanes 32 * (warp % 4) ..)
+constexpr int kEpiThreads = 128 * kEpiSets;
+constexpr int kTcThreads = 64 + kEpiThreads;
 constexpr int kMaxStages = 8;
 constexpr int kStageBytes = 16384;
 constexpr int kHeaderBytes = 2048;          // biases [5][C], head weight [C], head bias
@@ -83,7 +86,7 @@ struct Geo {
   static constexpr int OFF_XP = OFF_R + SZ_L1;       // overlay: X0 (input) then P1 = pool(e1)
   static constexpr int SZ_XP = (XCH * LBO1 > SZ_L2) ? XCH * LBO1 : SZ_L2;
   static constexpr int OFF_RING = OFF_XP + SZ_XP;
-  static constexpr int SCR_BYTES = 2 * 4 * C * 4;    // epilogue row-exchange scratch: [2 buffers][4 warps][C floats]
+  static constexpr int SCR_BYTES = kEpiSets * 2 * 4 * C * 4;   // epilogue row-exchange scratch: [set][2 buffers][4 warps][C floats]
   static constexpr int STAGES_FIT = (227 * 1024 - kHeaderBytes - kBarBytes - SCR_BYTES - OFF_RING) / STAGE_BYTES;
   static constexpr int MAX_STAGES = CG == 2 ? 12 : kMaxStages;   // measured: depth >= 6 changes nothing (bf16 and tf32)
   static constexpr int STAGES = STAGES_FIT < MAX_STAGES ? STAGES_FIT : MAX_STAGES;   // weight ring depth
@@ -222,12 +225,14 @@ __device__ __forceinline__ void zero_rows(uint32_t buf, uint32_t lbo, int nch, i
 
 enum { kE1 = 0, kE2 = 1, kB = 2, kD2 = 3, kD1 = 4 };
 
-// Epilogue of one 128-row accumulator tile, executed by the four epilogue warps (thread = row m).
+// Epilogue of channels [cb, ce) of one 128-row accumulator tile, executed by the four warps of one epilogue set
+// (thread = row m; named barrier 1 + set among them).  A layer with two or more tiles gives whole tiles to the sets
+// alternately; a single-tile layer is split by channel halves (never d1, whose head sums over all channels).
 template <int C, int BF16, int MODE>
 __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_base, int tile, int q, int lane,
                                               const float* __restrict__ par, int n_valid_int,
                                               float* __restrict__ probs_group, float* __restrict__ scr,
-                                              const int* __restrict__ list_g) {
+                                              const int* __restrict__ list_g, int cb, int ce, int set) {
   using G = Geo<C, BF16>;
   const int m = 32 * q + lane;
   const float* bias = par + MODE * C;
@@ -237,7 +242,7 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
   // Row m + 1 of lane 31 lives in the next warp's TMEM quadrant: lane 0 of every warp publishes its E1 row
   // in shared memory (scr: [4 warps][C], double buffered by the caller), one named barrier per tile.
 #pragma unroll 1
-  for (int c0 = 0; c0 < C; c0 += 16) {
+  for (int c0 = cb; c0 < ce; c0 += 16) {
     uint32_t r[16];
     tmem_ld_x16(taddr + (uint32_t)(C + c0), r);
     tmem_ld_wait();
@@ -247,7 +252,7 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
         *reinterpret_cast<uint4*>(scr + q * C + c0 + 4 * k) = make_uint4(r[4 * k], r[4 * k + 1], r[4 * k + 2], r[4 * k + 3]);
     }
   }
-  asm volatile("bar.sync 1, 128;" ::: "memory");
+  asm volatile("bar.sync %0, 128;" ::"r"(1 + set) : "memory");
   const float* nxt = scr + (q < 3 ? q + 1 : 3) * C;   // E1 row of the next quadrant's first lane (q = 3: unused)
   // which interval of the group this row belongs to, its position, and whether it is a real output
   int interval, l;
@@ -275,7 +280,7 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
   }
   float logit = 0.0f;
 #pragma unroll 1
-  for (int c0 = 0; c0 < C; c0 += 16) {
+  for (int c0 = cb; c0 < ce; c0 += 16) {
     uint32_t r[16], r1[16];
     tmem_ld_x16(taddr + (uint32_t)c0, r);
     tmem_ld_x16(taddr + (uint32_t)(C + c0), r1);
@@ -326,7 +331,7 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
   }
 }
 
-// Interval histograms of one group -> X0 (operand-rounded, chunked layout).  128 threads.  X0 shares
+// Interval histograms of one group -> X0 (operand-rounded, chunked layout).  All kEpiThreads epilogue threads.  X0 shares
 // its memory with P1, so every row the e1 MMAs can read for a valid output is (re)written: the lead
 // rows and the gap rows l >= 100 of every interval as zeros.
 template <int C, int BF16>
@@ -341,7 +346,7 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
   if (tid < G::LEAD1)
     for (int c = 0; c < G::XCH; ++c) st_smem16(x0 + (uint32_t)c * G::LBO1 + (uint32_t)tid * 16u, zero4);
   if (BF16) {
-    for (int it = tid; it < G::T * 128; it += 128) {
+    for (int it = tid; it < G::T * 128; it += kEpiThreads) {
       const int t = it >> 7, l = it & 127;
       bool live = l < 100 && t < n_valid_int;
       const long long src = !live ? 0 : (list ? (long long)list[g0 + t] : g0 + t);
@@ -361,7 +366,7 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
     // side by side in the K = 16 of one kind::f16 MMA: chunk 0 = a1 of the 8 channels, chunk 1 = a2.  With the
     // weights as [w1 | w1] (pass 0) and [w2 | 0] (pass 1) two MMAs per tap pair give a1 w1 + a2 w1 + a1 w2, i.e.
     // ~2^-16 relative per product (plain TF32: 2^-12) for 2/3 of the MMAs a three-pass TF32 split needs.
-    for (int it = tid; it < G::T * 128; it += 128) {
+    for (int it = tid; it < G::T * 128; it += kEpiThreads) {
       const int t = it >> 7, l = it & 127;
       bool live = l < 100 && t < n_valid_int;
       const long long src = !live ? 0 : (list ? (long long)list[g0 + t] : g0 + t);
@@ -380,7 +385,7 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
       st_smem16(x0 + G::LBO1 + row, q2);
     }
   } else {
-    for (int it = tid; it < G::T * 256; it += 128) {
+    for (int it = tid; it < G::T * 256; it += kEpiThreads) {
       const int t = it >> 8, qc = (it >> 7) & 1, l = it & 127;
       bool live = l < 100 && t < n_valid_int;
       const long long src = !live ? 0 : (list ? (long long)list[g0 + t] : g0 + t);
@@ -557,7 +562,7 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
       mbar_init(bar0 + 8u * (2 * G::STAGES + s), 1);
     }
     for (int k = 0; k < 5; ++k) mbar_init(accum_bar(k), 1);
-    for (int k = 0; k < 6; ++k) { mbar_init(epi_bar(k), 128); mbar_init(pepi_bar(k), 128); }
+    for (int k = 0; k < 6; ++k) { mbar_init(epi_bar(k), kEpiThreads); mbar_init(pepi_bar(k), kEpiThreads); }
     fence_mbar_init();
   }
   if (warp == 1) {
@@ -676,9 +681,9 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
       }
     }
   } else {
-    // ===================== epilogue warps (128 threads): thread = accumulator row
-    const int q = warp & 3, et = tid - 64;
-    float* scr0 = reinterpret_cast<float*>(smem + G::OFF_SCR);
+    // ===================== epilogue warps: two sets of 128 threads, thread = accumulator row
+    const int q = warp & 3, et = tid - 64, set = (warp - 2) >> 2;
+    float* scr0 = reinterpret_cast<float*>(smem + G::OFF_SCR) + set * 2 * 4 * C;
     int ecount = 0;                          // accumulator tiles drained so far (selects the scratch buffer)
     auto scr = [&]() { return scr0 + (ecount++ & 1) * 4 * C; };
     uint32_t pa[5] = {0, 0, 0, 0, 0};
@@ -700,34 +705,48 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
       float* pg_out = list ? probs : probs + g0 * kBins;
       const int* lg = list ? list + g0 : nullptr;
       const int* lgn = list ? list + gn0 : nullptr;
+      // the NT tiles of a layer: whole tiles alternate between the sets; a single tile is split by channel halves
+      // (C = 16: a half is less than one 16-channel chunk, set 0 takes it all)
+      auto layer = [&](auto mode, int nt, int nv, const int* lgx) {
+        constexpr int MODE = decltype(mode)::value;
+        if (nt >= 2) {
+          for (int t = set; t < nt; t += kEpiSets)
+            epilogue_tile<C, BF16, MODE>(sb, tmem_base, t, q, lane, par, nv, pg_out, scr(), lgx, 0, C, set);
+        } else if (C >= 32 && MODE != kD1) {
+          epilogue_tile<C, BF16, MODE>(sb, tmem_base, 0, q, lane, par, nv, pg_out, scr(), lgx, set * (C / 2), (set + 1) * (C / 2), set);
+        } else if (set == 0) {
+          epilogue_tile<C, BF16, MODE>(sb, tmem_base, 0, q, lane, par, nv, pg_out, scr(), lgx, 0, C, set);
+        }
+      };
+      using std::integral_constant;
       if (first) {
         load_x0<C, BF16>(sb, hist, g0, n_valid, split_e1, et, list, seg_cnt);
         done(0);
         wait_acc(0);
-        for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kE1>(sb, tmem_base, t, q, lane, par, n_valid, pg_out, scr(), lg);
+        layer(integral_constant<int, kE1>{}, G::T, n_valid, lg);
         done(1);
         first = false;
       }
       wait_acc(1);
-      for (int t = 0; t < G::T / 2; ++t) epilogue_tile<C, BF16, kE2>(sb, tmem_base, t, q, lane, par, n_valid, pg_out, scr(), lg);
+      layer(integral_constant<int, kE2>{}, G::T / 2, n_valid, lg);
       done(2);
       if (has_next) {                                // P1 is dead (e2's MMAs retired): stage the next input
         load_x0<C, BF16>(sb, hist, gn0, n_valid_next, split_e1, et, list, seg_cnt);
         done(0);
       }
       wait_acc(2);
-      for (int t = 0; t < (G::T + 3) / 4; ++t) epilogue_tile<C, BF16, kB>(sb, tmem_base, t, q, lane, par, n_valid, pg_out, scr(), lg);
+      layer(integral_constant<int, kB>{}, (G::T + 3) / 4, n_valid, lg);
       done(3);
       wait_acc(3);
-      for (int t = 0; t < G::T / 2; ++t) epilogue_tile<C, BF16, kD2>(sb, tmem_base, t, q, lane, par, n_valid, pg_out, scr(), lg);
+      layer(integral_constant<int, kD2>{}, G::T / 2, n_valid, lg);
       done(4);
       if (has_next) {
         wait_acc(0);
-        for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kE1>(sb, tmem_base, t, q, lane, par, n_valid_next, pg_out, scr(), lgn);
+        layer(integral_constant<int, kE1>{}, G::T, n_valid_next, lgn);
         done(1);
       }
       wait_acc(4);
-      for (int t = 0; t < G::T; ++t) epilogue_tile<C, BF16, kD1>(sb, tmem_base, t, q, lane, par, n_valid, pg_out, scr(), lg);
+      layer(integral_constant<int, kD1>{}, G::T, n_valid, lg);
       done(5);
     }
   }
