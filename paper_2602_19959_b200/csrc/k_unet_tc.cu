@@ -41,9 +41,9 @@ using namespace umma;
 
 namespace {
 
-constexpr int kEpiSets = 2;                 // two sets of four epilogue warps (a warp reaches TMEM lanes 32 * (warp % 4) ..)
-constexpr int kEpiThreads = 128 * kEpiSets;
-constexpr int kTcThreads = 64 + kEpiThreads;
+// Epilogue warps come in sets of four (a warp reaches TMEM lanes 32 * (warp % 4) ..): two sets at 64 channels
+// (MMA-bound), four at 32 / 16 channels (epilogue work ~ C, MMA work ~ C^2: those widths are epilogue-bound).
+constexpr int epi_sets(int C) { return C == 64 ? 2 : 4; }
 constexpr int kMaxStages = 8;
 constexpr int kStageBytes = 16384;
 constexpr int kHeaderBytes = 2048;          // biases [5][C], head weight [C], head bias
@@ -86,7 +86,9 @@ struct Geo {
   static constexpr int OFF_XP = OFF_R + SZ_L1;       // overlay: X0 (input) then P1 = pool(e1)
   static constexpr int SZ_XP = (XCH * LBO1 > SZ_L2) ? XCH * LBO1 : SZ_L2;
   static constexpr int OFF_RING = OFF_XP + SZ_XP;
-  static constexpr int SCR_BYTES = kEpiSets * 2 * 4 * C * 4;   // epilogue row-exchange scratch: [set][2 buffers][4 warps][C floats]
+  static constexpr int SETS = epi_sets(C);
+  static constexpr int EPI_THREADS = 128 * SETS, THREADS = 64 + EPI_THREADS;
+  static constexpr int SCR_BYTES = SETS * 2 * 4 * C * 4;   // epilogue row-exchange scratch: [set][2 buffers][4 warps][C floats]
   static constexpr int STAGES_FIT = (227 * 1024 - kHeaderBytes - kBarBytes - SCR_BYTES - OFF_RING) / STAGE_BYTES;
   static constexpr int MAX_STAGES = CG == 2 ? 12 : kMaxStages;   // measured: depth >= 6 changes nothing (bf16 and tf32)
   static constexpr int STAGES = STAGES_FIT < MAX_STAGES ? STAGES_FIT : MAX_STAGES;   // weight ring depth
@@ -226,8 +228,8 @@ __device__ __forceinline__ void zero_rows(uint32_t buf, uint32_t lbo, int nch, i
 enum { kE1 = 0, kE2 = 1, kB = 2, kD2 = 3, kD1 = 4 };
 
 // Epilogue of channels [cb, ce) of one 128-row accumulator tile, executed by the four warps of one epilogue set
-// (thread = row m; named barrier 1 + set among them).  A layer with two or more tiles gives whole tiles to the sets
-// alternately; a single-tile layer is split by channel halves (never d1, whose head sums over all channels).
+// (thread = row m; named barrier 1 + set among them).  The (tile, channel half) units of a layer go round-robin to
+// the sets (whole tiles for d1, whose head sums over all channels).
 template <int C, int BF16, int MODE>
 __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_base, int tile, int q, int lane,
                                               const float* __restrict__ par, int n_valid_int,
@@ -331,7 +333,7 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
   }
 }
 
-// Interval histograms of one group -> X0 (operand-rounded, chunked layout).  All kEpiThreads epilogue threads.  X0 shares
+// Interval histograms of one group -> X0 (operand-rounded, chunked layout).  All epilogue threads.  X0 shares
 // its memory with P1, so every row the e1 MMAs can read for a valid output is (re)written: the lead
 // rows and the gap rows l >= 100 of every interval as zeros.
 template <int C, int BF16>
@@ -346,7 +348,7 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
   if (tid < G::LEAD1)
     for (int c = 0; c < G::XCH; ++c) st_smem16(x0 + (uint32_t)c * G::LBO1 + (uint32_t)tid * 16u, zero4);
   if (BF16) {
-    for (int it = tid; it < G::T * 128; it += kEpiThreads) {
+    for (int it = tid; it < G::T * 128; it += G::EPI_THREADS) {
       const int t = it >> 7, l = it & 127;
       bool live = l < 100 && t < n_valid_int;
       const long long src = !live ? 0 : (list ? (long long)list[g0 + t] : g0 + t);
@@ -366,7 +368,7 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
     // side by side in the K = 16 of one kind::f16 MMA: chunk 0 = a1 of the 8 channels, chunk 1 = a2.  With the
     // weights as [w1 | w1] (pass 0) and [w2 | 0] (pass 1) two MMAs per tap pair give a1 w1 + a2 w1 + a1 w2, i.e.
     // ~2^-16 relative per product (plain TF32: 2^-12) for 2/3 of the MMAs a three-pass TF32 split needs.
-    for (int it = tid; it < G::T * 128; it += kEpiThreads) {
+    for (int it = tid; it < G::T * 128; it += G::EPI_THREADS) {
       const int t = it >> 7, l = it & 127;
       bool live = l < 100 && t < n_valid_int;
       const long long src = !live ? 0 : (list ? (long long)list[g0 + t] : g0 + t);
@@ -385,7 +387,7 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
       st_smem16(x0 + G::LBO1 + row, q2);
     }
   } else {
-    for (int it = tid; it < G::T * 256; it += kEpiThreads) {
+    for (int it = tid; it < G::T * 256; it += G::EPI_THREADS) {
       const int t = it >> 8, qc = (it >> 7) & 1, l = it & 127;
       bool live = l < 100 && t < n_valid_int;
       const long long src = !live ? 0 : (list ? (long long)list[g0 + t] : g0 + t);
@@ -525,7 +527,7 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
 }
 
 template <int C, int BF16, int CG>
-__global__ void __launch_bounds__(kTcThreads, 1)
+__global__ void __launch_bounds__((Geo<C, BF16, CG>::THREADS), 1)
 k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __restrict__ wpack, int split_e1,
           float* __restrict__ probs, const int* __restrict__ list, const int* __restrict__ n_list,
           const int* __restrict__ seg_cnt) {
@@ -553,8 +555,8 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
   const unsigned char* wimg = wpack + (size_t)rank * P.total;       // this CTA's weight image
 
   // ---- one-time setup: zero the activation buffers (gap / halo rows must be zero), parameters, barriers
-  for (int i = tid; i < G::OFF_RING / 16; i += kTcThreads) reinterpret_cast<uint4*>(smem)[i] = make_uint4(0, 0, 0, 0);
-  for (int i = tid; i < 6 * C + 1; i += kTcThreads) par[i] = reinterpret_cast<const float*>(wimg)[i];
+  for (int i = tid; i < G::OFF_RING / 16; i += G::THREADS) reinterpret_cast<uint4*>(smem)[i] = make_uint4(0, 0, 0, 0);
+  for (int i = tid; i < 6 * C + 1; i += G::THREADS) par[i] = reinterpret_cast<const float*>(wimg)[i];
   if (tid == 0) {
     for (int s = 0; s < G::STAGES; ++s) {
       mbar_init(bar0 + 8u * s, 1);
@@ -562,7 +564,7 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
       mbar_init(bar0 + 8u * (2 * G::STAGES + s), 1);
     }
     for (int k = 0; k < 5; ++k) mbar_init(accum_bar(k), 1);
-    for (int k = 0; k < 6; ++k) { mbar_init(epi_bar(k), kEpiThreads); mbar_init(pepi_bar(k), kEpiThreads); }
+    for (int k = 0; k < 6; ++k) { mbar_init(epi_bar(k), G::EPI_THREADS); mbar_init(pepi_bar(k), G::EPI_THREADS); }
     fence_mbar_init();
   }
   if (warp == 1) {
@@ -705,17 +707,14 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
       float* pg_out = list ? probs : probs + g0 * kBins;
       const int* lg = list ? list + g0 : nullptr;
       const int* lgn = list ? list + gn0 : nullptr;
-      // the NT tiles of a layer: whole tiles alternate between the sets; a single tile is split by channel halves
-      // (C = 16: a half is less than one 16-channel chunk, set 0 takes it all)
+      // The work units of a layer -- (tile, channel half) pairs; whole tiles for d1, whose head sums over all
+      // channels, and for C = 16, where a half is less than one 16-channel chunk -- go round-robin to the sets.
       auto layer = [&](auto mode, int nt, int nv, const int* lgx) {
         constexpr int MODE = decltype(mode)::value;
-        if (nt >= 2) {
-          for (int t = set; t < nt; t += kEpiSets)
-            epilogue_tile<C, BF16, MODE>(sb, tmem_base, t, q, lane, par, nv, pg_out, scr(), lgx, 0, C, set);
-        } else if (C >= 32 && MODE != kD1) {
-          epilogue_tile<C, BF16, MODE>(sb, tmem_base, 0, q, lane, par, nv, pg_out, scr(), lgx, set * (C / 2), (set + 1) * (C / 2), set);
-        } else if (set == 0) {
-          epilogue_tile<C, BF16, MODE>(sb, tmem_base, 0, q, lane, par, nv, pg_out, scr(), lgx, 0, C, set);
+        constexpr int HALVES = (C >= 32 && MODE != kD1) ? 2 : 1;
+        for (int u = set; u < nt * HALVES; u += G::SETS) {
+          const int t = u / HALVES, cb = (u % HALVES) * (C / HALVES);
+          epilogue_tile<C, BF16, MODE>(sb, tmem_base, t, q, lane, par, nv, pg_out, scr(), lgx, cb, cb + C / HALVES, set);
         }
       };
       using std::integral_constant;
@@ -875,12 +874,12 @@ void launch_impl(const float* hist, int n_int, const void* packed, int split_e1,
   const int n_pg = (n_groups + CG - 1) / CG, max_pairs = sm_count / CG;
   const int grid = CG * (n_pg < max_pairs ? n_pg : max_pairs);
   if (CG == 1) {
-    k_unet_tc<C, BF16, CG><<<grid, kTcThreads, G::SMEM, s>>>(hist, n_int, static_cast<const unsigned char*>(packed),
+    k_unet_tc<C, BF16, CG><<<grid, G::THREADS, G::SMEM, s>>>(hist, n_int, static_cast<const unsigned char*>(packed),
                                                             split_e1, probs, list, n_list, seg_cnt);
   } else {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
-    cfg.blockDim = dim3(kTcThreads);
+    cfg.blockDim = dim3(G::THREADS);
     cfg.dynamicSmemBytes = G::SMEM;
     cfg.stream = s;
     cudaLaunchAttribute at[1];
