@@ -57,10 +57,17 @@ __device__ __forceinline__ bool mbar_try_wait_hint(uint32_t bar, uint32_t parity
 // SM clock is a protocol bug: trap instead of hanging the device.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   if (mbar_try_wait(bar, parity)) return;
+#ifdef PVF_MBAR_NO_TIMEOUT
+  while (!mbar_try_wait_hint(bar, parity)) {}
+#else
+  // the clock is read every 256th failed poll only: a waiting warp wakes on every barrier event of the CTA,
+  // so the loop body is executed often and should stay short
   const long long t0 = clock64();
+  uint32_t polls = 0;
   while (!mbar_try_wait_hint(bar, parity)) {
-    if (clock64() - t0 > 4000000000LL) __trap();
+    if ((++polls & 255u) == 0u && clock64() - t0 > 4000000000LL) __trap();
   }
+#endif
 }
 
 // ---------------------------------------------------------------- proxies / fences
