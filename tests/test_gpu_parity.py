@@ -236,6 +236,53 @@ def test_width_sweep_parity(prec, ch):
     assert np.abs(probs.cpu().numpy().astype(np.float64) - ref["probs"]).max() <= TOL[prec]
 
 
+def _pv_efficiency(pv_z, z_found, count, window_mm=0.5):
+    """Toy 'physics' numbers on the hand-built `peaky` weights (stand-in for PAPER.md:41 Fig. 1, whose curves need the
+    trained weights): share of generated PVs with a found peak within +-0.5 mm, and found peaks per event that match
+    no generated PV."""
+    hit = tot = fake = 0
+    for e, truth in enumerate(pv_z):
+        z = np.sort(z_found[e, : count[e]].astype(np.float64))
+        tot += len(truth)
+        near = np.zeros(len(z), bool)
+        for t in truth:
+            d = np.abs(z - t) <= window_mm
+            hit += bool(d.any())
+            near |= d
+        fake += int((~near).sum())
+    return hit / max(tot, 1), fake / max(len(pv_z), 1)
+
+
+@pytest.mark.parametrize("ch", [64, 32, 16])
+def test_accuracy_vs_width_and_precision_table(ch):
+    """accuracy-vs-width/precision on `peaky` (config-1 event model, 160 events, each width with
+    its own `peaky` weights).  Asserts the tolerances; with PVF_WRITE_TABLES=1 appends the rows to
+    gpurun_out/accuracy_table_rows.md (copied to profiles/r01_accuracy_table.md)."""
+    import os
+    ev = make_events("run3", 160, 1001)
+    w = make_weights("peaky", 1, ch)
+    ref = O.run(ev.feat, ev.event_offsets, w)
+    eff_o, fake_o = _pv_efficiency(ev.pv_z, ref["peaks"]["z"], ref["peaks"]["count"])
+    rows = [f"| {ch} | oracle (FP64) | - | {int(ref['peaks']['count'].sum())} | - | {100 * eff_o:.1f} | {fake_o:.2f} |"]
+    for prec in ["fp32", "tf32", "fp16", "bf16"]:
+        pvf = _available(prec, w, ev)
+        probs, pk = _run(pvf, ev)
+        err = float(np.abs(probs.cpu().numpy().astype(np.float64) - ref["probs"]).max())
+        assert err <= TOL[prec], f"{prec} C={ch}: max|dP| {err:.3e}"
+        got = _np(pk)
+        m_all = n_all = 0
+        for e in range(ev.n_events):
+            m, n, _ = O.match_peaks(ref["peaks"]["bin"][e], got["bin"][e])
+            m_all += m; n_all += n
+        assert m_all >= 0.98 * n_all
+        eff, fake = _pv_efficiency(ev.pv_z, got["z"], got["count"])
+        assert abs(eff - eff_o) <= 0.01                           # precision does not change what the toy finds
+        rows.append(f"| {ch} | {prec} | {err:.2e} | {int(got['count'].sum())} | {m_all}/{n_all} | {100 * eff:.1f} | {fake:.2f} |")
+    if os.environ.get("PVF_WRITE_TABLES") == "1" and os.path.isdir("gpurun_out"):
+        with open("gpurun_out/accuracy_table_rows.md", "a") as f:
+            f.write("\n".join(rows) + "\n")
+
+
 @pytest.mark.parametrize("prec", ["fp32", "tf32", "bf16", "fp16"])
 def test_unet_entry_point_on_synthetic_histograms(prec):
     """UNet alone: zero input (bias-only), one-hot inputs at the interval edges (padding), large values."""
