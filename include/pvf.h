@@ -161,7 +161,9 @@ PVF_API pvf_status pvf_run_unet(pvf_handle h, const float* hist, int32_t n_event
                         void* cuda_stream);
 
 /* Copy the histogram of the last pvf_run ([n_events,40,8,100] float, canonical layout) into
- * dev_out, enqueued on cuda_stream. */
+ * dev_out, enqueued on cuda_stream.  In the tensor-core modes the pool holds the histograms of the
+ * intervals with at least one track only (the UNet kernel takes the others as zeros without reading
+ * them); this accessor fills the empty intervals with zeros, so dev_out is always the canonical H. */
 PVF_API pvf_status pvf_debug_copy_histogram(pvf_handle h, float* dev_out, int32_t n_events, void* cuda_stream);
 
 /* Mean stage times in ms over the pvf_run calls made since the previous call of this function (at
