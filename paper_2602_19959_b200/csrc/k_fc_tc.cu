@@ -239,7 +239,10 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
           const int nv = ntile - c0;
           // Ordered accumulation without branches (seg_step).  Only intervals that hold a track are written --
           // the UNet kernel never reads the histogram of an empty interval (it takes seg_cnt == 0 as zeros).
-          if (nv >= 16) {
+          if (nv >= 16 && ivv[15] == c) {        // sorted: the whole chunk belongs to the running interval
+#pragma unroll
+            for (int i = 0; i < 16; ++i) a += sp[i];
+          } else if (nv >= 16) {
 #pragma unroll
             for (int i = 0; i < 16; ++i) seg_step(a, c, ivv[i], sp[i], Hc);
           } else {                                // ragged last chunk: inactive columns add +0 to the same interval
