@@ -398,6 +398,28 @@ def test_cta_pair_is_bit_identical(prec, channels):
         _make(w, ev, "fp32", cta_pair=True)                       # tensor-core modes only
 
 
+@pytest.mark.parametrize("prec,elide", [("tf32", False), ("tf32", True), ("bf16", False), ("fp32", False)])
+def test_batch_without_any_track(prec, elide):
+    """Degenerate batch: 5 events, zero tracks in total (n_tracks == 0).  Every interval is the bias-only vector
+    UNet(0) (BASELINE.json north_star 'empty intervals'), identical across intervals and equal to the oracle's."""
+    w = make_weights("peaky", 4)
+    base = make_events("run3", 1, 3)
+    ev = type(base)(np.zeros((9, 0), np.float32), np.zeros(6, np.int32), [None] * 5)
+    ref = O.run(ev.feat, ev.event_offsets, w)
+    pvf = PVFinder(w, max_events=5, max_tracks=1, precision=prec, split_mask=SPLIT[prec], elide_empty=elide)
+    feat = torch.zeros((9, 1), device="cuda")
+    off = torch.zeros(6, dtype=torch.int32, device="cuda")
+    probs = torch.full((5, 4000), -1.0, device="cuda")
+    pk = pvf.alloc_peaks(5)
+    s = torch.cuda.Stream()
+    pvf.run(feat, off, 5, probs, pk, stream=s)
+    s.synchronize()
+    P = probs.cpu().numpy().reshape(5 * 40, 100)
+    assert np.all(P == P[0])
+    assert np.abs(P.reshape(5, 4000).astype(np.float64) - ref["probs"]).max() <= TOL[prec]
+    assert np.array_equal(pk["count"].cpu().numpy(), ref["peaks"]["count"])
+
+
 # ------------------------------------------------------------------ boundary behaviour
 def test_boundary_contract():
     ev = make_events("run3", 4, 77)
