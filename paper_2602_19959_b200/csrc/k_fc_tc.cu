@@ -33,14 +33,16 @@ namespace {
 constexpr int kEpiWarps = 13;                // one per (accumulator tile, 32-lane quadrant) that holds outputs
 constexpr int kMmaWarp = kEpiWarps;
 constexpr int kHidWarp0 = kMmaWarp + 1;
-constexpr int kFtThreads = (kEpiWarps + 1 + 8) * 32;   // 13 epilogue + 1 MMA + 8 hidden-layer warps
+constexpr int kHidWarps = 4;                 // two groups of two warps: a CTA runs the hidden layers of HALF of a tile
+constexpr int kFtThreads = (kEpiWarps + 1 + kHidWarps) * 32;   // 13 epilogue + 1 MMA + 4 hidden-layer warps
 constexpr int kHalfOut = kFcOut / 2;         // outputs per CTA half, packed densely: row 128 t + r = output 400 half + 128 t + r
 constexpr int kTile = 128;                   // tracks per tile (MMA N)
 constexpr int kRowsW = 512;                  // 4 channel tiles x 128 rows per CTA half
 constexpr int kLboW = kRowsW * 16;           // 8192: next 16-byte K chunk of the A operand
-constexpr int kLboH = kTile * 16;            // 2048: next 16-byte K chunk of the B operand
+constexpr int kHalfTile = kTile / 2;         // B-operand rows (tracks) this CTA of the pair supplies
+constexpr int kLboH = kHalfTile * 16;        // 1024: next 16-byte K chunk of the B operand
 constexpr int kWPart = 8 * kLboW;            // 65536 bytes: one part (hi or lo) of W5x for one half
-constexpr int kHPart = 8 * kLboH;            // 16384 bytes: one part of hx for one tile
+constexpr int kHPart = 8 * kLboH;            // 8192 bytes: one part of hx for this CTA's half of a tile
 constexpr int kWRow = 28;
 
 struct FtSmall {                             // the five hidden layers, zero padded
@@ -51,7 +53,7 @@ struct FtSmall {                             // the five hidden layers, zero pad
 };
 
 constexpr int OFF_W = 0;                               // [hi | lo][8 chunks][512 rows][16 B]
-constexpr int OFF_H = OFF_W + 2 * kWPart;              // [buf 0 | 1][hi | lo][8 chunks][128 tracks][16 B]
+constexpr int OFF_H = OFF_W + 2 * kWPart;              // [buf 0 | 1][hi | lo][8 chunks][64 tracks][16 B]
 constexpr int OFF_SMALL = OFF_H + 4 * kHPart;
 constexpr int OFF_IV = OFF_SMALL + ((int)sizeof(FtSmall) + 127) / 128 * 128;   // int [4][128]
 constexpr int kIvBufs = 4;                   // interval lists of four tiles in flight: the hidden-layer warps of tile
@@ -59,8 +61,9 @@ constexpr int kIvBufs = 4;                   // interval lists of four tiles in 
 constexpr int OFF_BARS = OFF_IV + kIvBufs * kTile * 4;
 constexpr int FT_SMEM = OFF_BARS + 256;
 static_assert(FT_SMEM <= 227 * 1024, "shared memory budget");
-// barriers (8 bytes each): h_full[2], h_empty[2], meta_empty[2], acc_full[4], acc_empty[4], then the TMEM slot
-enum { bHFull = 0, bHEmpty = 2, bMeta = 4, bAccFull = 8, bAccEmpty = 12, bSlot = 16 };
+// barriers (8 bytes each): h_full[2], peer_h_full[2] (leader: the peer's half is staged), h_empty[2], meta[4],
+// acc_full[4], acc_empty[4], peer_acc_empty[4] (leader: the peer's epilogue has drained the tile), then the TMEM slot
+enum { bHFull = 0, bPHFull = 2, bHEmpty = 4, bMeta = 6, bAccFull = 10, bAccEmpty = 14, bPAccEmpty = 18, bSlot = 22 };
 
 __device__ __forceinline__ float leaky_ft(float v) { return v >= 0.0f ? v : kLeaky * v; }
 __device__ __forceinline__ uint32_t tf32_of(float v) {
@@ -126,8 +129,8 @@ __device__ __forceinline__ void seg_step(float& a, int& c, int iv, float x, floa
 // [5] MMA total; [6] hidden wait h_empty, [7] hidden wait meta, [8] hidden total (group 0), [9] tiles
 __device__ unsigned long long g_fc_prof[160][16];
 #define FC_PROF_T0() const long long prof_t0 = clock64()
-#define FC_PROF_ADD(slot, cond) do { if (cond) g_fc_prof[blockIdx.x + gridDim.x * blockIdx.y][slot] += (unsigned long long)(clock64() - prof_t0); } while (0)
-#define FC_PROF_CNT(slot, cond) do { if (cond) g_fc_prof[blockIdx.x + gridDim.x * blockIdx.y][slot] += 1ull; } while (0)
+#define FC_PROF_ADD(slot, cond) do { if (cond) g_fc_prof[blockIdx.x][slot] += (unsigned long long)(clock64() - prof_t0); } while (0)
+#define FC_PROF_CNT(slot, cond) do { if (cond) g_fc_prof[blockIdx.x][slot] += 1ull; } while (0)
 #else
 #define FC_PROF_T0() do {} while (0)
 #define FC_PROF_ADD(slot, cond) do {} while (0)
@@ -143,7 +146,11 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
   const uint32_t sb = smem_u32(smem);
   const int tid = threadIdx.x, lane = tid & 31;
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
-  const int half = blockIdx.y;
+  // The two CTAs of a cluster (blockIdx.x = 2 j, 2 j + 1) serve the two halves of the outputs for the SAME events and share
+  // every MMA (cta_group::2, M = 256): each supplies its 128 output rows of W5x and the hidden activations of HALF of
+  // the tile's tracks (even sorted positions: rank 0, odd: rank 1), so the hidden layers are computed once per pair.
+  const int rank = (int)cluster_ctarank();
+  const int half = rank;
   FtSmall& S = *reinterpret_cast<FtSmall*>(smem + OFF_SMALL);
   int* s_iv = reinterpret_cast<int*>(smem + OFF_IV);
   auto bar = [&](int k) { return sb + OFF_BARS + 8u * k; };
@@ -171,15 +178,21 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
     S.bh[l][c] = c < kFcHidden ? par[kFcHid + l * kFcHidStride + kFcHidden * kFcHidden + c] : 0.0f;
   }
   if (tid == 0) {
-    for (int k = 0; k < 2; ++k) { mbar_init(bar(bHFull + k), 128); mbar_init(bar(bHEmpty + k), 1); }
+    for (int k = 0; k < 2; ++k) {
+      mbar_init(bar(bHFull + k), kHalfTile); mbar_init(bar(bPHFull + k), kHalfTile); mbar_init(bar(bHEmpty + k), 1);
+    }
     for (int k = 0; k < kIvBufs; ++k) mbar_init(bar(bMeta + k), 32 * kEpiWarps);
-    for (int k = 0; k < 4; ++k) { mbar_init(bar(bAccFull + k), 1); mbar_init(bar(bAccEmpty + k), k < 3 ? 128 : 32); }
+    for (int k = 0; k < 4; ++k) {
+      mbar_init(bar(bAccFull + k), 1);
+      mbar_init(bar(bAccEmpty + k), k < 3 ? 128 : 32);
+      mbar_init(bar(bPAccEmpty + k), k < 3 ? 128 : 32);
+    }
     fence_mbar_init();
   }
-  if (warp == kMmaWarp) tmem_alloc(smem_u32(const_cast<uint32_t*>(tmem_slot)), 512);
+  if (warp == kMmaWarp) tmem_alloc2(smem_u32(const_cast<uint32_t*>(tmem_slot)), 512);
   fence_proxy_async_smem();
   tc_fence_before_sync();
-  __syncthreads();
+  cluster_sync_all();
   tc_fence_after_sync();
   const uint32_t tmem_base = *tmem_slot;
 
@@ -197,10 +210,11 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
     const int q = warp & 3, mt = warp >> 2;
     const int r = 32 * q + lane, ol = 128 * mt + r;
     const bool valid = ol < kHalfOut;
+    const uint32_t lead_pacc = mapa_rank(bar(bPAccEmpty), 0);
     int it = 0;
     const bool pw = tid == 0;
     FC_PROF_T0();
-    for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
+    for (int e = (int)blockIdx.x >> 1; e < n_events; e += (int)gridDim.x >> 1) {
       int ev_lo;
       const int nk = kept_of(e, ev_lo);
       // output o = c * 100 + l lives at H[e][interval][o]: the dense row index is the offset itself.  Rows that
@@ -220,8 +234,11 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
         tc_fence_after_sync();
         const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)(mt * kTile);
         for (int c0 = 0; c0 < ntile; c0 += 16) {
-          uint32_t v[16];
-          tmem_ld_x16(taddr + (uint32_t)c0, v);
+          // sorted positions c0 .. c0+15: the even ones are columns c0/2 .. of the leader's half of N, the odd ones
+          // columns 64 + c0/2 .. of the peer's half
+          uint32_t ve[8], vo[8], v[16];
+          tmem_ld_x8(taddr + (uint32_t)(c0 >> 1), ve);
+          tmem_ld_x8(taddr + (uint32_t)(kHalfTile + (c0 >> 1)), vo);
           // intervals of the 16 tracks (broadcast 16-byte loads) while the TMEM load is in flight
           int ivv[16];
 #pragma unroll
@@ -230,6 +247,8 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
             ivv[4 * k + 0] = q4.x; ivv[4 * k + 1] = q4.y; ivv[4 * k + 2] = q4.z; ivv[4 * k + 3] = q4.w;
           }
           tmem_ld_wait();
+#pragma unroll
+          for (int k = 0; k < 8; ++k) { v[2 * k] = ve[k]; v[2 * k + 1] = vo[k]; }
           // all 16 softplus first: independent, so the SFU pipeline stays full; columns past the
           // tile's last track are computed on stale accumulators and then masked
           float sp[16];
@@ -255,29 +274,41 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
         }
         if (last) Hc[c] = a;                      // the event's last non-empty interval
         tc_fence_before_sync();
-        mbar_arrive(bar(bAccEmpty + mt));
+        if (rank == 0) mbar_arrive(bar(bAccEmpty + mt));
+        else mbar_arrive_cluster(lead_pacc + 8u * mt);
         mbar_arrive(bar(bMeta + (it & (kIvBufs - 1))));
       }
     }
     FC_PROF_ADD(2, pw);
   } else if (warp == kMmaWarp) {
-    // ===================== MMA issuer
-    constexpr uint32_t idesc = instr_desc(kFmtTF32, 128, kTile);
+    // ===================== MMA issuer (leader CTA only; the peer's warp just keeps the TMEM allocation)
+    if (rank == 0) {
+    constexpr uint32_t idesc = instr_desc(kFmtTF32, 256, kTile);
     constexpr uint32_t hi = (128u >> 4) | (1u << 14);
     constexpr uint32_t a_lbo = (uint32_t)(kLboW >> 4) << 16, b_lbo = (uint32_t)(kLboH >> 4) << 16;
     int it = 0;
     const bool pw = lane == 0;
     FC_PROF_T0();
-    for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
+    for (int e = (int)blockIdx.x >> 1; e < n_events; e += (int)gridDim.x >> 1) {
       int ev_lo;
       const int nk = kept_of(e, ev_lo);
       for (int base = 0; base < nk; base += kTile, ++it) {
         const int buf = it & 1;
-        { FC_PROF_T0(); mbar_wait(bar(bHFull + buf), (uint32_t)((it >> 1) & 1)); FC_PROF_ADD(3, pw); }
+        {
+          FC_PROF_T0();
+          mbar_wait(bar(bHFull + buf), (uint32_t)((it >> 1) & 1));       // both halves of the B operand are staged
+          mbar_wait(bar(bPHFull + buf), (uint32_t)((it >> 1) & 1));
+          FC_PROF_ADD(3, pw);
+        }
         tc_fence_after_sync();
 #pragma unroll
         for (int mt = 0; mt < 4; ++mt) {
-          { FC_PROF_T0(); mbar_wait(bar(bAccEmpty + mt), (uint32_t)((it & 1) ^ 1)); FC_PROF_ADD(4, pw); }
+          {
+            FC_PROF_T0();
+            mbar_wait(bar(bAccEmpty + mt), (uint32_t)((it & 1) ^ 1));     // both epilogues have drained tile mt
+            mbar_wait(bar(bPAccEmpty + mt), (uint32_t)((it & 1) ^ 1));
+            FC_PROF_ADD(4, pw);
+          }
           tc_fence_after_sync();
           if (elect_one()) {
 #pragma unroll
@@ -286,25 +317,30 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
               for (int s = 0; s < 4; ++s) {
                 const uint32_t a = a_lbo + ((sb + OFF_W + (pass == 2 ? kWPart : 0) + mt * 2048 + s * 2 * kLboW) >> 4);
                 const uint32_t b = b_lbo + ((sb + OFF_H + buf * 2 * kHPart + (pass == 1 ? kHPart : 0) + s * 2 * kLboH) >> 4);
-                mma_tf32_lh(tmem_base + (uint32_t)(mt * kTile), a, hi, b, hi, idesc, (pass | s) ? 1u : 0u);
+                mma2_tf32_lh(tmem_base + (uint32_t)(mt * kTile), a, hi, b, hi, idesc, (pass | s) ? 1u : 0u);
               }
             }
-            mma_commit(bar(bAccFull + mt));
-            if (mt == 3) mma_commit(bar(bHEmpty + buf));
+            mma_commit2(bar(bAccFull + mt), 3);            // to both CTAs' barriers
+            if (mt == 3) mma_commit2(bar(bHEmpty + buf), 3);
           }
           __syncwarp();
         }
       }
     }
     FC_PROF_ADD(5, pw);
+    }
   } else {
-    // ===================== hidden layers: two groups of 128 threads, thread = track, alternating tiles
-    const int g = (warp - kHidWarp0) >> 2, i = tid - 32 * kHidWarp0 - 128 * g;
+    // ===================== hidden layers: two groups of 64 threads for alternating tiles; thread i takes the track
+    // at sorted position 2 i + rank of the tile (B-operand row i of this CTA) and also looks up the interval of its
+    // neighbour 2 i + 1 - rank, so that both CTAs hold the interval list of the whole tile without exchanging data
+    const int g = (warp - kHidWarp0) >> 1, i = tid - 32 * kHidWarp0 - kHalfTile * g;
     const uint32_t hbase = sb + OFF_H + (uint32_t)g * 2 * kHPart + (uint32_t)i * 16u;
+    const uint32_t lead_phfull = mapa_rank(bar(bPHFull + g), 0);
+    const int p_own = 2 * i + rank, p_other = 2 * i + 1 - rank;
     int it = 0;
     const bool pw = g == 0 && i == 0;
     FC_PROF_T0();
-    for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
+    for (int e = (int)blockIdx.x >> 1; e < n_events; e += (int)gridDim.x >> 1) {
       int ev_lo;
       const int nk = kept_of(e, ev_lo);
       for (int base = 0; base < nk; base += kTile, ++it) {
@@ -313,11 +349,16 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
         { FC_PROF_T0(); mbar_wait(bar(bHEmpty + g), prev); FC_PROF_ADD(6, pw); }   // the MMAs that read this buffer have retired
         const int ib = it & (kIvBufs - 1);
         { FC_PROF_T0(); mbar_wait(bar(bMeta + ib), (uint32_t)(((it >> 2) & 1) ^ 1)); FC_PROF_ADD(7, pw); }   // the epilogue is done with s_iv[ib]
-        if (base + i < nk) {
+        if (base + p_other < nk) {
           int t;
           float zrel;
-          const int iv = entry_interval(perm[ev_lo + base + i], F.f[0], t, zrel);   // own or neighbouring interval
-          s_iv[ib * kTile + i] = iv * kFcOut;       // the epilogue wants the interval as its offset in H
+          s_iv[ib * kTile + p_other] = entry_interval(perm[ev_lo + base + p_other], F.f[0], t, zrel) * kFcOut;
+        }
+        if (base + p_own < nk) {
+          int t;
+          float zrel;
+          const int iv = entry_interval(perm[ev_lo + base + p_own], F.f[0], t, zrel);   // own or neighbouring interval
+          s_iv[ib * kTile + p_own] = iv * kFcOut;   // the epilogue wants the interval as its offset in H
           const float x[kFcIn] = {zrel, F.f[1][t], F.f[2][t], F.f[3][t], F.f[4][t], F.f[5][t], F.f[6][t], F.f[7][t], F.f[8][t]};
           float h[32], gg[28];
 #pragma unroll
@@ -361,16 +402,18 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
           }
         }
         fence_proxy_async_smem();
-        mbar_arrive(bar(bHFull + g));
+        mbar_arrive(bar(bHFull + g));                       // this CTA's epilogue (interval list) and, in the leader, the MMAs
+        if (rank == 1) mbar_arrive_cluster(lead_phfull);    // the peer's half of the B operand is staged
       }
     }
     FC_PROF_ADD(8, pw);
   }
+  __syncwarp();
   tc_fence_before_sync();
-  __syncthreads();
+  cluster_sync_all();                                       // the pair's shared memory and barriers stay alive until both are done
   if (warp == kMmaWarp) {
     __syncwarp();
-    tmem_dealloc(tmem_base, 512);
+    tmem_dealloc2(tmem_base, 512);
   }
 }
 
@@ -417,17 +460,20 @@ void launch_fc_hist_tc(const float* const feat[9], const int32_t* event_offsets,
   Feat9 F;
   for (int k = 0; k < 9; ++k) F.f[k] = feat[k];
   const int gx = n_events < sm_count / 2 ? n_events : sm_count / 2;
-  k_fc_hist_tc<<<dim3(gx, 2), kFtThreads, FT_SMEM, s>>>(F, event_offsets, perm, seg_off, seg_cnt, fc_params,
-                                                        static_cast<const unsigned char*>(w5img), n_events, hist, dump);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(2 * gx);
+  cfg.blockDim = dim3(kFtThreads);
+  cfg.dynamicSmemBytes = FT_SMEM;
+  cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;     // the two output halves of the same events form a CTA pair
+  at[0].val.clusterDim.x = 2;
+  at[0].val.clusterDim.y = 1;
+  at[0].val.clusterDim.z = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  cudaLaunchKernelEx(&cfg, k_fc_hist_tc, F, event_offsets, perm, seg_off, seg_cnt, fc_params,
+                     static_cast<const unsigned char*>(w5img), n_events, hist, dump);
 }
-
-#ifdef PVF_FC_PROF
-extern "C" __attribute__((visibility("default"))) int pvf_debug_fc_prof(unsigned long long* host_out, int reset) {
-  cudaDeviceSynchronize();
-  if (host_out) cudaMemcpyFromSymbol(host_out, g_fc_prof, sizeof(g_fc_prof));
-  if (reset) { static unsigned long long z[160][16]; cudaMemcpyToSymbol(g_fc_prof, z, sizeof(z)); }
-  return 0;
-}
-#endif
 
 }  // namespace pvf
