@@ -299,6 +299,12 @@ def main_ours(args, rank, world, local_rank):
         "roofline_fc_hist": {"bound": "hbm", "achieved": hbm_bytes_fc / (stage[1] * 1e-3) / 1e9,
                              "peak": peaks["hbm_gbs"], "unit": "GB/s",
                              "frac": hbm_bytes_fc / (stage[1] * 1e-3) / 1e9 / peaks["hbm_gbs"]},
+        # the FC + sum stage is bound by its 1600 SFU operations per track (800 x (ex2 + lg2)), not by HBM (DESIGN.md
+        # section 4.2): 148 SMs x 16 SFU lanes x 1.965 GHz = 4.65 Tops/s
+        "roofline_fc_hist_alu": {"bound": "alu", "achieved": ev.n_tracks * 1600 / (stage[1] * 1e-3) / 1e12,
+                                 "peak": 148 * 16 * 1.965e9 / 1e12, "unit": "T SFU-op/s",
+                                 "frac": ev.n_tracks * 1600 / (stage[1] * 1e-3) / (148 * 16 * 1.965e9),
+                                 "peak_source": "148 SMs x 16 SFU lanes/clk x 1.965 GHz max SM clock (guide unit counts)"},
         "e2e": {"value": e2e_value, "unit": "events/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": n_e2e, "api": "pvf_run_host (pinned host buffers)"},
         "gpu_launches": launches, "clocks": clocks,
