@@ -9,17 +9,20 @@
 //
 // Mapping.  The last layer is 88 % of the FC FLOPs.  Per tile of up to 128 sorted tracks of one event
 //     D[o, t] = sum_k W5x[o, k] * hx[t, k],   k < 25: weights x activations, k = 25: bias x 1, K = 32
-// with M = 128 rows = the 100 bins of ONE histogram channel (+28 zero rows), N = 128 tracks.  So an
-// accumulator lane is one output bin and an accumulator column is one track: the epilogue thread that
-// owns lane l walks the columns in sorted-track order, adds softplus(D) into one FP32 register and
-// stores it to H whenever the interval changes -- the same fixed-order sum as k_fc_hist, with no
-// cross-lane reduction and every H element written exactly once (zeros for empty intervals).
+// with M = output rows and N = 128 tracks.  So an accumulator lane is one output and an accumulator column
+// is one track: the epilogue thread that owns a lane walks the columns in sorted-track order, adds
+// softplus(D) into one FP32 register and stores it to H whenever the interval changes -- the same fixed-order
+// sum as k_fc_hist, with no cross-lane reduction; only intervals that hold a track are written (k_unet_tc takes
+// seg_cnt == 0 as zeros).
 // FP32 accuracy: W5x = W_hi + W_lo and hx = h_hi + h_lo (each part RN-rounded to TF32), three MMAs
 // W_hi h_hi + W_hi h_lo + W_lo h_hi accumulate in FP32 in TMEM (the dropped term is ~2^-22 relative).
-// A CTA serves one half of the outputs (blockIdx.y: channels 0-3 or 4-7; 128 KB of W5x hi+lo resident
-// in shared memory) for a strided subset of the events.  Roles: warps 0-7 epilogue, warp 8 MMA
-// issuer, warps 9-16 = two groups of 128 threads that run the five 25-wide hidden layers (FP32 FMA,
-// thread = track) for alternating tiles and stage h_hi / h_lo as the B operand (double buffered).
+// CTA pairs: the two CTAs of a cluster serve the two halves of the 800 outputs (400 each, packed densely into
+// 3 full accumulator tiles + 16 rows; 128 KB of W5x hi + lo resident in shared memory) for the same strided
+// subset of events and share every MMA (cta_group::2, M = 256): each supplies the hidden activations of half of
+// the tile's tracks (even / odd sorted positions), so the hidden layers run once per pair.
+// Roles: warps 0-12 epilogue (one accumulator tile quadrant each), warp 13 MMA issuer (leader CTA), warps
+// 14-17 = two groups of 64 threads that run the five 25-wide hidden layers (FP32 FMA, thread = track) for
+// alternating tiles and stage h_hi / h_lo as the B operand (double buffered).
 #include <cstring>
 
 #include "pvf_internal.cuh"

@@ -15,8 +15,12 @@
 // base address, and an epilogue thread (= one row) writes whole 16-byte chunks, conflict free.
 // Intervals sit at row stride 128 / 64 / 32 (L = 100 / 50 / 25); the rows between them are zero and
 // double as the "same" padding.  One persistent CTA takes a group of T intervals through all five
-// layers; each weight slice is streamed from L2 once per group (1D bulk copies into a ring of 8 KB
-// stages) and used by every tile of the group.
+// layers; each weight slice is streamed from L2 once per group (1D bulk copies into a ring of 16 KB
+// stages, 8 KB per CTA of a pair) and used by every tile of the group.
+//
+// CTA pairs (template parameter CG = 2, the default of the binding): a cluster of two CTAs runs every MMA as
+// one tcgen05.mma.cta_group::2 of M = 256 issued by the leader; each CTA keeps its own group's activations
+// and accumulators and supplies half of the weight rows (rank 0 the even tap of a pair, rank 1 the odd one).
 //
 // Schedule.  The MMA issuer never waits for an epilogue in steady state: d1 is split into the half
 // that reads the e1 skip (d1E, needs only e1's epilogue) and the half that reads up(d2) (d1U); d1E
@@ -25,8 +29,10 @@
 //     e2 | d1E.1 | b | d1E.2 | d2 | d1E.3 | e1(next) | d1U        (weight image is packed in this order)
 // TMEM holds two accumulator regions: A (d1, T tiles) and B (e1: T tiles; e2, b, d2: its first tiles).
 // Roles: warp 0 = weight producer, warp 1 = MMA issuer (warp-uniform schedule, one elected lane
-// issues), warps 2-5 = epilogue (TMEM -> registers -> bias, LeakyReLU, TF32/BF16 rounding, pool /
-// upsample -> shared memory; d1's epilogue fuses the 1x1 head + sigmoid and writes out_probs).
+// issues; in the peer CTA of a pair it relays "my half of the stage has landed"), warps 2.. = epilogue in
+// sets of four (TMEM -> registers -> bias, LeakyReLU, TF32/BF16 rounding, pool / upsample -> shared
+// memory; d1's epilogue fuses the 1x1 head + sigmoid and writes out_probs).
+// TF32 mode: the e1 layer (raw histogram input) can run as two passes on BF16 pieces (split_mask bit 0).
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 #include <cstring>
