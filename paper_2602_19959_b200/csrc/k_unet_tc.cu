@@ -473,6 +473,12 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
                 "a ring stage is either part of one source's K blocks or whole taps");
   constexpr uint32_t idesc = instr_desc(BF16 == 2 ? kFmtF16 : (BF16 ? kFmtBF16 : kFmtTF32), 128 * CG, G::NOUT);
   constexpr uint32_t idesc_x = instr_desc(kFmtBF16, 128 * CG, G::NOUT);
+  // The kernels have an odd number of taps: the last "pair" holds an even tap only, so its steps are MMAs of
+  // N = C (half the tensor time, half the B rows; the E1 columns of the accumulator are left alone).
+  constexpr uint32_t idesc_h = instr_desc(BF16 == 2 ? kFmtF16 : (BF16 ? kFmtBF16 : kFmtTF32), 128 * CG, G::NOUT / 2);
+  constexpr uint32_t idesc_xh = instr_desc(kFmtBF16, 128 * CG, G::NOUT / 2);
+  constexpr uint32_t b_lbo_h = (uint32_t)((G::NB / 2 * 16) >> 4) << 16;
+  constexpr int LAST0 = (Y::PAIRS - 1) * Y::NKB;                       // first step of the last tap pair (not e1)
   constexpr uint32_t hi = (128u >> 4) | (1u << 14);                    // SBO = 128 B, descriptor version 1
   constexpr uint32_t a_lbo = (uint32_t)(Y::LBO >> 4) << 16;
   constexpr uint32_t b_lbo = (uint32_t)((G::NB * 16) >> 4) << 16;
@@ -490,7 +496,7 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
       PVF_PROF_ADD(7);
     }
     tc_fence_after_sync();
-    const uint32_t b0 = b_lbo + ((sb + G::OFF_RING + rs.ring * G::STAGE_BYTES) >> 4);
+    const uint32_t b0 = (sb + G::OFF_RING + rs.ring * G::STAGE_BYTES) >> 4;
     uint32_t a0 = a_lbo + (sb >> 4);          // stage origin: descriptor low word of tile 0, step f
     if (S == sE1) {
       // e1: one K block per step; steps run [pass][tap pair]; both passes of the split read the same operand
@@ -514,12 +520,15 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
           } else {
             a = a0 + (uint32_t)((Y::a_off(i % Y::NKB) - Y::SRC0) >> 4) + (uint32_t)(2 * (i / Y::NKB));
           }
-          const uint32_t b = b0 + (uint32_t)(i * (G::STEP_BYTES >> 4));
+          const bool half_n = (S == sE1) ? ((f + i) % 13 == 12) : (f + i >= LAST0);
+          const uint32_t b = (half_n ? b_lbo_h : b_lbo) + b0 + (uint32_t)(i * (G::STEP_BYTES >> 4));
           const uint32_t acc = (i > 0) ? 1u : (f > f_begin ? 1u : acc0);
 #pragma unroll
           for (int t = 0; t < Y::NT; ++t) {
-            if (S == sE1 && BF16 == 0 && e1x) mma_lh<1, CG>(dcol + (uint32_t)(t * G::NOUT), a + 128u * t, hi, b, hi, idesc_x, acc);
-            else mma_lh<BF16, CG>(dcol + (uint32_t)(t * G::NOUT), a + 128u * t, hi, b, hi, idesc, acc);
+            if (S == sE1 && BF16 == 0 && e1x)
+              mma_lh<1, CG>(dcol + (uint32_t)(t * G::NOUT), a + 128u * t, hi, b, hi, half_n ? idesc_xh : idesc_x, acc);
+            else
+              mma_lh<BF16, CG>(dcol + (uint32_t)(t * G::NOUT), a + 128u * t, hi, b, hi, half_n ? idesc_h : idesc, acc);
           }
         }
       }
@@ -833,10 +842,12 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst_all) {
       unsigned char* step = dst + P.seg_off[d.seg] + (size_t)s * G::STEP_BYTES;
       if (d.seg == gE1 && !BF16 && split_e1) {
         // split e1 of the TF32 kernel: BF16 pieces w = w1 + w2; pass 0 holds [w1 | w1] (meets [a1 | a2]), pass 1 [w2 | 0]
+        const bool half_x = 2 * u + 1 >= d.taps;
+        const int nbx = half_x ? G::NB / 2 : G::NB;
         for (int h = 0; h < 2; ++h)
-          for (int nl = 0; nl < G::NB; ++nl)
+          for (int nl = 0; nl < nbx; ++nl)
             for (int e = 0; e < 8; ++e) {
-              const int n = rank * G::NB + nl;
+              const int n = rank * nbx + nl;
               const int co = n % C, j = 2 * u + n / C;
               const float v = j < d.taps ? W[((size_t)co * d.cin + e) * d.taps + j] : 0.0f;
               const uint16_t w1 = bf16_rne(v);
@@ -845,19 +856,22 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst_all) {
               memcpy(&w1f, &w1bits, 4);
               const uint16_t w2 = bf16_rne(v - w1f);
               const uint16_t out = pass == 0 ? w1 : (h == 0 ? w2 : (uint16_t)0);
-              memcpy(step + ((size_t)h * G::NB + nl) * 16 + e * 2, &out, 2);
+              memcpy(step + ((size_t)h * nbx + nl) * 16 + e * 2, &out, 2);
             }
         continue;
       }
+      // last tap pair (odd tap missing): an N = C step -- half as many B rows, all of the even tap, split over the pair
+      const bool half_n = 2 * u + 1 >= d.taps;
+      const int nb = half_n ? G::NB / 2 : G::NB;
       for (int h = 0; h < 2; ++h)
-        for (int nl = 0; nl < G::NB; ++nl)        // rows [0, C): even tap 2u, rows [C, 2C): odd tap 2u + 1
+        for (int nl = 0; nl < nb; ++nl)           // rows [0, C): even tap 2u, rows [C, 2C): odd tap 2u + 1
           for (int e = 0; e < G::PER; ++e) {
-            const int n = rank * G::NB + nl;
+            const int n = rank * nb + nl;
             const int co = n % C, j = 2 * u + n / C;
             const int cl = (2 * kk + h) * G::PER + e;            // channel inside the sub-layer's range
             const bool real = j < d.taps && ((d.seg == gE1) ? cl < kHistCh : true);
             const float v = real ? W[((size_t)co * d.cin + d.ch_base + cl) * d.taps + j] : 0.0f;
-            unsigned char* p = step + ((size_t)h * G::NB + nl) * 16 + e * G::ES;
+            unsigned char* p = step + ((size_t)h * nb + nl) * 16 + e * G::ES;
             if (BF16) {
               const uint16_t b = (BF16 == 2) ? fp16_rne(v) : bf16_rne(v);
               memcpy(p, &b, 2);
