@@ -135,7 +135,8 @@ template <int C, int BF16, int CG>
 __host__ __device__ inline Plan make_plan(int split_e1) {
   using G = Geo<C, BF16, CG>;
   Plan P{};
-  P.e1_steps = 13 * ((!BF16 && split_e1) ? 2 : 1);
+  // 16-bit modes: the 8 input channels fill half of an MMA's K = 16, so one e1 step takes TWO tap pairs (7 steps)
+  P.e1_steps = BF16 ? 7 : 13 * (split_e1 ? 2 : 1);
   P.seg_steps[gE2] = 8 * G::NKB1;
   P.seg_steps[gD1Ea] = G::D1E_A;
   P.seg_steps[gB] = 3 * G::NKB1;
@@ -480,7 +481,9 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
   constexpr uint32_t b_lbo_h = (uint32_t)((G::NB / 2 * 16) >> 4) << 16;
   constexpr int LAST0 = (Y::PAIRS - 1) * Y::NKB;                       // first step of the last tap pair (not e1)
   constexpr uint32_t hi = (128u >> 4) | (1u << 14);                    // SBO = 128 B, descriptor version 1
-  constexpr uint32_t a_lbo = (uint32_t)(Y::LBO >> 4) << 16;
+  // e1 in the 16-bit modes: the second 16-byte K chunk of A is the SAME 8-channel buffer two rows further down
+  // (LBO = 32 bytes), i.e. the input of the next tap pair -- one MMA does tap pairs 2w and 2w + 1
+  constexpr uint32_t a_lbo = (S == sE1 && BF16) ? (2u << 16) : ((uint32_t)(Y::LBO >> 4) << 16);
   constexpr uint32_t b_lbo = (uint32_t)((G::NB * 16) >> 4) << 16;
   const uint32_t dcol = tmem_base + (uint32_t)Y::DCOL;
   for (int f = f_begin; f < f_end; f += SPS) {
@@ -513,14 +516,14 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
         if (i < n) {
           uint32_t a;
           if (S == sE1) {
-            const int step = f + i, pass = step / 13, u = step - 13 * pass;
+            const int step = f + i, pass = step / 13, u = BF16 ? 2 * step : step - 13 * pass;
             a = a0 + (uint32_t)(Y::SRC0 >> 4) + (uint32_t)(Y::LEAD + 2 * u - Y::PAD);
           } else if (Y::HALF >= SPS) {
             a = a0 + (uint32_t)(i * ((2 * Y::LBO) >> 4));
           } else {
             a = a0 + (uint32_t)((Y::a_off(i % Y::NKB) - Y::SRC0) >> 4) + (uint32_t)(2 * (i / Y::NKB));
           }
-          const bool half_n = (S == sE1) ? ((f + i) % 13 == 12) : (f + i >= LAST0);
+          const bool half_n = (S == sE1) ? (BF16 ? f + i == 6 : (f + i) % 13 == 12) : (f + i >= LAST0);
           const uint32_t b = (half_n ? b_lbo_h : b_lbo) + b0 + (uint32_t)(i * (G::STEP_BYTES >> 4));
           const uint32_t acc = (i > 0) ? 1u : (f > f_begin ? 1u : acc0);
 #pragma unroll
@@ -837,7 +840,8 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst_all) {
     for (int s = 0; s < P.seg_steps[d.seg]; ++s) {
       const int f = d.f0 + s;                     // step index inside the sub-layer
       int u, kk, pass = 0;                        // tap pair, K block
-      if (d.seg == gE1) { pass = f / 13; u = f % 13; kk = 0; }     // e1 split runs [pass][tap pair]
+      if (d.seg == gE1 && BF16) { u = 2 * f; kk = 0; }             // 16-bit e1: K chunk h of step f holds tap pair 2f + h
+      else if (d.seg == gE1) { pass = f / 13; u = f % 13; kk = 0; }   // e1 split runs [pass][tap pair]
       else { u = f / d.nkb; kk = f % d.nkb; }
       unsigned char* step = dst + P.seg_off[d.seg] + (size_t)s * G::STEP_BYTES;
       if (d.seg == gE1 && !BF16 && split_e1) {
@@ -867,8 +871,9 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst_all) {
         for (int nl = 0; nl < nb; ++nl)           // rows [0, C): even tap 2u, rows [C, 2C): odd tap 2u + 1
           for (int e = 0; e < G::PER; ++e) {
             const int n = rank * nb + nl;
-            const int co = n % C, j = 2 * u + n / C;
-            const int cl = (2 * kk + h) * G::PER + e;            // channel inside the sub-layer's range
+            const bool e1x2 = d.seg == gE1 && BF16;
+            const int co = n % C, j = 2 * (u + (e1x2 ? h : 0)) + n / C;
+            const int cl = e1x2 ? e : (2 * kk + h) * G::PER + e;   // channel inside the sub-layer's range
             const bool real = j < d.taps && ((d.seg == gE1) ? cl < kHistCh : true);
             const float v = real ? W[((size_t)co * d.cin + d.ch_base + cl) * d.taps + j] : 0.0f;
             unsigned char* p = step + ((size_t)h * nb + nl) * 16 + e * G::ES;
