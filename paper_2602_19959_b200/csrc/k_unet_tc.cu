@@ -136,7 +136,8 @@ __host__ __device__ inline Plan make_plan(int split_e1) {
   using G = Geo<C, BF16, CG>;
   Plan P{};
   // 16-bit modes: the 8 input channels fill half of an MMA's K = 16, so one e1 step takes TWO tap pairs (7 steps)
-  P.e1_steps = BF16 ? 7 : 13 * (split_e1 ? 2 : 1);
+  // TF32 with the e1 split: 13 steps [a1 | a2] x [w1 | w1] + 7 steps [a1(pair 2w) | a1(pair 2w+1)] x [w2 | w2]
+  P.e1_steps = BF16 ? 7 : (split_e1 ? 20 : 13);
   P.seg_steps[gE2] = 8 * G::NKB1;
   P.seg_steps[gD1Ea] = G::D1E_A;
   P.seg_steps[gB] = 3 * G::NKB1;
@@ -484,6 +485,7 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
   // e1 in the 16-bit modes: the second 16-byte K chunk of A is the SAME 8-channel buffer two rows further down
   // (LBO = 32 bytes), i.e. the input of the next tap pair -- one MMA does tap pairs 2w and 2w + 1
   constexpr uint32_t a_lbo = (S == sE1 && BF16) ? (2u << 16) : ((uint32_t)(Y::LBO >> 4) << 16);
+  constexpr uint32_t a_lbo_x2 = (2u << 16) - a_lbo;     // added for the second pass of the split e1 (TF32 kernel)
   constexpr uint32_t b_lbo = (uint32_t)((G::NB * 16) >> 4) << 16;
   const uint32_t dcol = tmem_base + (uint32_t)Y::DCOL;
   for (int f = f_begin; f < f_end; f += SPS) {
@@ -516,14 +518,15 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
         if (i < n) {
           uint32_t a;
           if (S == sE1) {
-            const int step = f + i, pass = step / 13, u = BF16 ? 2 * step : step - 13 * pass;
+            const int step = f + i, pass = step / 13, u = BF16 ? 2 * step : (pass ? 2 * (step - 13) : step);
             a = a0 + (uint32_t)(Y::SRC0 >> 4) + (uint32_t)(Y::LEAD + 2 * u - Y::PAD);
+            if (!BF16 && pass) a += a_lbo_x2;              // [a1 of pair u | a1 of pair u + 1]
           } else if (Y::HALF >= SPS) {
             a = a0 + (uint32_t)(i * ((2 * Y::LBO) >> 4));
           } else {
             a = a0 + (uint32_t)((Y::a_off(i % Y::NKB) - Y::SRC0) >> 4) + (uint32_t)(2 * (i / Y::NKB));
           }
-          const bool half_n = (S == sE1) ? (BF16 ? f + i == 6 : (f + i) % 13 == 12) : (f + i >= LAST0);
+          const bool half_n = (S == sE1) ? (BF16 ? f + i == 6 : (f + i == 12 || f + i == 19)) : (f + i >= LAST0);
           const uint32_t b = (half_n ? b_lbo_h : b_lbo) + b0 + (uint32_t)(i * (G::STEP_BYTES >> 4));
           const uint32_t acc = (i > 0) ? 1u : (f > f_begin ? 1u : acc0);
 #pragma unroll
@@ -845,21 +848,23 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst_all) {
       else { u = f / d.nkb; kk = f % d.nkb; }
       unsigned char* step = dst + P.seg_off[d.seg] + (size_t)s * G::STEP_BYTES;
       if (d.seg == gE1 && !BF16 && split_e1) {
-        // split e1 of the TF32 kernel: BF16 pieces w = w1 + w2; pass 0 holds [w1 | w1] (meets [a1 | a2]), pass 1 [w2 | 0]
+        // split e1 of the TF32 kernel: BF16 pieces w = w1 + w2; pass 0 (13 steps) holds [w1 | w1] (meets [a1 | a2]),
+        // pass 1 (7 steps) [w2 of pair 2w | w2 of pair 2w + 1] (meets [a1 two rows apart])
+        if (pass) u = 2 * (f - 13);
         const bool half_x = 2 * u + 1 >= d.taps;
         const int nbx = half_x ? G::NB / 2 : G::NB;
         for (int h = 0; h < 2; ++h)
           for (int nl = 0; nl < nbx; ++nl)
             for (int e = 0; e < 8; ++e) {
               const int n = rank * nbx + nl;
-              const int co = n % C, j = 2 * u + n / C;
+              const int co = n % C, j = 2 * (u + (pass ? h : 0)) + n / C;
               const float v = j < d.taps ? W[((size_t)co * d.cin + e) * d.taps + j] : 0.0f;
               const uint16_t w1 = bf16_rne(v);
               uint32_t w1bits = (uint32_t)w1 << 16;
               float w1f;
               memcpy(&w1f, &w1bits, 4);
               const uint16_t w2 = bf16_rne(v - w1f);
-              const uint16_t out = pass == 0 ? w1 : (h == 0 ? w2 : (uint16_t)0);
+              const uint16_t out = pass == 0 ? w1 : w2;
               memcpy(step + ((size_t)h * nbx + nl) * 16 + e * 2, &out, 2);
             }
         continue;
