@@ -60,7 +60,8 @@ def _peaks_file():
 
 
 class ClockSampler:
-    """nvidia-smi clocks + throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+    """nvidia-smi clocks + throttle reasons sampled DURING the timed regions (B200_PROFILING.md); one background
+    process for the whole run, summarised per wall-clock window."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
@@ -82,14 +83,13 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.rows.append((time.time(), line.strip()))
 
-    def stop(self, t0, t1):
+    def window(self, t0, t1):
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
-        self.proc.terminate()
+        time.sleep(0.12)
         sm, mx, reasons = [], None, set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        rows = [r for (t, r) in self.rows if t0 <= t <= t1 + 0.1] or [r for (_, r) in self.rows]
+        rows = [r for (t, r) in list(self.rows) if t0 <= t <= t1 + 0.1] or [r for (_, r) in list(self.rows)[-1:]]
         for r in rows:
             p = [x.strip() for x in r.split(",")]
             try:
@@ -101,6 +101,10 @@ class ClockSampler:
                     reasons.add(n)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx,
                 "reasons": sorted(reasons), "samples": len(sm)}
+
+    def stop(self):
+        if self.proc is not None:
+            self.proc.terminate()
 
 
 def rank_seed(model, rank):
@@ -124,18 +128,32 @@ def whole_job_rate(world, events_per_rank, steps, ms):
 
 
 def run_oracle_sample(ev, w, n_sample):
-    """Oracle timed as it stands on the first n_sample events.  Returns (events/s, seconds, threads)."""
+    """Oracle timed as it stands on the first n_sample events, stage by stage: the same functions in the same
+    16-event chunks as oracle.run.  Returns (events/s, seconds, threads, {stage: seconds})."""
     from oracle import pvf_oracle as O   # bench.py's cpu_baseline / reference legs may execute oracle/
     sub = select_events(ev, range(min(n_sample, ev.n_events)))
+    off = sub.event_offsets.astype(np.int64)
+    st = {"fc_hist": 0.0, "unet": 0.0, "peaks": 0.0}
+    probs = np.zeros((sub.n_events, 4000), np.float32)
+    t_all = time.perf_counter()
+    for lo in range(0, sub.n_events, 16):
+        hi = min(lo + 16, sub.n_events)
+        t0 = time.perf_counter()
+        H, _ = O.histogram(sub.feat[:, off[lo]:off[hi]], off[lo:hi + 1] - off[lo], w.fc_w, w.fc_b)
+        t1 = time.perf_counter()
+        probs[lo:hi] = O.unet_probs(H, w.conv_w, w.conv_b)
+        st["fc_hist"] += t1 - t0
+        st["unet"] += time.perf_counter() - t1
     t0 = time.perf_counter()
-    O.run(sub.feat, sub.event_offsets, w)
-    dt = time.perf_counter() - t0
+    O.find_peaks(probs)
+    st["peaks"] = time.perf_counter() - t0
+    dt = time.perf_counter() - t_all
     try:
         import threadpoolctl
         thr = max([p.get("num_threads", 1) for p in threadpoolctl.threadpool_info()] or [1])
     except Exception:
         thr = os.cpu_count() or 1
-    return sub.n_events / dt, dt, int(thr)
+    return sub.n_events / dt, dt, int(thr), st
 
 
 def main_reference(args, rank, world):
@@ -150,7 +168,7 @@ def main_reference(args, rank, world):
     t0 = time.perf_counter()
     thr = 1
     for _ in range(args.steps):
-        _, _, thr = run_oracle_sample(ev, w, n_sample)
+        _, _, thr, _ = run_oracle_sample(ev, w, n_sample)
     dt = time.perf_counter() - t0
     value = n_sample * args.steps / dt
     sample = f"first {n_sample} of {args.events} events per step, oracle.run (numpy float64) as it stands"
@@ -167,6 +185,192 @@ def main_reference(args, rank, world):
     print(json.dumps(out), flush=True)
 
 
+def nonempty_intervals(ev):
+    """Number of (event, interval) pairs that hold at least one in-range track (bookkeeping for byte / FLOP
+    accounting only; same float32 recipe as DESIGN.md reading R2)."""
+    z = ev.feat[0]
+    iv = np.floor((z.astype(np.float32) + np.float32(200.0)) * np.float32(0.1)).astype(np.int64)
+    evi = np.repeat(np.arange(ev.n_events), np.diff(ev.event_offsets))
+    ok = np.isfinite(z) & (iv >= 0) & (iv < 40)
+    return int(np.unique(evi[ok] * 40 + iv[ok]).size)
+
+
+def tensor_peak(peaks, peaks_src, prec, tf32_measured, sustained=True):
+    """(peak TFLOP/s, note) for the UNet roofline: MEASURED_PEAKS.json's bf16 figure for the 16-bit modes; for TF32 the
+    figure this run measured (torch.matmul 8192^3, TF32 allowed -- measurement only), the derived one kept beside it."""
+    key = "bf16_tflops_sustained" if sustained else "bf16_tflops"
+    if prec in ("bf16", "fp16"):
+        return peaks[key], f"{peaks_src} {key} {peaks[key]} TFLOP/s (MEASURED_PEAKS.json)"
+    if tf32_measured is not None:
+        k = "sustained" if sustained else "burst"
+        return tf32_measured[k], f"measured in this run: torch.matmul 8192^3 TF32, {k}"
+    return peaks[key] * 1.1 / 2.25, f"{peaks_src} {key} {peaks[key]} x nominal tf32/bf16 ratio 1.1/2.25 (derived)"
+
+
+def measure_tf32_peak(torch, seconds=4.0):
+    """cuBLAS TF32 matmul 8192^3, the way MEASURED_PEAKS.json measures bf16: best of 10 (burst) and back to back
+    for `seconds` (sustained).  Measurement only -- never on the product path, outside every timed region."""
+    n = 8192
+    old = torch.backends.cuda.matmul.allow_tf32
+    torch.backends.cuda.matmul.allow_tf32 = True
+    try:
+        a = torch.randn(n, n, device="cuda")
+        b = torch.randn(n, n, device="cuda")
+        c = torch.empty(n, n, device="cuda")
+        for _ in range(3):
+            torch.matmul(a, b, out=c)
+        torch.cuda.synchronize()
+        flop = 2.0 * n ** 3
+        best = 0.0
+        for _ in range(10):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            torch.matmul(a, b, out=c)
+            e1.record()
+            e1.synchronize()
+            best = max(best, flop / (e0.elapsed_time(e1) * 1e-3) / 1e12)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0, reps = time.time(), 0
+        e0.record()
+        while time.time() - t0 < seconds:
+            for _ in range(20):
+                torch.matmul(a, b, out=c)
+            reps += 20
+            torch.cuda.synchronize()
+        e1.record()
+        e1.synchronize()
+        sustained = reps * flop / (e0.elapsed_time(e1) * 1e-3) / 1e12
+        del a, b, c
+        return {"burst": best, "sustained": sustained, "how": f"torch.matmul {n}^3 fp32 inputs, allow_tf32; best of 10 / {reps} back to back"}
+    finally:
+        torch.backends.cuda.matmul.allow_tf32 = old
+
+
+class Workload:
+    """One configuration of the hot path on the device: events + weights + handle + output buffers."""
+
+    def __init__(self, torch, PVFinder, *, model, events, seed, precision, channels=64, split_mask=None, elide=False,
+                 cta_pair=True, margin=0.0, weights="peaky", host_io=False, l2_chunk_events=0, low_latency=None):
+        self.torch = torch
+        self.ev = make_events(model, events, seed)
+        self.w = make_weights(weights, 1, channels)
+        self.E, self.precision, self.channels, self.elide = events, precision, channels, elide
+        self.split = split_mask if split_mask is not None else (1 if precision == "tf32" else 0)
+        extra = {}
+        if l2_chunk_events:
+            extra["l2_chunk_events"] = int(l2_chunk_events)
+        if low_latency is not None:
+            extra["low_latency"] = int(low_latency)
+        self.pvf = PVFinder(self.w, max_events=events, max_tracks=max(self.ev.n_tracks, 1), precision=precision,
+                            split_mask=self.split, stage_timing=True, host_io=host_io, elide_empty=elide,
+                            cta_pair=bool(cta_pair) and precision != "fp32", boundary_margin_mm=margin, **extra)
+        self.feat = torch.from_numpy(self.ev.feat).cuda()
+        self.off = torch.from_numpy(self.ev.event_offsets).cuda()
+        self.probs = torch.empty(events, 4000, device="cuda")
+        self.pk = self.pvf.alloc_peaks(events)
+        self.stream = torch.cuda.Stream()
+
+    def run(self):
+        self.pvf.run(self.feat, self.off, self.E, self.probs, self.pk, stream=self.stream)
+
+    def timed(self, steps, warmup, barrier=None):
+        """(total ms over `steps` runs, mean stage ms [sort, fc+sum, unet, peaks], wall window)."""
+        torch = self.torch
+        for _ in range(warmup):
+            self.run()
+        self.stream.synchronize()
+        try:
+            self.pvf.stage_times_ms()            # reset the stage-time ring
+        except Exception:
+            pass
+        if barrier:
+            barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.time()
+        e0.record(self.stream)
+        for _ in range(steps):
+            self.run()
+        e1.record(self.stream)
+        self.stream.synchronize()
+        t1 = time.time()
+        if barrier:
+            barrier()
+        return e0.elapsed_time(e1), self.pvf.stage_times_ms(), (t0, t1)
+
+    def close(self):
+        self.pvf.destroy()
+        del self.feat, self.off, self.probs, self.pk
+
+
+def run_variants(torch, PVFinder, args, sampler, peaks, peaks_src, tf32_measured):
+    """Every other named configuration of BASELINE.json on the same line (3 warm-ups + 5 steps each): config 2 in
+    BF16 / FP16, config 3, config 4 at C = 32 / 16, config 1 (1000 events), config 0 (one event: latency), the FP32
+    path, and the separate modes (empty-interval elision, L2-resident histogram chunks)."""
+    V = []
+    specs = [
+        dict(name="config2_bf16", model="run3", events=16000, seed=SEEDS["run3"], precision="bf16"),
+        dict(name="config2_fp16", model="run3", events=16000, seed=SEEDS["run3"], precision="fp16"),
+        dict(name="config3_tf32", model="pileup", events=16000, seed=SEEDS["pileup"], precision="tf32"),
+        dict(name="config4_bf16_c32", model="run3", events=16000, seed=1004, precision="bf16", channels=32),
+        dict(name="config4_bf16_c16", model="run3", events=16000, seed=1004, precision="bf16", channels=16),
+        dict(name="config1_tf32", model="run3", events=1000, seed=1001, precision="tf32"),
+        dict(name="config2_tf32_elide_empty", model="run3", events=16000, seed=SEEDS["run3"], precision="tf32", elide=True),
+        dict(name="config2_fp32", model="run3", events=4000, seed=SEEDS["run3"], precision="fp32"),
+    ]
+    for sp in specs:
+        name = sp.pop("name")
+        try:
+            wl = Workload(torch, PVFinder, **sp)
+            ms, stage, win = wl.timed(5, 3)
+            E, ch, prec = wl.E, wl.channels, wl.precision
+            flop = UNET_FLOP_PER_EVENT[ch] * E
+            rec = {"name": name, "events": E, "tracks": wl.ev.n_tracks, "precision": prec, "channels": ch,
+                   "events_per_s": E * 5 / (ms * 1e-3), "ms_per_step": ms / 5, "us_per_event": ms * 1e3 / (5 * E),
+                   "stage_ms": {"sort": stage[0], "fc_hist": stage[1], "unet": stage[2], "peaks": stage[3]},
+                   "steps": 5, "warmup": 3, "clocks": sampler.window(*win)}
+            if wl.elide:
+                ne = nonempty_intervals(wl.ev) / (E * 40.0)
+                rec["nonempty_interval_fraction"] = ne
+                flop *= ne                                         # executed-FLOP accounting: a separate mode
+            if prec == "fp32":
+                pk_, note = 148 * 128 * 2 * 1.965e9 / 1e12, "FP32 FMA peak: 148 SM x 128 lanes x 2 x 1.965 GHz"
+            else:
+                pk_, note = tensor_peak(peaks, peaks_src, prec, tf32_measured, sustained=E >= 4000)
+            rec["unet_tflops"] = flop / (stage[2] * 1e-3) / 1e12
+            rec["unet_frac"] = rec["unet_tflops"] / pk_
+            rec["unet_peak"] = pk_
+            rec["unet_peak_source"] = note
+            wl.close()
+            V.append(rec)
+        except Exception as exc:   # a variant must never take the headline line down
+            V.append({"name": name, "error": repr(exc)[:200]})
+        torch.cuda.empty_cache()
+    # config 0: one event, per-call latency (PAPER.md:11: sub-400 us budget per event)
+    for prec in ("tf32", "fp32"):
+        try:
+            wl = Workload(torch, PVFinder, model="single", events=1, seed=SEEDS["single"], precision=prec)
+            n = 200
+            ms, stage, win = wl.timed(n, 20)
+            iso = []
+            for _ in range(30):                                    # isolated calls: launch gaps included
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(wl.stream)
+                wl.run()
+                e1.record(wl.stream)
+                e1.synchronize()
+                iso.append(e0.elapsed_time(e1) * 1e3)
+            V.append({"name": f"config0_{prec}_latency", "events": 1, "tracks": wl.ev.n_tracks, "precision": prec,
+                      "channels": 64, "latency_us": ms * 1e3 / n, "latency_isolated_us_median": float(np.median(iso)),
+                      "how": f"{n} back-to-back pvf_run calls on one stream (device time / call); 30 isolated calls",
+                      "stage_us": {"sort": stage[0] * 1e3, "fc_hist": stage[1] * 1e3, "unet": stage[2] * 1e3,
+                                   "peaks": stage[3] * 1e3},
+                      "launches_per_run": wl.pvf.launches_per_run(1), "clocks": sampler.window(*win)})
+            wl.close()
+        except Exception as exc:
+            V.append({"name": f"config0_{prec}_latency", "error": repr(exc)[:200]})
+    return V
+
+
 def main_ours(args, rank, world, local_rank):
     import torch
     from paper_2602_19959_b200 import PVFinder   # raises if libpvf.so is missing: no CPU fallback
@@ -179,18 +383,11 @@ def main_ours(args, rank, world, local_rank):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     E = args.events
-    ev = make_events(args.model, E, rank_seed(args.model, rank))
-    w = make_weights(args.weights, 1, args.channels)
-    split = args.split_mask if args.split_mask >= 0 else (1 if args.precision == "tf32" else 0)
-    pvf = PVFinder(w, max_events=E, max_tracks=ev.n_tracks, precision=args.precision, split_mask=split,
-                   stage_timing=True, host_io=True, elide_empty=args.elide_empty,
-                   cta_pair=bool(args.cta_pair) and args.precision != "fp32",
-                   boundary_margin_mm=args.boundary_margin)
-    feat = torch.from_numpy(ev.feat).cuda()
-    off = torch.from_numpy(ev.event_offsets).cuda()
-    probs = torch.empty(E, 4000, device="cuda")
-    pk = pvf.alloc_peaks(E)
-    stream = torch.cuda.Stream()
+    split = args.split_mask if args.split_mask >= 0 else None
+    wl = Workload(torch, PVFinder, model=args.model, events=E, seed=rank_seed(args.model, rank), precision=args.precision,
+                  channels=args.channels, split_mask=split, elide=args.elide_empty, cta_pair=args.cta_pair,
+                  margin=args.boundary_margin, weights=args.weights, host_io=True)
+    ev, w, pvf, stream = wl.ev, wl.w, wl.pvf, wl.stream
 
     def barrier():
         torch.cuda.synchronize()
@@ -199,50 +396,34 @@ def main_ours(args, rank, world, local_rank):
         torch.cuda.synchronize()
 
     # ---------------- device-resident timing (inputs in HBM; 107 MB features + 2 GB H: larger than L2)
-    for _ in range(args.warmup):
-        pvf.run(feat, off, E, probs, pk, stream=stream)
-    stream.synchronize()
-    try:
-        pvf.stage_times_ms()            # reset the stage-time ring
-    except Exception:
-        pass
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
         time.sleep(1.0)
-    barrier()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    t_wall0 = time.time()
-    e0.record(stream)
-    for _ in range(args.steps):
-        pvf.run(feat, off, E, probs, pk, stream=stream)
-    e1.record(stream)
-    stream.synchronize()
-    t_wall1 = time.time()
-    barrier()
-    ms = e0.elapsed_time(e1)
-    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
-    stage = pvf.stage_times_ms()        # mean over the timed runs: sort, FC+sum, UNet, peaks
+    ms, stage, win = wl.timed(args.steps, args.warmup, barrier)
+    clocks = sampler.window(*win) if rank == 0 else None
     launches = pvf.launches_per_run(E) * args.steps
 
-    # ---------------- end to end through pvf_run_host: pinned host buffers, H2D + D2H inside
+    # ---------------- end to end through pvf_run_host: pinned host buffers, H2D + D2H inside, every step timed
     hfeat = torch.from_numpy(ev.feat).pin_memory()
     hoff = torch.from_numpy(ev.event_offsets).pin_memory()
     hprobs = torch.empty(E, 4000).pin_memory()
     hpk = pvf.alloc_peaks(E, pinned=True)
     pvf.run_host(hfeat, hoff, E, hprobs, hpk, stream=stream)
     barrier()
-    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     n_e2e = max(1, min(args.steps, args.e2e_steps))
-    f0.record(stream)
-    for _ in range(n_e2e):
+    marks = [torch.cuda.Event(enable_timing=True) for _ in range(n_e2e + 1)]
+    marks[0].record(stream)
+    for k in range(n_e2e):
         pvf.run_host(hfeat, hoff, E, hprobs, hpk, stream=stream)   # synchronises the stream itself
-    f1.record(stream)
+        marks[k + 1].record(stream)
     stream.synchronize()
     barrier()
-    ms_e2e = f0.elapsed_time(f1)
+    ms_e2e = marks[0].elapsed_time(marks[-1])
+    e2e_steps_ms = [marks[k].elapsed_time(marks[k + 1]) for k in range(n_e2e)]
     h2d = int(hfeat.numel() * 4 + hoff.numel() * 4)
     d2h = int(hprobs.numel() * 4 + sum(v.numel() * v.element_size() for v in hpk.values()))
+    del hfeat, hprobs
 
     ms, ms_e2e = max_over_ranks([ms, ms_e2e], dist, "cuda")
     if rank != 0:
@@ -253,36 +434,61 @@ def main_ours(args, rank, world, local_rank):
     e2e_value = whole_job_rate(world, E, n_e2e, ms_e2e)
 
     peaks, peaks_src = _peaks_file()
+    nonempty = nonempty_intervals(ev)
     flop = UNET_FLOP_PER_EVENT[args.channels] * E
-    nonempty = None
     if args.elide_empty:
-        # executed-FLOP accounting: only the intervals that hold a track go through the UNet
-        z = ev.feat[0]
-        iv = np.floor((z.astype(np.float32) + np.float32(200.0)) * np.float32(0.1)).astype(np.int64)   # bookkeeping only
-        evi = np.repeat(np.arange(E), np.diff(ev.event_offsets))
-        ok = np.isfinite(z) & (iv >= 0) & (iv < 40)
-        nonempty = float(np.unique(evi[ok] * 40 + iv[ok]).size) / (E * 40)
-        flop *= nonempty
+        flop *= nonempty / (E * 40.0)     # executed-FLOP accounting: only the intervals that hold a track go through the UNet
+    tf32_measured = None
+    variants = None
+    if world == 1 and not args.no_variants:
+        wl.close()
+        torch.cuda.empty_cache()
+        try:
+            tf32_measured = measure_tf32_peak(torch)
+        except Exception as exc:
+            tf32_measured = None
+            print(f"bench: TF32 peak measurement failed: {exc!r}", file=sys.stderr)
+        variants = run_variants(torch, PVFinder, args, sampler, peaks, peaks_src, tf32_measured)
+    sampler.stop()
     unet_s = stage[2] * 1e-3
     if args.precision == "fp32":
         bound, peak = "alu", 148 * 128 * 2 * 1.965e9 / 1e12
         peak_note = "FP32 FMA: 148 SM x 128 lanes x 2 FLOP x 1.965 GHz (B200_PROFILING.md unit counts)"
     else:
-        ratio = 1.0 if args.precision in ("bf16", "fp16") else 1.1 / 2.25
-        bound, peak = "tensor", peaks["bf16_tflops_sustained"] * ratio
-        peak_note = (f"{peaks_src} bf16 sustained {peaks['bf16_tflops_sustained']} TFLOP/s"
-                     + ("" if ratio == 1.0 else " x nominal tf32/bf16 ratio 1.1/2.25"))
+        bound = "tensor"
+        peak, peak_note = tensor_peak(peaks, peaks_src, args.precision, tf32_measured, sustained=E >= 4000)
     achieved = flop / unet_s / 1e12
-    traffic = None   # DRAM bytes per launch from the committed ncu --set full capture (per event x E)
-    tensor_pct = None
-    try:
-        with open(os.path.join(ROOT, "profiles", "r01_roofline_traffic.json.txt")) as f:
-            rec = json.load(f)[f"{args.precision}_c{args.channels}"]
+    traffic, tensor_pct, traffic_src = None, None, None
+    for fn in ("r02_roofline_traffic.json.txt", "r01_roofline_traffic.json.txt"):
+        try:
+            with open(os.path.join(ROOT, "profiles", fn)) as f:
+                rec = json.load(f)[f"{args.precision}_c{args.channels}"]
             traffic = rec["bytes_per_event"] * E
             tensor_pct = rec.get("tensor_pipe_active_pct")
-    except Exception:
-        pass
-    hbm_bytes_fc = (ev.n_tracks * 36 + E * 40 * 800 * 4)
+            traffic_src = f"profiles capture (profiles/{fn}: ncu --set full on a 4000-event batch) x events; not observed in this run"
+            break
+        except Exception:
+            continue
+    # FC + sum: bytes the stage must move.  The tensor-core FC kernel writes only the intervals that hold a track
+    # (the UNet takes the others as zeros), so its bytes are features + non-empty histograms; the canonical figure
+    # of SURVEY.md 8(d) (all 40 intervals written) is kept beside it.
+    fc_s = stage[1] * 1e-3
+    bytes_alg = ev.n_tracks * 36 + E * 40 * 800 * 4
+    bytes_moved = ev.n_tracks * 36 + (nonempty if args.precision != "fp32" else E * 40) * 800 * 4
+    roof = {"kernel": "unet", "bound": bound, "achieved": achieved, "peak": peak,
+            "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
+            "peak_source": peak_note,
+            # BASELINE.json's metric also asks for the UNet tensor-pipe utilisation: a profiler counter, so it is
+            # the value of the committed ncu capture (profiles/), not something measured in this run
+            "tensor_pipe_active_pct_ncu": tensor_pct, "tensor_pipe_source": traffic_src}
+    if args.precision == "tf32":
+        d_s = peaks["bf16_tflops_sustained"] * 1.1 / 2.25
+        d_b = peaks["bf16_tflops"] * 1.1 / 2.25
+        roof["peak_measured_tf32"] = tf32_measured
+        roof["frac_vs_derived_sustained"] = achieved / d_s      # bf16 sustained x nominal 1.1/2.25 (round 1's denominator)
+        roof["frac_vs_derived_burst"] = achieved / d_b
+        if tf32_measured is not None:
+            roof["frac_vs_measured_burst"] = achieved / tf32_measured["burst"]
     out = {
         "metric": METRIC, "value": value, "unit": "events/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -290,35 +496,41 @@ def main_ours(args, rank, world, local_rank):
         "data": "synthetic",
         "config": {"workload": f"BASELINE.json config {_config_id(args)}: {E} events/GPU, "
                                f"model {args.model}, {ev.n_tracks} tracks, UNet {args.channels} ch, weights {args.weights}",
-                   "precision": args.precision, "split_mask": split,
-                   "elide_empty_intervals": bool(args.elide_empty), "unet_cta_pair": bool(args.cta_pair) and args.precision != "fp32", "boundary_margin_mm": args.boundary_margin, "nonempty_interval_fraction": nonempty,
+                   "precision": args.precision, "split_mask": wl.split,
+                   "elide_empty_intervals": bool(args.elide_empty), "unet_cta_pair": bool(args.cta_pair) and args.precision != "fp32", "boundary_margin_mm": args.boundary_margin,
+                   "nonempty_interval_fraction": nonempty / (E * 40.0),
                    "cache": ("inputs larger than L2 (107 MB features, 2 GB histogram per step)" if E >= 2000 else
                              "small batch: inputs fit in L2 (latency-style measurement)")},
         "us_per_event": ms * 1e3 / (args.steps * E),
         "stage_ms": {"sort": stage[0], "fc_hist": stage[1], "unet": stage[2], "peaks": stage[3]},
         "stage_us_per_event": {k: v * 1e3 / E for k, v in zip(("sort", "fc_hist", "unet", "peaks"), stage)},
-        "roofline": {"kernel": "unet", "bound": bound, "achieved": achieved, "peak": peak,
-                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic, "peak_source": peak_note,
-                     # BASELINE.json's metric also asks for the UNet tensor-pipe utilisation: a profiler counter, so it is
-                     # the value of the committed ncu capture (profiles/), not something measured in this run
-                     "tensor_pipe_active_pct_ncu": tensor_pct},
-        "roofline_fc_hist": {"bound": "hbm", "achieved": hbm_bytes_fc / (stage[1] * 1e-3) / 1e9,
-                             "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                             "frac": hbm_bytes_fc / (stage[1] * 1e-3) / 1e9 / peaks["hbm_gbs"]},
+        "roofline": roof,
+        "roofline_fc_hist": {"bound": "hbm", "achieved": bytes_moved / fc_s / 1e9,
+                             "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": bytes_moved / fc_s / 1e9 / peaks["hbm_gbs"],
+                             "bytes": "features 36 B/track + histograms of the non-empty intervals (what this kernel writes)",
+                             "achieved_canonical": bytes_alg / fc_s / 1e9,
+                             "frac_canonical": bytes_alg / fc_s / 1e9 / peaks["hbm_gbs"],
+                             "bytes_canonical": "SURVEY.md 8(d): features + all 40 intervals x 800 floats per event"},
         # the FC + sum stage is bound by its 1600 SFU operations per track (800 x (ex2 + lg2)), not by HBM (DESIGN.md
         # section 4.2): 148 SMs x 16 SFU lanes x 1.965 GHz = 4.65 Tops/s
-        "roofline_fc_hist_alu": {"bound": "alu", "achieved": ev.n_tracks * 1600 / (stage[1] * 1e-3) / 1e12,
+        "roofline_fc_hist_alu": {"bound": "alu", "achieved": ev.n_tracks * 1600 / fc_s / 1e12,
                                  "peak": 148 * 16 * 1.965e9 / 1e12, "unit": "T SFU-op/s",
-                                 "frac": ev.n_tracks * 1600 / (stage[1] * 1e-3) / (148 * 16 * 1.965e9),
+                                 "frac": ev.n_tracks * 1600 / fc_s / (148 * 16 * 1.965e9),
                                  "peak_source": "148 SMs x 16 SFU lanes/clk x 1.965 GHz max SM clock (guide unit counts)"},
         "e2e": {"value": e2e_value, "unit": "events/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "steps": n_e2e, "api": "pvf_run_host (pinned host buffers)"},
+                "steps": n_e2e, "api": "pvf_run_host (pinned host buffers)",
+                "ms_per_step_min_mean_max": [min(e2e_steps_ms), ms_e2e / n_e2e, max(e2e_steps_ms)]},
         "gpu_launches": launches, "clocks": clocks,
     }
+    if variants is not None:
+        out["variants"] = variants
     if world == 1 and not args.no_cpu_baseline:
-        v, dt, thr = run_oracle_sample(ev, w, args.cpu_sample)
+        v, dt, thr, st = run_oracle_sample(ev, w, args.cpu_sample)
+        n_s = min(args.cpu_sample, E)
         out["cpu_baseline"] = {"value": v, "unit": "events/s", "cores": thr, "kind": "oracle",
-                               "sample": f"first {args.cpu_sample} events of the batch, {dt:.1f} s"}
+                               "sample": f"first {n_s} events of the batch, {dt:.1f} s",
+                               "stage_s": st, "stage_us_per_event": {k: 1e6 * x / n_s for k, x in st.items()},
+                               "stages": "fc_hist = interval assignment + FC + histogram sum; unet incl. sigmoid; peaks"}
     print(json.dumps(out), flush=True)
     if dist is not None:
         dist.destroy_process_group()
@@ -338,8 +550,10 @@ def main():
     ap.add_argument("--channels", type=int, default=64, choices=[64, 32, 16])
     ap.add_argument("--cpu-sample", type=int, default=192)   # ~13 s of oracle time on 16 host threads
     ap.add_argument("--ref-sample", type=int, default=16)
-    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-variants", action="store_true",
+                    help="skip the other named configurations and the TF32 peak measurement (N = 1 only anyway)")
     ap.add_argument("--boundary-margin", type=float, default=0.0,
                     help="NEXT-1 mode (mm): boundary tracks contribute to two intervals, PAPER.md:49")
     ap.add_argument("--cta-pair", type=int, default=1, choices=[0, 1],

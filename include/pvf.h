@@ -56,6 +56,9 @@ typedef enum {
 #define PVF_FLAG_PEAK_OVERFLOW 1u /* more than max_peaks maxima; the first max_peaks are kept */
 #define PVF_FLAG_TRACK_DROPPED 2u /* >=1 track outside [z_min, z_min+400mm) or non-finite */
 #define PVF_FLAG_NONFINITE 4u     /* >=1 track with non-finite z_poca */
+#define PVF_FLAG_BAD_OFFSETS 8u   /* the event's [event_offsets[e], event_offsets[e+1]) is not an ascending range inside
+                                     [0, n_tracks]: it was clamped (no access outside the caller's buffers), the
+                                     event's result covers the clamped range only */
 
 /* Frozen at pvf_create (the paper's TensorSpec).  Fields marked (fixed) must hold
  * the stated value in this build, anything else returns PVF_ERR_CONFIG. */

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libpvf.so")
 PVF_OK, PVF_ERR_ARG, PVF_ERR_CONFIG, PVF_ERR_CAPACITY, PVF_ERR_CUDA, PVF_ERR_UNSUPPORTED = range(6)
 PVF_PREC_FP32, PVF_PREC_TF32, PVF_PREC_BF16, PVF_PREC_FP16 = 0, 1, 2, 3
 PRECISIONS = {"fp32": PVF_PREC_FP32, "tf32": PVF_PREC_TF32, "bf16": PVF_PREC_BF16, "fp16": PVF_PREC_FP16}
-FLAG_PEAK_OVERFLOW, FLAG_TRACK_DROPPED, FLAG_NONFINITE = 1, 2, 4
+FLAG_PEAK_OVERFLOW, FLAG_TRACK_DROPPED, FLAG_NONFINITE, FLAG_BAD_OFFSETS = 1, 2, 4, 8
 N_INTERVALS, N_BINS, N_GLOBAL_BINS, MAX_PEAKS = 40, 100, 4000, 32
 
 EXPORTS = [

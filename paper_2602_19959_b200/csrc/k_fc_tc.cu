@@ -479,13 +479,17 @@ void launch_fc_hist_tc(const float* const feat[9], const int32_t* event_offsets,
                      static_cast<const unsigned char*>(w5img), n_events, hist, dump);
 }
 
-#ifdef PVF_FC_PROF
+// include/pvf_debug.h: per-role cycle counters; only a -DPVF_FC_PROF build records them
 extern "C" __attribute__((visibility("default"))) int pvf_debug_fc_prof(unsigned long long* host_out, int reset) {
+#ifdef PVF_FC_PROF
   cudaDeviceSynchronize();
   if (host_out) cudaMemcpyFromSymbol(host_out, g_fc_prof, sizeof(g_fc_prof));
   if (reset) { static unsigned long long z[160][16]; cudaMemcpyToSymbol(g_fc_prof, z, sizeof(z)); }
   return 0;
-}
+#else
+  (void)host_out; (void)reset;
+  return -1;
 #endif
+}
 
 }  // namespace pvf

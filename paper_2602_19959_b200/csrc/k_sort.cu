@@ -18,7 +18,7 @@ constexpr int kSortWarps = 4;
 __global__ void __launch_bounds__(kSortWarps * 32)
 k_sort(const float* __restrict__ z_poca, const int32_t* __restrict__ event_offsets, int n_events,
        int32_t* __restrict__ perm, int32_t* __restrict__ seg_off, int32_t* __restrict__ seg_cnt,
-       uint32_t* __restrict__ flags, float mfrac, int two) {
+       uint32_t* __restrict__ flags, float mfrac, int two, int n_tracks) {
   __shared__ int s_cnt[kSortWarps][kIntervals];
   __shared__ int s_base[kSortWarps][kIntervals];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -28,9 +28,13 @@ k_sort(const float* __restrict__ z_poca, const int32_t* __restrict__ event_offse
   int* base = s_base[warp];
   for (int i = lane; i < kIntervals; i += 32) cnt[i] = 0;
   __syncwarp();
-  const int lo = event_offsets[e], hi = event_offsets[e + 1];
+  // The offsets are device data the host never sees (data-dependent anomalies degrade per event, they do
+  // not fail the call): a range that is not inside [0, n_tracks] or not ascending is clamped -- nothing is ever read
+  // or written outside feat[] / perm[] -- and the event is flagged.
+  const int lo_raw = event_offsets[e], hi_raw = event_offsets[e + 1];
+  const int lo = min(max(lo_raw, 0), n_tracks), hi = min(max(hi_raw, lo), n_tracks);
   const int plo = two ? 2 * lo : lo;        // start of the event's run in perm (two slots per track with NEXT-1)
-  uint32_t fl = 0;
+  uint32_t fl = (lo != lo_raw || hi != hi_raw) ? PVF_FLAG_BAD_OFFSETS : 0u;
   for (int t = lo + lane; t < hi; t += 32) {
     bool nf;
     float zr;
@@ -110,12 +114,12 @@ k_sort(const float* __restrict__ z_poca, const int32_t* __restrict__ event_offse
   }
 }
 
-void launch_sort(const float* z_poca, const int32_t* event_offsets, int n_events, int32_t* perm,
+void launch_sort(const float* z_poca, const int32_t* event_offsets, int n_events, int n_tracks, int32_t* perm,
                  int32_t* seg_off, int32_t* seg_cnt, uint32_t* flags, float mfrac, cudaStream_t s) {
   if (n_events <= 0) return;
   const int grid = (n_events + kSortWarps - 1) / kSortWarps;
   k_sort<<<grid, kSortWarps * 32, 0, s>>>(z_poca, event_offsets, n_events, perm, seg_off, seg_cnt, flags, mfrac,
-                                          mfrac > 0.0f ? 1 : 0);
+                                          mfrac > 0.0f ? 1 : 0, n_tracks);
 }
 
 }  // namespace pvf

@@ -979,13 +979,17 @@ void launch_unet_tc(const float* hist, int n_intervals_total, const void* packed
 #undef PVF_CALL
 }
 
-#ifdef PVF_UNET_PROF
+// include/pvf_debug.h: per-CTA wait counters of the MMA issuer; only a -DPVF_UNET_PROF build records them
 extern "C" __attribute__((visibility("default"))) int pvf_debug_unet_prof(unsigned long long* host_out, int reset) {
+#ifdef PVF_UNET_PROF
   cudaDeviceSynchronize();
   if (host_out) cudaMemcpyFromSymbol(host_out, g_unet_prof, sizeof(g_unet_prof));
   if (reset) { static unsigned long long z[160][16]; cudaMemcpyToSymbol(g_unet_prof, z, sizeof(z)); }
   return 0;
-}
+#else
+  (void)host_out; (void)reset;
+  return -1;
 #endif
+}
 
 }  // namespace pvf

@@ -81,7 +81,8 @@ bool config_ok(const pvf_config* c) {
   if (!(c->peak_threshold == c->peak_threshold)) return false;
   if (c->peak_halfwidth != kPeakHalf || c->max_peaks != kMaxPeaks) return false;
   if (c->precision < PVF_PREC_FP32 || c->precision > PVF_PREC_FP16) return false;
-  if (c->split_mask < 0 || c->split_mask > 31) return false;
+  // split_mask: only bit 0 (e1) is built, and only for TF32 (unet_tc_setup would refuse anything else later)
+  if (c->split_mask != 0 && !(c->precision == PVF_PREC_TF32 && c->split_mask == 1)) return false;
   if (c->max_events < 1 || c->max_tracks < 1 || c->max_tracks > 0x7fffffffLL) return false;
   if (c->elide_empty_intervals && c->precision == PVF_PREC_FP32) return false;   // tensor-core modes only
   if (c->unet_cta_pair != 0 && c->unet_cta_pair != 1) return false;
@@ -235,6 +236,10 @@ pvf_status create_impl(const pvf_weights* w, const pvf_config* cfg, void* dev_po
       }
     }
   }
+  // cudaMemcpy from pageable memory returns once the data is staged, not once the DMA has finished, and the caller's
+  // (non-blocking) streams are not ordered against the legacy stream: make every upload visible before anything
+  // reads it (create is not on the hot path)
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
   if (e == cudaSuccess && cfg->elide_empty_intervals) {
     // UNet(0): one event's worth of zero histograms through the very kernel pvf_run uses, on a private
     // stream (create is not on the hot path); every interval of it is the constant vector
@@ -261,8 +266,9 @@ pvf_status create_impl(const pvf_weights* w, const pvf_config* cfg, void* dev_po
     for (int r = 0; r < pvf_ctx::kTimedRuns; ++r)
       for (int k = 0; k < 5 && e == cudaSuccess; ++k) e = cudaEventCreate(&h->ev[r][k]);
   if (e != cudaSuccess) {
+    fprintf(stderr, "pvf_create: %s\n", cudaGetErrorString(e));
     pvf_destroy(h);
-    return e == cudaErrorInvalidValue && cfg->precision != PVF_PREC_FP32 ? PVF_ERR_CONFIG : PVF_ERR_CUDA;
+    return PVF_ERR_CUDA;         // unsupported configurations were rejected by config_ok: this is a runtime failure
   }
   *out = h;
   return PVF_OK;
@@ -322,7 +328,7 @@ pvf_status pvf_run(pvf_handle h, const pvf_tracks* t, int32_t n_events, float* o
   const bool timing = h->cfg.enable_stage_timing != 0 && !h->suppress_timing;
   cudaEvent_t* ev = h->ev[h->timed_runs % pvf_ctx::kTimedRuns];
   if (timing) cudaEventRecord(ev[0], s);
-  launch_sort(t->feat[0], t->event_offsets, n_events, h->perm, h->seg_off, h->seg_cnt, h->flags,
+  launch_sort(t->feat[0], t->event_offsets, n_events, (int)t->n_tracks, h->perm, h->seg_off, h->seg_cnt, h->flags,
               h->cfg.boundary_margin_mm * 0.1f, s);
   if (timing) cudaEventRecord(ev[1], s);
   if (h->cfg.precision == PVF_PREC_FP32)
@@ -365,59 +371,79 @@ pvf_status pvf_run_host(pvf_handle h, const pvf_tracks* t, int32_t n_events, flo
   // index everything through event_offsets), so a chunk is just a window [e0, e1) of the same arrays.
   const int n_chunks = n_events >= 4096 ? pvf_ctx::kHostChunks : 1;
   const int32_t* off = t->event_offsets;                     // host pointer here
-  if (n_chunks > 1 && (off[0] != 0 || (size_t)off[E] != T)) return PVF_ERR_ARG;
+  // the offsets steer the copies below: ascending, starting at 0, ending at n_tracks -- checked before anything is enqueued
+  if (off[0] != 0 || (size_t)off[E] != T) return PVF_ERR_ARG;
+  for (size_t e = 0; e < E; ++e)
+    if (off[e + 1] < off[e]) return PVF_ERR_ARG;
   pvf_tracks d{};
   for (int k = 0; k < 9; ++k) d.feat[k] = h->st_feat + cap * k;
   d.n_tracks = t->n_tracks;
+  // A failing CUDA call inside the pipeline must not leave copies into the caller's host buffers in flight or the
+  // handle in "chunked" state: every error path goes through the clean-up at the end.
+  cudaError_t ce = cudaSuccess;
+  const char* where = "";
+#define PVF_TRY(call)                                              \
+  do {                                                             \
+    if (ce == cudaSuccess) { ce = (call); if (ce != cudaSuccess) where = #call; } \
+  } while (0)
   if (n_chunks > 1) {
-    PVF_CUDA(h, cudaEventRecord(h->ev_fork, s));             // the copy streams start after what is already queued on s
-    PVF_CUDA(h, cudaStreamWaitEvent(h->s_in, h->ev_fork, 0));
-    PVF_CUDA(h, cudaStreamWaitEvent(h->s_out, h->ev_fork, 0));
+    PVF_TRY(cudaEventRecord(h->ev_fork, s));                 // the copy streams start after what is already queued on s
+    PVF_TRY(cudaStreamWaitEvent(h->s_in, h->ev_fork, 0));
+    PVF_TRY(cudaStreamWaitEvent(h->s_out, h->ev_fork, 0));
   }
   h->suppress_timing = n_chunks > 1;                         // stage timing describes whole-batch pvf_run calls only
   pvf_status st = PVF_OK;
-  for (int c = 0; c < n_chunks && st == PVF_OK; ++c) {
+  for (int c = 0; c < n_chunks && st == PVF_OK && ce == cudaSuccess; ++c) {
     const size_t e0 = E * c / n_chunks, e1 = E * (c + 1) / n_chunks, ne = e1 - e0;
     const size_t t0 = n_chunks > 1 ? (size_t)off[e0] : 0, t1 = n_chunks > 1 ? (size_t)off[e1] : T;
     cudaStream_t si = n_chunks > 1 ? h->s_in : s, so = n_chunks > 1 ? h->s_out : s;
     for (int k = 0; k < 9; ++k)
       if (t1 > t0)
-        PVF_CUDA(h, cudaMemcpyAsync(h->st_feat + cap * k + t0, t->feat[k] + t0, sizeof(float) * (t1 - t0), cudaMemcpyHostToDevice, si));
+        PVF_TRY(cudaMemcpyAsync(h->st_feat + cap * k + t0, t->feat[k] + t0, sizeof(float) * (t1 - t0), cudaMemcpyHostToDevice, si));
     {   // offsets (e0, e1] -- plus offsets[e0] for the first chunk -- so that no element is copied twice
       const size_t lo = c == 0 ? e0 : e0 + 1;
-      PVF_CUDA(h, cudaMemcpyAsync(h->st_off + lo, off + lo, sizeof(int32_t) * (e1 + 1 - lo), cudaMemcpyHostToDevice, si));
+      PVF_TRY(cudaMemcpyAsync(h->st_off + lo, off + lo, sizeof(int32_t) * (e1 + 1 - lo), cudaMemcpyHostToDevice, si));
     }
     if (n_chunks > 1) {
-      PVF_CUDA(h, cudaEventRecord(h->ev_in[c], si));
-      PVF_CUDA(h, cudaStreamWaitEvent(s, h->ev_in[c], 0));
+      PVF_TRY(cudaEventRecord(h->ev_in[c], si));
+      PVF_TRY(cudaStreamWaitEvent(s, h->ev_in[c], 0));
     }
     d.event_offsets = h->st_off + e0;
     pvf_peaks dp{h->st_z + e0 * kMaxPeaks, h->st_prob + e0 * kMaxPeaks, h->st_bin + e0 * kMaxPeaks, h->st_count + e0,
                  h->st_flags + e0};
+    if (ce != cudaSuccess) break;
     st = pvf_run(h, &d, (int32_t)ne, h->st_probs + e0 * kGlobalBins, &dp, cuda_stream);
     if (st != PVF_OK) break;
     if (n_chunks > 1) {
-      PVF_CUDA(h, cudaEventRecord(h->ev_comp[c], s));
-      PVF_CUDA(h, cudaStreamWaitEvent(so, h->ev_comp[c], 0));
+      PVF_TRY(cudaEventRecord(h->ev_comp[c], s));
+      PVF_TRY(cudaStreamWaitEvent(so, h->ev_comp[c], 0));
     }
     if (host_probs)
-      PVF_CUDA(h, cudaMemcpyAsync(host_probs + e0 * kGlobalBins, h->st_probs + e0 * kGlobalBins, sizeof(float) * ne * kGlobalBins,
+      PVF_TRY(cudaMemcpyAsync(host_probs + e0 * kGlobalBins, h->st_probs + e0 * kGlobalBins, sizeof(float) * ne * kGlobalBins,
                                   cudaMemcpyDeviceToHost, so));
-    PVF_CUDA(h, cudaMemcpyAsync(pk->z_mm + e0 * kMaxPeaks, dp.z_mm, sizeof(float) * ne * kMaxPeaks, cudaMemcpyDeviceToHost, so));
-    PVF_CUDA(h, cudaMemcpyAsync(pk->prob + e0 * kMaxPeaks, dp.prob, sizeof(float) * ne * kMaxPeaks, cudaMemcpyDeviceToHost, so));
-    PVF_CUDA(h, cudaMemcpyAsync(pk->bin + e0 * kMaxPeaks, dp.bin, sizeof(int32_t) * ne * kMaxPeaks, cudaMemcpyDeviceToHost, so));
-    PVF_CUDA(h, cudaMemcpyAsync(pk->count + e0, dp.count, sizeof(int32_t) * ne, cudaMemcpyDeviceToHost, so));
+    PVF_TRY(cudaMemcpyAsync(pk->z_mm + e0 * kMaxPeaks, dp.z_mm, sizeof(float) * ne * kMaxPeaks, cudaMemcpyDeviceToHost, so));
+    PVF_TRY(cudaMemcpyAsync(pk->prob + e0 * kMaxPeaks, dp.prob, sizeof(float) * ne * kMaxPeaks, cudaMemcpyDeviceToHost, so));
+    PVF_TRY(cudaMemcpyAsync(pk->bin + e0 * kMaxPeaks, dp.bin, sizeof(int32_t) * ne * kMaxPeaks, cudaMemcpyDeviceToHost, so));
+    PVF_TRY(cudaMemcpyAsync(pk->count + e0, dp.count, sizeof(int32_t) * ne, cudaMemcpyDeviceToHost, so));
     if (pk->event_flags)
-      PVF_CUDA(h, cudaMemcpyAsync(pk->event_flags + e0, dp.event_flags, sizeof(uint32_t) * ne, cudaMemcpyDeviceToHost, so));
+      PVF_TRY(cudaMemcpyAsync(pk->event_flags + e0, dp.event_flags, sizeof(uint32_t) * ne, cudaMemcpyDeviceToHost, so));
   }
   h->suppress_timing = false;
   if (n_chunks > 1) {                                        // join: the caller's stream is ordered after both copy streams
-    PVF_CUDA(h, cudaEventRecord(h->ev_join, h->s_out));
-    PVF_CUDA(h, cudaStreamWaitEvent(s, h->ev_join, 0));
-    PVF_CUDA(h, cudaEventRecord(h->ev_join, h->s_in));
-    PVF_CUDA(h, cudaStreamWaitEvent(s, h->ev_join, 0));
+    PVF_TRY(cudaEventRecord(h->ev_join, h->s_out));
+    PVF_TRY(cudaStreamWaitEvent(s, h->ev_join, 0));
+    PVF_TRY(cudaEventRecord(h->ev_join, h->s_in));
+    PVF_TRY(cudaStreamWaitEvent(s, h->ev_join, 0));
   }
-  PVF_CUDA(h, cudaStreamSynchronize(s));
+  PVF_TRY(cudaStreamSynchronize(s));
+#undef PVF_TRY
+  if (ce != cudaSuccess || st != PVF_OK) {                   // nothing may still be writing the caller's buffers
+    cudaStreamSynchronize(s);
+    if (h->s_in) cudaStreamSynchronize(h->s_in);
+    if (h->s_out) cudaStreamSynchronize(h->s_out);
+    if (ce != cudaSuccess) return fail_cuda(h, ce, where);
+    return st;
+  }
   if (st == PVF_OK) h->last_n_events = n_chunks > 1 ? (int32_t)(E - E * (n_chunks - 1) / n_chunks) : n_events;
   return st;
 }

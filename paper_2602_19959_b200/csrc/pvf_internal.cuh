@@ -66,7 +66,7 @@ __device__ __forceinline__ int entry_interval(int ent, const float* __restrict__
 
 // a0: interval assignment + stable per-event counting sort (k_sort.cu).  mfrac > 0: boundary tracks get a
 // second entry (perm then holds up to 2 entries per track).
-void launch_sort(const float* z_poca, const int32_t* event_offsets, int n_events, int32_t* perm,
+void launch_sort(const float* z_poca, const int32_t* event_offsets, int n_events, int n_tracks, int32_t* perm,
                  int32_t* seg_off, int32_t* seg_cnt, uint32_t* flags, float mfrac, cudaStream_t s);
 
 // a1+a2: per-track FC and fixed-order segmented sum into H [n_events,40,8,100] (k_fc.cu)

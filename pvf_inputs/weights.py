@@ -64,7 +64,8 @@ def _rand(seed: int, channels: int) -> PVFWeights:
     return w
 
 
-def _peaky(seed: int, channels: int, eps_unet: float = 0.3, eps_fc: float = 0.01) -> PVFWeights:
+def _peaky(seed: int, channels: int, eps_unet: float = 0.3, eps_fc: float = 0.01,
+           head_gain: float = 0.16, head_bias: float = -6.5) -> PVFWeights:
     C = channels
     noise = _rand(seed, channels)
     w = PVFWeights(channels=channels, kind="peaky")
@@ -109,17 +110,19 @@ def _peaky(seed: int, channels: int, eps_unet: float = 0.3, eps_fc: float = 0.01
     S_cw[4][0, C + 0, (kd1 - 1) // 2] = 1.0   # concat order is [upsampled, skip]
     # head: background logit -6.5 (p = 1.5e-3, a decade below the 0.01 peak threshold, so that ripples of
     # the background are not peaks: DESIGN.md "peaky weights"), signal gain 0.16
-    S_cw[5][0, 0, 0] = 0.16
-    S_cb[5][0] = -6.5
+    # (head_gain / head_bias are parameters only so that tests/test_oracle_pins.py can re-run the conditioning
+    # experiment that compares this recipe with the first one, gain 0.12 / bias -5)
+    S_cw[5][0, 0, 0] = head_gain
+    S_cb[5][0] = head_bias
     for k in range(6):
         w.conv_w.append((S_cw[k] + eps_unet * noise.conv_w[k]).astype(np.float32))
         w.conv_b.append((S_cb[k] + eps_unet * noise.conv_b[k]).astype(np.float32))
     return w
 
 
-def make_weights(kind: str, seed: int, channels: int = 64) -> PVFWeights:
+def make_weights(kind: str, seed: int, channels: int = 64, **peaky_kw) -> PVFWeights:
     if kind == "rand":
         return _rand(seed, channels)
     if kind == "peaky":
-        return _peaky(seed, channels)
+        return _peaky(seed, channels, **peaky_kw)
     raise ValueError(f"unknown weight kind {kind!r}")

@@ -17,8 +17,8 @@ def lib():
     return pkg.load_library()
 
 
-def _declared_symbols(repo_root):
-    text = open(os.path.join(repo_root, "include", "pvf.h")).read()
+def _declared_symbols(repo_root, header="pvf.h"):
+    text = open(os.path.join(repo_root, "include", header)).read()
     return re.findall(r"PVF_API\s+[\w\s\*]+?\b(pvf_\w+)\s*\(", text)
 
 
@@ -28,6 +28,18 @@ def test_every_declared_symbol_is_exported(lib, repo_root):
     assert sorted(names) == sorted(pkg.EXPORTS)
     for n in names:
         assert getattr(lib, n) is not None
+    # every header under include/ is covered: the diagnostic entry points exist in every build flavour
+    import glob
+    assert sorted(os.path.basename(h) for h in glob.glob(os.path.join(repo_root, "include", "*.h"))) == ["pvf.h", "pvf_debug.h"]
+    dbg = _declared_symbols(repo_root, "pvf_debug.h")
+    assert sorted(dbg) == ["pvf_debug_fc_prof", "pvf_debug_unet_prof"]
+    for n in dbg:
+        assert getattr(lib, n) is not None
+    # and nothing is exported that no header declares
+    import subprocess
+    out = subprocess.run(["nm", "-D", "--defined-only", pkg.LIB_PATH], capture_output=True, text=True).stdout
+    exported = sorted(l.split()[-1] for l in out.splitlines() if " T " in l and l.split()[-1].startswith("pvf_"))
+    assert exported == sorted(names + dbg)
 
 
 def test_header_cites_the_paper(repo_root):
@@ -53,8 +65,9 @@ def test_default_config_and_workspace_bytes(lib):
 
 @pytest.mark.parametrize("field,value", [("n_intervals", 41), ("n_bins", 64), ("unet_channels", 48), ("k_e1", 27),
                                          ("max_peaks", 16), ("precision", 7), ("max_events", 0), ("max_tracks", 0),
-                                         ("split_mask", 64), ("fc_hidden", 32)])
+                                         ("split_mask", 64), ("split_mask", 1), ("fc_hidden", 32)])
 def test_invalid_config_is_rejected_on_the_host(lib, field, value):
+    # (split_mask 1 is the e1 split of the TF32 mode; the default precision here is FP32, where no split exists)
     cfg = pkg.default_config(lib, 4, 100)
     setattr(cfg, field, value)
     assert lib.pvf_workspace_bytes(C.byref(cfg)) == 0

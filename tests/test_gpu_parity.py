@@ -164,48 +164,109 @@ def test_edge_events_empty_dropped_nonfinite_and_long(prec):
     assert np.all(P[0] == P[0, 0]) and np.array_equal(P[0], P[3])
 
 
+@pytest.mark.parametrize("prec,margin", [("fp32", 0.0), ("tf32", 0.0), ("tf32", 0.5)])
+def test_corrupt_event_offsets_are_clamped_and_flagged(prec, margin):
+    """The device-side event_offsets are data the host never sees: ranges that leave [0, n_tracks] or run backwards
+    must not make any kernel touch memory outside the caller's / the pool's buffers (per-event
+    degradation instead of a failing call).  The pool is caller-supplied here with guard bytes behind it."""
+    ev = make_events("run3", 8, 91)
+    w = make_weights("peaky", 2)
+    ref = O.run(ev.feat, ev.event_offsets, w)
+    T = ev.n_tracks
+    pvf0 = _make(w, ev, prec, boundary_margin_mm=margin)
+    nbytes = pvf0.workspace_bytes()
+    guard = 1 << 20
+    pool = torch.full((nbytes + guard,), 0x5A, dtype=torch.uint8, device="cuda")
+    pvf = PVFinder(w, max_events=8, max_tracks=T, precision=prec, split_mask=SPLIT[prec], boundary_margin_mm=margin, pool=pool)
+    feat = torch.from_numpy(ev.feat).cuda()
+    probs = torch.full((8, 4000), -1.0, device="cuda")
+    pk = pvf.alloc_peaks(8)
+    s = torch.cuda.Stream()
+
+    def go(off):
+        probs.fill_(-1.0)
+        pvf.run(feat, torch.from_numpy(off).cuda(), 8, probs, pk, stream=s)
+        s.synchronize()
+        assert bool((pool[nbytes:] == 0x5A).all())                   # nothing written behind the pool
+        assert bool(torch.isfinite(probs).all()) and float(probs.min()) > 0.0
+        fl = pk["flags"].cpu().numpy().astype(np.uint32)
+        return (fl & pkg.FLAG_BAD_OFFSETS) != 0, probs.cpu().numpy().astype(np.float64)
+
+    # A: event 2 runs backwards (event 3 then also covers the last 17 tracks of event 1); the last event reaches far
+    # past the end of the track arrays (clamped to what is there, i.e. to its true range)
+    off = ev.event_offsets.copy()
+    off[3] = off[2] - 17
+    off[8] = T + 5000
+    bad, P = go(off)
+    assert list(bad) == [False, False, True, False, False, False, False, True]
+    if margin == 0.0:                  # events whose tracks no broken range touches are unaffected
+        assert np.abs(P[[0, 4, 5, 6, 7]] - ref["probs"][[0, 4, 5, 6, 7]]).max() <= TOL[prec]
+    # B: negative start, absurd end: both clamp to the true ranges
+    off = ev.event_offsets.copy()
+    off[0] = -40
+    off[8] = 2**31 - 1
+    bad, P = go(off)
+    assert list(bad) == [True] + [False] * 6 + [True]
+    if margin == 0.0:
+        assert np.abs(P - ref["probs"]).max() <= TOL[prec]
+    # and the same handle still serves a well-formed batch
+    probs2, _ = _run(pvf, ev)
+    assert np.abs(probs2.cpu().numpy().astype(np.float64) - ref["probs"]).max() <= TOL[prec] or margin > 0.0
+
+
 # ------------------------------------------------------------------ a3 + whole path
-def _available(prec, w, ev):
-    try:
-        return _make(w, ev, prec)
-    except pkg.PVFError as exc:
-        if exc.status == pkg.PVF_ERR_CONFIG:
-            pytest.skip(f"precision {prec} not built yet")
-        raise
-
-
 _ORACLE_CACHE = {}
 
 
-def _oracle_cached(kind, n_events):
-    """Oracle results are shared by the precisions of one weight kind (the oracle takes ~70 ms/event)."""
-    key = (kind, n_events)
+def _oracle_cached(kind, n_events, model="run3", seed=1001, ch=64, wseed=1, sample=None, n_total=None):
+    """Oracle results are shared by the precisions of one (events, weights) pair (the oracle takes ~70 ms/event).
+    sample: indices into a batch of n_total events -> the oracle sees only those (full-size tests)."""
+    key = (kind, n_events, model, seed, ch, wseed, None if sample is None else tuple(sample), n_total)
     if key not in _ORACLE_CACHE:
-        ev = make_events("run3", n_events, 1001)
-        w = make_weights(kind, 1)
-        _ORACLE_CACHE[key] = (ev, w, O.run(ev.feat, ev.event_offsets, w))
+        ev = make_events(model, n_events if n_total is None else n_total, seed)
+        w = make_weights(kind, wseed, ch)
+        sub = ev if sample is None else select_events(ev, sample)
+        _ORACLE_CACHE[key] = (ev, w, O.run(sub.feat, sub.event_offsets, w))
     return _ORACLE_CACHE[key]
 
 
-# share of ALL oracle peaks that must be matched within +-1 bin on `peaky` (north_star: 99.9 %; the BF16
-# variant has a stated 2e-2 probability tolerance, so peaks whose height is within that error of the
-# 0.01 threshold cannot be guaranteed: stated bar 99 %, DESIGN.md "Tolerances")
-PEAK_SHARE = {"fp32": 0.999, "tf32": 0.999, "bf16": 0.99, "fp16": 0.995}
+# north_star: "End-to-end peak positions must agree within 1 bin (0.1 mm) on at least 99.9% of oracle peaks" -- the
+# same bar for every precision and width, evaluated on `peaky` (on `rand` the criterion is ill-posed, DESIGN.md 3).
+PEAK_SHARE = 0.999
+
+
+def _peak_agreement(ref_probs, ref_bins, ref_count, got_bins, got_count):
+    """(matched, total, lost) over events where neither side hit the 32-peak cap; lost = [(event, bin, oracle P)]."""
+    m_all = n_all = 0
+    lost = []
+    for e in range(ref_probs.shape[0]):
+        if ref_count[e] >= 32 or got_count[e] >= 32:
+            continue
+        rb = [int(b) for b in ref_bins[e] if b >= 0]
+        tb = [int(b) for b in got_bins[e] if b >= 0]
+        m, n, _ = O.match_peaks(rb, tb)
+        m_all += m; n_all += n
+        if m < n:
+            lost += [(e, g, float(ref_probs[e, g])) for g in rb if not any(abs(g - t) <= 1 for t in tb)]
+    return m_all, n_all, lost
 
 
 @pytest.mark.parametrize("prec", ["fp32", "tf32", "bf16", "fp16"])
 @pytest.mark.parametrize("kind", ["rand", "peaky"])
 def test_whole_path_parity(prec, kind):
     # peaky: BASELINE.json config 1 (1000 events, ~5400 oracle peaks) so that 99.9 % is resolvable
-    ev, w, ref = _oracle_cached(kind, 1000 if kind == "peaky" else 48)
-    pvf = _available(prec, w, ev)
+    # rand (the config-0 literal weights): 300 events -- SURVEY.md 8c-P predicts the TF32 max|dP| to grow with the
+    # sample (6e-4 at 50 events -> 1.25e-3 at 300 single-pass, 8.3e-4 with the e1 split); the printed value says which
+    ev, w, ref = _oracle_cached(kind, 1000 if kind == "peaky" else 300)
+    pvf = _make(w, ev, prec)
     probs, pk = _run(pvf, ev)
     Pg = probs.cpu().numpy()
     err = np.abs(Pg.astype(np.float64) - ref["probs"]).max(axis=1)
+    print(f"[{prec}] {kind} {ev.n_events} events: max|dP| {err.max():.3e}")
     assert err.max() <= TOL[prec], f"max|dP| per event: {err.max():.3e}"
     got = _np(pk)
     tau = max(float(err.max()), 1e-7)
-    m_all = n_all = m_st = n_st = 0
+    m_st = n_st = 0
     for e in range(ev.n_events):
         cand = np.nonzero((ref["probs"][e] > 0.01) & (ref["probs"][e] > np.r_[-np.inf, ref["probs"][e][:-1]])
                           & (ref["probs"][e] >= np.r_[ref["probs"][e][1:], -np.inf]))[0]
@@ -213,13 +274,11 @@ def test_whole_path_parity(prec, kind):
         st = O.tau_stable_peaks(ref["probs"][e], cand, tau)
         m, n, _ = O.match_peaks(st, gcand)
         m_st += m; n_st += n
-        if ref["peaks"]["count"][e] < 32 and got["count"][e] < 32:
-            m, n, _ = O.match_peaks(ref["peaks"]["bin"][e], got["bin"][e])
-            m_all += m; n_all += n
     assert m_st == n_st, f"tau-stable peaks matched {m_st}/{n_st}"
     if kind == "peaky":
-        print(f"[{prec}] peaky: max|dP| {err.max():.3e}; peaks matched {m_all}/{n_all}; tau-stable {m_st}/{n_st}")
-        assert n_all > 3000 and m_all >= PEAK_SHARE[prec] * n_all, f"peaks matched {m_all}/{n_all}"
+        m_all, n_all, lost = _peak_agreement(ref["probs"], ref["peaks"]["bin"], ref["peaks"]["count"], got["bin"], got["count"])
+        print(f"[{prec}] peaky: peaks matched {m_all}/{n_all}; tau-stable {m_st}/{n_st}; lost (event, bin, P) {lost[:8]}")
+        assert n_all > 3000 and m_all >= PEAK_SHARE * n_all, f"peaks matched {m_all}/{n_all}; lost {lost[:8]}"
     # the library's own peak finder on its own probabilities is the oracle's definition, bit for bit
     own = O.find_peaks(Pg)
     assert np.array_equal(own["bin"], got["bin"]) and np.array_equal(own["z"].view(np.uint32), got["z"].view(np.uint32))
@@ -228,12 +287,20 @@ def test_whole_path_parity(prec, kind):
 @pytest.mark.parametrize("prec", ["fp32", "tf32", "bf16", "fp16"])
 @pytest.mark.parametrize("ch", [32, 16])
 def test_width_sweep_parity(prec, ch):
-    ev = make_events("run3", 16, 1004)
-    w = make_weights("rand", 1, ch)
-    ref = O.run(ev.feat, ev.event_offsets, w)
-    pvf = _available(prec, w, ev)
-    probs, _ = _run(pvf, ev)
+    """BASELINE.json config 4: "Sweep UNet width 16/32/64 channels ... per-width tolerance 2e-2 on probabilities plus
+    peak agreement within 1 bin against the FP64 oracle" -- probabilities on `rand` (48 events) and `peaky` (160
+    events), peak agreement on `peaky` at north_star's 99.9 % (width 64 is test_whole_path_parity)."""
+    ev, w, ref = _oracle_cached("rand", 48, seed=1004, ch=ch)
+    probs, _ = _run(_make(w, ev, prec), ev)
     assert np.abs(probs.cpu().numpy().astype(np.float64) - ref["probs"]).max() <= TOL[prec]
+    ev, w, ref = _oracle_cached("peaky", 160, seed=1001, ch=ch)
+    probs, pk = _run(_make(w, ev, prec), ev)
+    err = float(np.abs(probs.cpu().numpy().astype(np.float64) - ref["probs"]).max())
+    assert err <= TOL[prec], f"{prec} C={ch}: max|dP| {err:.3e}"
+    got = _np(pk)
+    m_all, n_all, lost = _peak_agreement(ref["probs"], ref["peaks"]["bin"], ref["peaks"]["count"], got["bin"], got["count"])
+    print(f"[{prec} C={ch}] peaky 160 events: max|dP| {err:.3e}; peaks matched {m_all}/{n_all}; lost {lost[:8]}")
+    assert n_all > 500 and m_all >= PEAK_SHARE * n_all, f"peaks matched {m_all}/{n_all}; lost {lost[:8]}"
 
 
 def _pv_efficiency(pv_z, z_found, count, window_mm=0.5):
@@ -256,31 +323,23 @@ def _pv_efficiency(pv_z, z_found, count, window_mm=0.5):
 @pytest.mark.parametrize("ch", [64, 32, 16])
 def test_accuracy_vs_width_and_precision_table(ch):
     """accuracy-vs-width/precision on `peaky` (config-1 event model, 160 events, each width with
-    its own `peaky` weights).  Asserts the tolerances; with PVF_WRITE_TABLES=1 appends the rows to
-    gpurun_out/accuracy_table_rows.md (copied to profiles/r01_accuracy_table.md)."""
-    import os
-    ev = make_events("run3", 160, 1001)
-    w = make_weights("peaky", 1, ch)
-    ref = O.run(ev.feat, ev.event_offsets, w)
+    its own `peaky` weights).  Asserts the tolerances and prints the table rows (pytest -s; profiles/*accuracy_table.md
+    is a copy of that output)."""
+    ev, w, ref = _oracle_cached("peaky", 160, seed=1001, ch=ch)
     eff_o, fake_o = _pv_efficiency(ev.pv_z, ref["peaks"]["z"], ref["peaks"]["count"])
     rows = [f"| {ch} | oracle (FP64) | - | {int(ref['peaks']['count'].sum())} | - | {100 * eff_o:.1f} | {fake_o:.2f} |"]
     for prec in ["fp32", "tf32", "fp16", "bf16"]:
-        pvf = _available(prec, w, ev)
+        pvf = _make(w, ev, prec)
         probs, pk = _run(pvf, ev)
         err = float(np.abs(probs.cpu().numpy().astype(np.float64) - ref["probs"]).max())
         assert err <= TOL[prec], f"{prec} C={ch}: max|dP| {err:.3e}"
         got = _np(pk)
-        m_all = n_all = 0
-        for e in range(ev.n_events):
-            m, n, _ = O.match_peaks(ref["peaks"]["bin"][e], got["bin"][e])
-            m_all += m; n_all += n
-        assert m_all >= 0.98 * n_all
+        m_all, n_all, lost = _peak_agreement(ref["probs"], ref["peaks"]["bin"], ref["peaks"]["count"], got["bin"], got["count"])
+        assert m_all >= PEAK_SHARE * n_all, f"{prec} C={ch}: peaks matched {m_all}/{n_all}; lost {lost[:8]}"
         eff, fake = _pv_efficiency(ev.pv_z, got["z"], got["count"])
         assert abs(eff - eff_o) <= 0.01                           # precision does not change what the toy finds
         rows.append(f"| {ch} | {prec} | {err:.2e} | {int(got['count'].sum())} | {m_all}/{n_all} | {100 * eff:.1f} | {fake:.2f} |")
-    if os.environ.get("PVF_WRITE_TABLES") == "1" and os.path.isdir("gpurun_out"):
-        with open("gpurun_out/accuracy_table_rows.md", "a") as f:
-            f.write("\n".join(rows) + "\n")
+    print("\n".join(rows))
 
 
 @pytest.mark.parametrize("prec", ["fp32", "tf32", "bf16", "fp16"])
@@ -293,12 +352,7 @@ def test_unet_entry_point_on_synthetic_histograms(prec):
     H[2] = np.random.default_rng(3).gamma(2.0, 4.0, size=(40, 8, 100)).astype(np.float32)
     ref = O.unet_probs(H.astype(np.float64), w.conv_w, w.conv_b)
     ev = make_events("single", 1, 1)
-    try:
-        pvf = PVFinder(w, max_events=E, max_tracks=1, precision=prec, split_mask=SPLIT[prec])
-    except pkg.PVFError as exc:
-        if exc.status == pkg.PVF_ERR_CONFIG:
-            pytest.skip(f"precision {prec} not built yet")
-        raise
+    pvf = PVFinder(w, max_events=E, max_tracks=1, precision=prec, split_mask=SPLIT[prec])
     out = torch.empty(E, 4000, device="cuda")
     s = torch.cuda.Stream()
     pvf.run_unet(torch.from_numpy(H).cuda(), E, out, stream=s)
@@ -538,25 +592,32 @@ def test_host_io_chunk_pipeline_matches_device_run(prec, margin):
 
 
 # ------------------------------------------------------------------ full size, bench launch configuration
-@pytest.mark.parametrize("prec,model", [("tf32", "run3"), ("bf16", "run3"), ("fp32", "run3"), ("tf32", "pileup"),
-                                        ("fp16", "pileup")])
-def test_full_batch_sampled_events(prec, model):
-    """BASELINE.json config 2 / config 3 (16000 events) in the launch configuration bench.py times; the
-    oracle computes sampled events one by one; properties hold for every event."""
+FULL_CASES = [  # (precision, event model, channels): BASELINE.json configs 2, 3 and 4 (16 000 events each)
+    ("tf32", "run3", 64), ("bf16", "run3", 64), ("fp16", "run3", 64),         # config 2 (+ config 4 at C = 64)
+    ("tf32", "pileup", 64), ("fp16", "pileup", 64),                            # config 3
+    ("bf16", "run3", 32), ("bf16", "run3", 16),                                # config 4 width sweep
+    ("fp32", "run3", 64),                                                      # CUDA-core path (2000 events)
+]
+
+
+@pytest.mark.parametrize("prec,model,ch", FULL_CASES)
+def test_full_batch_sampled_events(prec, model, ch):
+    """BASELINE.json configs 2 / 3 / 4 (16000 events) in the launch configuration bench.py times; the oracle
+    computes 256 events chosen by a seeded draw (plus the first and last two); properties hold for every event."""
     E = 16000 if prec != "fp32" else 2000
-    ev = make_events(model, E, 1002 if model == "run3" else 1003)
-    w = make_weights("peaky", 1)
-    pvf = _available(prec, w, ev)
+    seed = {"run3": 1002 if ch == 64 else 1004, "pileup": 1003}[model]
+    rng = np.random.default_rng(2602)
+    sample = sorted(set(rng.choice(E, 252, replace=False).tolist()) | {0, 1, E - 2, E - 1})
+    ev, w, ref = _oracle_cached("peaky", len(sample), model=model, seed=seed, ch=ch, sample=sample, n_total=E)
+    pvf = _make(w, ev, prec)
     probs, pk = _run(pvf, ev)
-    sample = [0, 1, E // 2, E - 2, E - 1, 4097, 777][: 7 if E > 5000 else 5]
-    sub = select_events(ev, sample)
-    ref = O.run(sub.feat, sub.event_offsets, w)
     got = probs[sample].cpu().numpy()
-    assert np.abs(got.astype(np.float64) - ref["probs"]).max() <= TOL[prec]
-    gb = pk["bin"][sample].cpu().numpy()
-    for i in range(len(sample)):
-        m, n, _ = O.match_peaks(ref["peaks"]["bin"][i], gb[i])
-        assert m >= n - 1
+    err = float(np.abs(got.astype(np.float64) - ref["probs"]).max())
+    assert err <= TOL[prec], f"max|dP| {err:.3e}"
+    gb, gc = pk["bin"][sample].cpu().numpy(), pk["count"][sample].cpu().numpy()
+    m_all, n_all, lost = _peak_agreement(ref["probs"], ref["peaks"]["bin"], ref["peaks"]["count"], gb, gc)
+    print(f"[{prec} {model} C={ch}] {E} events, {len(sample)} sampled: max|dP| {err:.3e}; peaks {m_all}/{n_all}; lost {lost[:8]}")
+    assert n_all > 1000 and m_all >= PEAK_SHARE * n_all, f"peaks matched {m_all}/{n_all}; lost {lost[:8]}"
     # properties at any size: probabilities in (0,1); peak bins ascending, counts consistent
     # (a float32 sigmoid saturates to exactly 1.0 for logits > ~17: dense pile-up peaks of the toy weights do)
     assert float(probs.min()) > 0.0 and float(probs.max()) <= 1.0 and bool(torch.isfinite(probs).all())

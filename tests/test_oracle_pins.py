@@ -383,3 +383,44 @@ def test_boundary_tracks_contribute_to_the_neighbouring_interval():
     iv2, zr2, _ = O.assign_intervals(feat2[0])
     nb2, z22 = O.boundary_neighbours(iv2, zr2, 0.5)
     assert iv2[0] == 7 and nb2[0] == 8 and abs(float(z22[0]) + 0.03) < 1e-5
+
+
+# ---------------------------------------------------------------- conditioning of the `peaky` head
+def test_peaky_head_recipe_conditioning():
+    """Why `peaky` uses head gain 0.16 / bias -6.5 and not the first recipe (0.12 / -5).
+    Oracle only: uniform noise of +-5e-4 -- half of north_star's 1e-3 probability tolerance, i.e. what ANY
+    implementation that merely meets the tolerance may add -- is put on the oracle's own probabilities (three
+    noise seeds) and the oracle's peak finder is run again.  First recipe: the background probability (0.007)
+    sits next to the 0.01 threshold, ripples of the background are oracle 'peaks', and more than 1 % of the
+    peaks are lost, most of them NOT because of their height.  Final recipe (background 0.0016): the only
+    peaks white noise of that size can still remove are the ones whose height is within the noise of the
+    threshold itself (P[g] <= 0.01 + 5e-4) -- a few per thousand, unavoidable for any threshold on a continuous
+    output.  Nothing of the CUDA path is involved here."""
+    ev = make_events("run3", 64, 1001)
+    amp = 5e-4
+    lost, lost_far = {}, {}
+    for name, kw in (("first", dict(head_gain=0.12, head_bias=-5.0)), ("final", {})):
+        w = make_weights("peaky", 1, **kw)
+        ref = O.run(ev.feat, ev.event_offsets, w)
+        P = ref["probs"]
+        bg = float(np.median(P))
+        assert (0.005 < bg < 0.01) if name == "first" else (bg < 0.0025)
+        m = n = far = 0
+        for seed in (7, 8, 9):
+            rng = np.random.default_rng(seed)
+            Q = (P.astype(np.float64) + rng.uniform(-amp, amp, P.shape)).astype(np.float32)
+            pk = O.find_peaks(Q)
+            for e in range(ev.n_events):
+                rb = [int(b) for b in ref["peaks"]["bin"][e] if b >= 0]
+                tb = [int(b) for b in pk["bin"][e] if b >= 0]
+                a, b, _ = O.match_peaks(rb, tb)
+                m += a
+                n += b
+                if a < b:      # lost peaks whose height is NOT within the noise of the threshold
+                    far += sum(1 for g in rb if not any(abs(g - t) <= 1 for t in tb) and P[e, g] > 0.01 + 2 * amp)
+        assert n > 900
+        lost[name], lost_far[name] = 1.0 - m / n, far
+    assert lost["first"] > 0.01, lost
+    assert lost_far["first"] > 0, lost_far                 # the first recipe loses peaks well above the threshold
+    assert lost["final"] < 0.5 * lost["first"], lost
+    assert lost_far["final"] == 0, lost_far                # the final one only threshold-adjacent ones
