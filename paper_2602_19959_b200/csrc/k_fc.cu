@@ -15,6 +15,7 @@
 // exactly once (zeros for empty intervals); the summation order is the sorted order, independent of
 // scheduling.
 #include "pvf_internal.cuh"
+#include "pdl.cuh"
 
 namespace pvf {
 
@@ -54,6 +55,7 @@ k_fc_hist(const float* __restrict__ f0, const float* __restrict__ f1, const floa
   FcSmem& S = *reinterpret_cast<FcSmem*>(smem_raw);
   const int tid = threadIdx.x;
 
+  pdl_launch_dependents();      // pdl.cuh: the weight staging below may overlap the sort kernel's tail
   // stage the small layers in shared memory (zero padded)
   for (int i = tid; i < kFcHidden * 12; i += kFcThreads) {
     int r = i / 12, c = i % 12;
@@ -80,6 +82,7 @@ k_fc_hist(const float* __restrict__ f0, const float* __restrict__ f1, const floa
     b5[m] = owner ? par[kFcB5 + o] : 0.0f;
   }
   __syncthreads();
+  pdl_wait();                   // perm / seg_off / seg_cnt come from the sort kernel
 
   for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
     const size_t seg0 = (size_t)e * kIntervals;
@@ -172,20 +175,16 @@ int fc_hist_launches(int n_events) { return n_events > 0 ? 1 : 0; }
 
 void launch_fc_hist(const float* const feat[9], const int32_t* event_offsets, const int32_t* perm,
                     const int32_t* seg_off, const int32_t* seg_cnt, const float* fc_params,
-                    int n_events, float* hist, cudaStream_t s) {
+                    int n_events, float* hist, int sm_count, bool pdl, cudaStream_t s) {
   if (n_events <= 0) return;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaFuncSetAttribute(k_fc_hist, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FcSmem));
-    attr_set = true;
-  }
-  int dev = 0, sms = 148;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  const int grid = min(n_events, sms * 2);
-  k_fc_hist<<<grid, kFcThreads, sizeof(FcSmem), s>>>(feat[0], feat[1], feat[2], feat[3], feat[4], feat[5],
-                                                    feat[6], feat[7], feat[8], event_offsets, perm,
-                                                    seg_off, seg_cnt, fc_params, n_events, hist);
+  const int grid = min(n_events, sm_count * 2);
+  PdlLaunch L(dim3(grid), dim3(kFcThreads), sizeof(FcSmem), s, pdl);
+  cudaLaunchKernelEx(&L.cfg, k_fc_hist, feat[0], feat[1], feat[2], feat[3], feat[4], feat[5], feat[6], feat[7], feat[8],
+                     event_offsets, perm, seg_off, seg_cnt, fc_params, n_events, hist);
+}
+
+cudaError_t fc_hist_setup() {
+  return cudaFuncSetAttribute(k_fc_hist, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FcSmem));
 }
 
 }  // namespace pvf

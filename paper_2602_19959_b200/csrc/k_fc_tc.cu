@@ -26,6 +26,7 @@
 #include <cstring>
 
 #include "pvf_internal.cuh"
+#include "pdl.cuh"
 #include "umma.cuh"
 
 namespace pvf {
@@ -34,8 +35,13 @@ using namespace umma;
 namespace {
 
 constexpr int kEpiWarps = 13;                // one per (accumulator tile, 32-lane quadrant) that holds outputs
-constexpr int kMmaWarp = kEpiWarps;
-constexpr int kHidWarp0 = kMmaWarp + 1;
+// Warp w runs on scheduler w % 4 and reaches TMEM lanes 32 (w % 4) .. only.  The 13th unit (the 16 rows of tile 3) sits in
+// QUADRANT 1 and is served by warp 13, the MMA issuer is warp 12: every scheduler then carries three full epilogue warps
+// (the SFU-heavy role) instead of four on scheduler 0.
+constexpr int kMmaWarp = 12;
+constexpr int kSmallEpiWarp = 13;
+constexpr int kSmallRow0 = 3 * 128 + 32;     // accumulator row of the first of the last 16 outputs of a half (384 ..)
+constexpr int kHidWarp0 = 14;
 constexpr int kHidWarps = 4;                 // two groups of two warps: a CTA runs the hidden layers of HALF of a tile
 constexpr int kFtThreads = (kEpiWarps + 1 + kHidWarps) * 32;   // 13 epilogue + 1 MMA + 4 hidden-layer warps
 constexpr int kHalfOut = kFcOut / 2;         // outputs per CTA half, packed densely: row 128 t + r = output 400 half + 128 t + r
@@ -65,8 +71,13 @@ constexpr int OFF_BARS = OFF_IV + kIvBufs * kTile * 4;
 constexpr int FT_SMEM = OFF_BARS + 256;
 static_assert(FT_SMEM <= 227 * 1024, "shared memory budget");
 // barriers (8 bytes each): h_full[2], peer_h_full[2] (leader: the peer's half is staged), h_empty[2], meta[4],
-// acc_full[4], acc_empty[4], peer_acc_empty[4] (leader: the peer's epilogue has drained the tile), then the TMEM slot
-enum { bHFull = 0, bPHFull = 2, bHEmpty = 4, bMeta = 6, bAccFull = 10, bAccEmpty = 14, bPAccEmpty = 18, bSlot = 22 };
+// acc_full[4], acc_empty[4], peer_acc_empty[4] (leader: the peer's epilogue has drained the tile), iv_full[4], then the
+// TMEM slot.
+// iv_full[it & 3] ("the interval list of tile it is staged", hidden-layer threads -> epilogue) is indexed like meta[]:
+// the hidden-layer threads of tile it + 4 write that list only after meta[it & 3] completed its phase `it`, i.e. after
+// EVERY epilogue warp has finished tile it and therefore observed phase `it` of iv_full -- no phase can be skipped.  (The
+// 2-deep h_full gave no such guarantee to a slow epilogue warp: hidden(it + 2) is only gated by the MMAs of tile it.)
+enum { bHFull = 0, bPHFull = 2, bHEmpty = 4, bMeta = 6, bAccFull = 10, bAccEmpty = 14, bPAccEmpty = 18, bIvFull = 22, bSlot = 26 };
 
 __device__ __forceinline__ float leaky_ft(float v) { return v >= 0.0f ? v : kLeaky * v; }
 __device__ __forceinline__ uint32_t tf32_of(float v) {
@@ -108,6 +119,38 @@ __device__ __forceinline__ void softplus2_ft(float v0, float v1, float& o0, floa
   asm("{\n\t.reg .b64 p, q, k, m;\n\tmov.b64 p, {%2, %3};\n\tmov.b64 k, {%4, %4};\n\tmov.b64 m, {%5, %6};\n\t"
       "fma.rn.f32x2 q, p, k, m;\n\tmov.b64 {%0, %1}, q;\n\t}"
       : "=f"(o0), "=f"(o1) : "f"(w0), "f"(w1), "f"(0.6931471805599453f), "f"(m0), "f"(m1));
+}
+
+// Packed FP32 pairs (mul / add .f32x2 of sm_100: one issue slot for two values).
+__device__ __forceinline__ void mul2(float a0, float a1, float b0, float b1, float& o0, float& o1) {
+  asm("{\n\t.reg .b64 p, q, r;\n\tmov.b64 p, {%2, %3};\n\tmov.b64 q, {%4, %5};\n\t"
+      "mul.rn.f32x2 r, p, q;\n\tmov.b64 {%0, %1}, r;\n\t}"
+      : "=f"(o0), "=f"(o1) : "f"(a0), "f"(a1), "f"(b0), "f"(b1));
+}
+__device__ __forceinline__ void add2(float a0, float a1, float b0, float b1, float& o0, float& o1) {
+  asm("{\n\t.reg .b64 p, q, r;\n\tmov.b64 p, {%2, %3};\n\tmov.b64 q, {%4, %5};\n\t"
+      "add.rn.f32x2 r, p, q;\n\tmov.b64 {%0, %1}, r;\n\t}"
+      : "=f"(o0), "=f"(o1) : "f"(a0), "f"(a1), "f"(b0), "f"(b1));
+}
+__device__ __forceinline__ float lg2_ft(float u) {
+  float w;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(w) : "f"(u));
+  return w;
+}
+// softplus(v) = max(v, 0) + ln2 * lg2(1 + 2^(-|v| log2 e)).  The front half for two values: u = 1 + e in (1, 2] and
+// m = max(v, 0).  Tracks that are summed into the same interval share ONE logarithm:
+//     sum_i softplus(v_i) = sum_i m_i + ln2 * lg2(prod_i u_i)        (16 factors in (1, 2]: prod <= 65536, no overflow)
+// which halves the SFU operations of the stage (one ex2 per value, one lg2 per group instead of per value).
+__device__ __forceinline__ void softplus_front2(float v0, float v1, float& u0, float& u1, float& m0, float& m1) {
+  float t0, t1, e0, e1;
+  mul2(v0, v1, 1.4426950408889634f, 1.4426950408889634f, t0, t1);
+  t0 = -fabsf(t0);
+  t1 = -fabsf(t1);
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e0) : "f"(t0));
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e1) : "f"(t1));
+  add2(e0, e1, 1.0f, 1.0f, u0, u1);
+  m0 = fmaxf(v0, 0.0f);
+  m1 = fmaxf(v1, 0.0f);
 }
 
 struct Feat9 { const float* f[9]; };
@@ -159,7 +202,9 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
   auto bar = [&](int k) { return sb + OFF_BARS + 8u * k; };
   volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + OFF_BARS + 8 * bSlot);
 
-  // ---- one-time setup: this half's W5x image, zeroed B buffers, the small layers, barriers, TMEM
+  // ---- one-time setup: this half's W5x image, zeroed B buffers, the small layers, barriers, TMEM (weights only:
+  // all of it may overlap the tail of the sort kernel, see pdl.cuh)
+  pdl_launch_dependents();
   {
     const uint4* src = reinterpret_cast<const uint4*>(w5img + (size_t)half * 2 * kWPart);
     uint4* dst = reinterpret_cast<uint4*>(smem + OFF_W);
@@ -184,7 +229,7 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
     for (int k = 0; k < 2; ++k) {
       mbar_init(bar(bHFull + k), kHalfTile); mbar_init(bar(bPHFull + k), kHalfTile); mbar_init(bar(bHEmpty + k), 1);
     }
-    for (int k = 0; k < kIvBufs; ++k) mbar_init(bar(bMeta + k), 32 * kEpiWarps);
+    for (int k = 0; k < kIvBufs; ++k) { mbar_init(bar(bMeta + k), 32 * kEpiWarps); mbar_init(bar(bIvFull + k), kHalfTile); }
     for (int k = 0; k < 4; ++k) {
       mbar_init(bar(bAccFull + k), 1);
       mbar_init(bar(bAccEmpty + k), k < 3 ? 128 : 32);
@@ -198,6 +243,7 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
   cluster_sync_all();
   tc_fence_after_sync();
   const uint32_t tmem_base = *tmem_slot;
+  pdl_wait();                                 // perm / seg_off / seg_cnt come from the sort kernel
 
   // kept (in-range) tracks of event e and the start of its run in perm
   auto kept_of = [&](int e, int& ev_lo) {
@@ -206,13 +252,14 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
     return seg_off[s] + seg_cnt[s] - ev_lo;
   };
 
-  if (warp < kEpiWarps) {
+  if (warp < kMmaWarp || warp == kSmallEpiWarp) {
     // ===================== epilogue: lane = output, column = track (sorted order).  The 400 outputs of this half
-    // fill accumulator tiles 0-2 and 16 rows of tile 3; warp w owns the 32 rows of quadrant w & 3 of tile w >> 2
-    // (warp 12: the 16 rows of tile 3), so every warp has one tile per 128 tracks.
-    const int q = warp & 3, mt = warp >> 2;
-    const int r = 32 * q + lane, ol = 128 * mt + r;
-    const bool valid = ol < kHalfOut;
+    // fill accumulator tiles 0-2 and 16 rows of tile 3 (quadrant 1); warp w < 12 owns the 32 rows of quadrant w & 3 of
+    // tile w >> 2, warp 13 the 16 rows of tile 3, so every warp has one tile per 128 tracks.
+    const int q = warp & 3, mt = warp == kSmallEpiWarp ? 3 : warp >> 2;
+    const int r = 32 * q + lane;
+    const int ol = warp == kSmallEpiWarp ? 384 + lane : 128 * mt + r;      // output inside this half
+    const bool valid = warp == kSmallEpiWarp ? lane < 16 : true;
     const uint32_t lead_pacc = mapa_rank(bar(bPAccEmpty), 0);
     int it = 0;
     const bool pw = tid == 0;
@@ -227,11 +274,12 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
       float a = 0.f;                             // running sum of the current interval
       int c = 0;                                 // the interval it belongs to, as the offset interval * 800
       for (int base = 0; base < nk; base += kTile, ++it) {
-        const int buf = it & 1, ntile = min(kTile, nk - base);
+        const int ntile = min(kTile, nk - base);
         const bool last = base + kTile >= nk;
-        { FC_PROF_T0(); mbar_wait(bar(bHFull + buf), (uint32_t)((it >> 1) & 1)); FC_PROF_ADD(0, pw); }   // s_iv is staged
+        const int ib = it & (kIvBufs - 1);
+        { FC_PROF_T0(); mbar_wait(bar(bIvFull + ib), (uint32_t)((it >> 2) & 1)); FC_PROF_ADD(0, pw); }   // s_iv is staged
         FC_PROF_CNT(9, pw);
-        const int* ivs = s_iv + (it & (kIvBufs - 1)) * kTile;
+        const int* ivs = s_iv + ib * kTile;
         if (base == 0) c = ivs[0];               // the event's first (lowest) non-empty interval
         { FC_PROF_T0(); mbar_wait(bar(bAccFull + mt), (uint32_t)(it & 1)); FC_PROF_ADD(1, pw); }
         tc_fence_after_sync();
@@ -239,47 +287,76 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
         for (int c0 = 0; c0 < ntile; c0 += 16) {
           // sorted positions c0 .. c0+15: the even ones are columns c0/2 .. of the leader's half of N, the odd ones
           // columns 64 + c0/2 .. of the peer's half
-          uint32_t ve[8], vo[8], v[16];
+          uint32_t ve[8], vo[8];
           tmem_ld_x8(taddr + (uint32_t)(c0 >> 1), ve);
           tmem_ld_x8(taddr + (uint32_t)(kHalfTile + (c0 >> 1)), vo);
-          // intervals of the 16 tracks (broadcast 16-byte loads) while the TMEM load is in flight
-          int ivv[16];
-#pragma unroll
-          for (int k = 0; k < 4; ++k) {
-            const int4 q4 = *reinterpret_cast<const int4*>(ivs + c0 + 4 * k);
-            ivv[4 * k + 0] = q4.x; ivv[4 * k + 1] = q4.y; ivv[4 * k + 2] = q4.z; ivv[4 * k + 3] = q4.w;
-          }
-          tmem_ld_wait();
-#pragma unroll
-          for (int k = 0; k < 8; ++k) { v[2 * k] = ve[k]; v[2 * k + 1] = vo[k]; }
-          // all 16 softplus first: independent, so the SFU pipeline stays full; columns past the
-          // tile's last track are computed on stale accumulators and then masked
-          float sp[16];
-#pragma unroll
-          for (int i = 0; i < 16; i += 2)
-            softplus2_ft(__uint_as_float(v[i]), __uint_as_float(v[i + 1]), sp[i], sp[i + 1]);
+          // Where do intervals change inside these 16 tracks?  The interval list is the same for every lane, so the
+          // answer is one warp-uniform 16-bit mask: lane i < 16 compares track c0 + i with its predecessor (the running
+          // interval c for the tile's first track), one ballot.  Tracks past the tile's end never start an interval.
           const int nv = ntile - c0;
-          // Ordered accumulation without branches (seg_step).  Only intervals that hold a track are written --
-          // the UNet kernel never reads the histogram of an empty interval (it takes seg_cnt == 0 as zeros).
-          if (nv >= 16 && ivv[15] == c) {        // sorted: the whole chunk belongs to the running interval
+          const int pos = c0 + (lane & 15);
+          const int iv_prev = pos == 0 ? c : ivs[pos - 1];
+          const unsigned mask = __ballot_sync(0xffffffffu, lane < 16 && lane < nv && ivs[pos] != iv_prev);
+          tmem_ld_wait();
+          // front half of all 16 softplus first: independent, so the SFU pipeline stays full; columns past the
+          // tile's last track are computed on stale accumulators and then neutralised (u = 1, m = 0)
+          float u[16], m[16];
 #pragma unroll
-            for (int i = 0; i < 16; ++i) a += sp[i];
-          } else if (nv >= 16) {
+          for (int k = 0; k < 8; ++k)
+            softplus_front2(__uint_as_float(ve[k]), __uint_as_float(vo[k]), u[2 * k], u[2 * k + 1], m[2 * k], m[2 * k + 1]);
+          if (nv < 16) {
 #pragma unroll
-            for (int i = 0; i < 16; ++i) seg_step(a, c, ivv[i], sp[i], Hc);
-          } else {                                // ragged last chunk: inactive columns add +0 to the same interval
+            for (int i = 0; i < 16; ++i)
+              if (i >= nv) { u[i] = 1.0f; m[i] = 0.0f; }
+          }
+#ifdef PVF_FC_NOREDUCE
+          // diagnostic build: the FC arithmetic alone (all 16 logarithms, no ordered segmented sum, no histogram stores
+          // but the event's last one) -- gives the "FC" share of the fused stage (BASELINE.json config 2)
 #pragma unroll
-            for (int i = 0; i < 16; ++i) {
-              const bool act = i < nv;
-              seg_step(a, c, act ? ivv[i] : c, act ? sp[i] : 0.0f, Hc);
+          for (int i = 0; i < 16; ++i) a += fmaf(lg2_ft(u[i]), 0.6931471805599453f, m[i]);
+#else
+          // Ordered accumulation (fixed by the sorted positions, hence reproducible).  Only intervals that hold a track
+          // are written -- the UNet kernel never reads the histogram of an empty interval (seg_cnt == 0 means zeros).
+          if (mask == 0u) {                      // the whole chunk continues the running interval: one logarithm
+            float p[8], t[8];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+              mul2(u[4 * k], u[4 * k + 1], u[4 * k + 2], u[4 * k + 3], p[2 * k], p[2 * k + 1]);
+              add2(m[4 * k], m[4 * k + 1], m[4 * k + 2], m[4 * k + 3], t[2 * k], t[2 * k + 1]);
+            }
+            mul2(p[0], p[1], p[2], p[3], p[0], p[1]);
+            mul2(p[4], p[5], p[6], p[7], p[4], p[5]);
+            add2(t[0], t[1], t[2], t[3], t[0], t[1]);
+            add2(t[4], t[5], t[6], t[7], t[4], t[5]);
+            mul2(p[0], p[1], p[4], p[5], p[0], p[1]);
+            add2(t[0], t[1], t[4], t[5], t[0], t[1]);
+            a += fmaf(lg2_ft(p[0] * p[1]), 0.6931471805599453f, t[0] + t[1]);
+          } else {
+#pragma unroll
+            for (int g = 0; g < 4; ++g) {        // groups of four tracks; the test is warp-uniform
+              if (((mask >> (4 * g)) & 15u) == 0u) {
+                float p0, p1, t0, t1;
+                mul2(u[4 * g], u[4 * g + 1], u[4 * g + 2], u[4 * g + 3], p0, p1);
+                add2(m[4 * g], m[4 * g + 1], m[4 * g + 2], m[4 * g + 3], t0, t1);
+                a += fmaf(lg2_ft(p0 * p1), 0.6931471805599453f, t0 + t1);
+              } else {                           // an interval starts here: track by track (seg_step)
+                const int4 q4 = *reinterpret_cast<const int4*>(ivs + c0 + 4 * g);
+                const int iq[4] = {q4.x, q4.y, q4.z, q4.w};
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                  const int i = 4 * g + k;
+                  seg_step(a, c, i < nv ? iq[k] : c, fmaf(lg2_ft(u[i]), 0.6931471805599453f, m[i]), Hc);
+                }
+              }
             }
           }
+#endif
         }
         if (last) Hc[c] = a;                      // the event's last non-empty interval
         tc_fence_before_sync();
         if (rank == 0) mbar_arrive(bar(bAccEmpty + mt));
         else mbar_arrive_cluster(lead_pacc + 8u * mt);
-        mbar_arrive(bar(bMeta + (it & (kIvBufs - 1))));
+        mbar_arrive(bar(bMeta + ib));
       }
     }
     FC_PROF_ADD(2, pw);
@@ -405,7 +482,8 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
           }
         }
         fence_proxy_async_smem();
-        mbar_arrive(bar(bHFull + g));                       // this CTA's epilogue (interval list) and, in the leader, the MMAs
+        mbar_arrive(bar(bIvFull + ib));                     // this CTA's epilogue: the interval list is staged
+        mbar_arrive(bar(bHFull + g));                       // the leader's MMA issuer: this half of the B operand is staged
         if (rank == 1) mbar_arrive_cluster(lead_phfull);    // the peer's half of the B operand is staged
       }
     }
@@ -435,7 +513,8 @@ float tf32_rna_h(float v) {
 size_t fc_tc_packed_bytes() { return (size_t)2 * 2 * kWPart; }      // 2 halves x (hi | lo)
 
 // W5 [800][25] and b5 [800] (PyTorch layouts) -> per half [hi | lo][8 K chunks][512 rows][4 floats];
-// row 128*mt + r holds output 400*half + 128*mt + r while 128*mt + r < 400 (zero rows otherwise); K index 25 = bias.
+// row 128*mt + r holds output 400*half + 128*mt + r for the first 384 outputs of a half, rows 416 .. 431 (tile 3, quadrant 1)
+// the last 16; all other rows are zero; K index 25 = bias.
 void fc_tc_pack(const float* w5, const float* b5, void* host_dst) {
   float* dst = static_cast<float*>(host_dst);
   memset(dst, 0, fc_tc_packed_bytes());
@@ -445,7 +524,7 @@ void fc_tc_pack(const float* w5, const float* b5, void* host_dst) {
       for (int k = 0; k <= kFcHidden; ++k) {
         const float v = k < kFcHidden ? w5[o * kFcHidden + k] : b5[o];
         const float hi = tf32_rna_h(v), lo = tf32_rna_h(v - hi);
-        const size_t idx = ((size_t)(k / 4) * kRowsW + row) * 4 + (k % 4);
+        const size_t idx = ((size_t)(k / 4) * kRowsW + (row < 384 ? row : kSmallRow0 + row - 384)) * 4 + (k % 4);
         dst[(size_t)half * 2 * (kWPart / 4) + idx] = hi;
         dst[(size_t)half * 2 * (kWPart / 4) + kWPart / 4 + idx] = lo;
       }
@@ -458,24 +537,13 @@ cudaError_t fc_tc_setup() {
 
 void launch_fc_hist_tc(const float* const feat[9], const int32_t* event_offsets, const int32_t* perm,
                        const int32_t* seg_off, const int32_t* seg_cnt, const float* fc_params, const void* w5img,
-                       int n_events, float* hist, float* dump, int sm_count, cudaStream_t s) {
+                       int n_events, float* hist, float* dump, int sm_count, bool pdl, cudaStream_t s) {
   if (n_events <= 0) return;
   Feat9 F;
   for (int k = 0; k < 9; ++k) F.f[k] = feat[k];
   const int gx = n_events < sm_count / 2 ? n_events : sm_count / 2;
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(2 * gx);
-  cfg.blockDim = dim3(kFtThreads);
-  cfg.dynamicSmemBytes = FT_SMEM;
-  cfg.stream = s;
-  cudaLaunchAttribute at[1];
-  at[0].id = cudaLaunchAttributeClusterDimension;     // the two output halves of the same events form a CTA pair
-  at[0].val.clusterDim.x = 2;
-  at[0].val.clusterDim.y = 1;
-  at[0].val.clusterDim.z = 1;
-  cfg.attrs = at;
-  cfg.numAttrs = 1;
-  cudaLaunchKernelEx(&cfg, k_fc_hist_tc, F, event_offsets, perm, seg_off, seg_cnt, fc_params,
+  PdlLaunch L(dim3(2 * gx), dim3(kFtThreads), FT_SMEM, s, pdl, 2);   // the two output halves of the same events form a CTA pair
+  cudaLaunchKernelEx(&L.cfg, k_fc_hist_tc, F, event_offsets, perm, seg_off, seg_cnt, fc_params,
                      static_cast<const unsigned char*>(w5img), n_events, hist, dump);
 }
 

@@ -10,6 +10,7 @@
 // index into perm) and length of interval i's run.  Integer shared-memory atomics only count;
 // placement uses match/ballot ranks, so the order is the stable one and is reproducible.
 #include "pvf_internal.cuh"
+#include "pdl.cuh"
 
 namespace pvf {
 
@@ -23,6 +24,8 @@ k_sort(const float* __restrict__ z_poca, const int32_t* __restrict__ event_offse
   __shared__ int s_base[kSortWarps][kIntervals];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int e = blockIdx.x * kSortWarps + warp;
+  pdl_launch_dependents();     // the FC kernel may start its prologue (weights to shared memory) now; it waits for
+                               // this grid's completion before it reads perm / seg_off / seg_cnt (pdl.cuh)
   if (e >= n_events) return;   // whole warp exits together; no block-level barrier below
   int* cnt = s_cnt[warp];
   int* base = s_base[warp];
