@@ -250,7 +250,7 @@ class Workload:
     """One configuration of the hot path on the device: events + weights + handle + output buffers."""
 
     def __init__(self, torch, PVFinder, *, model, events, seed, precision, channels=64, split_mask=None, elide=False,
-                 cta_pair=True, margin=0.0, weights="peaky", host_io=False, l2_chunk_events=0, low_latency=None):
+                 cta_pair=True, margin=0.0, weights="peaky", host_io=False, l2_chunk_events=0, stage_timing=True):
         self.torch = torch
         self.ev = make_events(model, events, seed)
         self.w = make_weights(weights, 1, channels)
@@ -259,11 +259,10 @@ class Workload:
         extra = {}
         if l2_chunk_events:
             extra["l2_chunk_events"] = int(l2_chunk_events)
-        if low_latency is not None:
-            extra["low_latency"] = int(low_latency)
+        self.stage_timing = stage_timing
         self.pvf = PVFinder(self.w, max_events=events, max_tracks=max(self.ev.n_tracks, 1), precision=precision,
-                            split_mask=self.split, stage_timing=True, host_io=host_io, elide_empty=elide,
-                            cta_pair=bool(cta_pair) and precision != "fp32", boundary_margin_mm=margin, **extra)
+                            split_mask=self.split, stage_timing=stage_timing, host_io=host_io, elide_empty=elide,
+                            cta_pair=bool(cta_pair), boundary_margin_mm=margin, **extra)
         self.feat = torch.from_numpy(self.ev.feat).cuda()
         self.off = torch.from_numpy(self.ev.event_offsets).cuda()
         self.probs = torch.empty(events, 4000, device="cuda")
@@ -295,7 +294,7 @@ class Workload:
         t1 = time.time()
         if barrier:
             barrier()
-        return e0.elapsed_time(e1), self.pvf.stage_times_ms(), (t0, t1)
+        return e0.elapsed_time(e1), (self.pvf.stage_times_ms() if self.stage_timing else None), (t0, t1)
 
     def close(self):
         self.pvf.destroy()
@@ -315,7 +314,10 @@ def run_variants(torch, PVFinder, args, sampler, peaks, peaks_src, tf32_measured
         dict(name="config4_bf16_c16", model="run3", events=16000, seed=1004, precision="bf16", channels=16),
         dict(name="config1_tf32", model="run3", events=1000, seed=1001, precision="tf32"),
         dict(name="config2_tf32_elide_empty", model="run3", events=16000, seed=SEEDS["run3"], precision="tf32", elide=True),
-        dict(name="config2_fp32", model="run3", events=4000, seed=SEEDS["run3"], precision="fp32"),
+        dict(name="config2_tf32_l2_chunks_1024", model="run3", events=16000, seed=SEEDS["run3"], precision="tf32",
+             l2_chunk_events=1024),
+        dict(name="config2_fp32", model="run3", events=16000, seed=SEEDS["run3"], precision="fp32"),
+        dict(name="config2_fp32_cuda_cores", model="run3", events=4000, seed=SEEDS["run3"], precision="fp32", cta_pair=False),
     ]
     for sp in specs:
         name = sp.pop("name")
@@ -332,10 +334,13 @@ def run_variants(torch, PVFinder, args, sampler, peaks, peaks_src, tf32_measured
                 ne = nonempty_intervals(wl.ev) / (E * 40.0)
                 rec["nonempty_interval_fraction"] = ne
                 flop *= ne                                         # executed-FLOP accounting: a separate mode
-            if prec == "fp32":
+            if prec == "fp32" and not sp.get("cta_pair", True):
                 pk_, note = 148 * 128 * 2 * 1.965e9 / 1e12, "FP32 FMA peak: 148 SM x 128 lanes x 2 x 1.965 GHz"
             else:
                 pk_, note = tensor_peak(peaks, peaks_src, prec, tf32_measured, sustained=E >= 4000)
+                if prec == "fp32":
+                    note += ("; FP32-accurate mode: nominal FLOPs against the TF32 peak -- every product costs one kind::tf32 "
+                             "and one kind::f16 MMA (2/3 and 1/3 of the executed tensor time), so 0.67 is this mode's ceiling")
             rec["unet_tflops"] = flop / (stage[2] * 1e-3) / 1e12
             rec["unet_frac"] = rec["unet_tflops"] / pk_
             rec["unet_peak"] = pk_
@@ -346,11 +351,14 @@ def run_variants(torch, PVFinder, args, sampler, peaks, peaks_src, tf32_measured
             V.append({"name": name, "error": repr(exc)[:200]})
         torch.cuda.empty_cache()
     # config 0: one event, per-call latency (sub-400 us budget per event)
-    for prec in ("tf32", "fp32"):
+    for prec in ("tf32", "fp16", "fp32"):
         try:
             wl = Workload(torch, PVFinder, model="single", events=1, seed=SEEDS["single"], precision=prec)
             n = 200
-            ms, stage, win = wl.timed(n, 20)
+            _, stage, _ = wl.timed(n, 20)                          # per-stage split: stage timing on (kernels not chained)
+            wl.close()
+            wl = Workload(torch, PVFinder, model="single", events=1, seed=SEEDS["single"], precision=prec, stage_timing=False)
+            ms, _, win = wl.timed(n, 20)                           # the latency: no events between the kernels, PDL chain
             iso = []
             for _ in range(30):                                    # isolated calls: launch gaps included
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -361,7 +369,8 @@ def run_variants(torch, PVFinder, args, sampler, peaks, peaks_src, tf32_measured
                 iso.append(e0.elapsed_time(e1) * 1e3)
             V.append({"name": f"config0_{prec}_latency", "events": 1, "tracks": wl.ev.n_tracks, "precision": prec,
                       "channels": 64, "latency_us": ms * 1e3 / n, "latency_isolated_us_median": float(np.median(iso)),
-                      "how": f"{n} back-to-back pvf_run calls on one stream (device time / call); 30 isolated calls",
+                      "how": f"{n} back-to-back pvf_run calls on one stream (device time / call), kernels chained by programmatic "
+                             "dependent launch; 30 isolated calls; stage_us from a second handle with stage timing (no PDL)",
                       "stage_us": {"sort": stage[0] * 1e3, "fc_hist": stage[1] * 1e3, "unet": stage[2] * 1e3,
                                    "peaks": stage[3] * 1e3},
                       "launches_per_run": wl.pvf.launches_per_run(1), "clocks": sampler.window(*win)})
@@ -451,7 +460,7 @@ def main_ours(args, rank, world, local_rank):
         variants = run_variants(torch, PVFinder, args, sampler, peaks, peaks_src, tf32_measured)
     sampler.stop()
     unet_s = stage[2] * 1e-3
-    if args.precision == "fp32":
+    if args.precision == "fp32" and not args.cta_pair:
         bound, peak = "alu", 148 * 128 * 2 * 1.965e9 / 1e12
         peak_note = "FP32 FMA: 148 SM x 128 lanes x 2 FLOP x 1.965 GHz (B200_PROFILING.md unit counts)"
     else:
@@ -474,7 +483,7 @@ def main_ours(args, rank, world, local_rank):
     # of SURVEY.md 8(d) (all 40 intervals written) is kept beside it.
     fc_s = stage[1] * 1e-3
     bytes_alg = ev.n_tracks * 36 + E * 40 * 800 * 4
-    bytes_moved = ev.n_tracks * 36 + (nonempty if args.precision != "fp32" else E * 40) * 800 * 4
+    bytes_moved = ev.n_tracks * 36 + (nonempty if (args.precision != "fp32" or args.cta_pair) else E * 40) * 800 * 4
     roof = {"kernel": "unet", "bound": bound, "achieved": achieved, "peak": peak,
             "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
             "peak_source": peak_note,
@@ -497,7 +506,7 @@ def main_ours(args, rank, world, local_rank):
         "config": {"workload": f"BASELINE.json config {_config_id(args)}: {E} events/GPU, "
                                f"model {args.model}, {ev.n_tracks} tracks, UNet {args.channels} ch, weights {args.weights}",
                    "precision": args.precision, "split_mask": wl.split,
-                   "elide_empty_intervals": bool(args.elide_empty), "unet_cta_pair": bool(args.cta_pair) and args.precision != "fp32", "boundary_margin_mm": args.boundary_margin,
+                   "elide_empty_intervals": bool(args.elide_empty), "unet_cta_pair": bool(args.cta_pair), "boundary_margin_mm": args.boundary_margin,
                    "nonempty_interval_fraction": nonempty / (E * 40.0),
                    "cache": ("inputs larger than L2 (107 MB features, 2 GB histogram per step)" if E >= 2000 else
                              "small batch: inputs fit in L2 (latency-style measurement)")},

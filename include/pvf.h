@@ -46,7 +46,9 @@ typedef enum {
  * FP32 FMAs in PVF_PREC_FP32, and in the tensor-core modes FP32 FMAs for the 25-wide layers plus a 3-pass
  * TF32 hi/lo split with FP32 accumulation for the 25 -> 800 layer. */
 typedef enum {
-  PVF_PREC_FP32 = 0, /* FP32 FMA direct convolution (CUDA cores); reference-accuracy path */
+  PVF_PREC_FP32 = 0, /* FP32-accurate.  With unet_cta_pair = 1: tcgen05 -- every product as a kind::tf32 MMA plus one kind::f16
+                        correction MMA on BF16 pieces (~2^-20 relative per product).  With
+                        unet_cta_pair = 0: FP32 FMA direct convolution on the CUDA cores, the bisecting reference */
   PVF_PREC_TF32 = 1, /* tcgen05 kind::tf32, operands RN-rounded to TF32, FP32 accumulate in TMEM */
   PVF_PREC_BF16 = 2, /* tcgen05 kind::f16 with BF16 operands, FP32 accumulate in TMEM */
   PVF_PREC_FP16 = 3  /* tcgen05 kind::f16 with FP16 operands (the paper's roadmap precision) */
@@ -83,17 +85,23 @@ typedef struct {
   int64_t max_tracks;      /* capacity the pool is sized for (>= 1) */
   int32_t enable_stage_timing; /* pre-creates CUDA events around the four stages; default 0 */
   int32_t enable_host_io;  /* reserve pool space for pvf_run_host's device staging; default 0 */
-  int32_t elide_empty_intervals; /* tensor-core modes only; default 0.  1: the UNet runs only over intervals that
+  int32_t elide_empty_intervals; /* tensor-core kernels only; default 0.  1: the UNet runs only over intervals that
                               hold at least one track, every empty interval gets the precomputed vector
                               UNet(0) -- bit-identical output, fewer executed FLOPs (our optimisation, not the
                               method's: SURVEY.md section 8f NEXT-2; reported separately by bench.py) */
   float boundary_margin_mm; /* default 0 = "each track adds to the interval holding its z_poca" (BASELINE.json
                               config 0).  > 0 (< 4.9): a track within this distance of an interval edge also
                               contributes to the neighbouring interval, PAPER.md:49 (NEXT-1; R12) */
-  int32_t unet_cta_pair;   /* tensor-core modes only; default 0.  1: the UNet kernel runs as clusters of two CTAs that
+  int32_t unet_cta_pair;   /* default 0 (with PVF_PREC_FP32, 0 also selects the CUDA-core kernels).  1: the UNet kernel runs as clusters of two CTAs that
                               share every tcgen05.mma (cta_group::2, M = 256): each CTA keeps its own intervals'
                               activations and half of the weight rows, so the weight stream and the B-operand
                               reads per SM are halved.  Same arithmetic, bit-identical output */
+  int32_t l2_chunk_events; /* default 0 = the histogram buffer holds the whole batch (128 KB per event of pool).  > 0:
+                              the pool holds the histograms of this many events only, and pvf_run walks the batch in
+                              chunks of that size -- FC + sum of a chunk, then its UNet -- so that the histograms are
+                              read back while still in the L2 cache instead of travelling through HBM (PAPER.md:86
+                              "memory layout fusion ... explicit workspace reuse").  Identical
+                              output.  1024 keeps the non-empty histograms (~52 KB per event) inside the 126 MB L2 */
 } pvf_config;
 
 /* Fill *cfg with BASELINE.json config 0 (64 channels, FP32) and the given capacities. */
@@ -166,7 +174,8 @@ PVF_API pvf_status pvf_run_unet(pvf_handle h, const float* hist, int32_t n_event
 /* Copy the histogram of the last pvf_run ([n_events,40,8,100] float, canonical layout) into
  * dev_out, enqueued on cuda_stream.  In the tensor-core modes the pool holds the histograms of the
  * intervals with at least one track only (the UNet kernel takes the others as zeros without reading
- * them); this accessor fills the empty intervals with zeros, so dev_out is always the canonical H. */
+ * them); this accessor fills the empty intervals with zeros, so dev_out is always the canonical H.  With
+ * l2_chunk_events the buffer holds the LAST chunk of the run only (n_events must not exceed its size). */
 PVF_API pvf_status pvf_debug_copy_histogram(pvf_handle h, float* dev_out, int32_t n_events, void* cuda_stream);
 
 /* Mean stage times in ms over the pvf_run calls made since the previous call of this function (at

@@ -38,7 +38,7 @@ class pvf_config(C.Structure):
         ("max_peaks", C.c_int32), ("precision", C.c_int32), ("split_mask", C.c_int32),
         ("max_events", C.c_int32), ("max_tracks", C.c_int64), ("enable_stage_timing", C.c_int32),
         ("enable_host_io", C.c_int32), ("elide_empty_intervals", C.c_int32),
-        ("boundary_margin_mm", C.c_float), ("unet_cta_pair", C.c_int32),
+        ("boundary_margin_mm", C.c_float), ("unet_cta_pair", C.c_int32), ("l2_chunk_events", C.c_int32),
     ]
 
 
@@ -129,8 +129,8 @@ class PVFinder:
         self.lib = lib or load_library()
         ch = channels if channels is not None else getattr(weights, "channels", 64)
         prec = PRECISIONS[precision] if isinstance(precision, str) else int(precision)
-        if cta_pair is None:                 # tensor-core modes default to CTA pairs (cta_group::2): faster, same bits
-            cta_pair = prec != PRECISIONS["fp32"]
+        if cta_pair is None:                 # CTA pairs (cta_group::2) by default: faster, same bits; precision "fp32" with
+            cta_pair = True                  # cta_pair=False selects the CUDA-core kernels (bisecting reference)
         self.cfg = default_config(self.lib, max_events, max_tracks, unet_channels=ch, precision=prec,
                                   split_mask=split_mask, enable_stage_timing=int(stage_timing),
                                   enable_host_io=int(host_io), elide_empty_intervals=int(elide_empty),

@@ -11,6 +11,7 @@
 // skip tensors are written straight into the second half of the decoder's concat buffers, pooled /
 // upsampled copies are produced by the epilogues, weights are read through L1/L2 in PyTorch layout.
 #include "pvf_internal.cuh"
+#include "pdl.cuh"
 
 namespace pvf {
 
@@ -84,6 +85,8 @@ __global__ void __launch_bounds__(kSimtThreads)
 k_unet_simt(const float* __restrict__ hist, int n_int, UnetParamsF32 p, float* __restrict__ probs) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   SimtSmem<C>& S = *reinterpret_cast<SimtSmem<C>*>(smem_raw);
+  pdl_launch_dependents();
+  pdl_wait();                   // the histograms come from the FC kernel (pdl.cuh)
   for (int n = blockIdx.x; n < n_int; n += gridDim.x) {
     const float* H = hist + (size_t)n * kFcOut;
     for (int i = threadIdx.x; i < kFcOut; i += kSimtThreads) (&S.h[0][0])[i] = H[i];
@@ -128,13 +131,16 @@ cudaError_t unet_simt_setup(int channels) {
 }
 
 void launch_unet_simt(const float* hist, int n_int, const UnetParamsF32& p, int channels, float* probs,
-                      cudaStream_t s) {
+                      bool pdl, cudaStream_t s) {
   if (n_int <= 0) return;
   const int grid = n_int < 148 * 64 ? n_int : 148 * 64;
   switch (channels) {
-    case 64: k_unet_simt<64><<<grid, kSimtThreads, sizeof(SimtSmem<64>), s>>>(hist, n_int, p, probs); break;
-    case 32: k_unet_simt<32><<<grid, kSimtThreads, sizeof(SimtSmem<32>), s>>>(hist, n_int, p, probs); break;
-    case 16: k_unet_simt<16><<<grid, kSimtThreads, sizeof(SimtSmem<16>), s>>>(hist, n_int, p, probs); break;
+    case 64: { PdlLaunch L(dim3(grid), dim3(kSimtThreads), sizeof(SimtSmem<64>), s, pdl);
+               cudaLaunchKernelEx(&L.cfg, k_unet_simt<64>, hist, n_int, p, probs); break; }
+    case 32: { PdlLaunch L(dim3(grid), dim3(kSimtThreads), sizeof(SimtSmem<32>), s, pdl);
+               cudaLaunchKernelEx(&L.cfg, k_unet_simt<32>, hist, n_int, p, probs); break; }
+    case 16: { PdlLaunch L(dim3(grid), dim3(kSimtThreads), sizeof(SimtSmem<16>), s, pdl);
+               cudaLaunchKernelEx(&L.cfg, k_unet_simt<16>, hist, n_int, p, probs); break; }
   }
 }
 

@@ -33,6 +33,14 @@
 // sets of four (TMEM -> registers -> bias, LeakyReLU, TF32/BF16 rounding, pool / upsample -> shared
 // memory; d1's epilogue fuses the 1x1 head + sigmoid and writes out_probs).
 // TF32 mode: the e1 layer (raw histogram input) can run as two passes on BF16 pieces (split_mask bit 0).
+//
+// FP32-accurate mode (format 3, "FX"; PVF_PREC_FP32 on the tensor cores, BASELINE.json config 0 "FP32"): every product a w is
+// taken as  tf32(a) tf32(w)  +  [a - tf32(a)] w  +  a [w - tf32(w)]  -- the first term one kind::tf32 MMA, the two small
+// terms ONE kind::f16 MMA over BF16 pieces stacked along K: A' = [a_lo (8 channels) | bf16(a) (the same 8 channels)],
+// B' = [bf16(w) | w_lo].  The small terms are 2^-11 of the product, so 8-bit pieces leave ~2^-20 relative error per
+// product at 2 MMA time units per (tap pair, 8 channels) -- a three-pass TF32 split needs 3.  Activations live in shared
+// memory as three arrays per buffer (HI: TF32 chunks, LO and HB: BF16 chunks; 8 bytes per value), which fits for groups
+// of ONE interval; the weight image interleaves a main and a correction step per (tap pair, K block).
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 #include <cstring>
@@ -40,6 +48,7 @@
 #include <vector>
 
 #include "pvf_internal.cuh"
+#include "pdl.cuh"
 #include "umma.cuh"
 
 namespace pvf {
@@ -65,16 +74,25 @@ enum { gE2 = 0, gD1Ea = 1, gB = 2, gD1Eb = 3, gD2 = 4, gD1Ec = 5, gE1 = 6, gD1U 
 // CG: CTAs per MMA -- 1, or 2 = a cluster of two CTAs (cta_group::2) that run one M = 256 MMA per step: each CTA
 // supplies its own 128 activation rows (its own group of intervals) and HALF of the weight rows (rank 0 the even
 // tap of a pair, rank 1 the odd tap), so per CTA the weight stream and the B-operand reads are halved.
-template <int C, int BF16, int CG = 1>
+// TT: intervals per group, 0 = the throughput default below.  TT = 1 is the small-batch (low-latency) instance: with
+// few intervals in the whole call (one event = 40) a group of one interval per CTA halves the serial MMA chain a CTA
+// walks and puts twice as many SMs to work.  Same MMAs per interval, same order.
+constexpr bool is16(int fmt) { return fmt == 1 || fmt == 2; }
+
+template <int C, int BF16, int CG = 1, int TT = 0>
 struct Geo {
-  static constexpr int ES = BF16 ? 2 : 4;            // operand element size
-  static constexpr int PER = 16 / ES;                // channels per 16-byte chunk
+  static constexpr bool B16 = is16(BF16);            // 2-byte operands
+  static constexpr bool FX = BF16 == 3;              // FP32-accurate: TF32 main array + BF16 correction arrays
+  static constexpr int ES = B16 ? 2 : 4;             // operand element size (main array)
+  static constexpr int PER = 16 / ES;                // channels per 16-byte chunk (main array)
   static constexpr int KPM = 2 * PER;                // channels per MMA (32 bytes of K)
-  static constexpr int NCH = C / PER;                // chunks of a C-channel activation
-  static constexpr int XCH = BF16 ? 2 : 4;           // chunks of the input buffer X0 (TF32: hi0 hi1 lo0 lo1)
+  static constexpr int NCH = C / PER;                // chunks of a C-channel activation (main array)
+  static constexpr int NCHB = FX ? 2 * NCH : NCH;    // chunks per buffer: FX adds LO (NCH/2 chunks of 8 BF16) and HB (same)
+  static constexpr int XCH = B16 ? 2 : 4;            // chunks of the input buffer X0 (FX: hi0 hi1 lo hb)
   static constexpr int NKB1 = C / KPM;               // MMA K blocks per tap over C channels
+  static constexpr int PH = FX ? 2 : 1;              // MMA steps per (tap pair, K block): FX = main + correction
   static constexpr int NOUT = 2 * C;                 // MMA N: the outputs of an (even, odd) tap pair side by side
-  static constexpr int T = (C == 64) ? 2 : (C == 32 ? 4 : (BF16 ? 8 : 4));   // intervals per group (TMEM: 4*T*C <= 512)
+  static constexpr int T = TT ? TT : (FX ? 1 : ((C == 64) ? 2 : (C == 32 ? 4 : (B16 ? 8 : 4))));   // intervals per group (TMEM: 4*T*C <= 512)
   static constexpr int LEAD1 = 16, LEAD2 = 8, LEAD3 = 8;
   // rows per chunk = lead halo + T interval slots; reads past the last slot (garbage output rows only)
   // land in the following chunk / buffer, which is always inside the CTA's allocation
@@ -85,8 +103,8 @@ struct Geo {
   static constexpr int STAGE_BYTES = kStageBytes / CG;
   static constexpr int SPS = STAGE_BYTES / STEP_BYTES;   // MMA steps per ring stage (independent of CG)
   // shared-memory map (bytes)
-  static constexpr int SZ_L1 = NCH * LBO1;           // a C-channel buffer at L = 100
-  static constexpr int SZ_L2 = NCH * LBO2;           //                     at L = 50
+  static constexpr int SZ_L1 = NCHB * LBO1;          // a C-channel buffer at L = 100
+  static constexpr int SZ_L2 = NCHB * LBO2;          //                     at L = 50
   static constexpr int OFF_E1 = 0;                   // e1 skip (dedicated)
   static constexpr int OFF_R = OFF_E1 + SZ_L1;       // overlay: (E2 | U2) then U1; P2 sits in U2's place
   static constexpr int OFF_XP = OFF_R + SZ_L1;       // overlay: X0 (input) then P1 = pool(e1)
@@ -111,15 +129,17 @@ struct Geo {
   static constexpr int TMEM_COLS = (2 * T * NOUT <= 32) ? 32 : (2 * T * NOUT <= 64) ? 64 : (2 * T * NOUT <= 128) ? 128
                                    : (2 * T * NOUT <= 256) ? 256 : 512;
   // d1E parts (steps): run while the epilogues of e2 / b / d2 drain; multiples of every SPS
-  static constexpr int D1E_STEPS = 13 * NKB1;        // 13 tap pairs
-  static constexpr int D1E_A = D1E_STEPS < 16 ? D1E_STEPS : 16;
-  static constexpr int D1E_B = (D1E_STEPS - D1E_A) < 16 ? (D1E_STEPS - D1E_A) : 16;
+  static constexpr int D1E_STEPS = 13 * NKB1 * PH;   // 13 tap pairs
+  static constexpr int D1E_A = D1E_STEPS < 16 * PH ? D1E_STEPS : 16 * PH;
+  static constexpr int D1E_B = (D1E_STEPS - D1E_A) < 16 * PH ? (D1E_STEPS - D1E_A) : 16 * PH;
   static constexpr int D1E_C = D1E_STEPS - D1E_A - D1E_B;
   static_assert(2 * SZ_L2 == SZ_L1, "E2 + U2 must tile the overlay region exactly");
-  static_assert(SMEM <= 227 * 1024 && STAGES >= 3, "shared memory budget");
+  static constexpr bool kFits = SMEM <= 227 * 1024 && STAGES >= 3;   // checked where a kernel is instantiated (the helper
+                                                                     // templates read layout constants from Geo<.., CG = 1>)
   static_assert(2 * T * NOUT <= 512, "TMEM budget");
-  static_assert(NCH % 2 == 0 && T % 2 == 0, "whole MMA K blocks per source; level-2 tiles whole");
-  static_assert(16 % SPS == 0, "d1E parts must start on ring-stage boundaries");
+  static_assert(NCH % 2 == 0 && (T % 2 == 0 || T == 1), "whole MMA K blocks per source; level-2 tiles whole (or one interval)");
+  static_assert(16 % SPS == 0 && SPS % PH == 0, "d1E parts must start on ring-stage boundaries; whole (main, correction) pairs per stage");
+  static_assert(!FX || T == 1, "the FP32-accurate format runs on groups of one interval");
 };
 
 // Steps and byte offsets of the weight-image segments (host packer, producer and issuer agree on it).
@@ -133,19 +153,20 @@ struct Plan {
 // With CG = 2 the image is two such images back to back (rank 0 | rank 1), each `total` bytes with its own header.
 template <int C, int BF16, int CG>
 __host__ __device__ inline Plan make_plan(int split_e1) {
-  using G = Geo<C, BF16, CG>;
+  using G = Geo<C, BF16, CG>;          // (nothing here depends on the group size)
   Plan P{};
   // 16-bit modes: the 8 input channels fill half of an MMA's K = 16, so one e1 step takes TWO tap pairs (7 steps)
   // TF32 with the e1 split: 13 steps [a1 | a2] x [w1 | w1] + 7 steps [a1(pair 2w) | a1(pair 2w+1)] x [w2 | w2]
-  P.e1_steps = BF16 ? 7 : (split_e1 ? 20 : 13);
-  P.seg_steps[gE2] = 8 * G::NKB1;
+  // FX: 13 tap pairs x (main, correction)
+  P.e1_steps = G::B16 ? 7 : (G::FX ? 26 : (split_e1 ? 20 : 13));
+  P.seg_steps[gE2] = 8 * G::NKB1 * G::PH;
   P.seg_steps[gD1Ea] = G::D1E_A;
-  P.seg_steps[gB] = 3 * G::NKB1;
+  P.seg_steps[gB] = 3 * G::NKB1 * G::PH;
   P.seg_steps[gD1Eb] = G::D1E_B;
-  P.seg_steps[gD2] = 8 * 2 * G::NKB1;
+  P.seg_steps[gD2] = 8 * 2 * G::NKB1 * G::PH;
   P.seg_steps[gD1Ec] = G::D1E_C;
   P.seg_steps[gE1] = P.e1_steps;
-  P.seg_steps[gD1U] = 13 * G::NKB1;
+  P.seg_steps[gD1U] = 13 * G::NKB1 * G::PH;
   int off = kHeaderBytes;
   for (int s = 0; s < kSegs; ++s) {
     P.seg_off[s] = off;
@@ -180,10 +201,11 @@ __device__ __forceinline__ void st_smem16(uint32_t addr, uint4 v) {
 }
 
 // 16 consecutive channels of one row -> 16-byte chunks (4 for TF32, 2 for BF16) at
-// dst + chunk * lbo, chunk counted from c0 / PER.
-template <int BF16>
+// dst + chunk * lbo, chunk counted from c0 / PER.  FX (NCHM = chunks of the main array): the TF32 chunks, then
+// lo = bf16(v - tf32(v)) into the LO array (chunks NCHM ..) and bf16(v) into the HB array (chunks 3 NCHM / 2 ..).
+template <int BF16, int NCHM>
 __device__ __forceinline__ void store_row16(uint32_t dst_row, uint32_t lbo, int c0, const float (&v)[16]) {
-  if (BF16) {
+  if (is16(BF16)) {
 #pragma unroll
     for (int k = 0; k < 2; ++k) {
       uint4 q;
@@ -194,6 +216,7 @@ __device__ __forceinline__ void store_row16(uint32_t dst_row, uint32_t lbo, int 
       st_smem16(dst_row + (uint32_t)(c0 / 8 + k) * lbo, q);
     }
   } else {
+    float lo[16];
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
       uint4 q;
@@ -202,29 +225,57 @@ __device__ __forceinline__ void store_row16(uint32_t dst_row, uint32_t lbo, int 
       q.z = to_tf32(v[4 * k + 2]);
       q.w = to_tf32(v[4 * k + 3]);
       st_smem16(dst_row + (uint32_t)(c0 / 4 + k) * lbo, q);
+      if (BF16 == 3) {
+        lo[4 * k + 0] = v[4 * k + 0] - __uint_as_float(q.x); lo[4 * k + 1] = v[4 * k + 1] - __uint_as_float(q.y);
+        lo[4 * k + 2] = v[4 * k + 2] - __uint_as_float(q.z); lo[4 * k + 3] = v[4 * k + 3] - __uint_as_float(q.w);
+      }
+    }
+    if (BF16 == 3) {
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        uint4 ql, qh;
+        ql.x = pack16<1>(lo[8 * k + 0], lo[8 * k + 1]); ql.y = pack16<1>(lo[8 * k + 2], lo[8 * k + 3]);
+        ql.z = pack16<1>(lo[8 * k + 4], lo[8 * k + 5]); ql.w = pack16<1>(lo[8 * k + 6], lo[8 * k + 7]);
+        qh.x = pack16<1>(v[8 * k + 0], v[8 * k + 1]); qh.y = pack16<1>(v[8 * k + 2], v[8 * k + 3]);
+        qh.z = pack16<1>(v[8 * k + 4], v[8 * k + 5]); qh.w = pack16<1>(v[8 * k + 6], v[8 * k + 7]);
+        st_smem16(dst_row + (uint32_t)(NCHM + c0 / 8 + k) * lbo, ql);
+        st_smem16(dst_row + (uint32_t)(NCHM + NCHM / 2 + c0 / 8 + k) * lbo, qh);
+      }
     }
   }
 }
 
 // Pooled row (identical in both lanes of a pair): the even lane stores the first half of the 16 channels,
 // the odd lane the second half, so every lane of the store instruction is active.
-template <int BF16>
+template <int BF16, int NCHM>
 __device__ __forceinline__ void store_pooled16(uint32_t dst_row, uint32_t lbo, int c0, const float (&v)[16], int odd) {
   float h[8];
 #pragma unroll
   for (int i = 0; i < 8; ++i) h[i] = odd ? v[8 + i] : v[i];
-  if (BF16) {
+  if (is16(BF16)) {
     uint4 q;
     q.x = pack16<BF16>(h[0], h[1]); q.y = pack16<BF16>(h[2], h[3]);
     q.z = pack16<BF16>(h[4], h[5]); q.w = pack16<BF16>(h[6], h[7]);
     st_smem16(dst_row + (uint32_t)(c0 / 8 + odd) * lbo, q);
   } else {
+    float lo[8];
 #pragma unroll
     for (int k = 0; k < 2; ++k) {
       uint4 q;
       q.x = to_tf32(h[4 * k + 0]); q.y = to_tf32(h[4 * k + 1]);
       q.z = to_tf32(h[4 * k + 2]); q.w = to_tf32(h[4 * k + 3]);
       st_smem16(dst_row + (uint32_t)(c0 / 4 + 2 * odd + k) * lbo, q);
+      if (BF16 == 3) {
+        lo[4 * k + 0] = h[4 * k + 0] - __uint_as_float(q.x); lo[4 * k + 1] = h[4 * k + 1] - __uint_as_float(q.y);
+        lo[4 * k + 2] = h[4 * k + 2] - __uint_as_float(q.z); lo[4 * k + 3] = h[4 * k + 3] - __uint_as_float(q.w);
+      }
+    }
+    if (BF16 == 3) {
+      uint4 ql, qh;
+      ql.x = pack16<1>(lo[0], lo[1]); ql.y = pack16<1>(lo[2], lo[3]); ql.z = pack16<1>(lo[4], lo[5]); ql.w = pack16<1>(lo[6], lo[7]);
+      qh.x = pack16<1>(h[0], h[1]); qh.y = pack16<1>(h[2], h[3]); qh.z = pack16<1>(h[4], h[5]); qh.w = pack16<1>(h[6], h[7]);
+      st_smem16(dst_row + (uint32_t)(NCHM + c0 / 8 + odd) * lbo, ql);
+      st_smem16(dst_row + (uint32_t)(NCHM + NCHM / 2 + c0 / 8 + odd) * lbo, qh);
     }
   }
 }
@@ -238,12 +289,12 @@ enum { kE1 = 0, kE2 = 1, kB = 2, kD2 = 3, kD1 = 4 };
 // Epilogue of channels [cb, ce) of one 128-row accumulator tile, executed by the four warps of one epilogue set
 // (thread = row m; named barrier 1 + set among them).  The (tile, channel half) units of a layer go round-robin to
 // the sets (whole tiles for d1, whose head sums over all channels).
-template <int C, int BF16, int MODE>
+template <int C, int BF16, int MODE, int TT>
 __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_base, int tile, int q, int lane,
                                               const float* __restrict__ par, int n_valid_int,
                                               float* __restrict__ probs_group, float* __restrict__ scr,
                                               const int* __restrict__ list_g, int cb, int ce, int set) {
-  using G = Geo<C, BF16>;
+  using G = Geo<C, BF16, 1, TT>;
   const int m = 32 * q + lane;
   const float* bias = par + MODE * C;
   // accumulator tile: columns [0, C) = E0 (even taps), [C, 2C) = E1 (odd taps); output row m = E0[m] + E1[m+1]
@@ -275,18 +326,18 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
   if (MODE == kE1) {
     dst_full = smem_base + G::OFF_E1 + (uint32_t)(G::LEAD1 + 128 * tile + m) * 16u; lbo_full = G::LBO1;
     dst_aux = smem_base + G::OFF_XP + (uint32_t)(G::LEAD2 + 64 * tile + (m >> 1)) * 16u; lbo_aux = G::LBO2;     // P1
-    if (tile == 0 && m < G::LEAD2) zero_rows(smem_base + G::OFF_XP, G::LBO2, G::NCH, m);
+    if (tile == 0 && m < G::LEAD2) zero_rows(smem_base + G::OFF_XP, G::LBO2, G::NCHB, m);
   } else if (MODE == kE2) {
     dst_full = smem_base + G::OFF_R + (uint32_t)(G::LEAD2 + 128 * tile + m) * 16u; lbo_full = G::LBO2;          // E2
     dst_aux = smem_base + G::OFF_R + G::SZ_L2 + (uint32_t)(G::LEAD3 + 64 * tile + (m >> 1)) * 16u; lbo_aux = G::LBO3;  // P2
-    if (tile == 0 && m < G::LEAD2) zero_rows(smem_base + G::OFF_R, G::LBO2, G::NCH, m);
-    if (tile == 0 && m >= 32 && m < 32 + G::LEAD3) zero_rows(smem_base + G::OFF_R + G::SZ_L2, G::LBO3, G::NCH, m - 32);
+    if (tile == 0 && m < G::LEAD2) zero_rows(smem_base + G::OFF_R, G::LBO2, G::NCHB, m);
+    if (tile == 0 && m >= 32 && m < 32 + G::LEAD3) zero_rows(smem_base + G::OFF_R + G::SZ_L2, G::LBO3, G::NCHB, m - 32);
   } else if (MODE == kB) {
     dst_full = smem_base + G::OFF_R + G::SZ_L2 + (uint32_t)(G::LEAD2 + 256 * tile + 2 * m) * 16u; lbo_full = G::LBO2;  // U2
-    if (tile == 0 && m < G::LEAD2) zero_rows(smem_base + G::OFF_R + G::SZ_L2, G::LBO2, G::NCH, m);
+    if (tile == 0 && m < G::LEAD2) zero_rows(smem_base + G::OFF_R + G::SZ_L2, G::LBO2, G::NCHB, m);
   } else if (MODE == kD2) {
     dst_full = smem_base + G::OFF_R + (uint32_t)(G::LEAD1 + 256 * tile + 2 * m) * 16u; lbo_full = G::LBO1;      // U1
-    if (tile == 0 && m < G::LEAD1) zero_rows(smem_base + G::OFF_R, G::LBO1, G::NCH, m);
+    if (tile == 0 && m < G::LEAD1) zero_rows(smem_base + G::OFF_R, G::LBO1, G::NCHB, m);
   }
   float logit = 0.0f;
 #pragma unroll 1
@@ -318,17 +369,19 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
       for (int i = 0; i < 16; ++i) v[i] = 0.0f;
     }
     if (MODE == kE1 || MODE == kE2) {
-      store_row16<BF16>(dst_full, lbo_full, c0, v);
       float pv[16];
 #pragma unroll
       for (int i = 0; i < 16; ++i) pv[i] = fmaxf(v[i], __shfl_xor_sync(0xffffffffu, v[i], 1));
-      store_pooled16<BF16>(dst_aux, lbo_aux, c0, pv, lane & 1);   // both lanes of a pair hold the same maxima
+      if (exists) {               // (a level-2 tile is wider than a one-interval group: its upper half has no buffer rows)
+        store_row16<BF16, G::NCH>(dst_full, lbo_full, c0, v);
+        store_pooled16<BF16, G::NCH>(dst_aux, lbo_aux, c0, pv, lane & 1);   // both lanes of a pair hold the same maxima
+      }
     } else if (exists) {          // kB, kD2: nearest upsample = the same chunk into rows 2m and 2m + 1;
       // groups of four lanes alternate which of the two rows goes first, so that one store instruction
       // covers all eight 16-byte slots of every 128-byte line evenly (no bank conflicts)
       const uint32_t swz = (uint32_t)((m >> 2) & 1) * 16u;
-      store_row16<BF16>(dst_full + swz, lbo_full, c0, v);
-      store_row16<BF16>(dst_full + (16u - swz), lbo_full, c0, v);
+      store_row16<BF16, G::NCH>(dst_full + swz, lbo_full, c0, v);
+      store_row16<BF16, G::NCH>(dst_full + (16u - swz), lbo_full, c0, v);
     }
   }
   if (MODE == kD1) {
@@ -344,18 +397,42 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
 // Interval histograms of one group -> X0 (operand-rounded, chunked layout).  All epilogue threads.  X0 shares
 // its memory with P1, so every row the e1 MMAs can read for a valid output is (re)written: the lead
 // rows and the gap rows l >= 100 of every interval as zeros.
-template <int C, int BF16>
 // seg_cnt (optional): tracks per interval; an interval without tracks is taken as zeros WITHOUT reading hist
 // (the tensor-core FC kernel does not write the histograms of empty intervals).
+template <int C, int BF16, int TT>
 __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restrict__ hist, long long g0,
                                         int n_valid_int, int split, int tid, const int* __restrict__ list,
                                         const int* __restrict__ seg_cnt) {
-  using G = Geo<C, BF16>;
+  using G = Geo<C, BF16, 1, TT>;
   const uint32_t x0 = smem_base + G::OFF_XP;
   const uint4 zero4 = make_uint4(0, 0, 0, 0);
   if (tid < G::LEAD1)
     for (int c = 0; c < G::XCH; ++c) st_smem16(x0 + (uint32_t)c * G::LBO1 + (uint32_t)tid * 16u, zero4);
-  if (BF16) {
+  if (G::FX) {
+    // FP32-accurate format: chunks 0, 1 = TF32 of channels 0-3 / 4-7 (HI), chunk 2 = bf16(x - tf32(x)) (LO), chunk 3 = bf16(x) (HB)
+    for (int it = tid; it < G::T * 128; it += G::EPI_THREADS) {
+      const int t = it >> 7, l = it & 127;
+      bool live = l < 100 && t < n_valid_int;
+      const long long src = !live ? 0 : (list ? (long long)list[g0 + t] : g0 + t);
+      if (live && seg_cnt != nullptr) live = __ldg(seg_cnt + src) > 0;
+      float x[8], r[8];
+      uint32_t hi[8];
+#pragma unroll
+      for (int c = 0; c < 8; ++c) {
+        x[c] = live ? __ldg(hist + src * kFcOut + c * kBins + l) : 0.0f;
+        hi[c] = to_tf32(x[c]);
+        r[c] = x[c] - __uint_as_float(hi[c]);
+      }
+      uint4 ql, qh;
+      ql.x = pack16<1>(r[0], r[1]); ql.y = pack16<1>(r[2], r[3]); ql.z = pack16<1>(r[4], r[5]); ql.w = pack16<1>(r[6], r[7]);
+      qh.x = pack16<1>(x[0], x[1]); qh.y = pack16<1>(x[2], x[3]); qh.z = pack16<1>(x[4], x[5]); qh.w = pack16<1>(x[6], x[7]);
+      const uint32_t row = (uint32_t)(G::LEAD1 + it) * 16u;
+      st_smem16(x0 + row, make_uint4(hi[0], hi[1], hi[2], hi[3]));
+      st_smem16(x0 + G::LBO1 + row, make_uint4(hi[4], hi[5], hi[6], hi[7]));
+      st_smem16(x0 + 2 * G::LBO1 + row, ql);
+      st_smem16(x0 + 3 * G::LBO1 + row, qh);
+    }
+  } else if (G::B16) {
     for (int it = tid; it < G::T * 128; it += G::EPI_THREADS) {
       const int t = it >> 7, l = it & 127;
       bool live = l < 100 && t < n_valid_int;
@@ -412,9 +489,9 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
 }
 
 // Compile-time description of sub-layer S as the MMA issuer sees it.
-template <int C, int BF16, int S>
+template <int C, int BF16, int S, int TT>
 struct Lay {
-  using G = Geo<C, BF16>;
+  using G = Geo<C, BF16, 1, TT>;
   static constexpr int TAPS = (S == sE1 || S == sD1U || S == sD1E) ? 25 : (S == sB ? 5 : 15);
   static constexpr int PAD = (TAPS - 1) / 2;
   static constexpr int PAIRS = (TAPS + 1) / 2;                 // (even, odd) tap pairs; the last odd tap is zero
@@ -422,7 +499,7 @@ struct Lay {
   static constexpr int LEVEL = (S == sE1 || S == sD1U || S == sD1E) ? 1 : (S == sB ? 3 : 2);
   static constexpr int LEAD = LEVEL == 1 ? G::LEAD1 : (LEVEL == 2 ? G::LEAD2 : G::LEAD3);
   static constexpr int LBO = LEVEL == 1 ? G::LBO1 : (LEVEL == 2 ? G::LBO2 : G::LBO3);
-  static constexpr int NT = LEVEL == 1 ? G::T : (LEVEL == 2 ? G::T / 2 : (G::T + 3) / 4);
+  static constexpr int NT = LEVEL == 1 ? G::T : (LEVEL == 2 ? (G::T + 1) / 2 : (G::T + 3) / 4);
   static constexpr int HALF = (S == sD2) ? NKB / 2 : NKB;      // K blocks served by the first source buffer
   static constexpr int SRC0 = (S == sE1) ? G::OFF_XP /* X0 */ : (S == sE2) ? G::OFF_XP /* P1 */
                               : (S == sB) ? G::OFF_R + G::SZ_L2 /* P2 */ : (S == sD2) ? G::OFF_R + G::SZ_L2 /* U2 */
@@ -433,16 +510,23 @@ struct Lay {
   __host__ __device__ static constexpr int a_off(int kk) {
     return kk < HALF ? SRC0 + 2 * kk * LBO : SRC1 + 2 * (kk - HALF) * LBO;
   }
+  // FX: the source buffers hold SRC_NCH main chunks, then SRC_NCH / 2 LO chunks, then SRC_NCH / 2 HB chunks; the
+  // correction MMA of K block kk reads LO chunk kk and HB chunk kk as the two 16-byte K chunks of its A operand
+  static constexpr int SRC_NCH = (S == sE1) ? 2 : G::NCH;
+  static constexpr int C_LBO = SRC_NCH / 2 * LBO;              // descriptor LBO of the correction operand (LO -> HB)
+  __host__ __device__ static constexpr int c_off(int kk) {
+    return (kk < HALF ? SRC0 + kk * LBO : SRC1 + (kk - HALF) * LBO) + SRC_NCH * LBO;
+  }
 };
 
 template <int BF16, int CG>
 __device__ __forceinline__ void mma_lh(uint32_t d, uint32_t a_lo, uint32_t a_hi, uint32_t b_lo, uint32_t b_hi,
                                        uint32_t idesc, uint32_t acc) {
   if (CG == 2) {
-    if (BF16) mma2_f16_lh(d, a_lo, a_hi, b_lo, b_hi, idesc, acc);
+    if (is16(BF16)) mma2_f16_lh(d, a_lo, a_hi, b_lo, b_hi, idesc, acc);
     else mma2_tf32_lh(d, a_lo, a_hi, b_lo, b_hi, idesc, acc);
   } else {
-    if (BF16) mma_f16_lh(d, a_lo, a_hi, b_lo, b_hi, idesc, acc);
+    if (is16(BF16)) mma_f16_lh(d, a_lo, a_hi, b_lo, b_hi, idesc, acc);
     else mma_tf32_lh(d, a_lo, a_hi, b_lo, b_hi, idesc, acc);
   }
 }
@@ -464,32 +548,38 @@ __device__ unsigned long long g_unet_prof[160][16];
 // used by all NT tiles.  The warp walks the (uniform) schedule; one elected lane issues a whole
 // stage worth of MMAs whose descriptors differ from the stage origin by compile-time constants.
 // f_begin must be a multiple of SPS.  acc0 = 0 starts fresh accumulators at step f_begin.
-template <int C, int BF16, int CG, int S>
+template <int C, int BF16, int CG, int TT, int S>
 __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_t bar0, RingState& rs,
                                         int f_begin, int f_end, uint32_t acc0, bool e1x = false) {
   // e1x (sub-layer e1 of the TF32 kernel only): the split e1 runs as kind::f16 MMAs on BF16 pieces (see load_x0)
-  using G = Geo<C, BF16, CG>;
-  using Y = Lay<C, BF16, S>;
-  constexpr int SPS = G::SPS;
-  static_assert(Y::HALF % SPS == 0 || SPS % Y::NKB == 0,
+  // Steps are MMA steps as they sit in the weight image ("physical"); FX has PH = 2 of them -- main (kind::tf32 on the HI
+  // array) and correction (kind::f16 on [LO | HB]) -- per (tap pair, K block) ("logical" step).
+  using G = Geo<C, BF16, CG, TT>;
+  using Y = Lay<C, BF16, S, TT>;
+  constexpr int SPS = G::SPS, PH = G::PH, SPL = SPS / PH;
+  constexpr bool B16 = G::B16, FX = G::FX;
+  static_assert(Y::HALF % SPL == 0 || SPL % Y::NKB == 0,
                 "a ring stage is either part of one source's K blocks or whole taps");
-  constexpr uint32_t idesc = instr_desc(BF16 == 2 ? kFmtF16 : (BF16 ? kFmtBF16 : kFmtTF32), 128 * CG, G::NOUT);
+  constexpr uint32_t fmt_main = BF16 == 2 ? kFmtF16 : (BF16 == 1 ? kFmtBF16 : kFmtTF32);
+  constexpr uint32_t idesc = instr_desc(fmt_main, 128 * CG, G::NOUT);
   constexpr uint32_t idesc_x = instr_desc(kFmtBF16, 128 * CG, G::NOUT);
   // The kernels have an odd number of taps: the last "pair" holds an even tap only, so its steps are MMAs of
   // N = C (half the tensor time, half the B rows; the E1 columns of the accumulator are left alone).
-  constexpr uint32_t idesc_h = instr_desc(BF16 == 2 ? kFmtF16 : (BF16 ? kFmtBF16 : kFmtTF32), 128 * CG, G::NOUT / 2);
+  constexpr uint32_t idesc_h = instr_desc(fmt_main, 128 * CG, G::NOUT / 2);
   constexpr uint32_t idesc_xh = instr_desc(kFmtBF16, 128 * CG, G::NOUT / 2);
   constexpr uint32_t b_lbo_h = (uint32_t)((G::NB / 2 * 16) >> 4) << 16;
-  constexpr int LAST0 = (Y::PAIRS - 1) * Y::NKB;                       // first step of the last tap pair (not e1)
+  constexpr int LAST0 = (Y::PAIRS - 1) * Y::NKB;                       // first logical step of the last tap pair (not e1)
   constexpr uint32_t hi = (128u >> 4) | (1u << 14);                    // SBO = 128 B, descriptor version 1
   // e1 in the 16-bit modes: the second 16-byte K chunk of A is the SAME 8-channel buffer two rows further down
   // (LBO = 32 bytes), i.e. the input of the next tap pair -- one MMA does tap pairs 2w and 2w + 1
-  constexpr uint32_t a_lbo = (S == sE1 && BF16) ? (2u << 16) : ((uint32_t)(Y::LBO >> 4) << 16);
+  constexpr uint32_t a_lbo = (S == sE1 && B16) ? (2u << 16) : ((uint32_t)(Y::LBO >> 4) << 16);
   constexpr uint32_t a_lbo_x2 = (2u << 16) - a_lbo;     // added for the second pass of the split e1 (TF32 kernel)
+  constexpr uint32_t c_lbo = (uint32_t)(Y::C_LBO >> 4) << 16;          // FX correction operand: LO chunk -> HB chunk
   constexpr uint32_t b_lbo = (uint32_t)((G::NB * 16) >> 4) << 16;
   const uint32_t dcol = tmem_base + (uint32_t)Y::DCOL;
   for (int f = f_begin; f < f_end; f += SPS) {
     const int n = min(SPS, f_end - f);
+    const int lf = f / PH;                      // logical step of the stage's first MMA
     {
       PVF_PROF_T0();
       mbar_wait(bar0 + 8u * rs.ring, rs.phase);
@@ -502,36 +592,50 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
     }
     tc_fence_after_sync();
     const uint32_t b0 = (sb + G::OFF_RING + rs.ring * G::STAGE_BYTES) >> 4;
-    uint32_t a0 = a_lbo + (sb >> 4);          // stage origin: descriptor low word of tile 0, step f
+    uint32_t a0 = a_lbo + (sb >> 4);          // stage origin: descriptor low word of tile 0, logical step lf
+    uint32_t c0 = c_lbo + (sb >> 4);          // same for the FX correction operand
     if (S == sE1) {
       // e1: one K block per step; steps run [pass][tap pair]; both passes of the split read the same operand
-    } else if (Y::HALF >= SPS) {
-      const int j0 = f / Y::NKB, kk0 = f % Y::NKB;
+    } else if (Y::HALF >= SPL) {
+      const int j0 = lf / Y::NKB, kk0 = lf % Y::NKB;
       const int off = kk0 < Y::HALF ? Y::SRC0 + 2 * kk0 * Y::LBO : Y::SRC1 + 2 * (kk0 - Y::HALF) * Y::LBO;
       a0 += (uint32_t)(off >> 4) + (uint32_t)(Y::LEAD + 2 * j0 - Y::PAD);
+      if (FX) {
+        const int offc = (kk0 < Y::HALF ? Y::SRC0 + kk0 * Y::LBO : Y::SRC1 + (kk0 - Y::HALF) * Y::LBO) + Y::SRC_NCH * Y::LBO;
+        c0 += (uint32_t)(offc >> 4) + (uint32_t)(Y::LEAD + 2 * j0 - Y::PAD);
+      }
     } else {
-      a0 += (uint32_t)(Y::SRC0 >> 4) + (uint32_t)(Y::LEAD + 2 * (f / Y::NKB) - Y::PAD);
+      a0 += (uint32_t)(Y::SRC0 >> 4) + (uint32_t)(Y::LEAD + 2 * (lf / Y::NKB) - Y::PAD);
+      c0 += (uint32_t)(Y::SRC0 >> 4) + (uint32_t)(Y::LEAD + 2 * (lf / Y::NKB) - Y::PAD);
     }
     if (elect_one()) {
 #pragma unroll
       for (int i = 0; i < SPS; ++i) {
         if (i < n) {
+          constexpr int dummy = 0; (void)dummy;
+          const int li = i / PH;                 // logical step inside the stage (compile time)
+          const bool corr = FX && (i % PH) == 1; // FX: the correction MMA of the logical step
           uint32_t a;
+          bool half_n;
           if (S == sE1) {
-            const int step = f + i, pass = step / 13, u = BF16 ? 2 * step : (pass ? 2 * (step - 13) : step);
+            const int step = lf + li, pass = step / 13, u = B16 ? 2 * step : (pass ? 2 * (step - 13) : step);
             a = a0 + (uint32_t)(Y::SRC0 >> 4) + (uint32_t)(Y::LEAD + 2 * u - Y::PAD);
-            if (!BF16 && pass) a += a_lbo_x2;              // [a1 of pair u | a1 of pair u + 1]
-          } else if (Y::HALF >= SPS) {
-            a = a0 + (uint32_t)(i * ((2 * Y::LBO) >> 4));
+            if (BF16 == 0 && pass) a += a_lbo_x2;              // [a1 of pair u | a1 of pair u + 1]
+            if (corr) a = c0 + (uint32_t)((Y::SRC0 + Y::SRC_NCH * Y::LBO) >> 4) + (uint32_t)(Y::LEAD + 2 * u - Y::PAD);
+            half_n = B16 ? step == 6 : (step == 12 || step == 19);
+          } else if (Y::HALF >= SPL) {
+            a = corr ? c0 + (uint32_t)(li * (Y::LBO >> 4)) : a0 + (uint32_t)(li * ((2 * Y::LBO) >> 4));
+            half_n = lf + li >= LAST0;
           } else {
-            a = a0 + (uint32_t)((Y::a_off(i % Y::NKB) - Y::SRC0) >> 4) + (uint32_t)(2 * (i / Y::NKB));
+            a = corr ? c0 + (uint32_t)((Y::c_off(li % Y::NKB) - Y::SRC0) >> 4) + (uint32_t)(2 * (li / Y::NKB))
+                     : a0 + (uint32_t)((Y::a_off(li % Y::NKB) - Y::SRC0) >> 4) + (uint32_t)(2 * (li / Y::NKB));
+            half_n = lf + li >= LAST0;
           }
-          const bool half_n = (S == sE1) ? (BF16 ? f + i == 6 : (f + i == 12 || f + i == 19)) : (f + i >= LAST0);
           const uint32_t b = (half_n ? b_lbo_h : b_lbo) + b0 + (uint32_t)(i * (G::STEP_BYTES >> 4));
           const uint32_t acc = (i > 0) ? 1u : (f > f_begin ? 1u : acc0);
 #pragma unroll
           for (int t = 0; t < Y::NT; ++t) {
-            if (S == sE1 && BF16 == 0 && e1x)
+            if ((S == sE1 && BF16 == 0 && e1x) || corr)
               mma_lh<1, CG>(dcol + (uint32_t)(t * G::NOUT), a + 128u * t, hi, b, hi, half_n ? idesc_xh : idesc_x, acc);
             else
               mma_lh<BF16, CG>(dcol + (uint32_t)(t * G::NOUT), a + 128u * t, hi, b, hi, half_n ? idesc_h : idesc, acc);
@@ -547,15 +651,18 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
   }
 }
 
-template <int C, int BF16, int CG>
-__global__ void __launch_bounds__((Geo<C, BF16, CG>::THREADS), 1)
+template <int C, int BF16, int CG, int TT>
+__global__ void __launch_bounds__((Geo<C, BF16, CG, TT>::THREADS), 1)
 k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __restrict__ wpack, int split_e1,
           float* __restrict__ probs, const int* __restrict__ list, const int* __restrict__ n_list,
           const int* __restrict__ seg_cnt) {
   // list / n_list (device, optional): process only intervals list[0 .. *n_list) of hist / probs (elision of
   // empty intervals); n_int is then only the capacity the grid was sized for
-  if (n_list != nullptr) n_int = *n_list;
-  using G = Geo<C, BF16, CG>;
+  pdl_launch_dependents();
+  if (n_list != nullptr) { pdl_wait(); n_int = *n_list; }
+  using G = Geo<C, BF16, CG, TT>;
+  static_assert(G::kFits, "shared memory budget");
+  static_assert(!G::FX || CG == 2, "the FP32-accurate format runs as CTA pairs");
   extern __shared__ __align__(1024) unsigned char smem[];
   const uint32_t sb = smem_u32(smem);
   const int tid = threadIdx.x, lane = tid & 31;
@@ -597,6 +704,7 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
   if (CG == 2) cluster_sync_all(); else __syncthreads();
   tc_fence_after_sync();
   const uint32_t tmem_base = *tmem_slot;
+  pdl_wait();      // everything above touched weights only; the histograms / seg_cnt come from the kernel before (pdl.cuh)
 
   // pair-groups: pair p of the grid takes groups CG*pg + rank for pg = p, p + pairs, ...; a CTA whose group lies
   // past the end (odd group count) runs the schedule on zeros and stores nothing
@@ -654,29 +762,29 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
       const bool has_next = pg + stride < n_pg;
       if (first) {
         wait_epi(0);
-        mma_seg<C, BF16, CG, sE1>(sb, tmem_base, bar0, rs, 0, P.e1_steps, 0u, split_e1 != 0);
+        mma_seg<C, BF16, CG, TT, sE1>(sb, tmem_base, bar0, rs, 0, P.e1_steps, 0u, split_e1 != 0);
         commit(0);
       }
       wait_epi(1);                                   // P1 staged, region B drained
-      mma_seg<C, BF16, CG, sE2>(sb, tmem_base, bar0, rs, 0, 8 * G::NKB1, 0u);
+      mma_seg<C, BF16, CG, TT, sE2>(sb, tmem_base, bar0, rs, 0, 8 * G::NKB1 * G::PH, 0u);
       commit(1);
       if (!first) wait_epi(5);                       // region A drained by the previous group's d1 epilogue
-      mma_seg<C, BF16, CG, sD1E>(sb, tmem_base, bar0, rs, 0, G::D1E_A, 0u);
+      mma_seg<C, BF16, CG, TT, sD1E>(sb, tmem_base, bar0, rs, 0, G::D1E_A, 0u);
       wait_epi(2);                                   // E2, P2 staged
-      mma_seg<C, BF16, CG, sB>(sb, tmem_base, bar0, rs, 0, 3 * G::NKB1, 0u);
+      mma_seg<C, BF16, CG, TT, sB>(sb, tmem_base, bar0, rs, 0, 3 * G::NKB1 * G::PH, 0u);
       commit(2);
-      mma_seg<C, BF16, CG, sD1E>(sb, tmem_base, bar0, rs, G::D1E_A, G::D1E_A + G::D1E_B, 1u);
+      mma_seg<C, BF16, CG, TT, sD1E>(sb, tmem_base, bar0, rs, G::D1E_A, G::D1E_A + G::D1E_B, 1u);
       wait_epi(3);                                   // U2 staged
-      mma_seg<C, BF16, CG, sD2>(sb, tmem_base, bar0, rs, 0, 8 * 2 * G::NKB1, 0u);
+      mma_seg<C, BF16, CG, TT, sD2>(sb, tmem_base, bar0, rs, 0, 8 * 2 * G::NKB1 * G::PH, 0u);
       commit(3);
-      mma_seg<C, BF16, CG, sD1E>(sb, tmem_base, bar0, rs, G::D1E_A + G::D1E_B, G::D1E_STEPS, 1u);
+      mma_seg<C, BF16, CG, TT, sD1E>(sb, tmem_base, bar0, rs, G::D1E_A + G::D1E_B, G::D1E_STEPS, 1u);
       wait_epi(4);                                   // U1 staged, region B drained
       if (has_next) {
         wait_epi(0);                                 // next group's X0 staged
-        mma_seg<C, BF16, CG, sE1>(sb, tmem_base, bar0, rs, 0, P.e1_steps, 0u, split_e1 != 0);
+        mma_seg<C, BF16, CG, TT, sE1>(sb, tmem_base, bar0, rs, 0, P.e1_steps, 0u, split_e1 != 0);
         commit(0);
       }
-      mma_seg<C, BF16, CG, sD1U>(sb, tmem_base, bar0, rs, 0, 13 * G::NKB1, 1u);
+      mma_seg<C, BF16, CG, TT, sD1U>(sb, tmem_base, bar0, rs, 0, 13 * G::NKB1 * G::PH, 1u);
       commit(4);
       first = false;
     }
@@ -735,12 +843,12 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
         constexpr int HALVES = (C >= 32 && MODE != kD1) ? 2 : 1;
         for (int u = set; u < nt * HALVES; u += G::SETS) {
           const int t = u / HALVES, cb = (u % HALVES) * (C / HALVES);
-          epilogue_tile<C, BF16, MODE>(sb, tmem_base, t, q, lane, par, nv, pg_out, scr(), lgx, cb, cb + C / HALVES, set);
+          epilogue_tile<C, BF16, MODE, TT>(sb, tmem_base, t, q, lane, par, nv, pg_out, scr(), lgx, cb, cb + C / HALVES, set);
         }
       };
       using std::integral_constant;
       if (first) {
-        load_x0<C, BF16>(sb, hist, g0, n_valid, split_e1, et, list, seg_cnt);
+        load_x0<C, BF16, TT>(sb, hist, g0, n_valid, split_e1, et, list, seg_cnt);
         done(0);
         wait_acc(0);
         layer(integral_constant<int, kE1>{}, G::T, n_valid, lg);
@@ -748,17 +856,17 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
         first = false;
       }
       wait_acc(1);
-      layer(integral_constant<int, kE2>{}, G::T / 2, n_valid, lg);
+      layer(integral_constant<int, kE2>{}, (G::T + 1) / 2, n_valid, lg);
       done(2);
       if (has_next) {                                // P1 is dead (e2's MMAs retired): stage the next input
-        load_x0<C, BF16>(sb, hist, gn0, n_valid_next, split_e1, et, list, seg_cnt);
+        load_x0<C, BF16, TT>(sb, hist, gn0, n_valid_next, split_e1, et, list, seg_cnt);
         done(0);
       }
       wait_acc(2);
       layer(integral_constant<int, kB>{}, (G::T + 3) / 4, n_valid, lg);
       done(3);
       wait_acc(3);
-      layer(integral_constant<int, kD2>{}, G::T / 2, n_valid, lg);
+      layer(integral_constant<int, kD2>{}, (G::T + 1) / 2, n_valid, lg);
       done(4);
       if (has_next) {
         wait_acc(0);
@@ -838,16 +946,18 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst_all) {
       {gE2, 1, C, 15, N1, 0, 0},        {gD1Ea, 4, 2 * C, 25, N1, C, 0},     {gB, 2, C, 5, N1, 0, 0},
       {gD1Eb, 4, 2 * C, 25, N1, C, A},  {gD2, 3, 2 * C, 15, 2 * N1, 0, 0},   {gD1Ec, 4, 2 * C, 25, N1, C, A + B},
       {gE1, 0, kHistCh, 25, 1, 0, 0},   {gD1U, 4, 2 * C, 25, N1, 0, 0}};
+  constexpr bool B16 = G::B16, FX = G::FX;
   for (const SegDef& d : defs) {
     const float* W = w->conv_w[d.layer];          // [C][cin][taps]
     for (int s = 0; s < P.seg_steps[d.seg]; ++s) {
-      const int f = d.f0 + s;                     // step index inside the sub-layer
+      const int fp = d.f0 + s;                    // physical step index inside the sub-layer
+      const int f = fp / G::PH, part = fp % G::PH;   // logical step; FX: part 0 = main (TF32), part 1 = correction (BF16)
       int u, kk, pass = 0;                        // tap pair, K block
-      if (d.seg == gE1 && BF16) { u = 2 * f; kk = 0; }             // 16-bit e1: K chunk h of step f holds tap pair 2f + h
+      if (d.seg == gE1 && B16) { u = 2 * f; kk = 0; }             // 16-bit e1: K chunk h of step f holds tap pair 2f + h
       else if (d.seg == gE1) { pass = f / 13; u = f % 13; kk = 0; }   // e1 split runs [pass][tap pair]
       else { u = f / d.nkb; kk = f % d.nkb; }
       unsigned char* step = dst + P.seg_off[d.seg] + (size_t)s * G::STEP_BYTES;
-      if (d.seg == gE1 && !BF16 && split_e1) {
+      if (d.seg == gE1 && BF16 == 0 && split_e1) {
         // split e1 of the TF32 kernel: BF16 pieces w = w1 + w2; pass 0 (13 steps) holds [w1 | w1] (meets [a1 | a2]),
         // pass 1 (7 steps) [w2 of pair 2w | w2 of pair 2w + 1] (meets [a1 two rows apart])
         if (pass) u = 2 * (f - 13);
@@ -872,17 +982,33 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst_all) {
       // last tap pair (odd tap missing): an N = C step -- half as many B rows, all of the even tap, split over the pair
       const bool half_n = 2 * u + 1 >= d.taps;
       const int nb = half_n ? G::NB / 2 : G::NB;
+      if (FX && part == 1) {
+        // correction step: K chunk 0 = bf16(w) of the 8 input channels of K block kk (meets a_lo), K chunk 1 =
+        // bf16(w - tf32(w)) of the same channels (meets bf16(a))
+        for (int h = 0; h < 2; ++h)
+          for (int nl = 0; nl < nb; ++nl)
+            for (int e = 0; e < 8; ++e) {
+              const int n = rank * nb + nl;
+              const int co = n % C, j = 2 * u + n / C;
+              const int cl = 8 * kk + e;
+              const bool real = j < d.taps && ((d.seg == gE1) ? cl < kHistCh : true);
+              const float v = real ? W[((size_t)co * d.cin + d.ch_base + cl) * d.taps + j] : 0.0f;
+              const uint16_t out = h == 0 ? bf16_rne(v) : bf16_rne(v - tf32_rna(v));
+              memcpy(step + ((size_t)h * nb + nl) * 16 + e * 2, &out, 2);
+            }
+        continue;
+      }
       for (int h = 0; h < 2; ++h)
         for (int nl = 0; nl < nb; ++nl)           // rows [0, C): even tap 2u, rows [C, 2C): odd tap 2u + 1
           for (int e = 0; e < G::PER; ++e) {
             const int n = rank * nb + nl;
-            const bool e1x2 = d.seg == gE1 && BF16;
+            const bool e1x2 = d.seg == gE1 && B16;
             const int co = n % C, j = 2 * (u + (e1x2 ? h : 0)) + n / C;
             const int cl = e1x2 ? e : (2 * kk + h) * G::PER + e;   // channel inside the sub-layer's range
             const bool real = j < d.taps && ((d.seg == gE1) ? cl < kHistCh : true);
             const float v = real ? W[((size_t)co * d.cin + d.ch_base + cl) * d.taps + j] : 0.0f;
             unsigned char* p = step + ((size_t)h * nb + nl) * 16 + e * G::ES;
-            if (BF16) {
+            if (B16) {
               const uint16_t b = (BF16 == 2) ? fp16_rne(v) : bf16_rne(v);
               memcpy(p, &b, 2);
             } else {
@@ -896,38 +1022,27 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst_all) {
   }
 }
 
-template <int C, int BF16, int CG>
+template <int C, int BF16, int CG, int TT = 0>
 void launch_impl(const float* hist, int n_int, const void* packed, int split_e1, float* probs, int sm_count,
-                 const int* list, const int* n_list, const int* seg_cnt, cudaStream_t s) {
-  using G = Geo<C, BF16, CG>;
+                 const int* list, const int* n_list, const int* seg_cnt, bool pdl, cudaStream_t s) {
+  using G = Geo<C, BF16, CG, TT>;
   const int n_groups = (n_int + G::T - 1) / G::T;
   const int n_pg = (n_groups + CG - 1) / CG, max_pairs = sm_count / CG;
   const int grid = CG * (n_pg < max_pairs ? n_pg : max_pairs);
-  if (CG == 1) {
-    k_unet_tc<C, BF16, CG><<<grid, G::THREADS, G::SMEM, s>>>(hist, n_int, static_cast<const unsigned char*>(packed),
-                                                            split_e1, probs, list, n_list, seg_cnt);
-  } else {
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(grid);
-    cfg.blockDim = dim3(G::THREADS);
-    cfg.dynamicSmemBytes = G::SMEM;
-    cfg.stream = s;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeClusterDimension;
-    at[0].val.clusterDim.x = CG;
-    at[0].val.clusterDim.y = 1;
-    at[0].val.clusterDim.z = 1;
-    cfg.attrs = at;
-    cfg.numAttrs = 1;
-    cudaLaunchKernelEx(&cfg, k_unet_tc<C, BF16, CG>, hist, n_int, static_cast<const unsigned char*>(packed), split_e1,
-                       probs, list, n_list, seg_cnt);
-  }
+  PdlLaunch L(dim3(grid), dim3(G::THREADS), G::SMEM, s, pdl, CG);
+  cudaLaunchKernelEx(&L.cfg, k_unet_tc<C, BF16, CG, TT>, hist, n_int, static_cast<const unsigned char*>(packed), split_e1,
+                     probs, list, n_list, seg_cnt);
 }
 
 template <int C, int BF16, int CG>
 cudaError_t setup_impl() {
-  return cudaFuncSetAttribute(k_unet_tc<C, BF16, CG>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              Geo<C, BF16, CG>::SMEM);
+  cudaError_t e = cudaFuncSetAttribute(k_unet_tc<C, BF16, CG, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       Geo<C, BF16, CG, 0>::SMEM);
+  constexpr int TS = (C == 64 && CG == 2 && BF16 != 3) ? 1 : 0;   // the small-batch instance (one interval per group)
+  if (e == cudaSuccess && TS == 1)
+    e = cudaFuncSetAttribute(k_unet_tc<C, BF16, CG, TS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             Geo<C, BF16, CG, TS>::SMEM);
+  return e;
 }
 
 #define PVF_TC_DISPATCH_CG(CALL, CG_)                             \
@@ -937,9 +1052,12 @@ cudaError_t setup_impl() {
     else if (channels == 32) { if (fm == 1) CALL(32, 1, CG_); else if (fm == 2) CALL(32, 2, CG_); else CALL(32, 0, CG_); } \
     else { if (fm == 1) CALL(16, 1, CG_); else if (fm == 2) CALL(16, 2, CG_); else CALL(16, 0, CG_); }        \
   } while (0)
+// PVF_PREC_FP32 on the tensor cores = the FP32-accurate format 3, CTA pairs only
 #define PVF_TC_DISPATCH(CALL)                                     \
   do {                                                            \
-    if (cta_pair) PVF_TC_DISPATCH_CG(CALL, 2); else PVF_TC_DISPATCH_CG(CALL, 1);   \
+    if (precision == PVF_PREC_FP32) {                             \
+      if (channels == 64) CALL(64, 3, 2); else if (channels == 32) CALL(32, 3, 2); else CALL(16, 3, 2);   \
+    } else if (cta_pair) PVF_TC_DISPATCH_CG(CALL, 2); else PVF_TC_DISPATCH_CG(CALL, 1);   \
   } while (0)
 
 }  // namespace
@@ -962,6 +1080,7 @@ cudaError_t unet_tc_setup(int channels, int precision, int split_mask, int cta_p
   if (channels != 64 && channels != 32 && channels != 16) return cudaErrorInvalidValue;
   if (split_mask & ~1) return cudaErrorInvalidValue;          // only the e1 split is built
   if (precision != PVF_PREC_TF32 && split_mask) return cudaErrorInvalidValue;   // the split is a TF32 remedy
+  if (precision == PVF_PREC_FP32 && !cta_pair) return cudaErrorInvalidValue;    // FP32 on the tensor cores runs as CTA pairs
   cudaError_t e = cudaSuccess;
 #define PVF_CALL(C_, B_, G_) e = setup_impl<C_, B_, G_>()
   PVF_TC_DISPATCH(PVF_CALL);
@@ -971,10 +1090,19 @@ cudaError_t unet_tc_setup(int channels, int precision, int split_mask, int cta_p
 
 void launch_unet_tc(const float* hist, int n_intervals_total, const void* packed_dev, int channels, int precision,
                     int split_mask, int cta_pair, float* probs, int sm_count, const int* list, const int* n_list,
-                    const int* seg_cnt, cudaStream_t s) {
+                    const int* seg_cnt, bool pdl, cudaStream_t s) {
   if (n_intervals_total <= 0) return;
+  // Small batches (NEXT-4): while one interval per CTA still fits the machine in a single round, groups
+  // of one interval finish sooner than groups of two on half as many SMs.  Same arithmetic per interval, identical bits.
+  if (channels == 64 && cta_pair && precision != PVF_PREC_FP32 && list == nullptr && n_intervals_total <= sm_count) {
+    const int fm = precision == PVF_PREC_BF16 ? 1 : (precision == PVF_PREC_FP16 ? 2 : 0);
+#define PVF_SMALL(B_) launch_impl<64, B_, 2, 1>(hist, n_intervals_total, packed_dev, split_mask & 1, probs, sm_count, list, n_list, seg_cnt, pdl, s)
+    if (fm == 1) PVF_SMALL(1); else if (fm == 2) PVF_SMALL(2); else PVF_SMALL(0);
+#undef PVF_SMALL
+    return;
+  }
 #define PVF_CALL(C_, B_, G_) \
-  launch_impl<C_, B_, G_>(hist, n_intervals_total, packed_dev, split_mask & 1, probs, sm_count, list, n_list, seg_cnt, s)
+  launch_impl<C_, B_, G_>(hist, n_intervals_total, packed_dev, split_mask & 1, probs, sm_count, list, n_list, seg_cnt, pdl, s)
   PVF_TC_DISPATCH(PVF_CALL);
 #undef PVF_CALL
 }

@@ -34,6 +34,7 @@ struct pvf_ctx {
   int32_t* seg_cnt = nullptr;
   uint32_t* flags = nullptr;
   float* hist = nullptr;
+  int32_t hist_events = 0;        // events the histogram buffer holds: max_events, or l2_chunk_events if that is smaller
   // host-io staging (enable_host_io)
   float* st_feat = nullptr;
   int32_t* st_off = nullptr;
@@ -51,7 +52,8 @@ struct pvf_ctx {
   static constexpr int kTimedRuns = 64;   // ring of per-run event sets (stage timing)
   cudaEvent_t ev[kTimedRuns][5] = {};
   int64_t timed_runs = 0;                 // runs recorded since the last pvf_stage_times_ms
-  int32_t last_n_events = 0;
+  int32_t last_n_events = 0;      // events whose histograms the buffer holds after the last run ...
+  int32_t last_e0 = 0;            // ... and the first of them (non-zero with l2_chunk_events: the last chunk)
   std::string cuda_err;
 };
 
@@ -70,6 +72,11 @@ void conv_shapes(int C, int shp[6][3]) {
   memcpy(shp, s, sizeof(s));
 }
 
+// Which kernels serve the configuration: the tcgen05 kernels (FC with the 25 -> 800 layer on tensor cores + k_unet_tc) for
+// every precision, except PVF_PREC_FP32 without CTA pairs = the CUDA-core kernels (k_fc_hist + k_unet_simt), kept as the
+// bisecting reference of the GPU side.
+bool uses_tc(const pvf_config* c) { return c->precision != PVF_PREC_FP32 || c->unet_cta_pair != 0; }
+
 bool config_ok(const pvf_config* c) {
   if (!c) return false;
   if (c->n_intervals != kIntervals || c->n_bins != kBins) return false;
@@ -84,10 +91,10 @@ bool config_ok(const pvf_config* c) {
   // split_mask: only bit 0 (e1) is built, and only for TF32 (unet_tc_setup would refuse anything else later)
   if (c->split_mask != 0 && !(c->precision == PVF_PREC_TF32 && c->split_mask == 1)) return false;
   if (c->max_events < 1 || c->max_tracks < 1 || c->max_tracks > 0x7fffffffLL) return false;
-  if (c->elide_empty_intervals && c->precision == PVF_PREC_FP32) return false;   // tensor-core modes only
   if (c->unet_cta_pair != 0 && c->unet_cta_pair != 1) return false;
-  if (c->unet_cta_pair && c->precision == PVF_PREC_FP32) return false;           // tensor-core modes only
+  if (c->elide_empty_intervals && !uses_tc(c)) return false;                     // tensor-core kernels only
   if (!(c->boundary_margin_mm >= 0.0f && c->boundary_margin_mm < 4.9f)) return false;
+  if (c->l2_chunk_events < 0) return false;
   if (c->boundary_margin_mm > 0.0f && c->max_tracks > (int64_t)kEntryMask) return false;
   return true;
 }
@@ -105,9 +112,9 @@ Layout make_layout(const pvf_config* c) {
     L.conv_b_off[k] = f; f += shp[k][0]; f = (f + 63) / 64 * 64;
   }
   L.conv_f32 = take(sizeof(float) * f);
-  L.tc_packed = take(c->precision == PVF_PREC_FP32 ? 0 : unet_tc_packed_bytes(c->unet_channels, c->precision, c->split_mask, c->unet_cta_pair));
+  L.tc_packed = take(!uses_tc(c) ? 0 : unet_tc_packed_bytes(c->unet_channels, c->precision, c->split_mask, c->unet_cta_pair));
   const size_t E = (size_t)c->max_events, T = (size_t)c->max_tracks;
-  L.fc_w5img = take(c->precision == PVF_PREC_FP32 ? 0 : fc_tc_packed_bytes());
+  L.fc_w5img = take(!uses_tc(c) ? 0 : fc_tc_packed_bytes());
   L.el_list = take(c->elide_empty_intervals ? sizeof(int32_t) * E * kIntervals : 0);
   L.el_count = take(c->elide_empty_intervals ? 256 : 0);
   L.el_p0 = take(c->elide_empty_intervals ? sizeof(float) * kGlobalBins : 0);
@@ -115,7 +122,8 @@ Layout make_layout(const pvf_config* c) {
   L.seg_off = take(sizeof(int32_t) * E * kIntervals);
   L.seg_cnt = take(sizeof(int32_t) * E * kIntervals);
   L.flags = take(sizeof(uint32_t) * E);
-  L.hist = take(sizeof(float) * (E * kIntervals * kFcOut + (c->precision == PVF_PREC_FP32 ? 0 : kFcDumpFloats)));
+  const size_t EH = (c->l2_chunk_events > 0 && (size_t)c->l2_chunk_events < E) ? (size_t)c->l2_chunk_events : E;
+  L.hist = take(sizeof(float) * (EH * kIntervals * kFcOut + (!uses_tc(c) ? 0 : kFcDumpFloats)));
   if (c->enable_host_io) {
     L.st_feat = take(sizeof(float) * 9 * T);
     L.st_off = take(sizeof(int32_t) * (E + 1));
@@ -143,7 +151,7 @@ pvf_status fail_cuda(pvf_ctx* h, cudaError_t e, const char* where) {
 
 // seg_cnt != nullptr: hist is the pool's histogram as the tensor-core FC kernel leaves it (empty intervals unwritten)
 void enqueue_unet(pvf_ctx* h, const float* hist, int n_events, float* out_probs, cudaStream_t s,
-                  const int* list = nullptr, const int* n_list = nullptr, const int* seg_cnt = nullptr);
+                  const int* list = nullptr, const int* n_list = nullptr, const int* seg_cnt = nullptr, bool pdl = false);
 
 bool peaks_ok(const pvf_peaks* p) { return p && p->z_mm && p->prob && p->bin && p->count; }
 
@@ -186,6 +194,7 @@ pvf_status create_impl(const pvf_weights* w, const pvf_config* cfg, void* dev_po
   h->seg_cnt = reinterpret_cast<int32_t*>(B + L.seg_cnt);
   h->flags = reinterpret_cast<uint32_t*>(B + L.flags);
   h->hist = reinterpret_cast<float*>(B + L.hist);
+  h->hist_events = (cfg->l2_chunk_events > 0 && cfg->l2_chunk_events < cfg->max_events) ? cfg->l2_chunk_events : cfg->max_events;
   if (cfg->enable_host_io) {
     h->st_feat = reinterpret_cast<float*>(B + L.st_feat);
     h->st_off = reinterpret_cast<int32_t*>(B + L.st_off);
@@ -220,8 +229,9 @@ pvf_status create_impl(const pvf_weights* w, const pvf_config* cfg, void* dev_po
     h->conv_ptrs.b[k] = h->conv_f32 + L.conv_b_off[k];
   }
   if (e == cudaSuccess) {
-    if (cfg->precision == PVF_PREC_FP32) {
+    if (!uses_tc(cfg)) {
       e = unet_simt_setup(cfg->unet_channels);
+      if (e == cudaSuccess) e = fc_hist_setup();
     } else {
       const size_t nb = unet_tc_packed_bytes(cfg->unet_channels, cfg->precision, cfg->split_mask, cfg->unet_cta_pair);
       std::vector<unsigned char> img(nb);
@@ -275,13 +285,13 @@ pvf_status create_impl(const pvf_weights* w, const pvf_config* cfg, void* dev_po
 }
 
 void enqueue_unet(pvf_ctx* h, const float* hist, int n_events, float* out_probs, cudaStream_t s, const int* list,
-                  const int* n_list, const int* seg_cnt) {
+                  const int* n_list, const int* seg_cnt, bool pdl) {
   const int n_int = n_events * kIntervals;
-  if (h->cfg.precision == PVF_PREC_FP32)
-    launch_unet_simt(hist, n_int, h->conv_ptrs, h->cfg.unet_channels, out_probs, s);
+  if (!uses_tc(&h->cfg))
+    launch_unet_simt(hist, n_int, h->conv_ptrs, h->cfg.unet_channels, out_probs, pdl, s);
   else
     launch_unet_tc(hist, n_int, h->tc_packed, h->cfg.unet_channels, h->cfg.precision, h->cfg.split_mask,
-                   h->cfg.unet_cta_pair, out_probs, h->sm_count, list, n_list, seg_cnt, s);
+                   h->cfg.unet_cta_pair, out_probs, h->sm_count, list, n_list, seg_cnt, pdl, s);
 }
 
 }  // namespace
@@ -299,6 +309,7 @@ void pvf_default_config(pvf_config* c, int32_t max_events, int64_t max_tracks) {
   c->max_events = max_events; c->max_tracks = max_tracks;
   c->enable_stage_timing = 0; c->enable_host_io = 0; c->elide_empty_intervals = 0; c->boundary_margin_mm = 0.0f;
   c->unet_cta_pair = 0;
+  c->l2_chunk_events = 0;
 }
 
 size_t pvf_workspace_bytes(const pvf_config* cfg) {
@@ -327,29 +338,46 @@ pvf_status pvf_run(pvf_handle h, const pvf_tracks* t, int32_t n_events, float* o
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   const bool timing = h->cfg.enable_stage_timing != 0 && !h->suppress_timing;
   cudaEvent_t* ev = h->ev[h->timed_runs % pvf_ctx::kTimedRuns];
+  // Programmatic dependent launch (pdl.cuh) chains the kernels of the run: each may start while its predecessor still
+  // runs and does its weight-only prologue before it waits for it.  Not with stage timing (an event record between two
+  // kernels orders them completely anyway) and not in the elision mode (a memset sits in the chain).
+  const bool pdl = !timing && !h->cfg.elide_empty_intervals;
+  const bool tc = uses_tc(&h->cfg);
   if (timing) cudaEventRecord(ev[0], s);
   launch_sort(t->feat[0], t->event_offsets, n_events, (int)t->n_tracks, h->perm, h->seg_off, h->seg_cnt, h->flags,
               h->cfg.boundary_margin_mm * 0.1f, s);
   if (timing) cudaEventRecord(ev[1], s);
-  if (h->cfg.precision == PVF_PREC_FP32)
-    launch_fc_hist(t->feat, t->event_offsets, h->perm, h->seg_off, h->seg_cnt, h->fc_params, n_events, h->hist, s);
-  else
-    launch_fc_hist_tc(t->feat, t->event_offsets, h->perm, h->seg_off, h->seg_cnt, h->fc_params, h->fc_w5img, n_events,
-                      h->hist, h->hist + (size_t)h->cfg.max_events * kIntervals * kFcOut, h->sm_count, s);
-  if (timing) cudaEventRecord(ev[2], s);
-  if (h->cfg.elide_empty_intervals) {
-    launch_compact_fill(h->seg_cnt, n_events * kIntervals, h->el_list, h->el_count, h->el_p0, out_probs, s);
-    enqueue_unet(h, h->hist, n_events, out_probs, s, h->el_list, h->el_count);   // the list holds non-empty intervals only
-  } else {
-    // tensor-core modes: k_fc_hist_tc leaves the histograms of empty intervals unwritten, the UNet takes them as zeros
-    enqueue_unet(h, h->hist, n_events, out_probs, s, nullptr, nullptr,
-                 h->cfg.precision == PVF_PREC_FP32 ? nullptr : h->seg_cnt);
+  // FC + segmented sum, then the UNet -- over the whole batch, or (l2_chunk_events > 0) chunk by chunk through ONE
+  // chunk-sized histogram buffer, so that the histograms are written and read back while they are still in the L2
+  // cache and never travel to HBM ("memory layout fusion ... explicit workspace reuse"; NEXT-2).
+  const int chunk = h->hist_events < n_events ? h->hist_events : n_events;
+  float* dump = h->hist + (size_t)h->hist_events * kIntervals * kFcOut;
+  if (timing && chunk < n_events) cudaEventRecord(ev[2], s);   // chunked: FC and UNet interleave, their sum is reported as "UNet"
+  for (int e0 = 0; e0 < n_events; e0 += chunk) {
+    const int ne = n_events - e0 < chunk ? n_events - e0 : chunk;
+    const int32_t* so = h->seg_off + (size_t)e0 * kIntervals;
+    const int32_t* sc = h->seg_cnt + (size_t)e0 * kIntervals;
+    if (!tc)
+      launch_fc_hist(t->feat, t->event_offsets, h->perm, so, sc, h->fc_params, ne, h->hist, h->sm_count, pdl, s);
+    else
+      launch_fc_hist_tc(t->feat, t->event_offsets, h->perm, so, sc, h->fc_params, h->fc_w5img, ne, h->hist, dump,
+                        h->sm_count, pdl, s);
+    if (timing && chunk >= n_events) cudaEventRecord(ev[2], s);
+    float* po = out_probs + (size_t)e0 * kGlobalBins;
+    if (h->cfg.elide_empty_intervals) {
+      launch_compact_fill(sc, ne * kIntervals, h->el_list, h->el_count, h->el_p0, po, s);
+      enqueue_unet(h, h->hist, ne, po, s, h->el_list, h->el_count);   // the list holds non-empty intervals only
+    } else {
+      // tensor-core modes: k_fc_hist_tc leaves the histograms of empty intervals unwritten, the UNet takes them as zeros
+      enqueue_unet(h, h->hist, ne, po, s, nullptr, nullptr, tc ? sc : nullptr, pdl);
+    }
   }
   if (timing) cudaEventRecord(ev[3], s);
   launch_peaks(out_probs, n_events, h->cfg.peak_threshold, h->flags, pk->z_mm, pk->prob, pk->bin, pk->count,
-               pk->event_flags, s);
+               pk->event_flags, pdl, s);
   if (timing) { cudaEventRecord(ev[4], s); ++h->timed_runs; }
-  h->last_n_events = n_events;
+  h->last_n_events = chunk < n_events ? (n_events - 1) % chunk + 1 : n_events;   // what the histogram buffer holds now
+  h->last_e0 = n_events - h->last_n_events;
   cudaError_t e = cudaPeekAtLastError();
   if (e != cudaSuccess) return fail_cuda(h, e, "pvf_run launch");
   return PVF_OK;
@@ -453,7 +481,7 @@ pvf_status pvf_find_peaks(pvf_handle h, const float* probs, int32_t n_events, co
   if (n_events == 0) return PVF_OK;
   if (!probs || !peaks_ok(pk)) return PVF_ERR_ARG;
   launch_peaks(probs, n_events, h->cfg.peak_threshold, nullptr, pk->z_mm, pk->prob, pk->bin, pk->count,
-               pk->event_flags, static_cast<cudaStream_t>(cuda_stream));
+               pk->event_flags, false, static_cast<cudaStream_t>(cuda_stream));
   cudaError_t e = cudaPeekAtLastError();
   if (e != cudaSuccess) return fail_cuda(h, e, "pvf_find_peaks launch");
   return PVF_OK;
@@ -474,11 +502,12 @@ pvf_status pvf_debug_copy_histogram(pvf_handle h, float* dev_out, int32_t n_even
   if (!h || !dev_out || !cuda_stream || n_events < 0) return PVF_ERR_ARG;
   if (n_events > h->last_n_events) return PVF_ERR_ARG;
   if (n_events == 0) return PVF_OK;
-  if (h->cfg.precision == PVF_PREC_FP32) {
+  if (!uses_tc(&h->cfg)) {
     PVF_CUDA(h, cudaMemcpyAsync(dev_out, h->hist, sizeof(float) * (size_t)n_events * kIntervals * kFcOut,
                                 cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(cuda_stream)));
   } else {   // the tensor-core FC kernel writes non-empty intervals only: empty ones are zeros by definition
-    launch_copy_hist_masked(h->hist, h->seg_cnt, n_events * kIntervals, dev_out, static_cast<cudaStream_t>(cuda_stream));
+    launch_copy_hist_masked(h->hist, h->seg_cnt + (size_t)h->last_e0 * kIntervals, n_events * kIntervals, dev_out,
+                            static_cast<cudaStream_t>(cuda_stream));
     PVF_CUDA(h, cudaPeekAtLastError());
   }
   return PVF_OK;
@@ -504,8 +533,9 @@ pvf_status pvf_stage_times_ms(pvf_handle h, float out_ms[4]) {
 
 int32_t pvf_launches_per_run(pvf_handle h, int32_t n_events) {
   if (!h || n_events <= 0) return 0;
-  return 1 /*sort*/ + fc_hist_launches(n_events) + 1 /*unet*/ + 1 /*peaks*/ +
-         (h->cfg.elide_empty_intervals ? 2 /*work list, constant fill*/ : 0);
+  const int chunks = (n_events + h->hist_events - 1) / h->hist_events;   // 1 unless l2_chunk_events splits the batch
+  return 1 /*sort*/ + chunks * (fc_hist_launches(n_events) + 1 /*unet*/ +
+                                (h->cfg.elide_empty_intervals ? 2 /*work list, constant fill*/ : 0)) + 1 /*peaks*/;
 }
 
 pvf_status pvf_destroy(pvf_handle h) {

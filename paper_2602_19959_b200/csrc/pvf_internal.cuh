@@ -64,6 +64,8 @@ __device__ __forceinline__ int entry_interval(int ent, const float* __restrict__
 }
 #endif
 
+// `pdl` on the launchers below: launch with programmatic stream serialization (pdl.cuh) -- the kernel may start while
+// its predecessor on the stream still runs and waits for it (griddepcontrol.wait) before it reads what that one wrote.
 // a0: interval assignment + stable per-event counting sort (k_sort.cu).  mfrac > 0: boundary tracks get a
 // second entry (perm then holds up to 2 entries per track).
 void launch_sort(const float* z_poca, const int32_t* event_offsets, int n_events, int n_tracks, int32_t* perm,
@@ -72,7 +74,8 @@ void launch_sort(const float* z_poca, const int32_t* event_offsets, int n_events
 // a1+a2: per-track FC and fixed-order segmented sum into H [n_events,40,8,100] (k_fc.cu)
 void launch_fc_hist(const float* const feat[9], const int32_t* event_offsets, const int32_t* perm,
                     const int32_t* seg_off, const int32_t* seg_cnt, const float* fc_params,
-                    int n_events, float* hist, cudaStream_t s);
+                    int n_events, float* hist, int sm_count, bool pdl, cudaStream_t s);
+cudaError_t fc_hist_setup();
 int fc_hist_launches(int n_events);
 
 // a1+a2, tensor-core version (k_fc_tc.cu): 25 -> 800 layer as 3-pass TF32 tcgen05 MMAs, sum in the epilogue
@@ -81,7 +84,7 @@ void fc_tc_pack(const float* w5, const float* b5, void* host_dst);
 cudaError_t fc_tc_setup();
 void launch_fc_hist_tc(const float* const feat[9], const int32_t* event_offsets, const int32_t* perm,
                        const int32_t* seg_off, const int32_t* seg_cnt, const float* fc_params, const void* w5img,
-                       int n_events, float* hist, float* dump, int sm_count, cudaStream_t s);
+                       int n_events, float* hist, float* dump, int sm_count, bool pdl, cudaStream_t s);
 // dump: kFcDumpFloats floats of scratch that the padding lanes of the accumulator tiles write their sums to
 constexpr size_t kFcDumpFloats = (size_t)kIntervals * kFcOut + 1024;
 
@@ -89,7 +92,7 @@ constexpr size_t kFcDumpFloats = (size_t)kIntervals * kFcOut + 1024;
 struct UnetParamsF32 { const float* w[6]; const float* b[6]; };
 cudaError_t unet_simt_setup(int channels);
 void launch_unet_simt(const float* hist, int n_intervals_total, const UnetParamsF32& p, int channels,
-                      float* probs, cudaStream_t s);
+                      float* probs, bool pdl, cudaStream_t s);
 
 // a3, tcgen05/TMEM path (k_unet_tc.cu)
 // cta_pair: 0 = one CTA per MMA (cta_group::1); 1 = clusters of two CTAs sharing every MMA (cta_group::2)
@@ -101,7 +104,7 @@ cudaError_t unet_tc_setup(int channels, int precision, int split_mask, int cta_p
 // seg_cnt (device, optional): tracks per interval; intervals with none are taken as zeros without reading hist
 void launch_unet_tc(const float* hist, int n_intervals_total, const void* packed_dev, int channels,
                     int precision, int split_mask, int cta_pair, float* probs, int sm_count, const int* list,
-                    const int* n_list, const int* seg_cnt, cudaStream_t s);
+                    const int* n_list, const int* seg_cnt, bool pdl, cudaStream_t s);
 
 // NEXT-2, empty-interval elision (k_compact.cu): work list of non-empty intervals + constant fill of the rest
 // canonical histogram out of the pool's: out[n] = seg_cnt[n] > 0 ? hist[n] : 0 (debug accessor, tensor-core modes)
@@ -112,6 +115,6 @@ void launch_compact_fill(const int32_t* seg_cnt, int n_total, int32_t* list, int
 // a4: peak finder (k_peaks.cu)
 void launch_peaks(const float* probs, int n_events, float threshold, const uint32_t* flags_in,
                   float* z_mm, float* prob, int32_t* bin, int32_t* count, uint32_t* flags_out,
-                  cudaStream_t s);
+                  bool pdl, cudaStream_t s);
 
 }  // namespace pvf

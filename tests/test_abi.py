@@ -89,5 +89,5 @@ def test_null_arguments(lib):
 
 
 def test_struct_sizes_match_header():
-    # int32 x2, float x2, int32 x4, int32 x5, float x2, int32 x5, int64, int32 x3, float, int32 (+4 tail padding)
+    # int32 x2, float x2, int32 x4, int32 x5, float x2, int32 x5, int64, int32 x3, float, int32 x2
     assert C.sizeof(pvf_config) == 112

@@ -21,8 +21,10 @@ import paper_2602_19959_b200 as pkg
 from paper_2602_19959_b200 import PVFinder
 
 # fp16 (NEXT-3, the paper's roadmap precision): 10-bit mantissa like TF32 but without the e1 split -> stated 2e-3
-TOL = {"fp32": 2e-5, "tf32": 1e-3, "bf16": 2e-2, "fp16": 2e-3}
-SPLIT = {"fp32": 0, "tf32": 1, "bf16": 0, "fp16": 0}
+# "fp32" = PVF_PREC_FP32 on the tensor cores (kind::tf32 + a BF16 correction MMA per product; the binding's default);
+# "simt" = PVF_PREC_FP32 with unet_cta_pair = 0: the CUDA-core kernels k_fc_hist + k_unet_simt (bisecting reference)
+TOL = {"fp32": 2e-5, "simt": 2e-5, "tf32": 1e-3, "bf16": 2e-2, "fp16": 2e-3}
+SPLIT = {"fp32": 0, "simt": 0, "tf32": 1, "bf16": 0, "fp16": 0}
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -49,8 +51,10 @@ def _run(pvf, ev, n=None):
 
 
 def _make(w, ev, prec="fp32", **kw):
-    return PVFinder(w, max_events=max(ev.n_events, 1), max_tracks=max(ev.n_tracks, 1), precision=prec,
-                    split_mask=kw.pop("split_mask", SPLIT[prec]), **kw)
+    if prec == "simt":
+        kw["cta_pair"] = False
+    return PVFinder(w, max_events=max(ev.n_events, 1), max_tracks=max(ev.n_tracks, 1),
+                    precision="fp32" if prec == "simt" else prec, split_mask=kw.pop("split_mask", SPLIT[prec]), **kw)
 
 
 def _np(pk):
@@ -86,8 +90,8 @@ def test_peaks_bit_exact_on_identical_probabilities():
 
 
 # ------------------------------------------------------------------ a0 + a1 + a2: histogram
-# fp32 -> k_fc_hist (FP32 FMA); tf32 -> k_fc_hist_tc (tcgen05, 3-pass TF32 split): same tolerance for both
-@pytest.mark.parametrize("prec", ["fp32", "tf32"])
+# simt -> k_fc_hist (FP32 FMA); tf32 -> k_fc_hist_tc (tcgen05, 3-pass TF32 split): same tolerance for both
+@pytest.mark.parametrize("prec", ["simt", "tf32"])
 @pytest.mark.parametrize("kind", ["rand", "peaky"])
 def test_histogram_parity_and_determinism(kind, prec):
     ev = make_events("run3", 48, 1001)
@@ -121,7 +125,7 @@ def test_histogram_parity_and_determinism(kind, prec):
     assert torch.allclose(H, H2, rtol=1e-5, atol=1e-5)
 
 
-@pytest.mark.parametrize("prec", ["fp32", "tf32"])
+@pytest.mark.parametrize("prec", ["simt", "fp32", "tf32"])
 def test_edge_events_empty_dropped_nonfinite_and_long(prec):
     w = make_weights("rand", 3)
     base = make_events("pileup", 3, 9)
@@ -164,7 +168,7 @@ def test_edge_events_empty_dropped_nonfinite_and_long(prec):
     assert np.all(P[0] == P[0, 0]) and np.array_equal(P[0], P[3])
 
 
-@pytest.mark.parametrize("prec,margin", [("fp32", 0.0), ("tf32", 0.0), ("tf32", 0.5)])
+@pytest.mark.parametrize("prec,margin", [("simt", 0.0), ("tf32", 0.0), ("tf32", 0.5)])
 def test_corrupt_event_offsets_are_clamped_and_flagged(prec, margin):
     """The device-side event_offsets are data the host never sees: ranges that leave [0, n_tracks] or run backwards
     must not make any kernel touch memory outside the caller's / the pool's buffers (per-event
@@ -177,7 +181,7 @@ def test_corrupt_event_offsets_are_clamped_and_flagged(prec, margin):
     nbytes = pvf0.workspace_bytes()
     guard = 1 << 20
     pool = torch.full((nbytes + guard,), 0x5A, dtype=torch.uint8, device="cuda")
-    pvf = PVFinder(w, max_events=8, max_tracks=T, precision=prec, split_mask=SPLIT[prec], boundary_margin_mm=margin, pool=pool)
+    pvf = _make(w, ev, prec, boundary_margin_mm=margin, pool=pool)
     feat = torch.from_numpy(ev.feat).cuda()
     probs = torch.full((8, 4000), -1.0, device="cuda")
     pk = pvf.alloc_peaks(8)
@@ -267,7 +271,7 @@ def _peak_agreement(ref_probs, ref_bins, ref_count, got_bins, got_count):
     return m_all, n_all, lost
 
 
-@pytest.mark.parametrize("prec", ["fp32", "tf32", "bf16", "fp16"])
+@pytest.mark.parametrize("prec", ["fp32", "simt", "tf32", "bf16", "fp16"])
 @pytest.mark.parametrize("kind", ["rand", "peaky"])
 def test_whole_path_parity(prec, kind):
     # peaky: BASELINE.json config 1 (1000 events, ~5400 oracle peaks) so that 99.9 % is resolvable
@@ -300,7 +304,7 @@ def test_whole_path_parity(prec, kind):
     assert np.array_equal(own["bin"], got["bin"]) and np.array_equal(own["z"].view(np.uint32), got["z"].view(np.uint32))
 
 
-@pytest.mark.parametrize("prec", ["fp32", "tf32", "bf16", "fp16"])
+@pytest.mark.parametrize("prec", ["fp32", "simt", "tf32", "bf16", "fp16"])
 @pytest.mark.parametrize("ch", [32, 16])
 def test_width_sweep_parity(prec, ch):
     """BASELINE.json config 4: "Sweep UNet width 16/32/64 channels ... per-width tolerance 2e-2 on probabilities plus
@@ -358,7 +362,7 @@ def test_accuracy_vs_width_and_precision_table(ch):
     print("\n".join(rows))
 
 
-@pytest.mark.parametrize("prec", ["fp32", "tf32", "bf16", "fp16"])
+@pytest.mark.parametrize("prec", ["fp32", "simt", "tf32", "bf16", "fp16"])
 def test_unet_entry_point_on_synthetic_histograms(prec):
     """UNet alone: zero input (bias-only), one-hot inputs at the interval edges (padding), large values."""
     w = make_weights("rand", 5)
@@ -368,7 +372,8 @@ def test_unet_entry_point_on_synthetic_histograms(prec):
     H[2] = np.random.default_rng(3).gamma(2.0, 4.0, size=(40, 8, 100)).astype(np.float32)
     ref = O.unet_probs(H.astype(np.float64), w.conv_w, w.conv_b)
     ev = make_events("single", 1, 1)
-    pvf = PVFinder(w, max_events=E, max_tracks=1, precision=prec, split_mask=SPLIT[prec])
+    pvf = PVFinder(w, max_events=E, max_tracks=1, precision="fp32" if prec == "simt" else prec, split_mask=SPLIT[prec],
+                   cta_pair=prec != "simt")
     out = torch.empty(E, 4000, device="cuda")
     s = torch.cuda.Stream()
     pvf.run_unet(torch.from_numpy(H).cuda(), E, out, stream=s)
@@ -379,7 +384,7 @@ def test_unet_entry_point_on_synthetic_histograms(prec):
 
 
 # ------------------------------------------------------------------ NEXT-1: boundary tracks in two intervals
-@pytest.mark.parametrize("prec", ["fp32", "tf32"])
+@pytest.mark.parametrize("prec", ["simt", "tf32"])
 def test_boundary_tracks_two_intervals(prec):
     """with a margin, tracks near an interval edge also contribute to the neighbour.  Histogram
     and probabilities against the oracle run with the same margin; an event packed with edge tracks
@@ -416,7 +421,7 @@ def test_boundary_tracks_two_intervals(prec):
 
 
 # ------------------------------------------------------------------ NEXT-2: empty-interval elision
-@pytest.mark.parametrize("prec", ["tf32", "bf16", "fp16"])
+@pytest.mark.parametrize("prec", ["tf32", "bf16", "fp16", "fp32"])
 def test_empty_interval_elision_is_bit_identical(prec):
     """The UNet run only over non-empty intervals + the constant UNet(0) vector elsewhere must reproduce the
     plain path bit for bit (an interval's result does not depend on its group mates); includes an event
@@ -438,7 +443,66 @@ def test_empty_interval_elision_is_bit_identical(prec):
     p3, _ = _run(elided, ev)                                      # and again (work-list order may differ)
     assert torch.equal(p2, p3)
     with pytest.raises(pkg.PVFError):
-        _make(w, ev, "fp32", elide_empty=True)                    # tensor-core modes only
+        _make(w, ev, "simt", elide_empty=True)                    # tensor-core kernels only
+
+
+# ------------------------------------------------------------------ NEXT-2: histograms through an L2-sized chunk buffer
+@pytest.mark.parametrize("prec,chunk", [("tf32", 5), ("bf16", 16), ("fp32", 7), ("simt", 7), ("tf32", 64)])
+def test_l2_chunked_histogram_buffer_is_bit_identical(prec, chunk):
+    """l2_chunk_events: the pool holds the histograms of `chunk` events only and pvf_run walks the batch chunk by chunk
+    (FC + sum, then UNet, per chunk).  Same kernels on the same data: output identical to the whole-batch path; the
+    pool shrinks by the histograms that are no longer kept (PAPER.md:86 'explicit workspace reuse')."""
+    ev = make_events("run3", 37, 558)
+    w = make_weights("peaky", 2)
+    plain = _make(w, ev, prec)
+    chunked = _make(w, ev, prec, l2_chunk_events=chunk)
+    p1, k1 = _run(plain, ev)
+    p2, k2 = _run(chunked, ev)
+    assert torch.equal(p1, p2) and all(torch.equal(k1[k], k2[k]) for k in k1)
+    if chunk < 37:
+        assert plain.workspace_bytes() - chunked.workspace_bytes() >= (37 - chunk) * 40 * 800 * 4 - 4096
+        assert chunked.launches_per_run(37) == 2 + 2 * ((37 + chunk - 1) // chunk)
+    else:
+        assert chunked.launches_per_run(37) == 4
+    # the debug accessor sees the last chunk
+    last = (37 - 1) % chunk + 1 if chunk < 37 else 37
+    H1 = torch.empty(37, 40, 8, 100, device="cuda")
+    H2 = torch.empty(last, 40, 8, 100, device="cuda")
+    s = torch.cuda.Stream()
+    plain.debug_copy_histogram(H1, 37, stream=s)
+    chunked.debug_copy_histogram(H2, last, stream=s)
+    s.synchronize()
+    assert torch.equal(H1[37 - last:], H2)
+    with pytest.raises(pkg.PVFError):
+        chunked.debug_copy_histogram(H1, last + 1, stream=s)
+
+
+# ------------------------------------------------------------------ NEXT-4: small batches (low-latency schedule)
+@pytest.mark.parametrize("prec", ["tf32", "bf16", "fp16", "fp32", "simt"])
+def test_small_batches_match_the_batch_path_bit_for_bit(prec):
+    """PAPER.md:11, 37 (per-event deployment under a sub-400 us budget): calls with 1, 2, 3 and 7 events -- up to 3 events
+    run the UNet with one interval per CTA (148 or fewer intervals in the call), all of them with the kernels chained by
+    programmatic dependent launch -- must give exactly the bits the same events get inside a 16-event batch; also with stage
+    timing on (no PDL)."""
+    ev = make_events("run3", 16, 559)
+    w = make_weights("peaky", 5)
+    big = _make(w, ev, prec)
+    pb, kb = _run(big, ev)
+    timed = _make(w, ev, prec, stage_timing=True)
+    pt, kt = _run(timed, ev)
+    assert torch.equal(pb, pt) and all(torch.equal(kb[k], kt[k]) for k in kb)
+    for n in (1, 2, 3, 7):
+        sub = select_events(ev, range(5, 5 + n))
+        small = _make(w, sub, prec)
+        ps, ks = _run(small, sub)
+        assert torch.equal(ps, pb[5:5 + n]), f"{n} events"
+        for k in ks:
+            assert torch.equal(ks[k], kb[k][5:5 + n]), (n, k)
+        for _ in range(2):                                        # back to back: the next call's sort must not overtake
+            ps2, _ = _run(small, sub)
+            assert torch.equal(ps2, ps)
+        pt2, _ = _run(timed, sub, n)
+        assert torch.equal(pt2[:n], ps)
 
 
 # ------------------------------------------------------------------ CTA pairs (cta_group::2)
@@ -464,11 +528,9 @@ def test_cta_pair_is_bit_identical(prec, channels):
         two_el = _make(w, ev, prec, cta_pair=True, elide_empty=True)
         p3, _ = _run(two_el, ev)
         assert torch.equal(p1, p3)
-    with pytest.raises(pkg.PVFError):
-        _make(w, ev, "fp32", cta_pair=True)                       # tensor-core modes only
 
 
-@pytest.mark.parametrize("prec,elide", [("tf32", False), ("tf32", True), ("bf16", False), ("fp32", False)])
+@pytest.mark.parametrize("prec,elide", [("tf32", False), ("tf32", True), ("bf16", False), ("fp32", False), ("simt", False)])
 def test_batch_without_any_track(prec, elide):
     """Degenerate batch: 5 events, zero tracks in total (n_tracks == 0).  Every interval is the bias-only vector
     UNet(0) (BASELINE.json north_star 'empty intervals'), identical across intervals and equal to the oracle's."""
@@ -476,7 +538,8 @@ def test_batch_without_any_track(prec, elide):
     base = make_events("run3", 1, 3)
     ev = type(base)(np.zeros((9, 0), np.float32), np.zeros(6, np.int32), [None] * 5)
     ref = O.run(ev.feat, ev.event_offsets, w)
-    pvf = PVFinder(w, max_events=5, max_tracks=1, precision=prec, split_mask=SPLIT[prec], elide_empty=elide)
+    pvf = PVFinder(w, max_events=5, max_tracks=1, precision="fp32" if prec == "simt" else prec, split_mask=SPLIT[prec],
+                   elide_empty=elide, cta_pair=prec != "simt")
     feat = torch.zeros((9, 1), device="cuda")
     off = torch.zeros(6, dtype=torch.int32, device="cuda")
     probs = torch.full((5, 4000), -1.0, device="cuda")
@@ -491,7 +554,8 @@ def test_batch_without_any_track(prec, elide):
 
 
 @pytest.mark.parametrize("model,prec,ch,elide,margin", [("run3", "tf32", 64, False, 0.0), ("pileup", "fp16", 64, True, 0.0),
-                                                        ("run3", "bf16", 32, False, 0.0), ("pileup", "tf32", 64, False, 0.5)])
+                                                        ("run3", "bf16", 32, False, 0.0), ("pileup", "tf32", 64, False, 0.5),
+                                                        ("run3", "fp32", 64, False, 0.0)])
 def test_repeated_full_size_runs_are_bit_identical(model, prec, ch, elide, margin):
     """Determinism under load: 12 back-to-back runs of a 16 000-event batch -- every CTA pair of both
     tensor-core kernels busy, all mbarrier hand-offs exercised thousands of times -- give identical bits."""
@@ -579,7 +643,7 @@ def test_host_io_and_stage_timing():
     assert torch.equal(hpk["z"], pk["z"].cpu())
 
 
-@pytest.mark.parametrize("prec,margin", [("tf32", 0.0), ("fp16", 0.5), ("fp32", 0.0)])
+@pytest.mark.parametrize("prec,margin", [("tf32", 0.0), ("fp16", 0.5), ("simt", 0.0)])
 def test_host_io_chunk_pipeline_matches_device_run(prec, margin):
     """pvf_run_host on >= 4096 events runs as 8 chunks with the copies on the library's own streams: the host
     results must equal the device-resident pvf_run of the same batch bit for bit (4101 events: ragged chunks;
@@ -612,7 +676,8 @@ FULL_CASES = [  # (precision, event model, channels): BASELINE.json configs 2, 3
     ("tf32", "run3", 64), ("bf16", "run3", 64), ("fp16", "run3", 64),         # config 2 (+ config 4 at C = 64)
     ("tf32", "pileup", 64), ("fp16", "pileup", 64),                            # config 3
     ("bf16", "run3", 32), ("bf16", "run3", 16),                                # config 4 width sweep
-    ("fp32", "run3", 64),                                                      # CUDA-core path (2000 events)
+    ("fp32", "run3", 64),                                                      # config 2 "FP32" on the tensor cores
+    ("simt", "run3", 64),                                                      # CUDA-core kernels (2000 events)
 ]
 
 
@@ -620,7 +685,7 @@ FULL_CASES = [  # (precision, event model, channels): BASELINE.json configs 2, 3
 def test_full_batch_sampled_events(prec, model, ch):
     """BASELINE.json configs 2 / 3 / 4 (16000 events) in the launch configuration bench.py times; the oracle
     computes 256 events chosen by a seeded draw (plus the first and last two); properties hold for every event."""
-    E = 16000 if prec != "fp32" else 2000
+    E = 16000 if prec != "simt" else 2000
     seed = {"run3": 1002 if ch == 64 else 1004, "pileup": 1003}[model]
     rng = np.random.default_rng(2602)
     sample = sorted(set(rng.choice(E, 252, replace=False).tolist()) | {0, 1, E - 2, E - 1})
