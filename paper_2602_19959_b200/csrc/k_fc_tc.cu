@@ -20,9 +20,9 @@
 // 3 full accumulator tiles + 16 rows; 128 KB of W5x hi + lo resident in shared memory) for the same strided
 // subset of events and share every MMA (cta_group::2, M = 256): each supplies the hidden activations of half of
 // the tile's tracks (even / odd sorted positions), so the hidden layers run once per pair.
-// Roles: warps 0-12 epilogue (one accumulator tile quadrant each), warp 13 MMA issuer (leader CTA), warps
-// 14-17 = two groups of 64 threads that run the five 25-wide hidden layers (FP32 FMA, thread = track) for
-// alternating tiles and stage h_hi / h_lo as the B operand (double buffered).
+// Roles: warps 0-11 and 13 epilogue (one accumulator tile quadrant each), warp 12 MMA issuer (leader CTA), warps
+// 14-21 = four groups of 64 threads that run the five 25-wide hidden layers (FP32 FMA, thread = track) for
+// tiles it, it + 1, it + 2, it + 3 and stage h_hi / h_lo as the B operand (one buffer per group).
 #include <cstring>
 
 #include "pvf_internal.cuh"
@@ -42,8 +42,12 @@ constexpr int kMmaWarp = 12;
 constexpr int kSmallEpiWarp = 13;
 constexpr int kSmallRow0 = 3 * 128 + 32;     // accumulator row of the first of the last 16 outputs of a half (384 ..)
 constexpr int kHidWarp0 = 14;
-constexpr int kHidWarps = 4;                 // two groups of two warps: a CTA runs the hidden layers of HALF of a tile
-constexpr int kFtThreads = (kEpiWarps + 1 + kHidWarps) * 32;   // 13 epilogue + 1 MMA + 4 hidden-layer warps
+#ifndef PVF_FC_HID_GROUPS
+#define PVF_FC_HID_GROUPS 4      // measured at 16 k events: 2 groups 2.40 ms, 3: 2.31 ms, 4: 2.16 ms
+#endif
+constexpr int kHidGroups = PVF_FC_HID_GROUPS;   // groups of two warps, each on its own tile: a CTA runs the hidden layers of HALF of a tile
+constexpr int kHidWarps = 2 * kHidGroups;
+constexpr int kFtThreads = (kEpiWarps + 1 + kHidWarps) * 32;   // 13 epilogue + 1 MMA + the hidden-layer warps
 constexpr int kHalfOut = kFcOut / 2;         // outputs per CTA half, packed densely: row 128 t + r = output 400 half + 128 t + r
 constexpr int kTile = 128;                   // tracks per tile (MMA N)
 constexpr int kRowsW = 512;                  // 4 channel tiles x 128 rows per CTA half
@@ -57,18 +61,18 @@ constexpr int kWRow = 28;
 struct FtSmall {                             // the five hidden layers, zero padded
   float w0[kFcHidden][12];
   float b0[28];
-  float wh[4][kFcHidden][kWRow];
+  float wh[4][kFcHidden][kWRow];           // TRANSPOSED: wh[l][k][o] = W_{l+1}[o][k] (one row = the weights of input k)
   float bh[4][28];
 };
 
 constexpr int OFF_W = 0;                               // [hi | lo][8 chunks][512 rows][16 B]
-constexpr int OFF_H = OFF_W + 2 * kWPart;              // [buf 0 | 1][hi | lo][8 chunks][64 tracks][16 B]
-constexpr int OFF_SMALL = OFF_H + 4 * kHPart;
+constexpr int OFF_H = OFF_W + 2 * kWPart;              // [one buffer per hidden-layer group][hi | lo][8 chunks][64 tracks][16 B]
+constexpr int OFF_SMALL = OFF_H + 2 * kHidGroups * kHPart;
 constexpr int OFF_IV = OFF_SMALL + ((int)sizeof(FtSmall) + 127) / 128 * 128;   // int [4][128]
-constexpr int kIvBufs = 4;                   // interval lists of four tiles in flight: the hidden-layer warps of tile
+constexpr int kIvBufs = 8;                   // interval lists of four tiles in flight: the hidden-layer warps of tile
                                              // i + 2 must not wait for the epilogue of tile i (measured: they did)
 constexpr int OFF_BARS = OFF_IV + kIvBufs * kTile * 4;
-constexpr int FT_SMEM = OFF_BARS + 256;
+constexpr int FT_SMEM = OFF_BARS + 512;
 static_assert(FT_SMEM <= 227 * 1024, "shared memory budget");
 // barriers (8 bytes each): h_full[2], peer_h_full[2] (leader: the peer's half is staged), h_empty[2], meta[4],
 // acc_full[4], acc_empty[4], peer_acc_empty[4] (leader: the peer's epilogue has drained the tile), iv_full[4], then the
@@ -77,7 +81,13 @@ static_assert(FT_SMEM <= 227 * 1024, "shared memory budget");
 // the hidden-layer threads of tile it + 4 write that list only after meta[it & 3] completed its phase `it`, i.e. after
 // EVERY epilogue warp has finished tile it and therefore observed phase `it` of iv_full -- no phase can be skipped.  (The
 // 2-deep h_full gave no such guarantee to a slow epilogue warp: hidden(it + 2) is only gated by the MMAs of tile it.)
-enum { bHFull = 0, bPHFull = 2, bHEmpty = 4, bMeta = 6, bAccFull = 10, bAccEmpty = 14, bPAccEmpty = 18, bIvFull = 22, bSlot = 26 };
+enum { bHFull = 0, bPHFull = bHFull + kHidGroups, bHEmpty = bPHFull + kHidGroups, bMeta = bHEmpty + kHidGroups,
+       bAccFull = bMeta + kIvBufs, bAccEmpty = bAccFull + 4, bPAccEmpty = bAccEmpty + 4, bIvFull = bPAccEmpty + 4,
+       bSlot = bIvFull + kIvBufs };
+static_assert(8 * bSlot + 4 <= 512, "barrier block");
+constexpr int kIvLog = 3;
+static_assert((1 << kIvLog) == kIvBufs && kIvBufs >= 2 * kHidGroups, "interval lists: a power of two, two per hidden-layer group");
+static_assert(FT_SMEM <= 227 * 1024, "shared memory budget");
 
 __device__ __forceinline__ float leaky_ft(float v) { return v >= 0.0f ? v : kLeaky * v; }
 __device__ __forceinline__ uint32_t tf32_of(float v) {
@@ -210,7 +220,7 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
     uint4* dst = reinterpret_cast<uint4*>(smem + OFF_W);
     for (int i = tid; i < 2 * kWPart / 16; i += kFtThreads) dst[i] = __ldg(src + i);
     uint4* hz = reinterpret_cast<uint4*>(smem + OFF_H);
-    for (int i = tid; i < 4 * kHPart / 16; i += kFtThreads) hz[i] = make_uint4(0, 0, 0, 0);
+    for (int i = tid; i < 2 * kHidGroups * kHPart / 16; i += kFtThreads) hz[i] = make_uint4(0, 0, 0, 0);
   }
   for (int i = tid; i < kFcHidden * 12; i += kFtThreads) {
     const int r = i / 12, c = i % 12;
@@ -218,15 +228,15 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
   }
   for (int i = tid; i < 28; i += kFtThreads) S.b0[i] = i < kFcHidden ? par[kFcB0 + i] : 0.0f;
   for (int i = tid; i < 4 * kFcHidden * kWRow; i += kFtThreads) {
-    const int l = i / (kFcHidden * kWRow), r = (i / kWRow) % kFcHidden, c = i % kWRow;
-    S.wh[l][r][c] = c < kFcHidden ? par[kFcHid + l * kFcHidStride + r * kFcHidden + c] : 0.0f;
+    const int l = i / (kFcHidden * kWRow), k = (i / kWRow) % kFcHidden, o = i % kWRow;
+    S.wh[l][k][o] = o < kFcHidden ? par[kFcHid + l * kFcHidStride + o * kFcHidden + k] : 0.0f;
   }
   for (int i = tid; i < 4 * 28; i += kFtThreads) {
     const int l = i / 28, c = i % 28;
     S.bh[l][c] = c < kFcHidden ? par[kFcHid + l * kFcHidStride + kFcHidden * kFcHidden + c] : 0.0f;
   }
   if (tid == 0) {
-    for (int k = 0; k < 2; ++k) {
+    for (int k = 0; k < kHidGroups; ++k) {
       mbar_init(bar(bHFull + k), kHalfTile); mbar_init(bar(bPHFull + k), kHalfTile); mbar_init(bar(bHEmpty + k), 1);
     }
     for (int k = 0; k < kIvBufs; ++k) { mbar_init(bar(bMeta + k), 32 * kEpiWarps); mbar_init(bar(bIvFull + k), kHalfTile); }
@@ -277,7 +287,7 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
         const int ntile = min(kTile, nk - base);
         const bool last = base + kTile >= nk;
         const int ib = it & (kIvBufs - 1);
-        { FC_PROF_T0(); mbar_wait(bar(bIvFull + ib), (uint32_t)((it >> 2) & 1)); FC_PROF_ADD(0, pw); }   // s_iv is staged
+        { FC_PROF_T0(); mbar_wait(bar(bIvFull + ib), (uint32_t)((it >> kIvLog) & 1)); FC_PROF_ADD(0, pw); }   // s_iv is staged
         FC_PROF_CNT(9, pw);
         const int* ivs = s_iv + ib * kTile;
         if (base == 0) c = ivs[0];               // the event's first (lowest) non-empty interval
@@ -373,11 +383,11 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
       int ev_lo;
       const int nk = kept_of(e, ev_lo);
       for (int base = 0; base < nk; base += kTile, ++it) {
-        const int buf = it & 1;
+        const int buf = it % kHidGroups;
         {
           FC_PROF_T0();
-          mbar_wait(bar(bHFull + buf), (uint32_t)((it >> 1) & 1));       // both halves of the B operand are staged
-          mbar_wait(bar(bPHFull + buf), (uint32_t)((it >> 1) & 1));
+          mbar_wait(bar(bHFull + buf), (uint32_t)((it / kHidGroups) & 1));       // both halves of the B operand are staged
+          mbar_wait(bar(bPHFull + buf), (uint32_t)((it / kHidGroups) & 1));
           FC_PROF_ADD(3, pw);
         }
         tc_fence_after_sync();
@@ -424,22 +434,30 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
       int ev_lo;
       const int nk = kept_of(e, ev_lo);
       for (int base = 0; base < nk; base += kTile, ++it) {
-        if ((it & 1) != g) continue;
-        const uint32_t prev = (uint32_t)(((it >> 1) & 1) ^ 1);
+        if (it % kHidGroups != g) continue;
+        // the track's inputs first (three dependent global loads: perm -> z_poca -> features), THEN the waits for the
+        // buffers they go to: the load latency overlaps whatever time the group has to wait anyway
+        const bool has_own = base + p_own < nk, has_other = base + p_other < nk;
+        int iv_other = 0, iv_own = 0;
+        float x[kFcIn] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        if (has_other) {
+          int t;
+          float zrel;
+          iv_other = entry_interval(perm[ev_lo + base + p_other], F.f[0], t, zrel);
+        }
+        if (has_own) {
+          int t;
+          iv_own = entry_interval(perm[ev_lo + base + p_own], F.f[0], t, x[0]);   // own or neighbouring interval
+#pragma unroll
+          for (int k = 1; k < kFcIn; ++k) x[k] = F.f[k][t];
+        }
+        const uint32_t prev = (uint32_t)(((it / kHidGroups) & 1) ^ 1);
         { FC_PROF_T0(); mbar_wait(bar(bHEmpty + g), prev); FC_PROF_ADD(6, pw); }   // the MMAs that read this buffer have retired
         const int ib = it & (kIvBufs - 1);
-        { FC_PROF_T0(); mbar_wait(bar(bMeta + ib), (uint32_t)(((it >> 2) & 1) ^ 1)); FC_PROF_ADD(7, pw); }   // the epilogue is done with s_iv[ib]
-        if (base + p_other < nk) {
-          int t;
-          float zrel;
-          s_iv[ib * kTile + p_other] = entry_interval(perm[ev_lo + base + p_other], F.f[0], t, zrel) * kFcOut;
-        }
-        if (base + p_own < nk) {
-          int t;
-          float zrel;
-          const int iv = entry_interval(perm[ev_lo + base + p_own], F.f[0], t, zrel);   // own or neighbouring interval
-          s_iv[ib * kTile + p_own] = iv * kFcOut;   // the epilogue wants the interval as its offset in H
-          const float x[kFcIn] = {zrel, F.f[1][t], F.f[2][t], F.f[3][t], F.f[4][t], F.f[5][t], F.f[6][t], F.f[7][t], F.f[8][t]};
+        { FC_PROF_T0(); mbar_wait(bar(bMeta + ib), (uint32_t)(((it >> kIvLog) & 1) ^ 1)); FC_PROF_ADD(7, pw); }   // the epilogue is done with s_iv[ib]
+        if (has_other) s_iv[ib * kTile + p_other] = iv_other * kFcOut;
+        if (has_own) {
+          s_iv[ib * kTile + p_own] = iv_own * kFcOut;   // the epilogue wants the interval as its offset in H
           float h[32], gg[28];
 #pragma unroll
           for (int o = 0; o < kFcHidden; ++o) {
@@ -450,22 +468,30 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
           }
 #pragma unroll 1                  // four identical layers share one copy of the code (I-cache footprint)
           for (int l = 0; l < 4; ++l) {
+            // input-major: for every input k the 25 accumulators take one independent FMA each (the weights of input k
+            // are one row of the transposed matrix: 7 broadcast 16-byte loads), so no FMA waits for the one before it.
+            // (Output-major -- one 25-long dependent chain per output, three chains interleaved by the compiler -- ran
+            // the hidden-layer warps at 0.3 instructions per clock and made them the critical path of the kernel.)
+            const float4* br = reinterpret_cast<const float4*>(S.bh[l]);
 #pragma unroll
-            for (int o = 0; o < kFcHidden; ++o) {
-              float a = S.bh[l][o];
-              const float4* wr = reinterpret_cast<const float4*>(S.wh[l][o]);
+            for (int q = 0; q < 7; ++q) {
+              const float4 b = br[q];
+              gg[4 * q] = b.x; gg[4 * q + 1] = b.y; gg[4 * q + 2] = b.z; gg[4 * q + 3] = b.w;
+            }
+#pragma unroll
+            for (int k = 0; k < kFcHidden; ++k) {
+              const float4* wr = reinterpret_cast<const float4*>(S.wh[l][k]);
 #pragma unroll
               for (int q = 0; q < 7; ++q) {
                 const float4 w = wr[q];
-                a = fmaf(w.x, h[4 * q], a);
-                if (4 * q + 1 < kFcHidden) a = fmaf(w.y, h[4 * q + 1], a);
-                if (4 * q + 2 < kFcHidden) a = fmaf(w.z, h[4 * q + 2], a);
-                if (4 * q + 3 < kFcHidden) a = fmaf(w.w, h[4 * q + 3], a);
+                gg[4 * q] = fmaf(w.x, h[k], gg[4 * q]);
+                if (4 * q + 1 < kFcHidden) gg[4 * q + 1] = fmaf(w.y, h[k], gg[4 * q + 1]);
+                if (4 * q + 2 < kFcHidden) gg[4 * q + 2] = fmaf(w.z, h[k], gg[4 * q + 2]);
+                if (4 * q + 3 < kFcHidden) gg[4 * q + 3] = fmaf(w.w, h[k], gg[4 * q + 3]);
               }
-              gg[o] = leaky_ft(a);
             }
 #pragma unroll
-            for (int o = 0; o < kFcHidden; ++o) h[o] = gg[o];
+            for (int o = 0; o < kFcHidden; ++o) h[o] = leaky_ft(gg[o]);
           }
           h[25] = 1.0f;                              // multiplies the bias column of W5x
 #pragma unroll
