@@ -395,7 +395,7 @@ def main_ours(args, rank, world, local_rank):
     split = args.split_mask if args.split_mask >= 0 else None
     wl = Workload(torch, PVFinder, model=args.model, events=E, seed=rank_seed(args.model, rank), precision=args.precision,
                   channels=args.channels, split_mask=split, elide=args.elide_empty, cta_pair=args.cta_pair,
-                  margin=args.boundary_margin, weights=args.weights, host_io=True)
+                  margin=args.boundary_margin, weights=args.weights, host_io=True, l2_chunk_events=args.l2_chunk_events)
     ev, w, pvf, stream = wl.ev, wl.w, wl.pvf, wl.stream
 
     def barrier():
@@ -507,7 +507,7 @@ def main_ours(args, rank, world, local_rank):
                                f"model {args.model}, {ev.n_tracks} tracks, UNet {args.channels} ch, weights {args.weights}",
                    "precision": args.precision, "split_mask": wl.split,
                    "elide_empty_intervals": bool(args.elide_empty), "unet_cta_pair": bool(args.cta_pair), "boundary_margin_mm": args.boundary_margin,
-                   "nonempty_interval_fraction": nonempty / (E * 40.0),
+                   "l2_chunk_events": args.l2_chunk_events, "nonempty_interval_fraction": nonempty / (E * 40.0),
                    "cache": ("inputs larger than L2 (107 MB features, 2 GB histogram per step)" if E >= 2000 else
                              "small batch: inputs fit in L2 (latency-style measurement)")},
         "us_per_event": ms * 1e3 / (args.steps * E),
@@ -567,6 +567,8 @@ def main():
                     help="NEXT-1 mode (mm): boundary tracks contribute to two intervals, PAPER.md:49")
     ap.add_argument("--cta-pair", type=int, default=1, choices=[0, 1],
                     help="UNet as clusters of two CTAs sharing every MMA (cta_group::2)")
+    ap.add_argument("--l2-chunk-events", type=int, default=0,
+                    help="NEXT-2 mode: histograms through a chunk-sized, L2-resident buffer (pvf_config.l2_chunk_events)")
     ap.add_argument("--elide-empty", action="store_true",
                     help="NEXT-2 mode: UNet only over non-empty intervals (reported with executed-FLOP accounting)")
     args = ap.parse_args()

@@ -34,6 +34,16 @@
 // memory; d1's epilogue fuses the 1x1 head + sigmoid and writes out_probs).
 // TF32 mode: the e1 layer (raw histogram input) can run as two passes on BF16 pieces (split_mask bit 0).
 //
+// Polyphase d1 (groups of an even number of intervals, i.e. every format but FX): d1 = conv25(cat[up2(d2), e1]) is computed on
+// the LOW-resolution rows i (outputs 2i and 2i + 1 = the two "phases" side by side in N):
+//   * the nearest-upsampled half needs no upsampling: out[2i + p] = sum_d d2[i + d] * Wp[d], d = -6 .. 6, with
+//     W0[d] = W[2d + 12] + W[2d + 13], W1[d] = W[2d + 11] + W[2d + 12] (taps that read the same low-resolution sample are
+//     added on the host) -- 13 MMA steps per K block on HALF as many rows instead of 13 tap pairs on all rows;
+//   * the skip half reads e1 de-interleaved (row i holds positions 2i and 2i + 1 as 2C channels): same MMA time as before,
+//     no row shift in the epilogue.
+// The accumulator tile is [low-resolution row][phase 0: C | phase 1: C]; the epilogue thread of row i computes both
+// logits and stores two probabilities.  ~15 % fewer MMA cycles per interval (SURVEY.md H1 "polyphase weights").
+//
 // FP32-accurate mode (format 3, "FX"; PVF_PREC_FP32 on the tensor cores, BASELINE.json config 0 "FP32"): every product a w is
 // taken as  tf32(a) tf32(w)  +  [a - tf32(a)] w  +  a [w - tf32(w)]  -- the first term one kind::tf32 MMA, the two small
 // terms ONE kind::f16 MMA over BF16 pieces stacked along K: A' = [a_lo (8 channels) | bf16(a) (the same 8 channels)],
@@ -41,6 +51,7 @@
 // product at 2 MMA time units per (tap pair, 8 channels) -- a three-pass TF32 split needs 3.  Activations live in shared
 // memory as three arrays per buffer (HI: TF32 chunks, LO and HB: BF16 chunks; 8 bytes per value), which fits for groups
 // of ONE interval; the weight image interleaves a main and a correction step per (tap pair, K block).
+#pragma nv_diag_suppress 128   // "loop is not reachable": template branches that return early for some instantiations
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 #include <cstring>
@@ -74,9 +85,9 @@ enum { gE2 = 0, gD1Ea = 1, gB = 2, gD1Eb = 3, gD2 = 4, gD1Ec = 5, gE1 = 6, gD1U 
 // CG: CTAs per MMA -- 1, or 2 = a cluster of two CTAs (cta_group::2) that run one M = 256 MMA per step: each CTA
 // supplies its own 128 activation rows (its own group of intervals) and HALF of the weight rows (rank 0 the even
 // tap of a pair, rank 1 the odd tap), so per CTA the weight stream and the B-operand reads are halved.
-// TT: intervals per group, 0 = the throughput default below.  TT = 1 is the small-batch (low-latency) instance: with
-// few intervals in the whole call (one event = 40) a group of one interval per CTA halves the serial MMA chain a CTA
-// walks and puts twice as many SMs to work.  Same MMAs per interval, same order.
+// TT: intervals per group, 0 = the default below (an explicit value is for experiments: groups of one interval were
+// measured as a small-batch schedule -- 41 -> 35 us for one event -- and dropped again when the polyphase d1, which needs
+// an even group, gave the same gain for every batch size with one code path and bit-identical results).
 constexpr bool is16(int fmt) { return fmt == 1 || fmt == 2; }
 
 template <int C, int BF16, int CG = 1, int TT = 0>
@@ -98,10 +109,15 @@ struct Geo {
   // land in the following chunk / buffer, which is always inside the CTA's allocation
   static constexpr int ROWS1 = LEAD1 + 128 * T, ROWS2 = LEAD2 + 64 * T, ROWS3 = LEAD3 + 32 * T;
   static constexpr int LBO1 = ROWS1 * 16, LBO2 = ROWS2 * 16, LBO3 = ROWS3 * 16;
+  static constexpr bool PP = (T % 2 == 0);           // polyphase d1 (see the header); FX (groups of one interval) runs d1 directly
   static constexpr int NB = NOUT / CG;               // B-operand rows this CTA holds
   static constexpr int STEP_BYTES = 2 * NB * 16;     // one MMA's B operand in this CTA: [2 chunks][NB rows][16 B]
-  static constexpr int STAGE_BYTES = kStageBytes / CG;
-  static constexpr int SPS = STAGE_BYTES / STEP_BYTES;   // MMA steps per ring stage (independent of CG)
+  // Ring stage.  One stage costs the producer, the relay and the MMA issuer a fixed ~400 cycles of mbarrier round trips
+  // each (measured: a single thread issues one bulk copy per ~380 cycles whatever its size), so a stage must hold at least
+  // that much tensor work: with the polyphase d1 most steps feed ONE tile (68 cycles), 4-step stages left the tensor pipe
+  // idle 30 % of the time.  A CTA of a pair therefore takes 16 KB stages like a single CTA (8 steps at C = 64) whenever
+  // three of them fit; the FX format (8-byte activations) keeps 8 KB.
+  static constexpr int STAGE_HALF = kStageBytes / CG;
   // shared-memory map (bytes)
   static constexpr int SZ_L1 = NCHB * LBO1;          // a C-channel buffer at L = 100
   static constexpr int SZ_L2 = NCHB * LBO2;          //                     at L = 50
@@ -113,8 +129,16 @@ struct Geo {
   static constexpr int SETS = epi_sets(C);
   static constexpr int EPI_THREADS = 128 * SETS, THREADS = 64 + EPI_THREADS;
   static constexpr int SCR_BYTES = SETS * 2 * 4 * C * 4;   // epilogue row-exchange scratch: [set][2 buffers][4 warps][C floats]
-  static constexpr int STAGES_FIT = (227 * 1024 - kHeaderBytes - kBarBytes - SCR_BYTES - OFF_RING) / STAGE_BYTES;
-  static constexpr int MAX_STAGES = CG == 2 ? 12 : kMaxStages;   // measured: depth >= 6 changes nothing (bf16 and tf32)
+  static constexpr int RING_FREE = 227 * 1024 - kHeaderBytes - kBarBytes - SCR_BYTES - OFF_RING;
+  static constexpr int STAGE_BIG = (kStageBytes / STEP_BYTES > 16) ? 16 * STEP_BYTES : kStageBytes;
+  static constexpr int STAGE_HUGE = 16 * STEP_BYTES;       // 16 steps (the most the d1E split points allow), if four fit
+  static constexpr int STAGE_BYTES = (RING_FREE / STAGE_HUGE >= 4) ? STAGE_HUGE : (RING_FREE / STAGE_BIG >= 3) ? STAGE_BIG : STAGE_HALF;
+  static constexpr int SPS = STAGE_BYTES / STEP_BYTES;   // MMA steps per ring stage
+  static constexpr int STAGES_FIT = RING_FREE / STAGE_BYTES;
+#ifndef PVF_UNET_MAX_STAGES
+#define PVF_UNET_MAX_STAGES 12
+#endif
+  static constexpr int MAX_STAGES = CG == 2 ? PVF_UNET_MAX_STAGES : kMaxStages;   // measured: depth >= 6 changes nothing (bf16 and tf32)
   static constexpr int STAGES = STAGES_FIT < MAX_STAGES ? STAGES_FIT : MAX_STAGES;   // weight ring depth
   static constexpr int OFF_PAR = OFF_RING + STAGES * STAGE_BYTES;   // biases + head (floats)
   static constexpr int OFF_SCR = OFF_PAR + kHeaderBytes;
@@ -129,7 +153,7 @@ struct Geo {
   static constexpr int TMEM_COLS = (2 * T * NOUT <= 32) ? 32 : (2 * T * NOUT <= 64) ? 64 : (2 * T * NOUT <= 128) ? 128
                                    : (2 * T * NOUT <= 256) ? 256 : 512;
   // d1E parts (steps): run while the epilogues of e2 / b / d2 drain; multiples of every SPS
-  static constexpr int D1E_STEPS = 13 * NKB1 * PH;   // 13 tap pairs
+  static constexpr int D1E_STEPS = 13 * NKB1 * PH * (PP ? 2 : 1);   // 13 tap pairs; polyphase: 13 offsets x 2C channels
   static constexpr int D1E_A = D1E_STEPS < 16 * PH ? D1E_STEPS : 16 * PH;
   static constexpr int D1E_B = (D1E_STEPS - D1E_A) < 16 * PH ? (D1E_STEPS - D1E_A) : 16 * PH;
   static constexpr int D1E_C = D1E_STEPS - D1E_A - D1E_B;
@@ -300,6 +324,33 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
   // accumulator tile: columns [0, C) = E0 (even taps), [C, 2C) = E1 (odd taps); output row m = E0[m] + E1[m+1]
   const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) +
                          (uint32_t)((MODE == kD1 ? G::COL_A : G::COL_B) + tile * G::NOUT);
+  if (MODE == kD1 && G::PP) {
+    // polyphase d1: row m = low-resolution position l of interval 2 tile + (m >> 6); columns [0, C) = output 2l,
+    // [C, 2C) = output 2l + 1.  No row shift: bias, LeakyReLU, the 1x1 head and the sigmoid per phase.
+    const int interval = 2 * tile + (m >> 6), l = m & 63;
+    const float* hw = par + 5 * C;
+    float logit0 = 0.0f, logit1 = 0.0f;
+#pragma unroll 1
+    for (int c0 = cb; c0 < ce; c0 += 16) {
+      uint32_t r[16], r1[16];
+      tmem_ld_x16(taddr + (uint32_t)c0, r);
+      tmem_ld_x16(taddr + (uint32_t)(C + c0), r1);
+      tmem_ld_wait();
+#pragma unroll
+      for (int i = 0; i < 16; ++i) {
+        logit0 = fmaf(hw[c0 + i], lrelu(__uint_as_float(r[i]) + bias[c0 + i]), logit0);
+        logit1 = fmaf(hw[c0 + i], lrelu(__uint_as_float(r1[i]) + bias[c0 + i]), logit1);
+      }
+    }
+    if (l < 50 && interval < n_valid_int) {
+      const float a0 = logit0 + par[6 * C], a1 = logit1 + par[6 * C];
+      // list_g != nullptr: the group's intervals are rows list_g[0..T) of the full output (empty-interval elision)
+      const size_t row = list_g ? (size_t)list_g[interval] : (size_t)interval;
+      *reinterpret_cast<float2*>(probs_group + row * kBins + 2 * l) =
+          make_float2(1.0f / (1.0f + expf(-a0)), 1.0f / (1.0f + expf(-a1)));
+    }
+    return;
+  }
   // Row m + 1 of lane 31 lives in the next warp's TMEM quadrant: lane 0 of every warp publishes its E1 row
   // in shared memory (scr: [4 warps][C], double buffered by the caller), one named barrier per tile.
 #pragma unroll 1
@@ -324,7 +375,11 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
   const bool exists = interval < G::T;          // level-3 tiles may be wider than the group
   uint32_t dst_full = 0, dst_aux = 0, lbo_full = 0, lbo_aux = 0;
   if (MODE == kE1) {
-    dst_full = smem_base + G::OFF_E1 + (uint32_t)(G::LEAD1 + 128 * tile + m) * 16u; lbo_full = G::LBO1;
+    if (G::PP) {   // de-interleaved skip: row = low-resolution position, positions 2i / 2i + 1 as channels [0, C) / [C, 2C)
+      dst_full = smem_base + G::OFF_E1 + (uint32_t)(G::LEAD2 + 64 * tile + (m >> 1)) * 16u; lbo_full = G::LBO2;
+    } else {
+      dst_full = smem_base + G::OFF_E1 + (uint32_t)(G::LEAD1 + 128 * tile + m) * 16u; lbo_full = G::LBO1;
+    }
     dst_aux = smem_base + G::OFF_XP + (uint32_t)(G::LEAD2 + 64 * tile + (m >> 1)) * 16u; lbo_aux = G::LBO2;     // P1
     if (tile == 0 && m < G::LEAD2) zero_rows(smem_base + G::OFF_XP, G::LBO2, G::NCHB, m);
   } else if (MODE == kE2) {
@@ -336,8 +391,13 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
     dst_full = smem_base + G::OFF_R + G::SZ_L2 + (uint32_t)(G::LEAD2 + 256 * tile + 2 * m) * 16u; lbo_full = G::LBO2;  // U2
     if (tile == 0 && m < G::LEAD2) zero_rows(smem_base + G::OFF_R + G::SZ_L2, G::LBO2, G::NCHB, m);
   } else if (MODE == kD2) {
-    dst_full = smem_base + G::OFF_R + (uint32_t)(G::LEAD1 + 256 * tile + 2 * m) * 16u; lbo_full = G::LBO1;      // U1
-    if (tile == 0 && m < G::LEAD1) zero_rows(smem_base + G::OFF_R, G::LBO1, G::NCHB, m);
+    if (G::PP) {   // polyphase d1 reads d2 itself (no upsampled copy): rows as E2's, in E2's place
+      dst_full = smem_base + G::OFF_R + (uint32_t)(G::LEAD2 + 128 * tile + m) * 16u; lbo_full = G::LBO2;
+      if (tile == 0 && m < G::LEAD2) zero_rows(smem_base + G::OFF_R, G::LBO2, G::NCHB, m);
+    } else {
+      dst_full = smem_base + G::OFF_R + (uint32_t)(G::LEAD1 + 256 * tile + 2 * m) * 16u; lbo_full = G::LBO1;      // U1
+      if (tile == 0 && m < G::LEAD1) zero_rows(smem_base + G::OFF_R, G::LBO1, G::NCHB, m);
+    }
   }
   float logit = 0.0f;
 #pragma unroll 1
@@ -373,9 +433,12 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
 #pragma unroll
       for (int i = 0; i < 16; ++i) pv[i] = fmaxf(v[i], __shfl_xor_sync(0xffffffffu, v[i], 1));
       if (exists) {               // (a level-2 tile is wider than a one-interval group: its upper half has no buffer rows)
-        store_row16<BF16, G::NCH>(dst_full, lbo_full, c0, v);
+        if (MODE == kE1 && G::PP) store_row16<BF16, 2 * G::NCH>(dst_full, lbo_full, c0 + (m & 1) * C, v);
+        else store_row16<BF16, G::NCH>(dst_full, lbo_full, c0, v);
         store_pooled16<BF16, G::NCH>(dst_aux, lbo_aux, c0, pv, lane & 1);   // both lanes of a pair hold the same maxima
       }
+    } else if (MODE == kD2 && G::PP) {
+      if (exists) store_row16<BF16, G::NCH>(dst_full, lbo_full, c0, v);
     } else if (exists) {          // kB, kD2: nearest upsample = the same chunk into rows 2m and 2m + 1;
       // groups of four lanes alternate which of the two rows goes first, so that one store instruction
       // covers all eight 16-byte slots of every 128-byte line evenly (no bank conflicts)
@@ -492,20 +555,24 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
 template <int C, int BF16, int S, int TT>
 struct Lay {
   using G = Geo<C, BF16, 1, TT>;
-  static constexpr int TAPS = (S == sE1 || S == sD1U || S == sD1E) ? 25 : (S == sB ? 5 : 15);
-  static constexpr int PAD = (TAPS - 1) / 2;
-  static constexpr int PAIRS = (TAPS + 1) / 2;                 // (even, odd) tap pairs; the last odd tap is zero
-  static constexpr int NKB = (S == sE1) ? 1 : (S == sD2 ? 2 * G::NKB1 : G::NKB1);     // K blocks per tap
-  static constexpr int LEVEL = (S == sE1 || S == sD1U || S == sD1E) ? 1 : (S == sB ? 3 : 2);
+  static constexpr bool D1 = (S == sD1U || S == sD1E);
+  static constexpr bool POLY = D1 && G::PP;                    // polyphase d1: low-resolution rows, 13 offsets, row step 1
+  static constexpr int TAPS = (S == sE1 || D1) ? 25 : (S == sB ? 5 : 15);
+  static constexpr int PAD = POLY ? 6 : (TAPS - 1) / 2;        // rows before the output row that the first step reads
+  static constexpr int RS = POLY ? 1 : 2;                      // rows per step: a tap pair moves two rows, an offset one
+  static constexpr int PAIRS = (TAPS + 1) / 2;                 // (even, odd) tap pairs (the last odd tap is zero) | offsets -6 .. 6
+  static constexpr bool HALF_LAST = !POLY;                     // the last tap pair holds one tap only: an N = C step
+  static constexpr int NKB = (S == sE1) ? 1 : ((S == sD2 || (S == sD1E && POLY)) ? 2 * G::NKB1 : G::NKB1);     // K blocks per step group
+  static constexpr int LEVEL = POLY ? 2 : ((S == sE1 || D1) ? 1 : (S == sB ? 3 : 2));
   static constexpr int LEAD = LEVEL == 1 ? G::LEAD1 : (LEVEL == 2 ? G::LEAD2 : G::LEAD3);
   static constexpr int LBO = LEVEL == 1 ? G::LBO1 : (LEVEL == 2 ? G::LBO2 : G::LBO3);
   static constexpr int NT = LEVEL == 1 ? G::T : (LEVEL == 2 ? (G::T + 1) / 2 : (G::T + 3) / 4);
   static constexpr int HALF = (S == sD2) ? NKB / 2 : NKB;      // K blocks served by the first source buffer
   static constexpr int SRC0 = (S == sE1) ? G::OFF_XP /* X0 */ : (S == sE2) ? G::OFF_XP /* P1 */
                               : (S == sB) ? G::OFF_R + G::SZ_L2 /* P2 */ : (S == sD2) ? G::OFF_R + G::SZ_L2 /* U2 */
-                              : (S == sD1U) ? G::OFF_R /* U1 */ : G::OFF_E1 /* E1 */;
+                              : (S == sD1U) ? G::OFF_R /* U1 | polyphase: d2 itself */ : G::OFF_E1 /* E1 */;
   static constexpr int SRC1 = (S == sD2) ? G::OFF_R /* E2 */ : SRC0;
-  static constexpr int DCOL = (S == sD1U || S == sD1E) ? G::COL_A : G::COL_B;
+  static constexpr int DCOL = D1 ? G::COL_A : G::COL_B;
   // byte offset (from the CTA's shared-memory base) of the first chunk of K block kk
   __host__ __device__ static constexpr int a_off(int kk) {
     return kk < HALF ? SRC0 + 2 * kk * LBO : SRC1 + 2 * (kk - HALF) * LBO;
@@ -568,7 +635,7 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
   constexpr uint32_t idesc_h = instr_desc(fmt_main, 128 * CG, G::NOUT / 2);
   constexpr uint32_t idesc_xh = instr_desc(kFmtBF16, 128 * CG, G::NOUT / 2);
   constexpr uint32_t b_lbo_h = (uint32_t)((G::NB / 2 * 16) >> 4) << 16;
-  constexpr int LAST0 = (Y::PAIRS - 1) * Y::NKB;                       // first logical step of the last tap pair (not e1)
+  constexpr int LAST0 = Y::HALF_LAST ? (Y::PAIRS - 1) * Y::NKB : (1 << 30);   // first logical step of the last tap pair (not e1)
   constexpr uint32_t hi = (128u >> 4) | (1u << 14);                    // SBO = 128 B, descriptor version 1
   // e1 in the 16-bit modes: the second 16-byte K chunk of A is the SAME 8-channel buffer two rows further down
   // (LBO = 32 bytes), i.e. the input of the next tap pair -- one MMA does tap pairs 2w and 2w + 1
@@ -599,14 +666,14 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
     } else if (Y::HALF >= SPL) {
       const int j0 = lf / Y::NKB, kk0 = lf % Y::NKB;
       const int off = kk0 < Y::HALF ? Y::SRC0 + 2 * kk0 * Y::LBO : Y::SRC1 + 2 * (kk0 - Y::HALF) * Y::LBO;
-      a0 += (uint32_t)(off >> 4) + (uint32_t)(Y::LEAD + 2 * j0 - Y::PAD);
+      a0 += (uint32_t)(off >> 4) + (uint32_t)(Y::LEAD + Y::RS * j0 - Y::PAD);
       if (FX) {
         const int offc = (kk0 < Y::HALF ? Y::SRC0 + kk0 * Y::LBO : Y::SRC1 + (kk0 - Y::HALF) * Y::LBO) + Y::SRC_NCH * Y::LBO;
-        c0 += (uint32_t)(offc >> 4) + (uint32_t)(Y::LEAD + 2 * j0 - Y::PAD);
+        c0 += (uint32_t)(offc >> 4) + (uint32_t)(Y::LEAD + Y::RS * j0 - Y::PAD);
       }
     } else {
-      a0 += (uint32_t)(Y::SRC0 >> 4) + (uint32_t)(Y::LEAD + 2 * (lf / Y::NKB) - Y::PAD);
-      c0 += (uint32_t)(Y::SRC0 >> 4) + (uint32_t)(Y::LEAD + 2 * (lf / Y::NKB) - Y::PAD);
+      a0 += (uint32_t)(Y::SRC0 >> 4) + (uint32_t)(Y::LEAD + Y::RS * (lf / Y::NKB) - Y::PAD);
+      c0 += (uint32_t)(Y::SRC0 >> 4) + (uint32_t)(Y::LEAD + Y::RS * (lf / Y::NKB) - Y::PAD);
     }
     if (elect_one()) {
 #pragma unroll
@@ -627,8 +694,8 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
             a = corr ? c0 + (uint32_t)(li * (Y::LBO >> 4)) : a0 + (uint32_t)(li * ((2 * Y::LBO) >> 4));
             half_n = lf + li >= LAST0;
           } else {
-            a = corr ? c0 + (uint32_t)((Y::c_off(li % Y::NKB) - Y::SRC0) >> 4) + (uint32_t)(2 * (li / Y::NKB))
-                     : a0 + (uint32_t)((Y::a_off(li % Y::NKB) - Y::SRC0) >> 4) + (uint32_t)(2 * (li / Y::NKB));
+            a = corr ? c0 + (uint32_t)((Y::c_off(li % Y::NKB) - Y::SRC0) >> 4) + (uint32_t)(Y::RS * (li / Y::NKB))
+                     : a0 + (uint32_t)((Y::a_off(li % Y::NKB) - Y::SRC0) >> 4) + (uint32_t)(Y::RS * (li / Y::NKB));
             half_n = lf + li >= LAST0;
           }
           const uint32_t b = (half_n ? b_lbo_h : b_lbo) + b0 + (uint32_t)(i * (G::STEP_BYTES >> 4));
@@ -874,7 +941,7 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
         done(1);
       }
       wait_acc(4);
-      layer(integral_constant<int, kD1>{}, G::T, n_valid, lg);
+      layer(integral_constant<int, kD1>{}, G::PP ? G::T / 2 : G::T, n_valid, lg);
       done(5);
     }
   }
@@ -957,6 +1024,37 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst_all) {
       else if (d.seg == gE1) { pass = f / 13; u = f % 13; kk = 0; }   // e1 split runs [pass][tap pair]
       else { u = f / d.nkb; kk = f % d.nkb; }
       unsigned char* step = dst + P.seg_off[d.seg] + (size_t)s * G::STEP_BYTES;
+      if (G::PP && d.layer == 4) {
+        // polyphase d1 (see the header): step = (offset u - 6, K block); B rows [0, C) = phase 0, [C, 2C) = phase 1.
+        //   upsampled half (gD1U):  Wp[u][ci][co] = W[co][ci][2u - p] + W[co][ci][2u - p + 1]     (taps outside 0 .. 24 are absent)
+        //   skip half (gD1E*):      K channel q * C + ci = skip channel ci at position 2i + q:  W[co][C + ci][2u + q - p]
+        const bool up_half = d.seg == gD1U;
+        const int nkb = up_half ? N1 : 2 * N1;
+        const int uo = f / nkb, kb = f % nkb;
+        for (int h = 0; h < 2; ++h)
+          for (int nl = 0; nl < G::NB; ++nl)
+            for (int e = 0; e < G::PER; ++e) {
+              const int n = rank * G::NB + nl, ph = n / C, co = n % C;
+              const int cl = (2 * kb + h) * G::PER + e;
+              float v = 0.0f;
+              if (up_half) {
+                for (int j = 2 * uo - ph; j <= 2 * uo - ph + 1; ++j)
+                  if (j >= 0 && j < d.taps) v += W[((size_t)co * d.cin + cl) * d.taps + j];
+              } else {
+                const int q = cl / C, ci = cl % C, j = 2 * uo + q - ph;
+                if (j >= 0 && j < d.taps) v = W[((size_t)co * d.cin + C + ci) * d.taps + j];
+              }
+              unsigned char* pdst = step + ((size_t)h * G::NB + nl) * 16 + e * G::ES;
+              if (B16) {
+                const uint16_t b = (BF16 == 2) ? fp16_rne(v) : bf16_rne(v);
+                memcpy(pdst, &b, 2);
+              } else {
+                const float out = tf32_rna(v);
+                memcpy(pdst, &out, 4);
+              }
+            }
+        continue;
+      }
       if (d.seg == gE1 && BF16 == 0 && split_e1) {
         // split e1 of the TF32 kernel: BF16 pieces w = w1 + w2; pass 0 (13 steps) holds [w1 | w1] (meets [a1 | a2]),
         // pass 1 (7 steps) [w2 of pair 2w | w2 of pair 2w + 1] (meets [a1 two rows apart])
@@ -1027,7 +1125,10 @@ void launch_impl(const float* hist, int n_int, const void* packed, int split_e1,
                  const int* list, const int* n_list, const int* seg_cnt, bool pdl, cudaStream_t s) {
   using G = Geo<C, BF16, CG, TT>;
   const int n_groups = (n_int + G::T - 1) / G::T;
-  const int n_pg = (n_groups + CG - 1) / CG, max_pairs = sm_count / CG;
+#ifndef PVF_UNET_GRID_DIV
+#define PVF_UNET_GRID_DIV 1      // experiments only: run on 1/N of the SMs (is a chip-wide resource the limit?)
+#endif
+  const int n_pg = (n_groups + CG - 1) / CG, max_pairs = sm_count / CG / PVF_UNET_GRID_DIV;
   const int grid = CG * (n_pg < max_pairs ? n_pg : max_pairs);
   PdlLaunch L(dim3(grid), dim3(G::THREADS), G::SMEM, s, pdl, CG);
   cudaLaunchKernelEx(&L.cfg, k_unet_tc<C, BF16, CG, TT>, hist, n_int, static_cast<const unsigned char*>(packed), split_e1,
@@ -1038,10 +1139,6 @@ template <int C, int BF16, int CG>
 cudaError_t setup_impl() {
   cudaError_t e = cudaFuncSetAttribute(k_unet_tc<C, BF16, CG, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        Geo<C, BF16, CG, 0>::SMEM);
-  constexpr int TS = (C == 64 && CG == 2 && BF16 != 3) ? 1 : 0;   // the small-batch instance (one interval per group)
-  if (e == cudaSuccess && TS == 1)
-    e = cudaFuncSetAttribute(k_unet_tc<C, BF16, CG, TS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             Geo<C, BF16, CG, TS>::SMEM);
   return e;
 }
 
@@ -1092,15 +1189,6 @@ void launch_unet_tc(const float* hist, int n_intervals_total, const void* packed
                     int split_mask, int cta_pair, float* probs, int sm_count, const int* list, const int* n_list,
                     const int* seg_cnt, bool pdl, cudaStream_t s) {
   if (n_intervals_total <= 0) return;
-  // Small batches (NEXT-4): while one interval per CTA still fits the machine in a single round, groups
-  // of one interval finish sooner than groups of two on half as many SMs.  Same arithmetic per interval, identical bits.
-  if (channels == 64 && cta_pair && precision != PVF_PREC_FP32 && list == nullptr && n_intervals_total <= sm_count) {
-    const int fm = precision == PVF_PREC_BF16 ? 1 : (precision == PVF_PREC_FP16 ? 2 : 0);
-#define PVF_SMALL(B_) launch_impl<64, B_, 2, 1>(hist, n_intervals_total, packed_dev, split_mask & 1, probs, sm_count, list, n_list, seg_cnt, pdl, s)
-    if (fm == 1) PVF_SMALL(1); else if (fm == 2) PVF_SMALL(2); else PVF_SMALL(0);
-#undef PVF_SMALL
-    return;
-  }
 #define PVF_CALL(C_, B_, G_) \
   launch_impl<C_, B_, G_>(hist, n_intervals_total, packed_dev, split_mask & 1, probs, sm_count, list, n_list, seg_cnt, pdl, s)
   PVF_TC_DISPATCH(PVF_CALL);

@@ -480,9 +480,9 @@ def test_l2_chunked_histogram_buffer_is_bit_identical(prec, chunk):
 # ------------------------------------------------------------------ NEXT-4: small batches (low-latency schedule)
 @pytest.mark.parametrize("prec", ["tf32", "bf16", "fp16", "fp32", "simt"])
 def test_small_batches_match_the_batch_path_bit_for_bit(prec):
-    """PAPER.md:11, 37 (per-event deployment under a sub-400 us budget): calls with 1, 2, 3 and 7 events -- up to 3 events
-    run the UNet with one interval per CTA (148 or fewer intervals in the call), all of them with the kernels chained by
-    programmatic dependent launch -- must give exactly the bits the same events get inside a 16-event batch; also with stage
+    """PAPER.md:11, 37 (per-event deployment under a sub-400 us budget): calls with 1, 2, 3 and 7 events -- a handful of
+    CTAs per kernel, one CTA per event in the peak finder, the kernels chained by programmatic dependent launch -- must
+    give exactly the bits the same events get inside a 16-event batch; also with stage
     timing on (no PDL)."""
     ev = make_events("run3", 16, 559)
     w = make_weights("peaky", 5)
