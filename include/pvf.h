@@ -79,8 +79,9 @@ typedef struct {
   int32_t peak_halfwidth;  /* (fixed) 3 */
   int32_t max_peaks;       /* (fixed) 32 */
   int32_t precision;       /* pvf_precision */
-  int32_t split_mask;      /* TF32 only: bit L (0=e1,1=e2,2=b,3=d2,4=d1) = hi/lo split precision for that conv
-                              layer (only bit 0 is built: two passes on BF16 pieces) */
+  int32_t split_mask;      /* PVF_PREC_TF32 only: 0, or 1 = the e1 layer (raw histogram input, the dominant TF32 error) runs as
+                              two passes on BF16 pieces.  Anything else is PVF_ERR_CONFIG: FP32
+                              accuracy on every layer is PVF_PREC_FP32, not a mask value */
   int32_t max_events;      /* capacity the pool is sized for (>= 1) */
   int64_t max_tracks;      /* capacity the pool is sized for (>= 1) */
   int32_t enable_stage_timing; /* pre-creates CUDA events around the four stages; default 0 */
