@@ -150,8 +150,14 @@ struct Geo {
   // TMEM columns: region A = [0, T*2C) (d1), region B = [T*2C, 2*T*2C) (e1; e2, b, d2 use its head);
   // an accumulator tile is 2C columns: E0 (even taps) | E1 (odd taps)
   static constexpr int COL_A = 0, COL_B = T * NOUT;
-  static constexpr int TMEM_COLS = (2 * T * NOUT <= 32) ? 32 : (2 * T * NOUT <= 64) ? 64 : (2 * T * NOUT <= 128) ? 128
-                                   : (2 * T * NOUT <= 256) ? 256 : 512;
+  // FX: the two halves of d1 accumulate in SEPARATE tiles (region A for the skip half, A2 for the upsampled half) and
+  // the epilogue adds them in FP32: a tensor-core accumulator is not rounded to nearest, and with 400+ accumulating MMAs
+  // per tile that rounding is what is left of the error once the products are FP32-accurate (measured on config 1: one
+  // tile max |dP| 1.9e-5, two tiles 1.2e-5; a third tile for the last part of the skip half changed nothing)
+  static constexpr int COL_A2 = 2 * T * NOUT;
+  static constexpr int TMEM_USED = (FX ? 3 : 2) * T * NOUT;
+  static constexpr int TMEM_COLS = (TMEM_USED <= 32) ? 32 : (TMEM_USED <= 64) ? 64 : (TMEM_USED <= 128) ? 128
+                                   : (TMEM_USED <= 256) ? 256 : 512;
   // d1E parts (steps): run while the epilogues of e2 / b / d2 drain; multiples of every SPS
   static constexpr int D1E_STEPS = 13 * NKB1 * PH * (PP ? 2 : 1);   // 13 tap pairs; polyphase: 13 offsets x 2C channels
   static constexpr int D1E_A = D1E_STEPS < 16 * PH ? D1E_STEPS : 16 * PH;
@@ -160,7 +166,7 @@ struct Geo {
   static_assert(2 * SZ_L2 == SZ_L1, "E2 + U2 must tile the overlay region exactly");
   static constexpr bool kFits = SMEM <= 227 * 1024 && STAGES >= 3;   // checked where a kernel is instantiated (the helper
                                                                      // templates read layout constants from Geo<.., CG = 1>)
-  static_assert(2 * T * NOUT <= 512, "TMEM budget");
+  static_assert(TMEM_USED <= 512, "TMEM budget");
   static_assert(NCH % 2 == 0 && (T % 2 == 0 || T == 1), "whole MMA K blocks per source; level-2 tiles whole (or one interval)");
   static_assert(16 % SPS == 0 && SPS % PH == 0, "d1E parts must start on ring-stage boundaries; whole (main, correction) pairs per stage");
   static_assert(!FX || T == 1, "the FP32-accurate format runs on groups of one interval");
@@ -358,6 +364,13 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
     uint32_t r[16];
     tmem_ld_x16(taddr + (uint32_t)(C + c0), r);
     tmem_ld_wait();
+    if (MODE == kD1 && G::FX) {
+      uint32_t s1[16];
+      tmem_ld_x16(taddr + (uint32_t)(G::COL_A2 - G::COL_A + C + c0), s1);
+      tmem_ld_wait();
+#pragma unroll
+      for (int i = 0; i < 16; ++i) r[i] = __float_as_uint(__uint_as_float(r[i]) + __uint_as_float(s1[i]));
+    }
     if (lane == 0) {
 #pragma unroll
       for (int k = 0; k < 4; ++k)
@@ -406,6 +419,17 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
     tmem_ld_x16(taddr + (uint32_t)c0, r);
     tmem_ld_x16(taddr + (uint32_t)(C + c0), r1);
     tmem_ld_wait();
+    if (MODE == kD1 && G::FX) {               // the upsampled half of d1 sits in its own accumulator tile (region A2)
+      uint32_t s0[16], s1[16];
+      tmem_ld_x16(taddr + (uint32_t)(G::COL_A2 - G::COL_A + c0), s0);
+      tmem_ld_x16(taddr + (uint32_t)(G::COL_A2 - G::COL_A + C + c0), s1);
+      tmem_ld_wait();
+#pragma unroll
+      for (int i = 0; i < 16; ++i) {
+        r[i] = __float_as_uint(__uint_as_float(r[i]) + __uint_as_float(s0[i]));
+        r1[i] = __float_as_uint(__uint_as_float(r1[i]) + __uint_as_float(s1[i]));
+      }
+    }
     float v[16], nx[16];
 #pragma unroll
     for (int k = 0; k < 4; ++k) {             // whole-warp broadcast loads (cheaper than 16 predicated scalar loads)
@@ -572,7 +596,7 @@ struct Lay {
                               : (S == sB) ? G::OFF_R + G::SZ_L2 /* P2 */ : (S == sD2) ? G::OFF_R + G::SZ_L2 /* U2 */
                               : (S == sD1U) ? G::OFF_R /* U1 | polyphase: d2 itself */ : G::OFF_E1 /* E1 */;
   static constexpr int SRC1 = (S == sD2) ? G::OFF_R /* E2 */ : SRC0;
-  static constexpr int DCOL = D1 ? G::COL_A : G::COL_B;
+  static constexpr int DCOL = (S == sD1U && G::FX) ? G::COL_A2 : (D1 ? G::COL_A : G::COL_B);
   // byte offset (from the CTA's shared-memory base) of the first chunk of K block kk
   __host__ __device__ static constexpr int a_off(int kk) {
     return kk < HALF ? SRC0 + 2 * kk * LBO : SRC1 + 2 * (kk - HALF) * LBO;
@@ -851,7 +875,7 @@ k_unet_tc(const float* __restrict__ hist, int n_int, const unsigned char* __rest
         mma_seg<C, BF16, CG, TT, sE1>(sb, tmem_base, bar0, rs, 0, P.e1_steps, 0u, split_e1 != 0);
         commit(0);
       }
-      mma_seg<C, BF16, CG, TT, sD1U>(sb, tmem_base, bar0, rs, 0, 13 * G::NKB1 * G::PH, 1u);
+      mma_seg<C, BF16, CG, TT, sD1U>(sb, tmem_base, bar0, rs, 0, 13 * G::NKB1 * G::PH, G::FX ? 0u : 1u);   // FX: its own tile
       commit(4);
       first = false;
     }
