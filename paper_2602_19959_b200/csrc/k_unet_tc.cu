@@ -104,6 +104,9 @@ struct Geo {
   static constexpr int PH = FX ? 2 : 1;              // MMA steps per (tap pair, K block): FX = main + correction
   static constexpr int NOUT = 2 * C;                 // MMA N: the outputs of an (even, odd) tap pair side by side
   static constexpr int T = TT ? TT : (FX ? 1 : ((C == 64) ? 2 : (C == 32 ? 4 : (B16 ? 8 : 4))));   // intervals per group (TMEM: 4*T*C <= 512)
+  // Lead (halo) rows of a chunk.  (12 lead rows at levels 2 / 3 -- chunk pitch 64 mod 128 bytes, so that the chunk pairs an
+  // (even, odd) lane pair writes fall into different bank halves -- were measured: C = 32 BF16 5.57 -> 5.98 ms per 8000 events,
+  // the tensor core's own operand reads prefer the 128-byte-aligned pitch.)
   static constexpr int LEAD1 = 16, LEAD2 = 8, LEAD3 = 8;
   // rows per chunk = lead halo + T interval slots; reads past the last slot (garbage output rows only)
   // land in the following chunk / buffer, which is always inside the CTA's allocation
@@ -121,9 +124,11 @@ struct Geo {
   // shared-memory map (bytes)
   static constexpr int SZ_L1 = NCHB * LBO1;          // a C-channel buffer at L = 100
   static constexpr int SZ_L2 = NCHB * LBO2;          //                     at L = 50
+  static constexpr int SZ_E1 = PP ? 2 * SZ_L2 : SZ_L1;   // e1 skip: de-interleaved on level-2 rows (polyphase d1) | level-1 rows
+  static constexpr int SZ_R = PP ? 2 * SZ_L2 : SZ_L1;    // (E2 | U2), then d2 in E2's place (polyphase) | U1 over both
   static constexpr int OFF_E1 = 0;                   // e1 skip (dedicated)
-  static constexpr int OFF_R = OFF_E1 + SZ_L1;       // overlay: (E2 | U2) then U1; P2 sits in U2's place
-  static constexpr int OFF_XP = OFF_R + SZ_L1;       // overlay: X0 (input) then P1 = pool(e1)
+  static constexpr int OFF_R = OFF_E1 + SZ_E1;       // overlay: (E2 | U2) then U1 / d2; P2 sits in U2's place
+  static constexpr int OFF_XP = OFF_R + SZ_R;        // overlay: X0 (input) then P1 = pool(e1)
   static constexpr int SZ_XP = (XCH * LBO1 > SZ_L2) ? XCH * LBO1 : SZ_L2;
   static constexpr int OFF_RING = OFF_XP + SZ_XP;
   static constexpr int SETS = epi_sets(C);
@@ -163,7 +168,7 @@ struct Geo {
   static constexpr int D1E_A = D1E_STEPS < 16 * PH ? D1E_STEPS : 16 * PH;
   static constexpr int D1E_B = (D1E_STEPS - D1E_A) < 16 * PH ? (D1E_STEPS - D1E_A) : 16 * PH;
   static constexpr int D1E_C = D1E_STEPS - D1E_A - D1E_B;
-  static_assert(2 * SZ_L2 == SZ_L1, "E2 + U2 must tile the overlay region exactly");
+  static_assert(PP || 2 * SZ_L2 == SZ_L1, "E2 + U2 must tile the overlay region exactly (direct d1: U1 overlays both)");
   static constexpr bool kFits = SMEM <= 227 * 1024 && STAGES >= 3;   // checked where a kernel is instantiated (the helper
                                                                      // templates read layout constants from Geo<.., CG = 1>)
   static_assert(TMEM_USED <= 512, "TMEM budget");
