@@ -165,8 +165,11 @@ struct Geo {
                                    : (TMEM_USED <= 256) ? 256 : 512;
   // d1E parts (steps): run while the epilogues of e2 / b / d2 drain; multiples of every SPS
   static constexpr int D1E_STEPS = 13 * NKB1 * PH * (PP ? 2 : 1);   // 13 tap pairs; polyphase: 13 offsets x 2C channels
-  static constexpr int D1E_A = D1E_STEPS < 16 * PH ? D1E_STEPS : 16 * PH;
-  static constexpr int D1E_B = (D1E_STEPS - D1E_A) < 16 * PH ? (D1E_STEPS - D1E_A) : 16 * PH;
+  // polyphase: a step feeds T/2 tiles instead of T, so the parts that cover the e2 / b epilogues are twice as many steps
+  // (with 16 the issuer waited 3 % of its time for each of the two epilogues)
+  static constexpr int D1E_PART = ((PP && C == 64) ? 32 : 16) * PH;   // (narrower widths: measured slower with 32)
+  static constexpr int D1E_A = D1E_STEPS < D1E_PART ? D1E_STEPS : D1E_PART;
+  static constexpr int D1E_B = (D1E_STEPS - D1E_A) < D1E_PART ? (D1E_STEPS - D1E_A) : D1E_PART;
   static constexpr int D1E_C = D1E_STEPS - D1E_A - D1E_B;
   static_assert(PP || 2 * SZ_L2 == SZ_L1, "E2 + U2 must tile the overlay region exactly (direct d1: U1 overlays both)");
   static constexpr bool kFits = SMEM <= 227 * 1024 && STAGES >= 3;   // checked where a kernel is instantiated (the helper
