@@ -128,8 +128,13 @@ struct Geo {
   static constexpr int SZ_R = PP ? 2 * SZ_L2 : SZ_L1;    // (E2 | U2), then d2 in E2's place (polyphase) | U1 over both
   static constexpr int OFF_E1 = 0;                   // e1 skip (dedicated)
   static constexpr int OFF_R = OFF_E1 + SZ_E1;       // overlay: (E2 | U2) then U1 / d2; P2 sits in U2's place
-  static constexpr int OFF_XP = OFF_R + SZ_R;        // overlay: X0 (input) then P1 = pool(e1)
-  static constexpr int SZ_XP = (XCH * LBO1 > SZ_L2) ? XCH * LBO1 : SZ_L2;
+  static constexpr int OFF_XP = OFF_R + SZ_R;        // X0 (input); direct d1: overlaid by P1 = pool(e1)
+  // Polyphase: P1 lives in U2's place (second half of R) -- free from d2's MMAs (the last readers of U2) until e2's epilogue
+  // writes P2 there, and the NEXT group's e1 epilogue (the writer of P1) only runs after this group's d2 MMAs have retired.
+  // XP then holds X0 alone, which is what buys TF32 a fourth 16 KB ring stage.  Direct d1 (FX): U1 covers all of R while the
+  // next e1 epilogue runs, so P1 stays in XP.
+  static constexpr int OFF_P1 = PP ? OFF_R + SZ_L2 : OFF_XP;
+  static constexpr int SZ_XP = PP ? XCH * LBO1 : ((XCH * LBO1 > SZ_L2) ? XCH * LBO1 : SZ_L2);
   static constexpr int OFF_RING = OFF_XP + SZ_XP;
   static constexpr int SETS = epi_sets(C);
   static constexpr int EPI_THREADS = 128 * SETS, THREADS = 64 + EPI_THREADS;
@@ -401,8 +406,8 @@ __device__ __forceinline__ void epilogue_tile(uint32_t smem_base, uint32_t tmem_
     } else {
       dst_full = smem_base + G::OFF_E1 + (uint32_t)(G::LEAD1 + 128 * tile + m) * 16u; lbo_full = G::LBO1;
     }
-    dst_aux = smem_base + G::OFF_XP + (uint32_t)(G::LEAD2 + 64 * tile + (m >> 1)) * 16u; lbo_aux = G::LBO2;     // P1
-    if (tile == 0 && m < G::LEAD2) zero_rows(smem_base + G::OFF_XP, G::LBO2, G::NCHB, m);
+    dst_aux = smem_base + G::OFF_P1 + (uint32_t)(G::LEAD2 + 64 * tile + (m >> 1)) * 16u; lbo_aux = G::LBO2;     // P1
+    if (tile == 0 && m < G::LEAD2) zero_rows(smem_base + G::OFF_P1, G::LBO2, G::NCHB, m);
   } else if (MODE == kE2) {
     dst_full = smem_base + G::OFF_R + (uint32_t)(G::LEAD2 + 128 * tile + m) * 16u; lbo_full = G::LBO2;          // E2
     dst_aux = smem_base + G::OFF_R + G::SZ_L2 + (uint32_t)(G::LEAD3 + 64 * tile + (m >> 1)) * 16u; lbo_aux = G::LBO3;  // P2
@@ -600,7 +605,7 @@ struct Lay {
   static constexpr int LBO = LEVEL == 1 ? G::LBO1 : (LEVEL == 2 ? G::LBO2 : G::LBO3);
   static constexpr int NT = LEVEL == 1 ? G::T : (LEVEL == 2 ? (G::T + 1) / 2 : (G::T + 3) / 4);
   static constexpr int HALF = (S == sD2) ? NKB / 2 : NKB;      // K blocks served by the first source buffer
-  static constexpr int SRC0 = (S == sE1) ? G::OFF_XP /* X0 */ : (S == sE2) ? G::OFF_XP /* P1 */
+  static constexpr int SRC0 = (S == sE1) ? G::OFF_XP /* X0 */ : (S == sE2) ? G::OFF_P1 /* P1 */
                               : (S == sB) ? G::OFF_R + G::SZ_L2 /* P2 */ : (S == sD2) ? G::OFF_R + G::SZ_L2 /* U2 */
                               : (S == sD1U) ? G::OFF_R /* U1 | polyphase: d2 itself */ : G::OFF_E1 /* E1 */;
   static constexpr int SRC1 = (S == sD2) ? G::OFF_R /* E2 */ : SRC0;
