@@ -185,7 +185,8 @@ PVF_API pvf_status pvf_debug_copy_histogram(pvf_handle h, float* dev_out, int32_
  * Needs enable_stage_timing; PVF_ERR_UNSUPPORTED if no run was recorded. */
 PVF_API pvf_status pvf_stage_times_ms(pvf_handle h, float out_ms[4]);
 
-/* Number of kernels pvf_run enqueues for n_events (host arithmetic; for launch accounting). */
+/* Number of KERNELS pvf_run enqueues for n_events (host arithmetic; for launch accounting).  The elision mode also enqueues one
+ * 4-byte cudaMemsetAsync per chunk (the work-list counter), which is not a kernel and is not counted. */
 PVF_API int32_t pvf_launches_per_run(pvf_handle h, int32_t n_events);
 
 PVF_API pvf_status pvf_destroy(pvf_handle h);
