@@ -39,10 +39,20 @@ k_peaks(const float* __restrict__ probs, int n_events, float thr, const uint32_t
   pdl_wait();                                         // the probabilities come from the kernel before this one
   if (e >= n_events) return;
   const float4* P4 = reinterpret_cast<const float4*>(probs + (size_t)e * kGlobalBins);
-  for (int i = tid; i < kGlobalBins / 4; i += kPeakThreads) {
-    const float4 v = P4[i];
-    const int s = pk_slot(4 * i);                     // 4 i .. 4 i + 3 never straddle a multiple of 32
-    sP[s] = v.x; sP[s + 1] = v.y; sP[s + 2] = v.z; sP[s + 3] = v.w;
+  constexpr int kLoads = (kGlobalBins / 4 + kPeakThreads - 1) / kPeakThreads;   // 8: all in flight at once (one event: the
+  float4 v[kLoads];                                                              // L2 round trips would otherwise add up)
+#pragma unroll
+  for (int k = 0; k < kLoads; ++k) {
+    const int i = tid + k * kPeakThreads;
+    if (i < kGlobalBins / 4) v[k] = P4[i];
+  }
+#pragma unroll
+  for (int k = 0; k < kLoads; ++k) {
+    const int i = tid + k * kPeakThreads;
+    if (i < kGlobalBins / 4) {
+      const int s = pk_slot(4 * i);                   // 4 i .. 4 i + 3 never straddle a multiple of 32
+      sP[s] = v[k].x; sP[s + 1] = v[k].y; sP[s + 2] = v[k].z; sP[s + 3] = v[k].w;
+    }
   }
   __syncthreads();
   const float ninf = __int_as_float(0xff800000);
