@@ -490,6 +490,8 @@ def main_ours(args, rank, world, local_rank):
             # BASELINE.json's metric also asks for the UNet tensor-pipe utilisation: a profiler counter, so it is
             # the value of the committed ncu capture (profiles/), not something measured in this run
             "tensor_pipe_active_pct_ncu": tensor_pct, "tensor_pipe_source": traffic_src}
+    roof["frac_vs_nominal_dense_peak"] = achieved / {"tf32": 1100.0, "bf16": 2250.0, "fp16": 2250.0, "fp32": 1100.0}[args.precision] \
+        if bound == "tensor" else None      # B200_PROFILING.md nominal dense peaks at the maximum clock, for context
     if args.precision == "tf32":
         d_s = peaks["bf16_tflops_sustained"] * 1.1 / 2.25
         d_b = peaks["bf16_tflops"] * 1.1 / 2.25
