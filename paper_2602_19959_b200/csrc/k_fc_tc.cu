@@ -83,7 +83,7 @@ static_assert(FT_SMEM <= 227 * 1024, "shared memory budget");
 // 2-deep h_full gave no such guarantee to a slow epilogue warp: hidden(it + 2) is only gated by the MMAs of tile it.)
 enum { bHFull = 0, bPHFull = bHFull + kHidGroups, bHEmpty = bPHFull + kHidGroups, bMeta = bHEmpty + kHidGroups,
        bAccFull = bMeta + kIvBufs, bAccEmpty = bAccFull + 4, bPAccEmpty = bAccEmpty + 4, bIvFull = bPAccEmpty + 4,
-       bSlot = bIvFull + kIvBufs };
+       bW5 = bIvFull + kIvBufs, bSlot = bW5 + 1 };
 static_assert(8 * bSlot + 4 <= 512, "barrier block");
 constexpr int kIvLog = 3;
 static_assert((1 << kIvLog) == kIvBufs && kIvBufs >= 2 * kHidGroups, "interval lists: a power of two, two per hidden-layer group");
@@ -215,10 +215,17 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
   // ---- one-time setup: this half's W5x image, zeroed B buffers, the small layers, barriers, TMEM (weights only:
   // all of it may overlap the tail of the sort kernel, see pdl.cuh)
   pdl_launch_dependents();
+  // The 128 KB of W5x go by bulk copies (TMA engine) issued first thing by one thread; they land while the other threads
+  // stage the small layers and zero the operand buffers (a load / store loop of all threads took ~4 us, most of what a
+  // one-event call spends in this kernel before its first track).
+  if (tid == 0) {
+    mbar_init(bar(bW5), 1);
+    fence_mbar_init();
+    mbar_arrive_expect_tx(bar(bW5), (uint32_t)(2 * kWPart));
+    for (int k = 0; k < 2 * kWPart / 16384; ++k)
+      bulk_g2s(sb + OFF_W + k * 16384, w5img + (size_t)half * 2 * kWPart + (size_t)k * 16384, 16384u, bar(bW5));
+  }
   {
-    const uint4* src = reinterpret_cast<const uint4*>(w5img + (size_t)half * 2 * kWPart);
-    uint4* dst = reinterpret_cast<uint4*>(smem + OFF_W);
-    for (int i = tid; i < 2 * kWPart / 16; i += kFtThreads) dst[i] = __ldg(src + i);
     uint4* hz = reinterpret_cast<uint4*>(smem + OFF_H);
     for (int i = tid; i < 2 * kHidGroups * kHPart / 16; i += kFtThreads) hz[i] = make_uint4(0, 0, 0, 0);
   }
@@ -246,6 +253,7 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
       mbar_init(bar(bPAccEmpty + k), k < 3 ? 128 : 32);
     }
     fence_mbar_init();
+    mbar_wait(bar(bW5), 0u);                     // this CTA's W5x image has landed (the peer's: before the cluster barrier below)
   }
   if (warp == kMmaWarp) tmem_alloc2(smem_u32(const_cast<uint32_t*>(tmem_slot)), 512);
   fence_proxy_async_smem();
