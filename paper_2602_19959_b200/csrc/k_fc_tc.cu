@@ -11,9 +11,10 @@
 //     D[o, t] = sum_k W5x[o, k] * hx[t, k],   k < 25: weights x activations, k = 25: bias x 1, K = 32
 // with M = output rows and N = 128 tracks.  So an accumulator lane is one output and an accumulator column
 // is one track: the epilogue thread that owns a lane walks the columns in sorted-track order, adds
-// softplus(D) into one FP32 register and stores it to H whenever the interval changes -- the same fixed-order
-// sum as k_fc_hist, with no cross-lane reduction; only intervals that hold a track are written (k_unet_tc takes
-// seg_cnt == 0 as zeros).
+// softplus(D) into one FP32 register and stores it to H whenever the interval changes -- a sum whose order is fixed
+// by the sorted positions, with no cross-lane reduction; only intervals that hold a track are written (k_unet_tc
+// takes seg_cnt == 0 as zeros).  Tracks of the same interval share one logarithm per group (16-track chunk or group
+// of four; see softplus_front2): sum softplus(v) = sum max(v, 0) + ln 2 lg2(prod (1 + e^-|v|)).
 // FP32 accuracy: W5x = W_hi + W_lo and hx = h_hi + h_lo (each part RN-rounded to TF32), three MMAs
 // W_hi h_hi + W_hi h_lo + W_lo h_hi accumulate in FP32 in TMEM (the dropped term is ~2^-22 relative).
 // CTA pairs: the two CTAs of a cluster serve the two halves of the 800 outputs (400 each, packed densely into

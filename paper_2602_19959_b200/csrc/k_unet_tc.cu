@@ -16,7 +16,7 @@
 // Intervals sit at row stride 128 / 64 / 32 (L = 100 / 50 / 25); the rows between them are zero and
 // double as the "same" padding.  One persistent CTA takes a group of T intervals through all five
 // layers; each weight slice is streamed from L2 once per group (1D bulk copies into a ring of 16 KB
-// stages, 8 KB per CTA of a pair) and used by every tile of the group.
+// stages -- also per CTA of a pair, see Geo::STAGE_BYTES) and used by every tile of the group.
 //
 // CTA pairs (template parameter CG = 2, the default of the binding): a cluster of two CTAs runs every MMA as
 // one tcgen05.mma.cta_group::2 of M = 256 issued by the leader; each CTA keeps its own group's activations
@@ -27,7 +27,8 @@
 // is cut in three parts that run while the epilogues of e2, b and d2 drain, and the NEXT group's e1
 // runs before d1U so that its epilogue overlaps d1U:
 //     e2 | d1E.1 | b | d1E.2 | d2 | d1E.3 | e1(next) | d1U        (weight image is packed in this order)
-// TMEM holds two accumulator regions: A (d1, T tiles) and B (e1: T tiles; e2, b, d2: its first tiles).
+// TMEM holds two accumulator regions: A (d1: T/2 low-resolution tiles, polyphase; direct d1: T tiles) and B (e1: T tiles; e2, b,
+// d2: its first tiles); FX adds A2 (the upsampled half of d1 accumulates on its own).
 // Roles: warp 0 = weight producer, warp 1 = MMA issuer (warp-uniform schedule, one elected lane
 // issues; in the peer CTA of a pair it relays "my half of the stage has landed"), warps 2.. = epilogue in
 // sets of four (TMEM -> registers -> bias, LeakyReLU, TF32/BF16 rounding, pool / upsample -> shared
@@ -42,7 +43,7 @@
 //   * the skip half reads e1 de-interleaved (row i holds positions 2i and 2i + 1 as 2C channels): same MMA time as before,
 //     no row shift in the epilogue.
 // The accumulator tile is [low-resolution row][phase 0: C | phase 1: C]; the epilogue thread of row i computes both
-// logits and stores two probabilities.  ~15 % fewer MMA cycles per interval (SURVEY.md H1 "polyphase weights").
+// logits and stores two probabilities.  ~17 % fewer MMA cycles per interval (SURVEY.md H1 "polyphase weights").
 //
 // FP32-accurate mode (format 3, "FX"; PVF_PREC_FP32 on the tensor cores, BASELINE.json config 0 "FP32"): every product a w is
 // taken as  tf32(a) tf32(w)  +  [a - tf32(a)] w  +  a [w - tf32(w)]  -- the first term one kind::tf32 MMA, the two small
