@@ -481,26 +481,34 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
             // are one row of the transposed matrix: 7 broadcast 16-byte loads), so no FMA waits for the one before it.
             // (Output-major -- one 25-long dependent chain per output, three chains interleaved by the compiler -- ran
             // the hidden-layer warps at 0.3 instructions per clock and made them the critical path of the kernel.)
-            const float4* br = reinterpret_cast<const float4*>(S.bh[l]);
+            // The 25 accumulators live as 13 packed pairs (fma.rn.f32x2: one issue slot for two outputs); the weight row
+            // and the bias arrive as 64-bit pairs straight from the 16-byte loads, so nothing is repacked but the input.
+            unsigned long long acc2[14];
+            const ulonglong2* br = reinterpret_cast<const ulonglong2*>(S.bh[l]);
 #pragma unroll
             for (int q = 0; q < 7; ++q) {
-              const float4 b = br[q];
-              gg[4 * q] = b.x; gg[4 * q + 1] = b.y; gg[4 * q + 2] = b.z; gg[4 * q + 3] = b.w;
+              const ulonglong2 b = br[q];
+              acc2[2 * q] = b.x; acc2[2 * q + 1] = b.y;
             }
 #pragma unroll
             for (int k = 0; k < kFcHidden; ++k) {
-              const float4* wr = reinterpret_cast<const float4*>(S.wh[l][k]);
+              const ulonglong2* wr = reinterpret_cast<const ulonglong2*>(S.wh[l][k]);
+              unsigned long long hh;
+              asm("mov.b64 %0, {%1, %1};" : "=l"(hh) : "f"(h[k]));
 #pragma unroll
               for (int q = 0; q < 7; ++q) {
-                const float4 w = wr[q];
-                gg[4 * q] = fmaf(w.x, h[k], gg[4 * q]);
-                if (4 * q + 1 < kFcHidden) gg[4 * q + 1] = fmaf(w.y, h[k], gg[4 * q + 1]);
-                if (4 * q + 2 < kFcHidden) gg[4 * q + 2] = fmaf(w.z, h[k], gg[4 * q + 2]);
-                if (4 * q + 3 < kFcHidden) gg[4 * q + 3] = fmaf(w.w, h[k], gg[4 * q + 3]);
+                const ulonglong2 w = wr[q];
+                asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc2[2 * q]) : "l"(w.x), "l"(hh));
+                if (4 * q + 2 < kFcHidden) asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc2[2 * q + 1]) : "l"(w.y), "l"(hh));
               }
             }
 #pragma unroll
-            for (int o = 0; o < kFcHidden; ++o) h[o] = leaky_ft(gg[o]);
+            for (int o = 0; o < kFcHidden; o += 2) {
+              float lo, hi2;
+              asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi2) : "l"(acc2[o / 2]));
+              h[o] = leaky_ft(lo);
+              if (o + 1 < kFcHidden) h[o + 1] = leaky_ft(hi2);
+            }
           }
           h[25] = 1.0f;                              // multiplies the bias column of W5x
 #pragma unroll
