@@ -25,6 +25,7 @@
 // 14-21 = four groups of 64 threads that run the five 25-wide hidden layers (FP32 FMA, thread = track) for
 // tiles it, it + 1, it + 2, it + 3 and stage h_hi / h_lo as the B operand (one buffer per group).
 #include <cstring>
+#include <type_traits>
 
 #include "pvf_internal.cuh"
 #include "pdl.cuh"
@@ -303,7 +304,10 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
         { FC_PROF_T0(); mbar_wait(bar(bAccFull + mt), (uint32_t)(it & 1)); FC_PROF_ADD(1, pw); }
         tc_fence_after_sync();
         const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)(mt * kTile);
-        for (int c0 = 0; c0 < ntile; c0 += 16) {
+        // One chunk of 16 sorted positions.  TAIL (compile time) = the tile's last, partly filled chunk: only that copy of the
+        // code masks the columns past the last track (as one body the masking cost every chunk 16 compares + 32 selects).
+        auto chunk = [&](const int c0, auto tail_tag) {
+          constexpr bool TAIL = decltype(tail_tag)::value;
           // sorted positions c0 .. c0+15: the even ones are columns c0/2 .. of the leader's half of N, the odd ones
           // columns 64 + c0/2 .. of the peer's half
           uint32_t ve[8], vo[8];
@@ -312,7 +316,7 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
           // Where do intervals change inside these 16 tracks?  The interval list is the same for every lane, so the
           // answer is one warp-uniform 16-bit mask: lane i < 16 compares track c0 + i with its predecessor (the running
           // interval c for the tile's first track), one ballot.  Tracks past the tile's end never start an interval.
-          const int nv = ntile - c0;
+          const int nv = TAIL ? ntile - c0 : 16;
           const int pos = c0 + (lane & 15);
           const int iv_prev = pos == 0 ? c : ivs[pos - 1];
           const unsigned mask = __ballot_sync(0xffffffffu, lane < 16 && lane < nv && ivs[pos] != iv_prev);
@@ -323,7 +327,7 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
 #pragma unroll
           for (int k = 0; k < 8; ++k)
             softplus_front2(__uint_as_float(ve[k]), __uint_as_float(vo[k]), u[2 * k], u[2 * k + 1], m[2 * k], m[2 * k + 1]);
-          if (nv < 16) {
+          if (TAIL) {
 #pragma unroll
             for (int i = 0; i < 16; ++i)
               if (i >= nv) { u[i] = 1.0f; m[i] = 0.0f; }
@@ -370,7 +374,10 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
             }
           }
 #endif
-        }
+        };
+        int c0 = 0;
+        for (; c0 + 16 <= ntile; c0 += 16) chunk(c0, std::false_type{});
+        if (c0 < ntile) chunk(c0, std::true_type{});
         if (last) Hc[c] = a;                      // the event's last non-empty interval
         tc_fence_before_sync();
         if (rank == 0) mbar_arrive(bar(bAccEmpty + mt));
