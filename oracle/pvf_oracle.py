@@ -63,9 +63,8 @@ def assign_intervals(z_poca):
     u = (u * np.float32(0.1)).astype(np.float32)
     fl = np.floor(u).astype(np.float32)
     zrel = (u - fl).astype(np.float32)          # exact in float32
-    i = fl.astype(np.int64)
-    ok = finite & (i >= 0) & (i < N_INTERVALS)
-    interval = np.where(ok, i, -1).astype(np.int32)
+    ok = finite & (fl >= np.float32(0.0)) & (fl < np.float32(N_INTERVALS))   # decided on the float: |z| may be 1e30
+    interval = np.where(ok, fl, np.float32(-1.0)).astype(np.int32)
     return interval, zrel, ~finite
 
 

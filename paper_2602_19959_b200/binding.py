@@ -180,7 +180,7 @@ class PVFinder:
     @staticmethod
     def _tracks_struct(feat, event_offsets):
         """feat: float32 tensor [9, n_tracks] (rows contiguous = SoA); event_offsets int32 [E+1]."""
-        assert feat.dim() == 2 and feat.shape[0] == 9 and feat.stride(1) == 1
+        assert feat.dim() == 2 and feat.shape[0] == 9 and (feat.shape[1] == 0 or feat.stride(1) == 1)
         s = pvf_tracks()
         for k in range(9):
             s.feat[k] = feat[k].data_ptr()

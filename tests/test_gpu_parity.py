@@ -553,6 +553,105 @@ def test_batch_without_any_track(prec, elide):
     assert np.array_equal(pk["count"].cpu().numpy(), ref["peaks"]["count"])
 
 
+def _structured_batch(rng, pool):
+    """1-12 events whose track counts sit on the tile / chunk edges of the kernels (0, 1, 16 +- 1, 128 +- 1, 256 +- 1, 513)
+    and whose z_poca follow one of six adversarial layouts; other features are drawn from `pool`."""
+    counts = [0, 0, 1, 2, 3, 15, 16, 17, 31, 32, 33, 63, 64, 65, 127, 128, 129, 130, 191, 192, 193, 255, 256, 257, 300, 385, 513]
+    E = int(rng.choice([1, 2, 3, 5, 8, 12]))
+    feats, offs = [], [0]
+    for _ in range(E):
+        n = int(rng.choice(counts))
+        f = pool.feat[:, rng.integers(0, pool.n_tracks, n)].copy()
+        mode = int(rng.integers(0, 6))
+        if mode == 0:                                     # anywhere in the region
+            z = rng.uniform(-200, 200, n)
+        elif mode == 1:                                   # all in one interval
+            z = -200 + 10 * rng.integers(0, 40) + rng.uniform(0, 10, n)
+        elif mode == 2:                                   # exactly on an interval edge, or 1-2 float32 steps beside it
+            z = (-200.0 + 10.0 * rng.integers(0, 41, n)).astype(np.float32)
+            d = rng.integers(-2, 3, n)
+            for step in (1, 2):
+                z = np.where(d >= step, np.nextafter(z, np.float32(1e9)),
+                             np.where(d <= -step, np.nextafter(z, np.float32(-1e9)), z)).astype(np.float32)
+        elif mode == 3:                                   # two tight clusters
+            z = rng.uniform(-190, 190, 2)[rng.integers(0, 2, n)] + rng.normal(0, 0.3, n)
+        elif mode == 4:                                   # around the region's ends, about half outside
+            z = np.where(rng.random(n) < 0.5, -200, 200) + rng.normal(0, 2.0, n)
+        else:                                             # descending
+            z = np.sort(rng.uniform(-200, 200, n))[::-1]
+        z = np.asarray(z, np.float32)
+        if n and rng.random() < 0.2:                      # a few non-finite / absurd positions
+            bad = rng.integers(0, n, max(1, n // 20))
+            z[bad] = rng.choice(np.array([np.nan, np.inf, -np.inf, 1e30, -1e30], np.float32), bad.shape[0])
+        f[0] = z
+        feats.append(f)
+        offs.append(offs[-1] + n)
+    feat = np.ascontiguousarray(np.concatenate(feats, axis=1))
+    return type(pool)(feat, np.array(offs, np.int32), [None] * E)
+
+
+@pytest.mark.parametrize("block", range(4))
+def test_randomised_structured_batches(block):
+    """48 seeded batches (12 per block) with adversarial structure, each through a randomly drawn mode (precision, width,
+    boundary margin, elision, L2 chunks, spare capacity).  Exact in every case: the sort's flags, the zero pattern of H,
+    the peak finder on the kernel's own probabilities, bit-identical reruns, finite outputs.  These inputs are far outside
+    the paper's workloads (hundreds of tracks in ONE interval, FC weights of any seed), where activations -- and with them
+    the rounding error of every precision, the FP32 CUDA-core kernels included -- are several times larger than on
+    run3 / pile-up events; the numeric bounds here are therefore 3 x the stated tolerances for P and 1e-4 for H (observed
+    over 850 such cases: <= 1.6 x and 5.8e-5).  The stated tolerances themselves are asserted on the paper's workloads
+    by the tests above."""
+    pool = make_events("pileup", 64, 77)
+    for case in range(12 * block, 12 * block + 12):
+        rng = np.random.default_rng(10_000 + case)
+        ev = _structured_batch(rng, pool)
+        E = ev.n_events
+        prec = str(rng.choice(["simt", "fp32", "tf32", "bf16", "fp16"]))
+        ch = int(rng.choice([64, 64, 32, 16]))
+        margin = float(rng.choice([0.0, 0.0, 0.3, 1.0, 4.8]))
+        elide = bool(rng.random() < 0.3) and prec != "simt"
+        chunk = int(rng.choice([0, 0, 1, 3]))
+        extra = int(rng.choice([0, 1, 200]))
+        w = make_weights(str(rng.choice(["rand", "peaky"])), 100 + case, ch)
+        what = f"case {case}: E={E} T={ev.n_tracks} {prec} C={ch} margin={margin} elide={elide} chunk={chunk} extra={extra}"
+        ref = O.run(ev.feat, ev.event_offsets, w, want_hist=True, boundary_margin_mm=margin)
+        kw = dict(boundary_margin_mm=margin, elide_empty=elide)
+        if chunk:
+            kw["l2_chunk_events"] = chunk
+        if prec == "simt":
+            kw["cta_pair"] = False
+        pvf = PVFinder(w, max_events=E + extra, max_tracks=max(ev.n_tracks, 1) + extra,
+                       precision="fp32" if prec == "simt" else prec, split_mask=SPLIT[prec], **kw)
+        feat, off = _dev(ev)                               # [9, 0] when no event holds a track
+        probs = torch.full((E, 4000), -1.0, device="cuda")
+        pk = pvf.alloc_peaks(E)
+        s = torch.cuda.Stream()
+        pvf.run(feat, off, E, probs, pk, stream=s)
+        s.synchronize()
+        Pf = probs.cpu().numpy()
+        assert np.isfinite(Pf).all(), what
+        assert np.abs(Pf.astype(np.float64) - ref["probs"]).max() <= 3 * TOL[prec], what
+        got = _np(pk)
+        sort_flags = pkg.FLAG_TRACK_DROPPED | pkg.FLAG_NONFINITE
+        assert np.array_equal(got["flags"].astype(np.uint32) & sort_flags, ref["flags"] & sort_flags), what
+        own = O.find_peaks(Pf)                             # the oracle's peak finder on the kernel's probabilities
+        assert np.array_equal(got["count"], own["count"]) and np.array_equal(got["bin"], own["bin"]), what
+        assert np.array_equal(got["z"].view(np.uint32), own["z"].view(np.uint32)), what
+        assert np.array_equal(got["prob"].view(np.uint32), own["prob"].view(np.uint32)), what
+        if not chunk and not elide:
+            H = torch.empty(E, 40, 8, 100, device="cuda")
+            pvf.debug_copy_histogram(H, E, stream=s)
+            s.synchronize()
+            Hn = H.cpu().numpy().astype(np.float64)
+            assert (np.abs(Hn - ref["hist"]) / np.maximum(np.abs(ref["hist"]), 1.0)).max() <= 1e-4, what
+            assert np.array_equal(Hn == 0, ref["hist"] == 0), what
+        probs2 = torch.full((E, 4000), -1.0, device="cuda")
+        pk2 = pvf.alloc_peaks(E)
+        pvf.run(feat, off, E, probs2, pk2, stream=s)
+        s.synchronize()
+        assert torch.equal(probs, probs2) and all(torch.equal(pk[k], pk2[k]) for k in pk), what
+        pvf.destroy()
+
+
 @pytest.mark.parametrize("model,prec,ch,elide,margin", [("run3", "tf32", 64, False, 0.0), ("pileup", "fp16", 64, True, 0.0),
                                                         ("run3", "bf16", 32, False, 0.0), ("pileup", "tf32", 64, False, 0.5),
                                                         ("run3", "fp32", 64, False, 0.0)])
