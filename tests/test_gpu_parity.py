@@ -590,6 +590,23 @@ def _structured_batch(rng, pool):
     return type(pool)(feat, np.array(offs, np.int32), [None] * E)
 
 
+def _operand_format(prec):
+    """float64 -> the nearest value of the kernel's MMA operand format (TF32: cvt.rna, 10 mantissa bits; FP16 / BF16:
+    round to nearest even), as float64 -- for the oracle's `operand_round` tolerance study."""
+    def tf32(a):
+        u = np.asarray(a, np.float32).view(np.uint32).astype(np.uint64)
+        return (((u + 0x1000) >> 13) << 13).astype(np.uint32).view(np.float32).astype(np.float64)
+
+    def bf16(a):
+        u = np.asarray(a, np.float32).view(np.uint32).astype(np.uint64)
+        return (((u + 0x7fff + ((u >> 16) & 1)) >> 16) << 16).astype(np.uint32).view(np.float32).astype(np.float64)
+
+    def fp16(a):
+        return np.asarray(a, np.float32).astype(np.float16).astype(np.float64)
+
+    return {"tf32": tf32, "bf16": bf16, "fp16": fp16}[prec]
+
+
 @pytest.mark.parametrize("block", range(4))
 def test_randomised_structured_batches(block):
     """48 seeded batches (12 per block) with adversarial structure, each through a randomly drawn mode (precision, width,
@@ -630,6 +647,15 @@ def test_randomised_structured_batches(block):
         Pf = probs.cpu().numpy()
         assert np.isfinite(Pf).all(), what
         assert np.abs(Pf.astype(np.float64) - ref["probs"]).max() <= 3 * TOL[prec], what
+        if prec in ("tf32", "bf16", "fp16"):
+            # What the operand FORMAT alone costs on this input: the oracle with every conv operand rounded to the format
+            # (e1 excepted for TF32: the kernel splits that layer's operands) and exact accumulation.  The kernel must
+            # sit within the stated tolerance of THAT, however far the format itself drifts on such inputs.
+            layers = ["e2", "b", "d2", "d1"] + ([] if prec == "tf32" else ["e1"])
+            emu = O.run(ev.feat, ev.event_offsets, w, boundary_margin_mm=margin,
+                        operand_round={k: _operand_format(prec) for k in layers})
+            d_emu = np.abs(Pf.astype(np.float64) - emu["probs"]).max()
+            assert d_emu <= TOL[prec], f"{what}: |kernel - format emulation| {d_emu:.3e}"
         got = _np(pk)
         sort_flags = pkg.FLAG_TRACK_DROPPED | pkg.FLAG_NONFINITE
         assert np.array_equal(got["flags"].astype(np.uint32) & sort_flags, ref["flags"] & sort_flags), what
