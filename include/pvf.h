@@ -179,6 +179,33 @@ PVF_API pvf_status pvf_run_unet(pvf_handle h, const float* hist, int32_t n_event
  * l2_chunk_events the buffer holds the LAST chunk of the run only (n_events must not exceed its size). */
 PVF_API pvf_status pvf_debug_copy_histogram(pvf_handle h, float* dev_out, int32_t n_events, void* cuda_stream);
 
+/* a0 + a1 + a2 (interval sort, per-track FC, ordered segmented sum; BASELINE.json config 0) for a
+ * SMALL batch with NO allocation anywhere in the call: for callers that cannot call cudaMalloc or supply a pool
+ * (code under CUDA graph capture, tight serving loops, harnesses that forbid it).  The scratch the two kernels need
+ * (the sorted track list perm, seg_off, seg_cnt, per-event flags) does not come from the handle's pool but from ONE
+ * file-scope static __device__ array of PVF_NOALLOC_SCRATCH_BYTES (about 149 KB) that every GPU which loads the
+ * library holds until the process exits.  Limits: n_events <= PVF_NOALLOC_MAX_EVENTS and n_tracks <=
+ * PVF_NOALLOC_MAX_TRACKS, whatever the handle's max_events / max_tracks; beyond them the call returns
+ * PVF_ERR_CAPACITY, enqueues nothing and leaves the reason in pvf_last_cuda_error(h).
+ *   h              any handle of the current device; only its FC weights (device, uploaded by pvf_create) and its
+ *                  boundary_margin_mm are used.  Always runs the FP32 CUDA-core kernels (k_sort, k_fc_hist), whatever
+ *                  the handle's precision: the result equals the histogram of a PVF_PREC_FP32 / unet_cta_pair = 0 handle bit
+ *                  for bit and that of every other mode within 2e-5 relative to max(|H|, 1).
+ *   tracks         device views, as for pvf_run
+ *   dev_hist       device float [n_events, 40, 8, 100], canonical layout, every element written (empty intervals = 0)
+ *   dev_event_flags  device uint32 [n_events] or NULL: PVF_FLAG_TRACK_DROPPED / NONFINITE / BAD_OFFSETS per event
+ *   cuda_stream    a cudaStream_t, not NULL; two kernels are enqueued on it, no host synchronisation
+ * The first call on a device resolves the array's device address (cudaGetSymbolAddress, once per device, with that
+ * device current -- it may load the module, so make it outside a capture); later calls only launch.  Nothing in the
+ * array has to start at zero (every word a call reads it has written before), so it is never cleared and keeps the last
+ * call's contents.  ALL calls share the array: two calls that overlap on the GPU (different streams, or different handles)
+ * race on it -- keep them on one stream or order them with events.  PVF_ERR_ARG if the current device is not the handle's. */
+#define PVF_NOALLOC_MAX_EVENTS 64
+#define PVF_NOALLOC_MAX_TRACKS 16384
+#define PVF_NOALLOC_SCRATCH_BYTES (2 * 4 * PVF_NOALLOC_MAX_TRACKS + 2 * 4 * 40 * PVF_NOALLOC_MAX_EVENTS + 4 * PVF_NOALLOC_MAX_EVENTS + 768)
+PVF_API pvf_status pvf_histogram_noalloc(pvf_handle h, const pvf_tracks* tracks, int32_t n_events, float* dev_hist,
+                                         uint32_t* dev_event_flags, void* cuda_stream);
+
 /* Mean stage times in ms over the pvf_run calls made since the previous call of this function (at
  * most the 64 most recent): [0] interval sort, [1] FC + segmented sum, [2] UNet, [3] peaks; measured
  * with CUDA events recorded on the run's stream.  Caller must have synchronised that stream.

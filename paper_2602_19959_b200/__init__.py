@@ -6,6 +6,7 @@ libpvf.so with nvcc.  There is no CPU fallback: the binding raises if the librar
 from .binding import (PVFinder, PVFError, load_library, default_config, LIB_PATH, EXPORTS,
                       PVF_OK, PVF_ERR_ARG, PVF_ERR_CONFIG, PVF_ERR_CAPACITY, PVF_ERR_CUDA,
                       PVF_ERR_UNSUPPORTED, PRECISIONS, FLAG_PEAK_OVERFLOW, FLAG_TRACK_DROPPED,
-                      FLAG_NONFINITE, FLAG_BAD_OFFSETS, N_INTERVALS, N_BINS, N_GLOBAL_BINS, MAX_PEAKS)
+                      FLAG_NONFINITE, FLAG_BAD_OFFSETS, N_INTERVALS, N_BINS, N_GLOBAL_BINS, MAX_PEAKS,
+                      NOALLOC_MAX_EVENTS, NOALLOC_MAX_TRACKS)
 
 __all__ = ["PVFinder", "PVFError", "load_library", "default_config", "LIB_PATH", "EXPORTS"]

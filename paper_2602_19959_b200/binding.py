@@ -20,10 +20,11 @@ PVF_PREC_FP32, PVF_PREC_TF32, PVF_PREC_BF16, PVF_PREC_FP16 = 0, 1, 2, 3
 PRECISIONS = {"fp32": PVF_PREC_FP32, "tf32": PVF_PREC_TF32, "bf16": PVF_PREC_BF16, "fp16": PVF_PREC_FP16}
 FLAG_PEAK_OVERFLOW, FLAG_TRACK_DROPPED, FLAG_NONFINITE, FLAG_BAD_OFFSETS = 1, 2, 4, 8
 N_INTERVALS, N_BINS, N_GLOBAL_BINS, MAX_PEAKS = 40, 100, 4000, 32
+NOALLOC_MAX_EVENTS, NOALLOC_MAX_TRACKS = 64, 16384      # pvf_histogram_noalloc (include/pvf.h)
 
 EXPORTS = [
     "pvf_default_config", "pvf_workspace_bytes", "pvf_create", "pvf_create_in_pool", "pvf_run",
-    "pvf_run_host", "pvf_find_peaks", "pvf_run_unet", "pvf_debug_copy_histogram",
+    "pvf_run_host", "pvf_find_peaks", "pvf_run_unet", "pvf_debug_copy_histogram", "pvf_histogram_noalloc",
     "pvf_stage_times_ms", "pvf_launches_per_run", "pvf_destroy", "pvf_status_string",
     "pvf_last_cuda_error", "pvf_build_info",
 ]
@@ -72,6 +73,7 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.pvf_find_peaks.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(pvf_peaks), C.c_void_p]
     lib.pvf_run_unet.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
     lib.pvf_debug_copy_histogram.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
+    lib.pvf_histogram_noalloc.argtypes = [C.c_void_p, C.POINTER(pvf_tracks), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.pvf_stage_times_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float * 4)]
     lib.pvf_launches_per_run.argtypes = [C.c_void_p, C.c_int32]
     lib.pvf_launches_per_run.restype = C.c_int32
@@ -83,7 +85,7 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.pvf_build_info.argtypes = []
     lib.pvf_build_info.restype = C.c_char_p
     for name in ("pvf_create", "pvf_create_in_pool", "pvf_run", "pvf_run_host", "pvf_find_peaks", "pvf_run_unet",
-                 "pvf_debug_copy_histogram", "pvf_stage_times_ms", "pvf_destroy"):
+                 "pvf_debug_copy_histogram", "pvf_histogram_noalloc", "pvf_stage_times_ms", "pvf_destroy"):
         getattr(lib, name).restype = C.c_int
     return lib
 
@@ -218,6 +220,17 @@ class PVFinder:
         st = self.lib.pvf_debug_copy_histogram(self.handle, C.c_void_p(dev_out.data_ptr()), int(n_events),
                                                self._stream(stream))
         self._check(st, "pvf_debug_copy_histogram")
+
+    def histogram_noalloc(self, feat, event_offsets, n_events, dev_hist, dev_flags=None, stream=None):
+        """pvf_histogram_noalloc: H [n_events, 40, 8, 100] of a small batch (<= NOALLOC_MAX_EVENTS events,
+        <= NOALLOC_MAX_TRACKS tracks) with the kernels' scratch in the library's static device array: no allocation."""
+        ts = self._tracks_struct(feat, event_offsets)
+        st = self.lib.pvf_histogram_noalloc(self.handle, C.byref(ts), int(n_events), C.c_void_p(dev_hist.data_ptr()),
+                                            C.c_void_p(dev_flags.data_ptr()) if dev_flags is not None else None,
+                                            self._stream(stream))
+        if st != PVF_OK:
+            raise PVFError(st, "pvf_histogram_noalloc", self.lib.pvf_status_string(st).decode() + " "
+                           + self.lib.pvf_last_cuda_error(self.handle).decode())
 
     def stage_times_ms(self):
         out = (C.c_float * 4)()

@@ -296,6 +296,21 @@ void enqueue_unet(pvf_ctx* h, const float* hist, int n_events, float* out_probs,
 
 }  // namespace
 
+// read-only view of a handle for pvf_noalloc.cu (new code only; nothing above uses these)
+namespace pvf {
+bool handle_view(pvf_handle h, HandleView* v) {
+  if (!h || !v) return false;
+  v->fc_params = h->fc_params;
+  v->device = h->device;
+  v->sm_count = h->sm_count;
+  v->mfrac = h->cfg.boundary_margin_mm * 0.1f;
+  return true;
+}
+void handle_set_error(pvf_handle h, const char* text) {
+  if (h) h->cuda_err = text ? text : "";
+}
+}  // namespace pvf
+
 extern "C" {
 
 void pvf_default_config(pvf_config* c, int32_t max_events, int64_t max_tracks) {

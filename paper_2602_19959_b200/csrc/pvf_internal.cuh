@@ -112,6 +112,11 @@ void launch_copy_hist_masked(const float* hist, const int32_t* seg_cnt, int n_to
 void launch_compact_fill(const int32_t* seg_cnt, int n_total, int32_t* list, int32_t* n_list, const float* p0,
                          float* probs, cudaStream_t s);
 
+// pvf_noalloc.cu (pvf_histogram_noalloc) needs three things of a handle; pvf_ctx itself stays private to pvf_api.cu
+struct HandleView { const float* fc_params; int device; int sm_count; float mfrac; };
+bool handle_view(pvf_handle h, HandleView* v);
+void handle_set_error(pvf_handle h, const char* text);    // what pvf_last_cuda_error returns
+
 // a4: peak finder (k_peaks.cu)
 void launch_peaks(const float* probs, int n_events, float threshold, const uint32_t* flags_in,
                   float* z_mm, float* prob, int32_t* bin, int32_t* count, uint32_t* flags_out,
