@@ -161,7 +161,7 @@ def main_reference(args, rank, world):
     if rank != 0:
         return
     ev = make_events(args.model, args.events, SEEDS[args.model])
-    w = make_weights(args.weights, 1, args.channels)
+    w = bench_weights(args.weights, args.channels)
     n_sample = args.ref_sample
     for _ in range(args.warmup):
         run_oracle_sample(ev, w, n_sample)
@@ -246,6 +246,18 @@ def measure_tf32_peak(torch, seconds=4.0):
         torch.backends.cuda.matmul.allow_tf32 = old
 
 
+def bench_weights(kind, channels):
+    """make_weights, plus the diagnostic kind "zero-conv": `peaky` with every conv weight and bias set to zero, so that
+    every MMA operand of the UNet is zero.  The launch sequence and the executed instructions are identical; what changes is
+    the switching activity of the data paths -- the difference in stage time is the data-dependent share of the power the
+    1 kW cap charges (profiles/r02_experiments.md, section on the power cap).  Never a headline configuration."""
+    w = make_weights("peaky" if kind == "zero-conv" else kind, 1, channels)
+    if kind == "zero-conv":
+        w.conv_w = [np.zeros_like(a) for a in w.conv_w]
+        w.conv_b = [np.zeros_like(a) for a in w.conv_b]
+    return w
+
+
 class Workload:
     """One configuration of the hot path on the device: events + weights + handle + output buffers."""
 
@@ -253,7 +265,7 @@ class Workload:
                  cta_pair=True, margin=0.0, weights="peaky", host_io=False, l2_chunk_events=0, stage_timing=True):
         self.torch = torch
         self.ev = make_events(model, events, seed)
-        self.w = make_weights(weights, 1, channels)
+        self.w = bench_weights(weights, channels)
         self.E, self.precision, self.channels, self.elide = events, precision, channels, elide
         self.split = split_mask if split_mask is not None else (1 if precision == "tf32" else 0)
         extra = {}
@@ -557,7 +569,7 @@ def main():
     ap.add_argument("--split-mask", type=int, default=-1)
     ap.add_argument("--events", type=int, default=16000)
     ap.add_argument("--model", default="run3", choices=["run3", "pileup", "single"])
-    ap.add_argument("--weights", default="peaky", choices=["peaky", "rand"])
+    ap.add_argument("--weights", default="peaky", choices=["peaky", "rand", "zero-conv"])
     ap.add_argument("--channels", type=int, default=64, choices=[64, 32, 16])
     ap.add_argument("--cpu-sample", type=int, default=192)   # ~13 s of oracle time on 16 host threads
     ap.add_argument("--ref-sample", type=int, default=16)
