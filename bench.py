@@ -330,6 +330,10 @@ def run_variants(torch, PVFinder, args, sampler, peaks, peaks_src, tf32_measured
              l2_chunk_events=1024),
         dict(name="config2_fp32", model="run3", events=16000, seed=SEEDS["run3"], precision="fp32"),
         dict(name="config2_fp32_cuda_cores", model="run3", events=4000, seed=SEEDS["run3"], precision="fp32", cta_pair=False),
+        # diagnostic, never a headline: the same launches with all-zero UNet operands do not reach the 1 kW cap -- the
+        # stage time at the maximum clock, i.e. what the power cap costs (profiles/r02_experiments.md section 8)
+        dict(name="config2_tf32_zero_operands_power_cap_diagnostic", model="run3", events=16000, seed=SEEDS["run3"],
+             precision="tf32", weights="zero-conv"),
     ]
     for sp in specs:
         name = sp.pop("name")
@@ -353,6 +357,9 @@ def run_variants(torch, PVFinder, args, sampler, peaks, peaks_src, tf32_measured
                 if prec == "fp32":
                     note += ("; FP32-accurate mode: nominal FLOPs against the TF32 peak -- every product costs one kind::tf32 "
                              "and one kind::f16 MMA (2/3 and 1/3 of the executed tensor time), so 0.67 is this mode's ceiling")
+            if sp.get("weights") == "zero-conv":
+                pk_, note = 1100.0, ("nominal dense TF32 peak at 1.965 GHz (this run is not power-capped: compare the "
+                                                  "clocks entry with the headline's)")
             rec["unet_tflops"] = flop / (stage[2] * 1e-3) / 1e12
             rec["unet_frac"] = rec["unet_tflops"] / pk_
             rec["unet_peak"] = pk_

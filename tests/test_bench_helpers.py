@@ -46,3 +46,15 @@ def test_unet_mac_count_from_the_topology():
     def macs(C):
         return 100 * C * 8 * 25 + 50 * C * C * 15 + 25 * C * C * 5 + 50 * C * 2 * C * 15 + 100 * C * 2 * C * 25 + 100 * C
     assert macs(64) == 31_494_400 and macs(32) == 8_195_200 and macs(16) == 2_209_600
+
+
+def test_zero_conv_weights_are_a_diagnostic_of_peaky():
+    """bench.py --weights zero-conv: `peaky` FC weights, all conv weights and biases zero (power-cap diagnostic)."""
+    import numpy as np
+    import bench
+    from pvf_inputs import make_weights
+    w, ref = bench.bench_weights("zero-conv", 32), make_weights("peaky", 1, 32)
+    assert all(np.array_equal(a, b) for a, b in zip(w.fc_w, ref.fc_w)) and all(np.array_equal(a, b) for a, b in zip(w.fc_b, ref.fc_b))
+    assert all(a.shape == b.shape and not a.any() for a, b in zip(w.conv_w, ref.conv_w))
+    assert all(a.shape == b.shape and not a.any() for a, b in zip(w.conv_b, ref.conv_b))
+    assert bench.bench_weights("rand", 16).kind == "rand"
