@@ -15,6 +15,7 @@
 // by the sorted positions, with no cross-lane reduction; only intervals that hold a track are written (k_unet_tc
 // takes seg_cnt == 0 as zeros).  Tracks of the same interval share one logarithm per group (16-track chunk or group
 // of four; see softplus_front2): sum softplus(v) = sum max(v, 0) + ln 2 lg2(prod (1 + e^-|v|)).
+// The packed W5x is pre-scaled by log2(e): D holds t = v log2(e), the sums run in units of log2 and ln 2 is applied per stored sum.
 // FP32 accuracy: W5x = W_hi + W_lo and hx = h_hi + h_lo (each part RN-rounded to TF32), three MMAs
 // W_hi h_hi + W_hi h_lo + W_lo h_hi accumulate in FP32 in TMEM (the dropped term is ~2^-22 relative).
 // CTA pairs: the two CTAs of a cluster serve the two halves of the 800 outputs (400 each, packed densely into
@@ -100,39 +101,6 @@ __device__ __forceinline__ uint32_t tf32_of(float v) {
 __device__ __forceinline__ void st16(uint32_t addr, uint4 v) {
   asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
-// softplus(v) = max(v,0) + log(1 + exp(-|v|)) on the SFU (see k_fc.cu)
-// Raw ex2 / lg2 (no range fix-ups needed: the ex2 argument is <= 0, the lg2 argument is in (1, 2]).
-__device__ __forceinline__ float softplus_ft(float v) {
-  const float t = fabsf(v) * -1.4426950408889634f;
-  float e, w;
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(t));
-  const float u = 1.0f + e;
-  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(w) : "f"(u));
-  return fmaf(w, 0.6931471805599453f, fmaxf(v, 0.0f));
-}
-
-// Two softplus at once with the packed FP32 instructions of sm_100 (mul / add / fma .f32x2 = one issue slot for
-// two lanes' worth of work): the epilogue is issue-bound, so this removes a quarter of its softplus slots.
-__device__ __forceinline__ void softplus2_ft(float v0, float v1, float& o0, float& o1) {
-  float t0, t1, u0, u1, e0, e1, w0, w1;
-  asm("{\n\t.reg .b64 p, q, k;\n\tmov.b64 p, {%2, %3};\n\tmov.b64 k, {%4, %4};\n\t"
-      "mul.rn.f32x2 q, p, k;\n\tmov.b64 {%0, %1}, q;\n\t}"
-      : "=f"(t0), "=f"(t1) : "f"(v0), "f"(v1), "f"(1.4426950408889634f));
-  t0 = -fabsf(t0);
-  t1 = -fabsf(t1);
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e0) : "f"(t0));
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e1) : "f"(t1));
-  asm("{\n\t.reg .b64 p, q, k;\n\tmov.b64 p, {%2, %3};\n\tmov.b64 k, {%4, %4};\n\t"
-      "add.rn.f32x2 q, p, k;\n\tmov.b64 {%0, %1}, q;\n\t}"
-      : "=f"(u0), "=f"(u1) : "f"(e0), "f"(e1), "f"(1.0f));
-  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(w0) : "f"(u0));
-  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(w1) : "f"(u1));
-  const float m0 = fmaxf(v0, 0.0f), m1 = fmaxf(v1, 0.0f);
-  asm("{\n\t.reg .b64 p, q, k, m;\n\tmov.b64 p, {%2, %3};\n\tmov.b64 k, {%4, %4};\n\tmov.b64 m, {%5, %6};\n\t"
-      "fma.rn.f32x2 q, p, k, m;\n\tmov.b64 {%0, %1}, q;\n\t}"
-      : "=f"(o0), "=f"(o1) : "f"(w0), "f"(w1), "f"(0.6931471805599453f), "f"(m0), "f"(m1));
-}
-
 // Packed FP32 pairs (mul / add .f32x2 of sm_100: one issue slot for two values).
 __device__ __forceinline__ void mul2(float a0, float a1, float b0, float b1, float& o0, float& o1) {
   asm("{\n\t.reg .b64 p, q, r;\n\tmov.b64 p, {%2, %3};\n\tmov.b64 q, {%4, %5};\n\t"
@@ -153,33 +121,36 @@ __device__ __forceinline__ float lg2_ft(float u) {
 // m = max(v, 0).  Tracks that are summed into the same interval share ONE logarithm:
 //     sum_i softplus(v_i) = sum_i m_i + ln2 * lg2(prod_i u_i)        (16 factors in (1, 2]: prod <= 65536, no overflow)
 // which halves the SFU operations of the stage (one ex2 per value, one lg2 per group instead of per value).
-__device__ __forceinline__ void softplus_front2(float v0, float v1, float& u0, float& u1, float& m0, float& m1) {
-  float t0, t1, e0, e1;
-  mul2(v0, v1, 1.4426950408889634f, 1.4426950408889634f, t0, t1);
-  t0 = -fabsf(t0);
-  t1 = -fabsf(t1);
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e0) : "f"(t0));
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e1) : "f"(t1));
-  add2(e0, e1, 1.0f, 1.0f, u0, u1);
-  m0 = fmaxf(v0, 0.0f);
-  m1 = fmaxf(v1, 0.0f);
+// The packed W5x image is scaled by log2(e) (fc_tc_pack), so the accumulators hold t = v log2(e) and the whole sum runs in
+// units of log2: softplus(v) / ln 2 = max(t, 0) + lg2(1 + 2^-|t|); the factor ln 2 is applied once per stored sum
+// (kLn2 below) instead of one multiply per value in front of the ex2.
+// Front half for two values: e = 2^-|t| in (0, 1] and m = max(t, 0); the factor 1 + e is formed where it is used (prod2).
+__device__ __forceinline__ void softplus_front2(float t0, float t1, float& e0, float& e1, float& m0, float& m1) {
+  const float n0 = -fabsf(t0), n1 = -fabsf(t1);          // operand modifiers of the MUFU, no instructions of their own
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e0) : "f"(n0));
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e1) : "f"(n1));
+  m0 = fmaxf(t0, 0.0f);
+  m1 = fmaxf(t1, 0.0f);
 }
+// Running product of factors (1 + e) as one packed pair: start = (1 + e0, 1 + e1), then P <- P + e P = P (1 + e) per further
+// pair of factors -- one fma.rn.f32x2 for two factors (forming 1 + e and multiplying separately took two).
+__device__ __forceinline__ unsigned long long prod2_start(float e0, float e1) {
+  unsigned long long r;
+  asm("{\n\t.reg .b64 p, k;\n\tmov.b64 p, {%1, %2};\n\tmov.b64 k, {%3, %3};\n\tadd.rn.f32x2 %0, p, k;\n\t}"
+      : "=l"(r) : "f"(e0), "f"(e1), "f"(1.0f));
+  return r;
+}
+__device__ __forceinline__ void prod2_step(unsigned long long& P, float e0, float e1) {
+  asm("{\n\t.reg .b64 q;\n\tmov.b64 q, {%1, %2};\n\tfma.rn.f32x2 %0, q, %0, %0;\n\t}" : "+l"(P) : "f"(e0), "f"(e1));
+}
+__device__ __forceinline__ float prod2_finish(unsigned long long P) {
+  float a, b;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(P));
+  return a * b;
+}
+constexpr float kLn2 = 0.6931471805599453f;
 
 struct Feat9 { const float* f[9]; };
-
-// One step of the ordered segmented sum: a track of interval iv (given as the offset iv * 800) with value x joins
-// the running sum a of interval c.  When the interval changes, the finished sum goes to base[c] and the sum
-// restarts (0 + x == x exactly).  The compiler turns the rare branch into predicated instructions -- compare,
-// address, store, reset, add -- which beats a taken branch per track (measured: 5.4 -> 4.3 ms).
-__device__ __forceinline__ void seg_step(float& a, int& c, int iv, float x, float* __restrict__ base) {
-  if (__builtin_expect(iv != c, 0)) {
-    base[c] = a;
-    a = 0.0f;
-    c = iv;
-  }
-  a += x;
-}
-
 
 #ifdef PVF_FC_PROF
 // Diagnostic build only (-DPVF_FC_PROF): cycles per role and CTA (lane 0 of one warp per role):
@@ -288,7 +259,7 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
       int ev_lo;
       const int nk = kept_of(e, ev_lo);
       // output o = c * 100 + l lives at H[e][interval][o]: the dense row index is the offset itself.  Rows that
-      // hold no output send their (meaningless) sums to the dump slot, so seg_step's store predicate stays
+      // hold no output send their (meaningless) sums to the dump slot, so the boundary stores' predicate stays
       // warp-uniform.
       float* Hc = valid ? hist + (size_t)e * kIntervals * kFcOut + kHalfOut * half + ol : dump + r;   // + iv * 800 (= s_iv)
       float a = 0.f;                             // running sum of the current interval
@@ -323,52 +294,65 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
           tmem_ld_wait();
           // front half of all 16 softplus first: independent, so the SFU pipeline stays full; columns past the
           // tile's last track are computed on stale accumulators and then neutralised (u = 1, m = 0)
-          float u[16], m[16];
+          float ev[16], m[16];
 #pragma unroll
           for (int k = 0; k < 8; ++k)
-            softplus_front2(__uint_as_float(ve[k]), __uint_as_float(vo[k]), u[2 * k], u[2 * k + 1], m[2 * k], m[2 * k + 1]);
+            softplus_front2(__uint_as_float(ve[k]), __uint_as_float(vo[k]), ev[2 * k], ev[2 * k + 1], m[2 * k], m[2 * k + 1]);
           if (TAIL) {
 #pragma unroll
             for (int i = 0; i < 16; ++i)
-              if (i >= nv) { u[i] = 1.0f; m[i] = 0.0f; }
+              if (i >= nv) { ev[i] = 0.0f; m[i] = 0.0f; }     // factor 1, term 0
           }
 #ifdef PVF_FC_NOREDUCE
           // diagnostic build: the FC arithmetic alone (all 16 logarithms, no ordered segmented sum, no histogram stores
           // but the event's last one) -- gives the "FC" share of the fused stage (BASELINE.json config 2)
 #pragma unroll
-          for (int i = 0; i < 16; ++i) a += fmaf(lg2_ft(u[i]), 0.6931471805599453f, m[i]);
+          for (int i = 0; i < 16; ++i) a += lg2_ft(1.0f + ev[i]) + m[i];
 #else
           // Ordered accumulation (fixed by the sorted positions, hence reproducible).  Only intervals that hold a track
           // are written -- the UNet kernel never reads the histogram of an empty interval (seg_cnt == 0 means zeros).
           if (mask == 0u) {                      // the whole chunk continues the running interval: one logarithm
-            float p[8], t[8];
+            unsigned long long P = prod2_start(ev[0], ev[1]);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-              mul2(u[4 * k], u[4 * k + 1], u[4 * k + 2], u[4 * k + 3], p[2 * k], p[2 * k + 1]);
-              add2(m[4 * k], m[4 * k + 1], m[4 * k + 2], m[4 * k + 3], t[2 * k], t[2 * k + 1]);
-            }
-            mul2(p[0], p[1], p[2], p[3], p[0], p[1]);
-            mul2(p[4], p[5], p[6], p[7], p[4], p[5]);
+            for (int k = 1; k < 8; ++k) prod2_step(P, ev[2 * k], ev[2 * k + 1]);
+            float t[8];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) add2(m[4 * k], m[4 * k + 1], m[4 * k + 2], m[4 * k + 3], t[2 * k], t[2 * k + 1]);
             add2(t[0], t[1], t[2], t[3], t[0], t[1]);
             add2(t[4], t[5], t[6], t[7], t[4], t[5]);
-            mul2(p[0], p[1], p[4], p[5], p[0], p[1]);
             add2(t[0], t[1], t[4], t[5], t[0], t[1]);
-            a += fmaf(lg2_ft(p[0] * p[1]), 0.6931471805599453f, t[0] + t[1]);
+            a += lg2_ft(prod2_finish(P)) + (t[0] + t[1]);
           } else {
 #pragma unroll
-            for (int g = 0; g < 4; ++g) {        // groups of four tracks; the test is warp-uniform
-              if (((mask >> (4 * g)) & 15u) == 0u) {
-                float p0, p1, t0, t1;
-                mul2(u[4 * g], u[4 * g + 1], u[4 * g + 2], u[4 * g + 3], p0, p1);
+            for (int g = 0; g < 4; ++g) {        // groups of four tracks; the tests are warp-uniform
+              const unsigned gb = (mask >> (4 * g)) & 15u;
+              if (gb == 0u) {
+                unsigned long long P = prod2_start(ev[4 * g], ev[4 * g + 1]);
+                prod2_step(P, ev[4 * g + 2], ev[4 * g + 3]);
+                float t0, t1;
                 add2(m[4 * g], m[4 * g + 1], m[4 * g + 2], m[4 * g + 3], t0, t1);
-                a += fmaf(lg2_ft(p0 * p1), 0.6931471805599453f, t0 + t1);
-              } else {                           // an interval starts here: track by track (seg_step)
+                a += lg2_ft(prod2_finish(P)) + (t0 + t1);
+              } else {                           // an interval starts here: track by track
                 const int4 q4 = *reinterpret_cast<const int4*>(ivs + c0 + 4 * g);
                 const int iq[4] = {q4.x, q4.y, q4.z, q4.w};
+                float u0, u1, u2, u3;
+                add2(ev[4 * g], ev[4 * g + 1], 1.0f, 1.0f, u0, u1);
+                add2(ev[4 * g + 2], ev[4 * g + 3], 1.0f, 1.0f, u2, u3);
+                const float uu[4] = {u0, u1, u2, u3};
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
-                  const int i = 4 * g + k;
-                  seg_step(a, c, i < nv ? iq[k] : c, fmaf(lg2_ft(u[i]), 0.6931471805599453f, m[i]), Hc);
+                  const float x = lg2_ft(uu[k]) + m[4 * g + k];
+                  // Bit k of gb: an interval starts at this track (never set past the tile's last track): the finished sum
+                  // goes to H and the sum restarts (0 + x == x exactly).  The compiler predicates the store sequence on the
+                  // mask bits (one R2P for the group) -- cheaper than comparing interval ids per track, and cheaper than real
+                  // branches (measured: four straight-line cases behind warp-uniform branches, each segment sharing one
+                  // logarithm, were 5 % slower: the epilogue is bound by latency, not by issue slots).
+                  if (gb & (1u << k)) {
+                    Hc[c] = a * kLn2;              // sums run in units of log2 (softplus_front2)
+                    a = 0.0f;
+                    c = iq[k];
+                  }
+                  a += x;
                 }
               }
             }
@@ -378,7 +362,7 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
         int c0 = 0;
         for (; c0 + 16 <= ntile; c0 += 16) chunk(c0, std::false_type{});
         if (c0 < ntile) chunk(c0, std::true_type{});
-        if (last) Hc[c] = a;                      // the event's last non-empty interval
+        if (last) Hc[c] = a * kLn2;               // the event's last non-empty interval
         tc_fence_before_sync();
         if (rank == 0) mbar_arrive(bar(bAccEmpty + mt));
         else mbar_arrive_cluster(lead_pacc + 8u * mt);
@@ -474,7 +458,7 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
         if (has_other) s_iv[ib * kTile + p_other] = iv_other * kFcOut;
         if (has_own) {
           s_iv[ib * kTile + p_own] = iv_own * kFcOut;   // the epilogue wants the interval as its offset in H
-          float h[32], gg[28];
+          float h[32];
 #pragma unroll
           for (int o = 0; o < kFcHidden; ++o) {
             float a = S.b0[o];
@@ -572,7 +556,8 @@ void fc_tc_pack(const float* w5, const float* b5, void* host_dst) {
     for (int row = 0; row < kHalfOut; ++row) {
       const int o = kHalfOut * half + row;
       for (int k = 0; k <= kFcHidden; ++k) {
-        const float v = k < kFcHidden ? w5[o * kFcHidden + k] : b5[o];
+        // scaled by log2(e) in double, rounded once: the kernel's sums run in units of log2 (softplus_front2)
+        const float v = (float)((double)(k < kFcHidden ? w5[o * kFcHidden + k] : b5[o]) * 1.4426950408889634);
         const float hi = tf32_rna_h(v), lo = tf32_rna_h(v - hi);
         const size_t idx = ((size_t)(k / 4) * kRowsW + (row < 384 ? row : kSmallRow0 + row - 384)) * 4 + (k % 4);
         dst[(size_t)half * 2 * (kWPart / 4) + idx] = hi;
