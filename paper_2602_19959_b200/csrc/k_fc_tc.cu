@@ -101,12 +101,7 @@ __device__ __forceinline__ uint32_t tf32_of(float v) {
 __device__ __forceinline__ void st16(uint32_t addr, uint4 v) {
   asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
-// Packed FP32 pairs (mul / add .f32x2 of sm_100: one issue slot for two values).
-__device__ __forceinline__ void mul2(float a0, float a1, float b0, float b1, float& o0, float& o1) {
-  asm("{\n\t.reg .b64 p, q, r;\n\tmov.b64 p, {%2, %3};\n\tmov.b64 q, {%4, %5};\n\t"
-      "mul.rn.f32x2 r, p, q;\n\tmov.b64 {%0, %1}, r;\n\t}"
-      : "=f"(o0), "=f"(o1) : "f"(a0), "f"(a1), "f"(b0), "f"(b1));
-}
+// Packed FP32 pairs (add / fma .f32x2 of sm_100: one issue slot for two values).
 __device__ __forceinline__ void add2(float a0, float a1, float b0, float b1, float& o0, float& o1) {
   asm("{\n\t.reg .b64 p, q, r;\n\tmov.b64 p, {%2, %3};\n\tmov.b64 q, {%4, %5};\n\t"
       "add.rn.f32x2 r, p, q;\n\tmov.b64 {%0, %1}, r;\n\t}"
@@ -253,7 +248,7 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
     const bool valid = warp == kSmallEpiWarp ? lane < 16 : true;
     const uint32_t lead_pacc = mapa_rank(bar(bPAccEmpty), 0);
     int it = 0;
-    const bool pw = tid == 0;
+    [[maybe_unused]] const bool pw = tid == 0;
     FC_PROF_T0();
     for (int e = (int)blockIdx.x >> 1; e < n_events; e += (int)gridDim.x >> 1) {
       int ev_lo;
@@ -377,7 +372,7 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
     constexpr uint32_t hi = (128u >> 4) | (1u << 14);
     constexpr uint32_t a_lbo = (uint32_t)(kLboW >> 4) << 16, b_lbo = (uint32_t)(kLboH >> 4) << 16;
     int it = 0;
-    const bool pw = lane == 0;
+    [[maybe_unused]] const bool pw = lane == 0;
     FC_PROF_T0();
     for (int e = (int)blockIdx.x >> 1; e < n_events; e += (int)gridDim.x >> 1) {
       int ev_lo;
@@ -428,7 +423,7 @@ k_fc_hist_tc(Feat9 F, const int32_t* __restrict__ event_offsets, const int32_t* 
     const uint32_t lead_phfull = mapa_rank(bar(bPHFull + g), 0);
     const int p_own = 2 * i + rank, p_other = 2 * i + 1 - rank;
     int it = 0;
-    const bool pw = g == 0 && i == 0;
+    [[maybe_unused]] const bool pw = g == 0 && i == 0;
     FC_PROF_T0();
     for (int e = (int)blockIdx.x >> 1; e < n_events; e += (int)gridDim.x >> 1) {
       int ev_lo;
