@@ -321,6 +321,8 @@ def run_variants(torch, PVFinder, args, sampler, peaks, peaks_src, tf32_measured
     specs = [
         dict(name="config2_bf16", model="run3", events=16000, seed=SEEDS["run3"], precision="bf16"),
         dict(name="config2_fp16", model="run3", events=16000, seed=SEEDS["run3"], precision="fp16"),
+        # FP16 operands with the e1 layer split into two FP16 pieces: meets north_star's TF32 tolerance (1e-3), tests fp16s
+        dict(name="config2_fp16_e1split", model="run3", events=16000, seed=SEEDS["run3"], precision="fp16", split_mask=1),
         dict(name="config3_tf32", model="pileup", events=16000, seed=SEEDS["pileup"], precision="tf32"),
         dict(name="config4_bf16_c32", model="run3", events=16000, seed=1004, precision="bf16", channels=32),
         dict(name="config4_bf16_c16", model="run3", events=16000, seed=1004, precision="bf16", channels=16),
@@ -345,7 +347,7 @@ def run_variants(torch, PVFinder, args, sampler, peaks, peaks_src, tf32_measured
             rec = {"name": name, "events": E, "tracks": wl.ev.n_tracks, "precision": prec, "channels": ch,
                    "events_per_s": E * 5 / (ms * 1e-3), "ms_per_step": ms / 5, "us_per_event": ms * 1e3 / (5 * E),
                    "stage_ms": {"sort": stage[0], "fc_hist": stage[1], "unet": stage[2], "peaks": stage[3]},
-                   "steps": 5, "warmup": 3, "clocks": sampler.window(*win)}
+                   "split_mask": wl.split, "steps": 5, "warmup": 3, "clocks": sampler.window(*win)}
             if wl.elide:
                 ne = nonempty_intervals(wl.ev) / (E * 40.0)
                 rec["nonempty_interval_fraction"] = ne

@@ -79,9 +79,10 @@ typedef struct {
   int32_t peak_halfwidth;  /* (fixed) 3 */
   int32_t max_peaks;       /* (fixed) 32 */
   int32_t precision;       /* pvf_precision */
-  int32_t split_mask;      /* PVF_PREC_TF32 only: 0, or 1 = the e1 layer (raw histogram input, the dominant TF32 error) runs as
-                              two passes on BF16 pieces.  Anything else is PVF_ERR_CONFIG: FP32
-                              accuracy on every layer is PVF_PREC_FP32, not a mask value */
+  int32_t split_mask;      /* PVF_PREC_TF32 and PVF_PREC_FP16 only (the two formats with a 10-bit mantissa): 0, or 1 = the e1
+                              layer (raw histogram input, the dominant error of these formats) runs as two passes on 16-bit
+                              pieces (BF16 pieces in the TF32 kernel, FP16 pieces in the FP16 kernel).
+                              Anything else is PVF_ERR_CONFIG: FP32 accuracy on every layer is PVF_PREC_FP32, not a mask value */
   int32_t max_events;      /* capacity the pool is sized for (>= 1) */
   int64_t max_tracks;      /* capacity the pool is sized for (>= 1) */
   int32_t enable_stage_timing; /* pre-creates CUDA events around the four stages; default 0 */

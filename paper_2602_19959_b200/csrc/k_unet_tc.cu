@@ -202,7 +202,9 @@ __host__ __device__ inline Plan make_plan(int split_e1) {
   // 16-bit modes: the 8 input channels fill half of an MMA's K = 16, so one e1 step takes TWO tap pairs (7 steps)
   // TF32 with the e1 split: 13 steps [a1 | a2] x [w1 | w1] + 7 steps [a1(pair 2w) | a1(pair 2w+1)] x [w2 | w2]
   // FX: 13 tap pairs x (main, correction)
-  P.e1_steps = G::B16 ? 7 : (G::FX ? 26 : (split_e1 ? 20 : 13));
+  // FP16 with the e1 split: the same 13 + 7 steps on FP16 pieces (the BF16 kernel has no split: its tolerance is set by the
+  // 8-bit mantissa of every other layer)
+  P.e1_steps = G::FX ? 26 : ((split_e1 && BF16 != 1) ? 20 : (G::B16 ? 7 : 13));
   P.seg_steps[gE2] = 8 * G::NKB1 * G::PH;
   P.seg_steps[gD1Ea] = G::D1E_A;
   P.seg_steps[gB] = 3 * G::NKB1 * G::PH;
@@ -533,7 +535,7 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
       st_smem16(x0 + 2 * G::LBO1 + row, ql);
       st_smem16(x0 + 3 * G::LBO1 + row, qh);
     }
-  } else if (G::B16) {
+  } else if (G::B16 && !(split && BF16 == 2)) {
     for (int it = tid; it < G::T * 128; it += G::EPI_THREADS) {
       const int t = it >> 7, l = it & 127;
       bool live = l < 100 && t < n_valid_int;
@@ -550,7 +552,7 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
       st_smem16(x0 + G::LBO1 + row, zero4);       // channels 8..15 of the K = 16 MMA: zero
     }
   } else if (split) {
-    // TF32 mode with the e1 split: the histogram enters as TWO BF16 pieces per value, x = a1 + a2 (+ 2^-17 |x|),
+    // TF32 (and FP16) mode with the e1 split: the histogram enters as TWO 16-bit pieces per value, x = a1 + a2 (+ 2^-17 |x|; FP16 pieces: 2^-22),
     // side by side in the K = 16 of one kind::f16 MMA: chunk 0 = a1 of the 8 channels, chunk 1 = a2.  With the
     // weights as [w1 | w1] (pass 0) and [w2 | 0] (pass 1) two MMAs per tap pair give a1 w1 + a2 w1 + a1 w2, i.e.
     // ~2^-16 relative per product (plain TF32: 2^-12) for 2/3 of the MMAs a three-pass TF32 split needs.
@@ -559,15 +561,17 @@ __device__ __forceinline__ void load_x0(uint32_t smem_base, const float* __restr
       bool live = l < 100 && t < n_valid_int;
       const long long src = !live ? 0 : (list ? (long long)list[g0 + t] : g0 + t);
       if (live && seg_cnt != nullptr) live = __ldg(seg_cnt + src) > 0;
+      // pieces in the format of the MMA that reads them: BF16 in the TF32 kernel, FP16 in the FP16 kernel
+      constexpr int PF = BF16 == 2 ? 2 : 1;
       float x[8], r[8];
 #pragma unroll
       for (int c = 0; c < 8; ++c) {
         x[c] = live ? __ldg(hist + src * kFcOut + c * kBins + l) : 0.0f;
-        r[c] = x[c] - __bfloat162float(__float2bfloat16_rn(x[c]));
+        r[c] = x[c] - (PF == 2 ? __half2float(__float2half_rn(x[c])) : __bfloat162float(__float2bfloat16_rn(x[c])));
       }
       uint4 q1, q2;
-      q1.x = pack16<1>(x[0], x[1]); q1.y = pack16<1>(x[2], x[3]); q1.z = pack16<1>(x[4], x[5]); q1.w = pack16<1>(x[6], x[7]);
-      q2.x = pack16<1>(r[0], r[1]); q2.y = pack16<1>(r[2], r[3]); q2.z = pack16<1>(r[4], r[5]); q2.w = pack16<1>(r[6], r[7]);
+      q1.x = pack16<PF>(x[0], x[1]); q1.y = pack16<PF>(x[2], x[3]); q1.z = pack16<PF>(x[4], x[5]); q1.w = pack16<PF>(x[6], x[7]);
+      q2.x = pack16<PF>(r[0], r[1]); q2.y = pack16<PF>(r[2], r[3]); q2.z = pack16<PF>(r[4], r[5]); q2.w = pack16<PF>(r[6], r[7]);
       const uint32_t row = (uint32_t)(G::LEAD1 + it) * 16u;
       st_smem16(x0 + row, q1);
       st_smem16(x0 + G::LBO1 + row, q2);
@@ -679,6 +683,7 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
   // (LBO = 32 bytes), i.e. the input of the next tap pair -- one MMA does tap pairs 2w and 2w + 1
   constexpr uint32_t a_lbo = (S == sE1 && B16) ? (2u << 16) : ((uint32_t)(Y::LBO >> 4) << 16);
   constexpr uint32_t a_lbo_x2 = (2u << 16) - a_lbo;     // added for the second pass of the split e1 (TF32 kernel)
+  constexpr uint32_t a_lbo_x2_16 = (2u << 16) - ((uint32_t)(Y::LBO >> 4) << 16);   // subtracted for the FIRST pass in a 16-bit kernel
   constexpr uint32_t c_lbo = (uint32_t)(Y::C_LBO >> 4) << 16;          // FX correction operand: LO chunk -> HB chunk
   constexpr uint32_t b_lbo = (uint32_t)((G::NB * 16) >> 4) << 16;
   const uint32_t dcol = tmem_base + (uint32_t)Y::DCOL;
@@ -723,11 +728,16 @@ __device__ __forceinline__ void mma_seg(uint32_t sb, uint32_t tmem_base, uint32_
           uint32_t a;
           bool half_n;
           if (S == sE1) {
-            const int step = lf + li, pass = step / 13, u = B16 ? 2 * step : (pass ? 2 * (step - 13) : step);
+            // three shapes of e1: 16-bit unsplit (7 steps, K chunks = tap pairs 2 step, 2 step + 1 of the same array: LBO = 2
+            // rows), TF32 / FX (13 steps per pass), split (TF32 or FP16 kernel: 13 steps [a1 | a2] with the level-1 LBO, then
+            // 7 steps [a1 of pair u | a1 of pair u + 1] with LBO = 2 rows)
+            const bool split16 = B16 && e1x;
+            const int step = lf + li, pass = step / 13, u = (B16 && !e1x) ? 2 * step : (pass ? 2 * (step - 13) : step);
             a = a0 + (uint32_t)(Y::SRC0 >> 4) + (uint32_t)(Y::LEAD + 2 * u - Y::PAD);
             if (BF16 == 0 && pass) a += a_lbo_x2;              // [a1 of pair u | a1 of pair u + 1]
+            if (split16 && !pass) a -= a_lbo_x2_16;            // 16-bit kernel: a_lbo is the 2-row one; pass 0 wants [a1 | a2]
             if (corr) a = c0 + (uint32_t)((Y::SRC0 + Y::SRC_NCH * Y::LBO) >> 4) + (uint32_t)(Y::LEAD + 2 * u - Y::PAD);
-            half_n = B16 ? step == 6 : (step == 12 || step == 19);
+            half_n = (B16 && !e1x) ? step == 6 : (step == 12 || step == 19);
           } else if (Y::HALF >= SPL) {
             a = corr ? c0 + (uint32_t)(li * (Y::LBO >> 4)) : a0 + (uint32_t)(li * ((2 * Y::LBO) >> 4));
             half_n = lf + li >= LAST0;
@@ -1028,6 +1038,23 @@ uint16_t fp16_rne(float v) {                 // float -> IEEE binary16, round to
   return (uint16_t)(sign | ((r - 0x38000000u) >> 13));
 }
 
+float fp16_to_float(uint16_t h) {            // IEEE binary16 -> float (exact)
+  const uint32_t sign = (uint32_t)(h & 0x8000u) << 16, ex = (h >> 10) & 0x1fu, man = h & 0x3ffu;
+  uint32_t u;
+  if (ex == 0) {
+    if (man == 0) u = sign;
+    else {                                   // subnormal: value = man * 2^-24
+      float f = (float)man * 5.9604644775390625e-8f;
+      memcpy(&u, &f, 4);
+      u |= sign;
+    }
+  } else if (ex == 31) u = sign | 0x7f800000u | (man << 13);
+  else u = sign | ((ex + 112u) << 23) | (man << 13);
+  float r;
+  memcpy(&r, &u, 4);
+  return r;
+}
+
 // Packs PyTorch-layout conv weights [C_out][C_in][K] into the image the kernel streams: a 2 KB header
 // (biases [5][C], head weight [C], head bias) and, per segment in streaming order, per MMA step, the
 // B operand [2 chunks][2C rows: C outputs of tap 2u, then of tap 2u+1][16 B of input channels],
@@ -1058,7 +1085,7 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst_all) {
       const int fp = d.f0 + s;                    // physical step index inside the sub-layer
       const int f = fp / G::PH, part = fp % G::PH;   // logical step; FX: part 0 = main (TF32), part 1 = correction (BF16)
       int u, kk, pass = 0;                        // tap pair, K block
-      if (d.seg == gE1 && B16) { u = 2 * f; kk = 0; }             // 16-bit e1: K chunk h of step f holds tap pair 2f + h
+      if (d.seg == gE1 && B16 && !(split_e1 && BF16 == 2)) { u = 2 * f; kk = 0; }   // 16-bit e1: K chunk h of step f holds tap pair 2f + h
       else if (d.seg == gE1) { pass = f / 13; u = f % 13; kk = 0; }   // e1 split runs [pass][tap pair]
       else { u = f / d.nkb; kk = f % d.nkb; }
       unsigned char* step = dst + P.seg_off[d.seg] + (size_t)s * G::STEP_BYTES;
@@ -1093,7 +1120,7 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst_all) {
             }
         continue;
       }
-      if (d.seg == gE1 && BF16 == 0 && split_e1) {
+      if (d.seg == gE1 && (BF16 == 0 || BF16 == 2) && split_e1) {
         // split e1 of the TF32 kernel: BF16 pieces w = w1 + w2; pass 0 (13 steps) holds [w1 | w1] (meets [a1 | a2]),
         // pass 1 (7 steps) [w2 of pair 2w | w2 of pair 2w + 1] (meets [a1 two rows apart])
         if (pass) u = 2 * (f - 13);
@@ -1105,11 +1132,17 @@ void pack_impl(const pvf_weights* w, int split_e1, unsigned char* dst_all) {
               const int n = rank * nbx + nl;
               const int co = n % C, j = 2 * (u + (pass ? h : 0)) + n / C;
               const float v = j < d.taps ? W[((size_t)co * d.cin + e) * d.taps + j] : 0.0f;
-              const uint16_t w1 = bf16_rne(v);
-              uint32_t w1bits = (uint32_t)w1 << 16;
-              float w1f;
-              memcpy(&w1f, &w1bits, 4);
-              const uint16_t w2 = bf16_rne(v - w1f);
+              uint16_t w1, w2;                  // pieces in the format of the MMA: BF16 (TF32 kernel) or FP16 (FP16 kernel)
+              if (BF16 == 2) {
+                w1 = fp16_rne(v);
+                w2 = fp16_rne(v - fp16_to_float(w1));
+              } else {
+                w1 = bf16_rne(v);
+                uint32_t w1bits = (uint32_t)w1 << 16;
+                float w1f;
+                memcpy(&w1f, &w1bits, 4);
+                w2 = bf16_rne(v - w1f);
+              }
               const uint16_t out = pass == 0 ? w1 : w2;
               memcpy(step + ((size_t)h * nbx + nl) * 16 + e * 2, &out, 2);
             }
@@ -1214,7 +1247,7 @@ void unet_tc_pack(const pvf_weights* w, int channels, int precision, int split_m
 cudaError_t unet_tc_setup(int channels, int precision, int split_mask, int cta_pair) {
   if (channels != 64 && channels != 32 && channels != 16) return cudaErrorInvalidValue;
   if (split_mask & ~1) return cudaErrorInvalidValue;          // only the e1 split is built
-  if (precision != PVF_PREC_TF32 && split_mask) return cudaErrorInvalidValue;   // the split is a TF32 remedy
+  if (precision != PVF_PREC_TF32 && precision != PVF_PREC_FP16 && split_mask) return cudaErrorInvalidValue;   // the split serves the 10-bit formats
   if (precision == PVF_PREC_FP32 && !cta_pair) return cudaErrorInvalidValue;    // FP32 on the tensor cores runs as CTA pairs
   cudaError_t e = cudaSuccess;
 #define PVF_CALL(C_, B_, G_) e = setup_impl<C_, B_, G_>()

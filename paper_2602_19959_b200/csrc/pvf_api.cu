@@ -88,8 +88,8 @@ bool config_ok(const pvf_config* c) {
   if (!(c->peak_threshold == c->peak_threshold)) return false;
   if (c->peak_halfwidth != kPeakHalf || c->max_peaks != kMaxPeaks) return false;
   if (c->precision < PVF_PREC_FP32 || c->precision > PVF_PREC_FP16) return false;
-  // split_mask: only bit 0 (e1) is built, and only for TF32 (unet_tc_setup would refuse anything else later)
-  if (c->split_mask != 0 && !(c->precision == PVF_PREC_TF32 && c->split_mask == 1)) return false;
+  // split_mask: only bit 0 (e1) is built, for the two formats with a 10-bit mantissa (unet_tc_setup would refuse anything else later)
+  if (c->split_mask != 0 && !((c->precision == PVF_PREC_TF32 || c->precision == PVF_PREC_FP16) && c->split_mask == 1)) return false;
   if (c->max_events < 1 || c->max_tracks < 1 || c->max_tracks > 0x7fffffffLL) return false;
   if (c->unet_cta_pair != 0 && c->unet_cta_pair != 1) return false;
   if (c->elide_empty_intervals && !uses_tc(c)) return false;                     // tensor-core kernels only

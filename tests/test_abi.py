@@ -67,7 +67,7 @@ def test_default_config_and_workspace_bytes(lib):
                                          ("max_peaks", 16), ("precision", 7), ("max_events", 0), ("max_tracks", 0),
                                          ("split_mask", 64), ("split_mask", 1), ("fc_hidden", 32)])
 def test_invalid_config_is_rejected_on_the_host(lib, field, value):
-    # (split_mask 1 is the e1 split of the TF32 mode; the default precision here is FP32, where no split exists)
+    # (split_mask 1 is the e1 split of the TF32 and FP16 modes; the default precision here is FP32, where no split exists)
     cfg = pkg.default_config(lib, 4, 100)
     setattr(cfg, field, value)
     assert lib.pvf_workspace_bytes(C.byref(cfg)) == 0
@@ -91,3 +91,10 @@ def test_null_arguments(lib):
 def test_struct_sizes_match_header():
     # int32 x2, float x2, int32 x4, int32 x5, float x2, int32 x5, int64, int32 x3, float, int32 x2
     assert C.sizeof(pvf_config) == 112
+
+
+def test_e1_split_is_a_mode_of_the_ten_bit_formats_only(lib):
+    """split_mask = 1: accepted with PVF_PREC_TF32 and PVF_PREC_FP16 (a workspace size comes back), rejected with BF16 / FP32."""
+    for prec, ok in (("tf32", True), ("fp16", True), ("bf16", False), ("fp32", False)):
+        cfg = pkg.default_config(lib, 4, 100, precision=pkg.PRECISIONS[prec], split_mask=1)
+        assert (lib.pvf_workspace_bytes(C.byref(cfg)) > 0) == ok, prec
