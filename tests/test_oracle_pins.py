@@ -424,3 +424,22 @@ def test_peaky_head_recipe_conditioning():
     assert lost_far["first"] > 0, lost_far                 # the first recipe loses peaks well above the threshold
     assert lost["final"] < 0.5 * lost["first"], lost
     assert lost_far["final"] == 0, lost_far                # the final one only threshold-adjacent ones
+
+
+def test_e1_split_tolerance_study_for_the_ten_bit_formats():
+    """Why split_mask = 1 exists: with every conv operand rounded to a 10-bit-mantissa format (FP16 here; exact
+    accumulation) the probability error is dominated by the e1 layer, which reads the raw histogram; keeping e1's operands
+    exact -- what the two-piece split does to 2^-22 -- removes about a third to a half of the error.  Oracle only."""
+    ev = make_events("run3", 24, 1001)
+    w = make_weights("peaky", 1)
+    ref = O.run(ev.feat, ev.event_offsets, w)["probs"].astype(np.float64)
+
+    def fp16(a):
+        return np.asarray(a, np.float32).astype(np.float16).astype(np.float64)
+
+    every = {k: fp16 for k in ("e1", "e2", "b", "d2", "d1")}
+    split = {k: fp16 for k in ("e2", "b", "d2", "d1")}
+    e_all = np.abs(O.run(ev.feat, ev.event_offsets, w, operand_round=every)["probs"] - ref).max()
+    e_split = np.abs(O.run(ev.feat, ev.event_offsets, w, operand_round=split)["probs"] - ref).max()
+    assert 0 < e_split < 0.8 * e_all
+    assert e_split < 1e-3 and e_all < 2e-3          # the stated tolerances of fp16 + split (= TF32's) and of plain fp16
