@@ -350,7 +350,7 @@ def test_accuracy_vs_width_and_precision_table(ch):
     ev, w, ref = _oracle_cached("peaky", 160, seed=1001, ch=ch)
     eff_o, fake_o = _pv_efficiency(ev.pv_z, ref["peaks"]["z"], ref["peaks"]["count"])
     rows = [f"| {ch} | oracle (FP64) | - | {int(ref['peaks']['count'].sum())} | - | {100 * eff_o:.1f} | {fake_o:.2f} |"]
-    for prec in ["fp32", "tf32", "fp16", "bf16"]:
+    for prec in ["fp32", "tf32", "fp16s", "fp16", "bf16"]:
         pvf = _make(w, ev, prec)
         probs, pk = _run(pvf, ev)
         err = float(np.abs(probs.cpu().numpy().astype(np.float64) - ref["probs"]).max())
