@@ -63,7 +63,7 @@ class ClockSampler:
     """nvidia-smi clocks + throttle reasons sampled DURING the timed regions (B200_PROFILING.md); one background
     process for the whole run, summarised per wall-clock window."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap,power.draw.instant,power.limit")
 
     def __init__(self, index=0):
         self.rows, self.proc, self.thread, self.index = [], None, None, index
@@ -87,7 +87,7 @@ class ClockSampler:
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         time.sleep(0.12)
-        sm, mx, reasons = [], None, set()
+        sm, mx, reasons, pw, plim = [], None, set(), [], None
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         rows = [r for (t, r) in list(self.rows) if t0 <= t <= t1 + 0.1] or [r for (_, r) in list(self.rows)[-1:]]
         for r in rows:
@@ -99,8 +99,17 @@ class ClockSampler:
             for n, v in zip(names, p[2:6]):
                 if v.lower().startswith("active"):
                     reasons.add(n)
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx,
-                "reasons": sorted(reasons), "samples": len(sm)}
+            try:                                  # instantaneous board power: what sw_power_cap is about (the steps are power-bound)
+                pw.append(float(p[6])); plim = float(p[7])
+            except Exception:
+                pass
+        out = {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx,
+               "reasons": sorted(reasons), "samples": len(sm)}
+        if pw:
+            out["power_w"] = float(np.median(pw))    # instantaneous samples (100 ms apart) inside the window: median and maximum
+            out["power_w_max"] = float(np.max(pw))
+            out["power_limit_w"] = plim
+        return out
 
     def stop(self):
         if self.proc is not None:
