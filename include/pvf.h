@@ -51,7 +51,10 @@ typedef enum {
                         unet_cta_pair = 0: FP32 FMA direct convolution on the CUDA cores, the bisecting reference */
   PVF_PREC_TF32 = 1, /* tcgen05 kind::tf32, operands RN-rounded to TF32, FP32 accumulate in TMEM */
   PVF_PREC_BF16 = 2, /* tcgen05 kind::f16 with BF16 operands, FP32 accumulate in TMEM */
-  PVF_PREC_FP16 = 3  /* tcgen05 kind::f16 with FP16 operands (the paper's roadmap precision) */
+  PVF_PREC_FP16 = 3  /* tcgen05 kind::f16 with FP16 operands (the paper's roadmap precision), FP32 accumulation.
+                        Operands are rounded to FP16 with saturation to +-inf beyond 65504: histogram values and activations
+                        must stay below that (the synthetic workloads peak at a few hundred); with split_mask = 1 it meets the
+                        TF32 tolerance */
 } pvf_precision;
 
 /* Bits of pvf_peaks.event_flags (data-dependent anomalies never fail the call: PAPER.md:57). */
