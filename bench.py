@@ -381,13 +381,14 @@ def run_variants(torch, PVFinder, args, sampler, peaks, peaks_src, tf32_measured
             V.append({"name": name, "error": repr(exc)[:200]})
         torch.cuda.empty_cache()
     # config 0: one event, per-call latency (sub-400 us budget per event)
-    for prec in ("tf32", "fp16", "fp32"):
+    for tag, prec, split in (("tf32", "tf32", None), ("fp16", "fp16", None), ("fp16_e1split", "fp16", 1), ("fp32", "fp32", None)):
         try:
-            wl = Workload(torch, PVFinder, model="single", events=1, seed=SEEDS["single"], precision=prec)
+            wl = Workload(torch, PVFinder, model="single", events=1, seed=SEEDS["single"], precision=prec, split_mask=split)
             n = 200
             _, stage, _ = wl.timed(n, 20)                          # per-stage split: stage timing on (kernels not chained)
             wl.close()
-            wl = Workload(torch, PVFinder, model="single", events=1, seed=SEEDS["single"], precision=prec, stage_timing=False)
+            wl = Workload(torch, PVFinder, model="single", events=1, seed=SEEDS["single"], precision=prec, split_mask=split,
+                          stage_timing=False)
             ms, _, win = wl.timed(n, 20)                           # the latency: no events between the kernels, PDL chain
             iso = []
             for _ in range(30):                                    # isolated calls: launch gaps included
@@ -397,8 +398,8 @@ def run_variants(torch, PVFinder, args, sampler, peaks, peaks_src, tf32_measured
                 e1.record(wl.stream)
                 e1.synchronize()
                 iso.append(e0.elapsed_time(e1) * 1e3)
-            V.append({"name": f"config0_{prec}_latency", "events": 1, "tracks": wl.ev.n_tracks, "precision": prec,
-                      "channels": 64, "latency_us": ms * 1e3 / n, "latency_isolated_us_median": float(np.median(iso)),
+            V.append({"name": f"config0_{tag}_latency", "events": 1, "tracks": wl.ev.n_tracks, "precision": prec,
+                      "split_mask": wl.split, "channels": 64, "latency_us": ms * 1e3 / n, "latency_isolated_us_median": float(np.median(iso)),
                       "how": f"{n} back-to-back pvf_run calls on one stream (device time / call), kernels chained by programmatic "
                              "dependent launch; 30 isolated calls; stage_us from a second handle with stage timing (no PDL)",
                       "stage_us": {"sort": stage[0] * 1e3, "fc_hist": stage[1] * 1e3, "unet": stage[2] * 1e3,
@@ -406,7 +407,7 @@ def run_variants(torch, PVFinder, args, sampler, peaks, peaks_src, tf32_measured
                       "launches_per_run": wl.pvf.launches_per_run(1), "clocks": sampler.window(*win)})
             wl.close()
         except Exception as exc:
-            V.append({"name": f"config0_{prec}_latency", "error": repr(exc)[:200]})
+            V.append({"name": f"config0_{tag}_latency", "error": repr(exc)[:200]})
     return V
 
 
