@@ -806,6 +806,7 @@ FULL_CASES = [  # (precision, event model, channels): BASELINE.json configs 2, 3
     ("tf32", "pileup", 64), ("fp16", "pileup", 64),                            # config 3
     ("fp16s", "run3", 64), ("fp16s", "pileup", 64),                            # FP16 + e1 split at the TF32 tolerance
     ("bf16", "run3", 32), ("bf16", "run3", 16),                                # config 4 width sweep
+    ("tf32", "run3", 16), ("fp16s", "run3", 16),                               # the 10-bit formats at the narrowest width (9.1e-4)
     ("fp32", "run3", 64),                                                      # config 2 "FP32" on the tensor cores
     ("simt", "run3", 64),                                                      # CUDA-core kernels (2000 events)
 ]
