@@ -398,8 +398,38 @@ def run_variants(torch, PVFinder, args, sampler, peaks, peaks_src, tf32_measured
                 e1.record(wl.stream)
                 e1.synchronize()
                 iso.append(e0.elapsed_time(e1) * 1e3)
+            # the same call captured once in a CUDA graph (pvf_run allocates nothing and never synchronises; the
+            # programmatic dependent launches become programmatic edges) and replayed: what a per-event caller would do
+            graph_us, graph_iso = None, None
+            try:
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=wl.stream):
+                    wl.run()
+                with torch.cuda.stream(wl.stream):
+                    for _ in range(20):
+                        g.replay()
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record(wl.stream)
+                    for _ in range(n):
+                        g.replay()
+                    e1.record(wl.stream)
+                    e1.synchronize()
+                    graph_us = e0.elapsed_time(e1) * 1e3 / n
+                    gi = []
+                    for _ in range(30):
+                        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        e0.record(wl.stream)
+                        g.replay()
+                        e1.record(wl.stream)
+                        e1.synchronize()
+                        gi.append(e0.elapsed_time(e1) * 1e3)
+                    graph_iso = float(np.median(gi))
+                del g
+            except Exception:
+                pass
             V.append({"name": f"config0_{tag}_latency", "events": 1, "tracks": wl.ev.n_tracks, "precision": prec,
-                      "split_mask": wl.split, "channels": 64, "latency_us": ms * 1e3 / n, "latency_isolated_us_median": float(np.median(iso)),
+                      "split_mask": wl.split, "channels": 64, "latency_graph_us": graph_us,
+                      "latency_graph_isolated_us_median": graph_iso, "latency_us": ms * 1e3 / n, "latency_isolated_us_median": float(np.median(iso)),
                       "how": f"{n} back-to-back pvf_run calls on one stream (device time / call), kernels chained by programmatic "
                              "dependent launch; 30 isolated calls; stage_us from a second handle with stage timing (no PDL)",
                       "stage_us": {"sort": stage[0] * 1e3, "fc_hist": stage[1] * 1e3, "unet": stage[2] * 1e3,

@@ -151,7 +151,10 @@ PVF_API pvf_status pvf_create_in_pool(const pvf_weights* w, const pvf_config* cf
 /* The whole hot path for n_events events, enqueued on cuda_stream (a cudaStream_t; NULL is
  * rejected so that nothing can leak onto the default stream).  No allocation, no
  * host sync.  out_probs: device float [n_events, n_intervals*n_bins]; out_peaks: device views.
- * Errors detectable on the host return non-OK and enqueue nothing; n_events == 0 is a no-op. */
+ * Errors detectable on the host return non-OK and enqueue nothing; n_events == 0 is a no-op.
+ * The call may be captured in a CUDA graph (stream capture on cuda_stream) and replayed on new inputs written into the
+ * same buffers: it allocates nothing, never synchronises and touches no other stream; the programmatic dependent launches
+ * that chain its kernels become programmatic edges of the graph.  Not with enable_stage_timing (event records). */
 PVF_API pvf_status pvf_run(pvf_handle h, const pvf_tracks* tracks, int32_t n_events, float* out_probs,
                    const pvf_peaks* out_peaks, void* cuda_stream);
 

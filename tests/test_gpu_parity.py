@@ -508,6 +508,54 @@ def test_small_batches_match_the_batch_path_bit_for_bit(prec):
 
 
 # ------------------------------------------------------------------ CTA pairs (cta_group::2)
+@pytest.mark.parametrize("prec", ["tf32", "fp16s", "fp32", "simt"])
+def test_pvf_run_under_cuda_graph_capture(prec):
+    """PAPER.md:53 (no allocation, no host sync, no default-stream work per call) makes pvf_run capturable: the four launches
+    of a call -- chained by programmatic dependent launch -- are captured into a CUDA graph once and replayed on new inputs
+    written into the same buffers.  Replays must equal direct calls bit for bit (one event and seven), also after the inputs
+    changed, and pvf_histogram_noalloc (first call outside the capture) is capturable too."""
+    w = make_weights("peaky", 2)
+    evs = [make_events("run3", 7, 90 + k) for k in range(3)]
+    T = max(e.n_tracks for e in evs)
+    for n in (1, 7):
+        pvf = PVFinder(w, max_events=7, max_tracks=T, precision=PRECISION.get(prec, prec), split_mask=SPLIT[prec],
+                       cta_pair=prec != "simt")
+        feat = torch.zeros(9, T, device="cuda")
+        off = torch.zeros(8, dtype=torch.int32, device="cuda")
+        probs = torch.full((7, 4000), -1.0, device="cuda")
+        H = torch.full((7, 40, 8, 100), -1.0, device="cuda")
+        pk = pvf.alloc_peaks(7)
+        s = torch.cuda.Stream()
+
+        def load(ev):
+            feat[:, :ev.n_tracks] = torch.from_numpy(ev.feat).cuda()
+            off.copy_(torch.from_numpy(ev.event_offsets).cuda())
+            torch.cuda.synchronize()
+
+        load(evs[0])
+        pvf.run(feat[:, :T], off, n, probs, pk, stream=s)                 # warm-up outside the capture (module load,
+        pvf.histogram_noalloc(feat[:, :T], off, n, H, None, stream=s)     # address of the static scratch)
+        s.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            pvf.run(feat[:, :T], off, n, probs, pk, stream=s)
+            pvf.histogram_noalloc(feat[:, :T], off, n, H, None, stream=s)
+        for ev in evs[::-1]:
+            load(ev)
+            probs.fill_(-1.0)
+            H.fill_(-1.0)
+            g.replay()
+            torch.cuda.synchronize()
+            got_p, got_h, got_k = probs[:n].clone(), H[:n].clone(), {k: v[:n].clone() for k, v in pk.items()}
+            pvf.run(feat[:, :T], off, n, probs, pk, stream=s)
+            pvf.histogram_noalloc(feat[:, :T], off, n, H, None, stream=s)
+            s.synchronize()
+            assert torch.equal(got_p, probs[:n]) and torch.equal(got_h, H[:n])
+            assert all(torch.equal(got_k[k], pk[k][:n]) for k in pk)
+            assert float(got_p.min()) > 0.0
+        pvf.destroy()
+
+
 @pytest.mark.parametrize("prec,channels", [("tf32", 64), ("bf16", 64), ("fp16", 64), ("fp16s", 64), ("fp16s", 16), ("tf32", 32), ("bf16", 32),
                                            ("tf32", 16), ("bf16", 16)])
 def test_cta_pair_is_bit_identical(prec, channels):
