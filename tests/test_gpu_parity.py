@@ -508,6 +508,32 @@ def test_small_batches_match_the_batch_path_bit_for_bit(prec):
 
 
 # ------------------------------------------------------------------ CTA pairs (cta_group::2)
+def test_two_handles_on_two_streams_do_not_interfere():
+    """Handles share nothing (each owns its pool; PAPER.md:53 one workspace bound at init): two of them, different modes,
+    driven concurrently on two streams must give what each gives alone, every time."""
+    w = make_weights("peaky", 6)
+    ev_a, ev_b = make_events("run3", 300, 71), make_events("pileup", 200, 72)
+    a = _make(w, ev_a, "tf32", elide_empty=True)
+    b = _make(w, ev_b, "fp16s")
+    pa, ka = _run(a, ev_a)
+    pb, kb = _run(b, ev_b)
+    fa, oa = _dev(ev_a)
+    fb, ob = _dev(ev_b)
+    sa, sb_ = torch.cuda.Stream(), torch.cuda.Stream()
+    qa, qb = torch.empty_like(pa), torch.empty_like(pb)
+    ja, jb = a.alloc_peaks(300), b.alloc_peaks(200)
+    for _ in range(10):
+        qa.fill_(-1.0)
+        qb.fill_(-1.0)
+        torch.cuda.synchronize()
+        for _ in range(3):                                        # several calls in flight on both streams
+            a.run(fa, oa, 300, qa, ja, stream=sa)
+            b.run(fb, ob, 200, qb, jb, stream=sb_)
+        torch.cuda.synchronize()
+        assert torch.equal(qa, pa) and torch.equal(qb, pb)
+        assert all(torch.equal(ja[k], ka[k]) for k in ka) and all(torch.equal(jb[k], kb[k]) for k in kb)
+
+
 @pytest.mark.parametrize("prec", ["tf32", "fp16s", "fp32", "simt"])
 def test_pvf_run_under_cuda_graph_capture(prec):
     """PAPER.md:53 (no allocation, no host sync, no default-stream work per call) makes pvf_run capturable: the four launches
