@@ -87,7 +87,7 @@ typedef struct {
                               pieces (BF16 pieces in the TF32 kernel, FP16 pieces in the FP16 kernel).
                               Anything else is PVF_ERR_CONFIG: FP32 accuracy on every layer is PVF_PREC_FP32, not a mask value */
   int32_t max_events;      /* capacity the pool is sized for (>= 1) */
-  int64_t max_tracks;      /* capacity the pool is sized for (>= 1) */
+  int64_t max_tracks;      /* capacity the pool is sized for (>= 1, <= 536 870 911 = 2^29 - 1: the sorted list keeps a track index in 29 bits) */
   int32_t enable_stage_timing; /* pre-creates CUDA events around the four stages; default 0 */
   int32_t enable_host_io;  /* reserve pool space for pvf_run_host's device staging; default 0 */
   int32_t elide_empty_intervals; /* tensor-core kernels only; default 0.  1: the UNet runs only over intervals that

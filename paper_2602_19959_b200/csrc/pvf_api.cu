@@ -90,12 +90,12 @@ bool config_ok(const pvf_config* c) {
   if (c->precision < PVF_PREC_FP32 || c->precision > PVF_PREC_FP16) return false;
   // split_mask: only bit 0 (e1) is built, for the two formats with a 10-bit mantissa (unet_tc_setup would refuse anything else later)
   if (c->split_mask != 0 && !((c->precision == PVF_PREC_TF32 || c->precision == PVF_PREC_FP16) && c->split_mask == 1)) return false;
-  if (c->max_events < 1 || c->max_tracks < 1 || c->max_tracks > 0x7fffffffLL) return false;
+  // a perm entry keeps the track index in 29 bits (pvf_internal.cuh kEntryMask): 536 870 911 tracks per call at most
+  if (c->max_events < 1 || c->max_tracks < 1 || c->max_tracks > (int64_t)kEntryMask) return false;
   if (c->unet_cta_pair != 0 && c->unet_cta_pair != 1) return false;
   if (c->elide_empty_intervals && !uses_tc(c)) return false;                     // tensor-core kernels only
   if (!(c->boundary_margin_mm >= 0.0f && c->boundary_margin_mm < 4.9f)) return false;
   if (c->l2_chunk_events < 0) return false;
-  if (c->boundary_margin_mm > 0.0f && c->max_tracks > (int64_t)kEntryMask) return false;
   return true;
 }
 

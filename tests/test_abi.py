@@ -64,7 +64,7 @@ def test_default_config_and_workspace_bytes(lib):
 
 
 @pytest.mark.parametrize("field,value", [("n_intervals", 41), ("n_bins", 64), ("unet_channels", 48), ("k_e1", 27),
-                                         ("max_peaks", 16), ("precision", 7), ("max_events", 0), ("max_tracks", 0),
+                                         ("max_peaks", 16), ("precision", 7), ("max_events", 0), ("max_tracks", 0), ("max_tracks", 1 << 29),
                                          ("split_mask", 64), ("split_mask", 1), ("fc_hidden", 32)])
 def test_invalid_config_is_rejected_on_the_host(lib, field, value):
     # (split_mask 1 is the e1 split of the TF32 and FP16 modes; the default precision here is FP32, where no split exists)
