@@ -534,6 +534,44 @@ def test_two_handles_on_two_streams_do_not_interfere():
         assert all(torch.equal(ja[k], ka[k]) for k in ka) and all(torch.equal(jb[k], kb[k]) for k in kb)
 
 
+def test_host_threads_with_their_own_handles():
+    """The library keeps no mutable global state outside a handle (the static scratch of pvf_histogram_noalloc aside): four host
+    threads, each creating its own handle and stream and calling pvf_run 30 times (ctypes releases the GIL), all get the
+    result of the single-threaded run."""
+    import threading
+    w = make_weights("peaky", 8)
+    ev = make_events("run3", 64, 73)
+    want = {}
+    for prec in ("tf32", "bf16", "fp16s", "simt"):
+        p, k = _run(_make(w, ev, prec), ev)
+        want[prec] = (p, k)
+    errors = []
+
+    def worker(prec):
+        try:
+            torch.cuda.set_device(0)
+            pvf = _make(w, ev, prec)
+            feat, off = _dev(ev)
+            probs = torch.empty(64, 4000, device="cuda")
+            pk = pvf.alloc_peaks(64)
+            s = torch.cuda.Stream()
+            for _ in range(30):
+                pvf.run(feat, off, 64, probs, pk, stream=s)
+            s.synchronize()
+            if not torch.equal(probs, want[prec][0]) or not all(torch.equal(pk[k], want[prec][1][k]) for k in pk):
+                errors.append(f"{prec}: result differs")
+            pvf.destroy()
+        except Exception as exc:                                  # noqa: BLE001 -- reported below
+            errors.append(f"{prec}: {exc!r}")
+
+    threads = [threading.Thread(target=worker, args=(p,)) for p in ("tf32", "bf16", "fp16s", "simt")]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+
+
 @pytest.mark.parametrize("prec", ["tf32", "fp16s", "fp32", "simt"])
 def test_pvf_run_under_cuda_graph_capture(prec):
     """PAPER.md:53 (no allocation, no host sync, no default-stream work per call) makes pvf_run capturable: the four launches
